@@ -1,0 +1,340 @@
+/*
+ * cobalt_oracle.c -- float64 CPU ORACLE for the Cobalt correlator hot path.
+ *
+ * THIS IS TEST INFRASTRUCTURE, NOT THE PRODUCT.  Only tests/, __graft_entry__.smoke()
+ * and bench.py's cpu_baseline / --impl reference legs may load it.  It shares no code,
+ * header, table or constant generator with the CUDA path under
+ * paper_1801_04834_b200/csrc/ and never includes anything from there.
+ *
+ * What it computes (PAPER.md = /root/reference/PAPER.md, "P:Lnnn" = line nnn):
+ *   P:L89  (sec 3.2)  "Data is converted from fixed to floating point"            -> oracle_unpack_*
+ *   P:L360 (sec 7.5)  "channelizes subbands in a polyphase filter using FIR
+ *                      filters and FFT kernels. We carry FIR filter history
+ *                      samples across to the next block."                          -> oracle_fir, oracle_dft
+ *   P:L360, P:L368    "fine delay compensation and bandpass correction"; phase
+ *                      angles in double precision, rotate each sample               -> oracle_rotate
+ *   P:L360            "computes the correlations of all pairs of antenna fields
+ *                      and averages in time"                                        -> oracle_correlate
+ * The paper prints no formulas; every formula below is the reading fixed in
+ * SURVEY.md sec 8(c) / DESIGN.md "Readings" (A1..A20) and is written out in the
+ * order of that algorithm listing, in plain loops, in double precision: direct
+ * FIR convolution, naive O(C^2) DFT, explicit per-baseline multiply-accumulate.
+ * No blocking, no fusion, no FFT.  OpenMP only splits an outermost independent
+ * index (stream, or channel) across cores; it never changes a summation order.
+ *
+ * Pins (tests/test_oracle_pins.py): P2 firwin, P3 DC, P4 tone closed form, P5
+ * impulse, P6 numpy.fft special case, P7 Hermitian, P8 identical streams, P9
+ * delay slope, P10 history carry, P11 brute force (oracle_channel_direct below
+ * + a numpy brute force), P12 linearity, P13 statistics.  No function here is
+ * "parity unpinned".
+ *
+ * Layouts (all row-major, last index fastest):
+ *   samples  [S][2][N][2]      int16 or int8, (re,im) interleaved, one subband
+ *   hist     [S][2][(T-1)*C][2] double, the (T-1)*C samples preceding samples[..][0]
+ *   g        [T*C]             double prototype filter
+ *   F, z     [S][2][n_t][C][2] double (channel index j ascending in frequency)
+ *   vis      [C][n_bl][2][2][2] double, n_bl = S(S+1)/2, baseline (i<=k) at k(k+1)/2+i,
+ *                               then [pol of i][pol of k][re,im]
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define ORACLE_PI 3.14159265358979323846264338327950288
+
+/* Number of threads the OpenMP loops will use (1 without OpenMP). */
+int oracle_num_threads(void) {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+/* ------------------------------------------------------------------ step 1 */
+/* fixed -> floating point.  Two's complement value, no scaling, no
+ * flagging of extreme values (reading A12). */
+void oracle_unpack_i16(const int16_t *in, long long n, double *out) {
+    for (long long i = 0; i < n; ++i) out[i] = (double)in[i];
+}
+void oracle_unpack_i8(const int8_t *in, long long n, double *out) {
+    for (long long i = 0; i < n; ++i) out[i] = (double)in[i];
+}
+
+/* ------------------------------------------------------------------ step 2 */
+/* Reading A1 (BASELINE.json configs: "16-tap FIR (Hann-windowed sinc)"):
+ * g[n] = sinc((n-(L-1)/2)/C) * (0.5 - 0.5 cos(2 pi n/(L-1))), L = T*C, then
+ * divided by sum(g) so that the DC gain is 1. */
+void oracle_fir_prototype(int C, int T, double *g) {
+    const int L = T * C;
+    double sum = 0.0;
+    for (int n = 0; n < L; ++n) {
+        double u = ((double)n - 0.5 * (double)(L - 1)) / (double)C;
+        double sinc = (u == 0.0) ? 1.0 : sin(ORACLE_PI * u) / (ORACLE_PI * u);
+        double hann = 0.5 - 0.5 * cos(2.0 * ORACLE_PI * (double)n / (double)(L - 1));
+        g[n] = sinc * hann;
+        sum += g[n];
+    }
+    for (int n = 0; n < L; ++n) g[n] /= sum;
+}
+
+/* ------------------------------------------------------------------ step 3 */
+/* P:L360 / P:L150 "many FIR filters feeding into an FFT".  One stream.
+ * xh = history followed by the block: xh[(T-1)*C + n] = x[n].
+ * y[t][ph] = sum_{k=0}^{T-1} g[(T-1-k)*C + ph] * x[(t-k)*C + ph]   (reading A2:
+ * k = 0 is the newest block and takes the LAST C prototype taps). */
+void oracle_fir(int C, int T, const double *g, const double *xh /*[(T-1)*C + n_t*C][2]*/,
+                long long n_t, double *y /*[n_t][C][2]*/) {
+    const long long off = (long long)(T - 1) * C;
+    for (long long t = 0; t < n_t; ++t) {
+        for (int ph = 0; ph < C; ++ph) {
+            double re = 0.0, im = 0.0;
+            for (int k = 0; k < T; ++k) {
+                double w = g[(T - 1 - k) * C + ph];
+                long long idx = off + (t - k) * C + ph;
+                re += w * xh[2 * idx];
+                im += w * xh[2 * idx + 1];
+            }
+            y[2 * (t * C + ph)] = re;
+            y[2 * (t * C + ph) + 1] = im;
+        }
+    }
+}
+
+/* ------------------------------------------------------------- steps 4 + 5 */
+/* P:L340 (the paper calls cuFFT): forward, negative exponent, unnormalised
+ * (reading A4), written as the naive O(C^2) sum.
+ * D[t][c] = sum_ph y[t][ph] exp(-2 pi i ((ph*c) mod C)/C);
+ * F[t][j] = D[t][(j + C/2) mod C]   (reading A5: ascending frequency). */
+void oracle_dft(int C, const double *y /*[n_t][C][2]*/, long long n_t, double *F /*[n_t][C][2]*/) {
+    double *cs = (double *)malloc(sizeof(double) * 2 * (size_t)C);
+    for (int m = 0; m < C; ++m) {
+        cs[2 * m] = cos(-2.0 * ORACLE_PI * (double)m / (double)C);
+        cs[2 * m + 1] = sin(-2.0 * ORACLE_PI * (double)m / (double)C);
+    }
+    for (long long t = 0; t < n_t; ++t) {
+        for (int j = 0; j < C; ++j) {
+            int c = (j + C / 2) % C;
+            double re = 0.0, im = 0.0;
+            for (int ph = 0; ph < C; ++ph) {
+                int m = (int)(((long long)ph * c) % C);
+                double yr = y[2 * (t * C + ph)], yi = y[2 * (t * C + ph) + 1];
+                re += yr * cs[2 * m] - yi * cs[2 * m + 1];
+                im += yr * cs[2 * m + 1] + yi * cs[2 * m];
+            }
+            F[2 * (t * C + j)] = re;
+            F[2 * (t * C + j) + 1] = im;
+        }
+    }
+    free(cs);
+}
+
+/* ------------------------------------------------------------- steps 6 + 7 */
+/* Reading A6: f[j] = f_sb + (j - C/2) f_s/C.  P:L368 + BASELINE.json north_star:
+ * z = F * b[j] * exp(-2 pi i frac(f[j] tau)), everything in double here. */
+double oracle_channel_frequency(int C, double f_sb, double f_s, int j) {
+    return f_sb + ((double)j - 0.5 * (double)C) * f_s / (double)C;
+}
+void oracle_rotate(int C, double f_sb, double f_s, double tau, const double *bandpass /*[C]*/,
+                   long long n_t, double *F /*[n_t][C][2] in/out*/) {
+    for (int j = 0; j < C; ++j) {
+        double cyc = oracle_channel_frequency(C, f_sb, f_s, j) * tau;
+        double frac = cyc - floor(cyc);
+        double wr = bandpass[j] * cos(-2.0 * ORACLE_PI * frac);
+        double wi = bandpass[j] * sin(-2.0 * ORACLE_PI * frac);
+        for (long long t = 0; t < n_t; ++t) {
+            double a = F[2 * (t * C + j)], b = F[2 * (t * C + j) + 1];
+            F[2 * (t * C + j)] = a * wr - b * wi;
+            F[2 * (t * C + j) + 1] = a * wi + b * wr;
+        }
+    }
+}
+
+/* ------------------------------------------------------------------ step 8 */
+/* P:L360.  V[j][bl(i,k)][p][q] = sum_t z[i][p][t][j] conj(z[k][q][t][j]), i <= k
+ * (readings A9, A10: plain sum, no division, autos keep all four products). */
+void oracle_correlate(int S, int C, long long n_t, const double *z /*[S][2][n_t][C][2]*/,
+                      double *vis /*[C][n_bl][2][2][2]*/) {
+    const long long n_bl = (long long)S * (S + 1) / 2;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int j = 0; j < C; ++j) {
+        for (int k = 0; k < S; ++k) {
+            for (int i = 0; i <= k; ++i) {
+                long long bl = (long long)k * (k + 1) / 2 + i;
+                for (int p = 0; p < 2; ++p) {
+                    for (int q = 0; q < 2; ++q) {
+                        const double *zi = z + 2 * ((((long long)i * 2 + p) * n_t) * C);
+                        const double *zk = z + 2 * ((((long long)k * 2 + q) * n_t) * C);
+                        double re = 0.0, im = 0.0;
+                        for (long long t = 0; t < n_t; ++t) {
+                            double ar = zi[2 * (t * C + j)], ai = zi[2 * (t * C + j) + 1];
+                            double br = zk[2 * (t * C + j)], bi = zk[2 * (t * C + j) + 1];
+                            re += ar * br + ai * bi;
+                            im += ai * br - ar * bi;
+                        }
+                        double *o = vis + 2 * ((((long long)j * n_bl + bl) * 2 + p) * 2 + q);
+                        o[0] = re;
+                        o[1] = im;
+                    }
+                }
+            }
+        }
+    }
+}
+
+/* --------------------------------------------------- the F-stage, per stream */
+/* Steps 1-7 and 9 for every stream of one subband, from double-precision
+ * samples (x may come from oracle_unpack_* or, for pins that must avoid
+ * quantisation, directly from the test).  hist is read, then replaced by the
+ * last (T-1)*C consumed samples (step 9, "carry FIR filter history").
+ * delays may be NULL (no rotation, no bandpass: z = F). */
+int oracle_fstage_f64(int S, int C, int T, long long N, const double *x /*[S][2][N][2]*/,
+                      const double *g /*[T*C]*/, double *hist /*[S][2][(T-1)*C][2]*/,
+                      const double *delays /*[S] or NULL*/, const double *bandpass /*[C]*/,
+                      double f_sb, double f_s, double *z /*[S][2][n_t][C][2]*/) {
+    const long long n_t = N / C;          /* reading A11: trailing N - n_t*C samples unused */
+    const long long nu = n_t * C;
+    const long long nh = (long long)(T - 1) * C;
+    int fail = 0;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int sp = 0; sp < 2 * S; ++sp) {
+        double *xh = (double *)malloc(sizeof(double) * 2 * (size_t)(nh + nu));
+        double *y = (double *)malloc(sizeof(double) * 2 * (size_t)(nu > 0 ? nu : 1));
+        if (!xh || !y) {
+            fail = 1;
+            free(xh);
+            free(y);
+            continue;
+        }
+        double *h = hist + 2 * (long long)sp * nh;
+        memcpy(xh, h, sizeof(double) * 2 * (size_t)nh);
+        memcpy(xh + 2 * nh, x + 2 * (long long)sp * N, sizeof(double) * 2 * (size_t)nu);
+        double *zz = z + 2 * (long long)sp * nu;
+        oracle_fir(C, T, g, xh, n_t, y);
+        oracle_dft(C, y, n_t, zz);
+        if (delays) oracle_rotate(C, f_sb, f_s, delays[sp / 2], bandpass, n_t, zz);
+        memcpy(h, xh + 2 * nu, sizeof(double) * 2 * (size_t)nh);   /* last nh of hist||block */
+        free(xh);
+        free(y);
+    }
+    return fail;
+}
+
+/* ---------------------------------------------------------- whole subband */
+/* One subband through steps 1-9 from integer samples.  bits = 16 or 8.
+ * z_out may be NULL; otherwise receives z [S][2][n_t][C][2].
+ * Returns 0, or 1 on allocation failure / bad bits. */
+int oracle_process_subband(int S, int C, int T, long long N, int bits, const void *samples,
+                           double *hist, const double *delays, const double *bandpass,
+                           double f_sb, double f_s, double *vis, double *z_out) {
+    const long long n_t = N / C;
+    const long long n_in = (long long)S * 2 * N * 2;
+    if (bits != 16 && bits != 8) return 1;
+    double *x = (double *)malloc(sizeof(double) * (size_t)n_in);
+    double *g = (double *)malloc(sizeof(double) * (size_t)T * C);
+    double *z = z_out ? z_out : (double *)malloc(sizeof(double) * 2 * (size_t)S * 2 * n_t * C);
+    if (!x || !g || !z) {
+        free(x);
+        free(g);
+        if (!z_out) free(z);
+        return 1;
+    }
+    if (bits == 16) oracle_unpack_i16((const int16_t *)samples, n_in, x);
+    else oracle_unpack_i8((const int8_t *)samples, n_in, x);
+    oracle_fir_prototype(C, T, g);
+    int rc = oracle_fstage_f64(S, C, T, N, x, g, hist, delays, bandpass, f_sb, f_s, z);
+    if (!rc) oracle_correlate(S, C, n_t, z, vis);
+    free(x);
+    free(g);
+    if (!z_out) free(z);
+    return rc;
+}
+
+/* ------------------------------------------------- pin P11: single-sum form */
+/* An independent route to one channel, with a different loop structure from
+ * steps 3-5: window the last T*C samples with g in natural order and take one
+ * DFT bin of the whole window,
+ *   D[t][c] = sum_{n=0}^{TC-1} g[n] x[(t-(T-1))C + n] exp(-2 pi i c n / C),
+ * with the exponential evaluated per term by cos/sin of the reduced argument.
+ * Produces z for channel j (ascending-frequency index) of every input, then the
+ * visibilities of that channel by direct double loops.  Used for sampled checks
+ * at full size (one (subband, channel) at a time) and as the brute-force pin.
+ * x is double [S][2][N][2]; hist as above (not updated). */
+int oracle_channel_direct(int S, int C, int T, long long N, const double *x, const double *hist,
+                          const double *g, const double *delays, const double *bandpass,
+                          double f_sb, double f_s, int j,
+                          double *zc /*[2S][n_t][2]*/, double *vis_c /*[n_bl][2][2][2]*/) {
+    const long long n_t = N / C;
+    const long long nh = (long long)(T - 1) * C;
+    const int L = T * C;
+    const int c = (j + C / 2) % C;
+    double *er = (double *)malloc(sizeof(double) * (size_t)L);
+    double *ei = (double *)malloc(sizeof(double) * (size_t)L);
+    if (!er || !ei) {
+        free(er);
+        free(ei);
+        return 1;
+    }
+    for (int n = 0; n < L; ++n) {
+        long long m = ((long long)c * n) % C;            /* reduce before the trig call */
+        er[n] = g[n] * cos(2.0 * ORACLE_PI * (double)m / (double)C);
+        ei[n] = -g[n] * sin(2.0 * ORACLE_PI * (double)m / (double)C);
+    }
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int sp = 0; sp < 2 * S; ++sp) {
+        const double *xs = x + 2 * (long long)sp * N;
+        const double *hs = hist + 2 * (long long)sp * nh;
+        double wr = 1.0, wi = 0.0;
+        if (delays) {
+            double cyc = (f_sb + ((double)j - 0.5 * (double)C) * f_s / (double)C) * delays[sp / 2];
+            double frac = cyc - floor(cyc);
+            wr = bandpass[j] * cos(2.0 * ORACLE_PI * frac);
+            wi = -bandpass[j] * sin(2.0 * ORACLE_PI * frac);
+        }
+        for (long long t = 0; t < n_t; ++t) {
+            double re = 0.0, im = 0.0;
+            long long base = (t - (T - 1)) * C;          /* index of window start in the block */
+            for (int n = 0; n < L; ++n) {
+                long long idx = base + n;
+                double xr, xi;
+                if (idx < 0) {
+                    xr = hs[2 * (nh + idx)];
+                    xi = hs[2 * (nh + idx) + 1];
+                } else {
+                    xr = xs[2 * idx];
+                    xi = xs[2 * idx + 1];
+                }
+                re += xr * er[n] - xi * ei[n];
+                im += xr * ei[n] + xi * er[n];
+            }
+            zc[2 * (sp * n_t + t)] = re * wr - im * wi;
+            zc[2 * (sp * n_t + t) + 1] = re * wi + im * wr;
+        }
+    }
+    if (vis_c) {
+        for (int k = 0; k < S; ++k)
+            for (int i = 0; i <= k; ++i)
+                for (int p = 0; p < 2; ++p)
+                    for (int q = 0; q < 2; ++q) {
+                        const double *a = zc + 2 * ((long long)(2 * i + p) * n_t);
+                        const double *b = zc + 2 * ((long long)(2 * k + q) * n_t);
+                        double re = 0.0, im = 0.0;
+                        for (long long t = 0; t < n_t; ++t) {
+                            re += a[2 * t] * b[2 * t] + a[2 * t + 1] * b[2 * t + 1];
+                            im += a[2 * t + 1] * b[2 * t] - a[2 * t] * b[2 * t + 1];
+                        }
+                        long long bl = (long long)k * (k + 1) / 2 + i;
+                        double *o = vis_c + 2 * ((bl * 2 + p) * 2 + q);
+                        o[0] = re;
+                        o[1] = im;
+                    }
+    }
+    free(er);
+    free(ei);
+    return 0;
+}
