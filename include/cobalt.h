@@ -1,0 +1,169 @@
+/*
+ * cobalt.h -- C ABI of the B200-native Cobalt correlator hot path.
+ *
+ * One thing is built: the correlator pipeline of "Cobalt: A GPU-based correlator and
+ * beamformer for LOFAR" (arXiv:1801.04834), sec 7.5 ("P:L360"):
+ *
+ *   "The correlator pipeline first channelizes subbands in a polyphase filter using FIR
+ *    filters and FFT kernels.  We carry FIR filter history samples across to the next block.
+ *    The pipeline then applies fine delay compensation and bandpass correction. [...] the
+ *    delay and bandpass kernel transposes data on write-back [...].  The last kernel computes
+ *    the correlations of all pairs of antenna fields and averages in time to approximately 1 s."
+ *
+ * plus the fixed->floating conversion of P:L89 (sec 3.2) and the precision rule of P:L368
+ * (phase angles in double precision, everything else single precision).  The paper prints
+ * no formulas; the exact arithmetic is the reading listed in DESIGN.md ("Readings A1..A20",
+ * taken from SURVEY.md sec 8(c)), summarised at cobalt_process() below.
+ *
+ * Conventions
+ *   - Every function returns a cobalt_status (0 = OK, negative = error) and never throws,
+ *     aborts or prints.  cobalt_strerror() names a code; cobalt_last_error() gives detail.
+ *   - "device" pointers are CUDA device pointers valid on the plan's device; "host" pointers
+ *     are ordinary (for cobalt_process_host: preferably pinned) host memory.
+ *   - The caller owns every buffer it passes and the stream.  The plan owns the FIR weights,
+ *     FIR history, phase table and the intermediate (channelised) scratch.
+ *   - cobalt_process() only ENQUEUES work on `cuda_stream` and returns; buffers must stay
+ *     alive and unmodified until the stream reaches the end of the call.
+ *   - All sizes are validated; nothing is read or written outside the documented extents.
+ *   - There is no CPU fallback: without a CUDA device of compute capability 10.x every
+ *     entry point that needs the device returns COBALT_ERR_UNSUPPORTED_DEVICE / COBALT_ERR_CUDA.
+ *
+ * Symbols (S stations, B subbands, C channels, T = 16 taps, N samples per pol per subband
+ * per call, n_t = floor(N/C) spectra, N_u = n_t*C consumed samples, n_bl = S(S+1)/2).
+ */
+#ifndef COBALT_B200_H
+#define COBALT_B200_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct cobalt_plan_s cobalt_plan_t;   /* opaque */
+
+typedef enum {
+    COBALT_OK = 0,
+    COBALT_ERR_BAD_ARG = -1,             /* argument out of range / NULL pointer          */
+    COBALT_ERR_NO_MEMORY = -2,           /* host or device allocation failed              */
+    COBALT_ERR_CUDA = -3,                /* a CUDA runtime call failed (see last_error)   */
+    COBALT_ERR_UNSUPPORTED_DEVICE = -4   /* no device, or device is not sm_100 class      */
+} cobalt_status;
+
+typedef enum {
+    /* X-stage on tcgen05 tensor cores, fp16 operands, fp32 accumulation in TMEM.
+     * Tolerance vs the float64 oracle: ||dV||_F / ||V||_F <= 2e-3 per (subband, channel). */
+    COBALT_MODE_TENSOR_FP16 = 0,
+    /* Everything in fp32 (SIMT FMA correlator).  Tolerance: max |dV| / sqrt(V_ii V_kk) <= 1e-4. */
+    COBALT_MODE_EXACT_FP32 = 1
+} cobalt_mode;
+
+typedef struct {
+    int stations, subbands, channels, taps, input_bits, mode;
+    long long samples_per_integration;   /* N                                              */
+    long long n_spectra;                 /* n_t = floor(N / C)   (reading A11)             */
+    long long n_consumed;                /* N_u = n_t * C                                   */
+    long long n_baselines;               /* n_bl = S (S+1) / 2, autocorrelations included  */
+    long long input_bytes;               /* B*S*2*N*2*(bits/8): extent read from `samples` */
+    long long output_bytes;              /* B*C*n_bl*4*8: extent written to `visibilities` */
+    long long scratch_bytes;             /* device memory owned by the plan                */
+    int chunk_subbands;                  /* subbands processed per internal launch group   */
+    int sm_count;
+    double sample_rate_hz;
+} cobalt_info_t;
+
+/* ---------------------------------------------------------------------------------------
+ * cobalt_plan: validate the observation constants, allocate all device state on the current
+ * CUDA device, build the FIR weights.  ("Most kernel parameters are fixed throughout
+ * an observation"; the paper's run-time compilation becomes template specialisation on
+ * (channels, input_bits).)
+ *   stations  >= 1 (dual polarisation each), subbands >= 1,
+ *   channels  in {16, 64, 256}, taps == 16, input_bits in {16, 8},
+ *   samples_per_integration >= channels.
+ * The prototype filter is the Hann-windowed sinc of reading A1 (== scipy.signal.firwin(16 C,
+ * 1/C, window="hann")), evaluated in double and rounded once to fp32.  History starts as zeros
+ * (reading A3).  Default subband centre frequencies f_sb[s] = 100 MHz + (12 + s) * f_s, default
+ * f_s = 195312.5 Hz (reading A6); default mode COBALT_MODE_TENSOR_FP16.
+ * On failure *out = NULL. */
+int cobalt_plan(cobalt_plan_t **out, int stations, int subbands, int channels, int taps,
+                long long samples_per_integration, int input_bits);
+
+/* ---------------------------------------------------------------------------------------
+ * cobalt_process: one integration period of the whole hot path, enqueued on `cuda_stream`
+ * (a cudaStream_t passed as void*; NULL = the legacy default stream).
+ *
+ *   d_samples      device, [B][S][2 pol][N][2 (re,im)] int16 (input_bits 16) or int8 (8),
+ *                  time contiguous per polarisation (reading A13); read only.
+ *   d_delays       device, [S] double, seconds; one value per station, both pols (A7).
+ *   d_bandpass     device, [C] float, real weight multiplying the voltages (A8).
+ *   d_visibilities device, [B][C][n_bl][2][2] complex64 (float re, float im); fully
+ *                  overwritten.  Baseline (i <= k) at index k(k+1)/2 + i, then
+ *                  [pol of i][pol of k] (A9).
+ *
+ * Per subband s and stream (station a, pol p), with x = the integer samples as floats
+ * (bit-exact two's complement value, A12) preceded by the carried history:
+ *   y[t][ph] = sum_{k<16} g[(15-k) C + ph] x[(t-k) C + ph]                      (A2)
+ *   D[t][c]  = sum_ph y[t][ph] exp(-2 pi i ph c / C),  F[t][j] = D[t][(j + C/2) mod C]  (A4, A5)
+ *   f[s][j]  = f_sb[s] + (j - C/2) f_s / C                                       (A6)
+ *   z[t][j]  = F[t][j] b[j] exp(-2 pi i frac(f[s][j] tau_a))   (frac in fp64)
+ *   V[s][j][bl(i,k)][p][q] = sum_t z_{i,p}[t][j] conj(z_{k,q}[t][j])              (A9, A10)
+ * and the last 15 C consumed samples of every stream become the new history (stateful!).
+ * Only the first N_u = floor(N/C) C samples of each stream are consumed (A11). */
+int cobalt_process(cobalt_plan_t *plan, void *cuda_stream, const void *d_samples,
+                   const double *d_delays, const float *d_bandpass, void *d_visibilities);
+
+/* Same computation with HOST buffers (same layouts).  The library streams subband chunks
+ * host->device, computes, and streams visibilities device->host on internal streams, double
+ * buffered, and returns after everything has completed (synchronous).  Pinned host memory is
+ * needed for the copies to overlap; pageable memory works but serialises. */
+int cobalt_process_host(cobalt_plan_t *plan, const void *h_samples, const double *h_delays,
+                        const float *h_bandpass, void *h_visibilities);
+
+/* Frees all plan state.  cobalt_destroy(NULL) is a no-op returning COBALT_OK.  The caller must
+ * have synchronised every stream that still runs work of this plan. */
+int cobalt_destroy(cobalt_plan_t *plan);
+
+/* --------------------------------------------------------------------------- settings */
+/* Subband centre (sky) frequencies in Hz, host array [B] (A6).  Takes effect next call. */
+int cobalt_set_subband_frequencies(cobalt_plan_t *plan, const double *h_hz);
+int cobalt_set_sample_rate(cobalt_plan_t *plan, double hz);
+/* Switch COBALT_MODE_*; reallocates the intermediate scratch, keeps the history. */
+int cobalt_set_mode(cobalt_plan_t *plan, int mode);
+/* Subbands per internal launch group (>= 1, clipped to B).  Reallocates scratch. */
+int cobalt_set_chunk_subbands(cobalt_plan_t *plan, int chunk);
+/* Zero the FIR history (as after cobalt_plan).  Enqueued on the legacy default stream and
+ * synchronised before returning. */
+int cobalt_reset(cobalt_plan_t *plan);
+int cobalt_info(const cobalt_plan_t *plan, cobalt_info_t *info);
+const char *cobalt_strerror(int status);
+/* Text of the most recent failure on this plan (valid until the next call on it). */
+const char *cobalt_last_error(const cobalt_plan_t *plan);
+
+/* --------------------------------------------------------------------------- measurement */
+/* When enabled, cobalt_process() brackets each stage of each chunk with CUDA events on the
+ * caller's stream.  cobalt_get_timing() synchronises those events and returns, for the most
+ * recent cobalt_process() call, the summed device time in ms of the F-stage kernels (phase
+ * table + unpack/FIR/FFT/rotate/transpose + history update) and of the X-stage kernels, and
+ * the number of kernels the call launched.  Any output pointer may be NULL. */
+int cobalt_set_timing(cobalt_plan_t *plan, int enabled);
+int cobalt_get_timing(cobalt_plan_t *plan, double *f_stage_ms, double *x_stage_ms, int *kernel_launches);
+
+/* --------------------------------------------------------------------------- debug taps */
+/* (used by the parity tests to pin individual steps; not needed in production)           */
+/* FIR weights exactly as the kernels use them, host [16][C] float, weight of tap k (k = 0 is
+ * the newest block) and branch ph at [k*C + ph] == fp32(g[(15-k) C + ph]). */
+int cobalt_debug_fir_weights(const cobalt_plan_t *plan, float *h_weights);
+/* Step a1 alone: n integer components (int16 or int8 per input_bits) -> n floats, device. */
+int cobalt_debug_unpack(void *cuda_stream, int input_bits, const void *d_in, long long n, float *d_out);
+/* Steps a1-a7 for ONE subband `sb` of d_samples (full [B][..] array as in cobalt_process):
+ * d_z receives z as [C][2S][n_t] complex64 (input index = 2*station + pol).  Reads the history
+ * of that subband but does NOT advance it.  In TENSOR_FP16 mode the values are the fp16
+ * operands (converted back to fp32) that the X-stage would consume. */
+int cobalt_debug_channelised(cobalt_plan_t *plan, void *cuda_stream, const void *d_samples,
+                             const double *d_delays, const float *d_bandpass, int sb, void *d_z);
+/* Step a8-a9 alone for one subband: d_z [C][2S][n_t] complex64 (caller supplied) ->
+ * d_vis [C][n_bl][2][2] complex64, through the X-stage of the current mode. */
+int cobalt_debug_correlate(cobalt_plan_t *plan, void *cuda_stream, const void *d_z, void *d_vis);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* COBALT_B200_H */

@@ -1,0 +1,290 @@
+"""Thin ctypes binding of libcobalt_b200.so (include/cobalt.h): argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels under ``csrc/``; PyTorch supplies device
+memory and streams.  There is no CPU fallback: ``load()`` raises when the shared library is
+missing, and every entry point returns an error status without a B200-class device.
+
+The functions ``cobalt_plan / cobalt_process / cobalt_process_host / cobalt_destroy / ...`` take
+the same arguments as the C ABI (tensors or numpy arrays are turned into raw pointers);
+``Correlator`` is a small convenience wrapper around them.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+_PKG = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_PKG, "libcobalt_b200.so")
+
+COBALT_OK = 0
+COBALT_ERR_BAD_ARG = -1
+COBALT_ERR_NO_MEMORY = -2
+COBALT_ERR_CUDA = -3
+COBALT_ERR_UNSUPPORTED_DEVICE = -4
+COBALT_MODE_TENSOR_FP16 = 0
+COBALT_MODE_EXACT_FP32 = 1
+
+F_S = 195312.5
+
+# every symbol include/cobalt.h declares (tests check the library exports exactly these)
+ABI_SYMBOLS = (
+    "cobalt_plan", "cobalt_process", "cobalt_process_host", "cobalt_destroy",
+    "cobalt_set_subband_frequencies", "cobalt_set_sample_rate", "cobalt_set_mode",
+    "cobalt_set_chunk_subbands", "cobalt_reset", "cobalt_info", "cobalt_strerror", "cobalt_last_error",
+    "cobalt_set_timing", "cobalt_get_timing",
+    "cobalt_debug_fir_weights", "cobalt_debug_unpack", "cobalt_debug_channelised", "cobalt_debug_correlate",
+)
+
+
+class CobaltError(RuntimeError):
+    def __init__(self, status: int, detail: str = ""):
+        self.status = status
+        super().__init__(f"cobalt status {status} ({_strerror(status)}){': ' + detail if detail else ''}")
+
+
+class cobalt_info_t(ctypes.Structure):
+    _fields_ = [
+        ("stations", ctypes.c_int), ("subbands", ctypes.c_int), ("channels", ctypes.c_int), ("taps", ctypes.c_int),
+        ("input_bits", ctypes.c_int), ("mode", ctypes.c_int),
+        ("samples_per_integration", ctypes.c_longlong), ("n_spectra", ctypes.c_longlong),
+        ("n_consumed", ctypes.c_longlong), ("n_baselines", ctypes.c_longlong),
+        ("input_bytes", ctypes.c_longlong), ("output_bytes", ctypes.c_longlong), ("scratch_bytes", ctypes.c_longlong),
+        ("chunk_subbands", ctypes.c_int), ("sm_count", ctypes.c_int), ("sample_rate_hz", ctypes.c_double),
+    ]
+
+
+_lib = None
+_vp = ctypes.c_void_p
+
+
+def load(path: str | None = None):
+    """dlopen the CUDA library.  Raises (never falls back) when it has not been built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = path or LIB_PATH
+    if not os.path.exists(path):
+        raise ImportError(f"{path} is missing: run `python -c 'import __graft_entry__ as g; g.build()'` "
+                          "(nvcc, sm_100a).  There is no CPU fallback.")
+    lib = ctypes.CDLL(path)
+    lib.cobalt_plan.argtypes = [ctypes.POINTER(_vp), ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+                                ctypes.c_longlong, ctypes.c_int]
+    lib.cobalt_process.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp]
+    lib.cobalt_process_host.argtypes = [_vp, _vp, _vp, _vp, _vp]
+    lib.cobalt_destroy.argtypes = [_vp]
+    lib.cobalt_set_subband_frequencies.argtypes = [_vp, _vp]
+    lib.cobalt_set_sample_rate.argtypes = [_vp, ctypes.c_double]
+    lib.cobalt_set_mode.argtypes = [_vp, ctypes.c_int]
+    lib.cobalt_set_chunk_subbands.argtypes = [_vp, ctypes.c_int]
+    lib.cobalt_reset.argtypes = [_vp]
+    lib.cobalt_info.argtypes = [_vp, ctypes.POINTER(cobalt_info_t)]
+    lib.cobalt_strerror.argtypes = [ctypes.c_int]
+    lib.cobalt_strerror.restype = ctypes.c_char_p
+    lib.cobalt_last_error.argtypes = [_vp]
+    lib.cobalt_last_error.restype = ctypes.c_char_p
+    lib.cobalt_set_timing.argtypes = [_vp, ctypes.c_int]
+    lib.cobalt_get_timing.argtypes = [_vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double),
+                                      ctypes.POINTER(ctypes.c_int)]
+    lib.cobalt_debug_fir_weights.argtypes = [_vp, _vp]
+    lib.cobalt_debug_unpack.argtypes = [_vp, ctypes.c_int, _vp, ctypes.c_longlong, _vp]
+    lib.cobalt_debug_channelised.argtypes = [_vp, _vp, _vp, _vp, _vp, ctypes.c_int, _vp]
+    lib.cobalt_debug_correlate.argtypes = [_vp, _vp, _vp, _vp]
+    for name in ABI_SYMBOLS:
+        fn = getattr(lib, name)
+        if name not in ("cobalt_strerror", "cobalt_last_error"):
+            fn.restype = ctypes.c_int
+    _lib = lib
+    return lib
+
+
+def _strerror(status: int) -> str:
+    try:
+        return load().cobalt_strerror(status).decode()
+    except Exception:  # library missing: still give a readable message
+        return "?"
+
+
+def _ptr(x):
+    """Raw address of a torch tensor / numpy array / int / None."""
+    if x is None:
+        return None
+    if isinstance(x, int):
+        return x
+    if hasattr(x, "data_ptr"):
+        return x.data_ptr()
+    if hasattr(x, "ctypes"):
+        return x.ctypes.data
+    raise TypeError(f"cannot take the address of {type(x)}")
+
+
+def _stream_ptr(stream):
+    if stream is None:
+        import torch
+
+        return torch.cuda.current_stream().cuda_stream
+    if isinstance(stream, int):
+        return stream
+    return stream.cuda_stream
+
+
+def _check(status: int, plan=None):
+    if status != COBALT_OK:
+        detail = load().cobalt_last_error(plan).decode() if _lib is not None else ""
+        raise CobaltError(status, detail)
+
+
+# ------------------------------------------------------------------ C ABI, same names
+def cobalt_plan(stations, subbands, channels, taps, samples_per_integration, input_bits):
+    h = _vp()
+    _check(load().cobalt_plan(ctypes.byref(h), stations, subbands, channels, taps, samples_per_integration, input_bits))
+    return h
+
+
+def cobalt_process(plan, stream, d_samples, d_delays, d_bandpass, d_visibilities):
+    _check(load().cobalt_process(plan, _stream_ptr(stream), _ptr(d_samples), _ptr(d_delays), _ptr(d_bandpass),
+                                 _ptr(d_visibilities)), plan)
+
+
+def cobalt_process_host(plan, h_samples, h_delays, h_bandpass, h_visibilities):
+    _check(load().cobalt_process_host(plan, _ptr(h_samples), _ptr(h_delays), _ptr(h_bandpass), _ptr(h_visibilities)), plan)
+
+
+def cobalt_destroy(plan):
+    _check(load().cobalt_destroy(plan))
+
+
+def cobalt_info(plan) -> cobalt_info_t:
+    info = cobalt_info_t()
+    _check(load().cobalt_info(plan, ctypes.byref(info)), plan)
+    return info
+
+
+class Correlator:
+    """Owns one cobalt_plan.  Tensors are torch CUDA tensors (device memory + streams only)."""
+
+    def __init__(self, stations, subbands, channels, samples_per_integration, input_bits=16, taps=16, mode=None):
+        self._h = cobalt_plan(stations, subbands, channels, taps, samples_per_integration, input_bits)
+        if mode is not None:
+            self.set_mode(mode)
+        self.info = cobalt_info(self._h)
+
+    # -- lifetime
+    def close(self):
+        if getattr(self, "_h", None) is not None:
+            import torch
+
+            torch.cuda.synchronize()
+            cobalt_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    # -- settings
+    def set_mode(self, mode):
+        _check(load().cobalt_set_mode(self._h, mode), self._h)
+        self.info = cobalt_info(self._h)
+
+    def set_chunk_subbands(self, chunk):
+        _check(load().cobalt_set_chunk_subbands(self._h, chunk), self._h)
+        self.info = cobalt_info(self._h)
+
+    def set_subband_frequencies(self, hz):
+        import numpy as np
+
+        a = np.ascontiguousarray(hz, dtype=np.float64)
+        assert a.shape == (self.info.subbands,)
+        _check(load().cobalt_set_subband_frequencies(self._h, a.ctypes.data), self._h)
+
+    def set_sample_rate(self, hz):
+        _check(load().cobalt_set_sample_rate(self._h, float(hz)), self._h)
+
+    def reset(self):
+        _check(load().cobalt_reset(self._h), self._h)
+
+    def set_timing(self, enabled=True):
+        _check(load().cobalt_set_timing(self._h, int(enabled)), self._h)
+
+    def get_timing(self):
+        f, x, n = ctypes.c_double(), ctypes.c_double(), ctypes.c_int()
+        _check(load().cobalt_get_timing(self._h, ctypes.byref(f), ctypes.byref(x), ctypes.byref(n)), self._h)
+        return f.value, x.value, n.value
+
+    # -- the hot path
+    def vis_shape(self):
+        i = self.info
+        return (i.subbands, i.channels, i.n_baselines, 2, 2)
+
+    def process(self, samples, delays, bandpass, out=None, stream=None):
+        """samples int16/int8 [B][S][2][N][2], delays float64 [S], bandpass float32 [C] (CUDA tensors)
+        -> complex64 [B][C][n_bl][2][2].  Enqueues on ``stream`` (default: torch's current stream)."""
+        import torch
+
+        i = self.info
+        want = torch.int16 if i.input_bits == 16 else torch.int8
+        assert samples.is_cuda and samples.is_contiguous() and samples.dtype == want
+        assert tuple(samples.shape) == (i.subbands, i.stations, 2, i.samples_per_integration, 2), tuple(samples.shape)
+        assert delays.is_cuda and delays.dtype == torch.float64 and delays.is_contiguous() and delays.numel() == i.stations
+        assert bandpass.is_cuda and bandpass.dtype == torch.float32 and bandpass.is_contiguous() and bandpass.numel() == i.channels
+        if out is None:
+            out = torch.empty(self.vis_shape(), dtype=torch.complex64, device=samples.device)
+        assert out.is_cuda and out.is_contiguous() and out.dtype == torch.complex64 and tuple(out.shape) == self.vis_shape()
+        cobalt_process(self._h, stream, samples, delays, bandpass, out)
+        return out
+
+    def process_host(self, samples, delays, bandpass, out):
+        """Host buffers (numpy arrays or pinned CPU tensors), same layouts; synchronous."""
+        i = self.info
+        for a, nbytes in ((samples, i.input_bytes), (delays, 8 * i.stations), (bandpass, 4 * i.channels),
+                          (out, i.output_bytes)):
+            n = a.numel() * a.element_size() if hasattr(a, "numel") else a.nbytes
+            assert n == nbytes, (n, nbytes)
+        cobalt_process_host(self._h, samples, delays, bandpass, out)
+        return out
+
+    # -- debug taps
+    def fir_weights(self):
+        import numpy as np
+
+        w = np.empty((16, self.info.channels), dtype=np.float32)
+        _check(load().cobalt_debug_fir_weights(self._h, w.ctypes.data), self._h)
+        return w
+
+    def channelised(self, samples, delays, bandpass, sb=0, stream=None):
+        import torch
+
+        i = self.info
+        z = torch.empty((i.channels, 2 * i.stations, i.n_spectra), dtype=torch.complex64, device=samples.device)
+        _check(load().cobalt_debug_channelised(self._h, _stream_ptr(stream), samples.data_ptr(), delays.data_ptr(),
+                                               bandpass.data_ptr(), sb, z.data_ptr()), self._h)
+        return z
+
+    def correlate(self, z, stream=None):
+        import torch
+
+        i = self.info
+        assert z.is_cuda and z.is_contiguous() and z.dtype == torch.complex64
+        assert tuple(z.shape) == (i.channels, 2 * i.stations, i.n_spectra)
+        vis = torch.empty((i.channels, i.n_baselines, 2, 2), dtype=torch.complex64, device=z.device)
+        _check(load().cobalt_debug_correlate(self._h, _stream_ptr(stream), z.data_ptr(), vis.data_ptr()), self._h)
+        return vis
+
+
+def unpack(x, stream=None):
+    """Step a1 alone: int16/int8 CUDA tensor -> float32 CUDA tensor of the same shape."""
+    import torch
+
+    assert x.is_cuda and x.is_contiguous() and x.dtype in (torch.int16, torch.int8)
+    out = torch.empty(x.shape, dtype=torch.float32, device=x.device)
+    bits = 16 if x.dtype == torch.int16 else 8
+    _check(load().cobalt_debug_unpack(_stream_ptr(stream), bits, x.data_ptr(), x.numel(), out.data_ptr()))
+    return out

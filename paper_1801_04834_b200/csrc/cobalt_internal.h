@@ -1,0 +1,113 @@
+// Internal declarations shared by the CUDA translation units of libcobalt_b200.so.
+// Nothing here is part of the ABI (see include/cobalt.h) and nothing here is shared with oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <cuda_fp16.h>
+
+#include <cstdint>
+#include <string>
+#include <vector>
+
+#include "cobalt.h"
+
+namespace cobalt {
+
+constexpr int kTaps = 16;          // P:L360 FIR filter; BASELINE.json: 16-tap
+constexpr int kSubTile = 16;       // spectra per FIR->FFT hand-over
+constexpr int kKTile = 64;         // spectra per X-stage K tile (= one 128-byte fp16 row)
+constexpr int kMaxMmaGroups = 2;   // MMA groups per X-stage job
+
+// ---------------------------------------------------------------------------------------------
+// Layout of the channelised intermediate ("z", step a7, "transposes data on write-back").
+//
+// TENSOR_FP16: per subband  [C][n_kt][2 planes (re, im)][Mpad rows][64 t] fp16,
+//   rows = inputs (2*station + pol) padded with zero rows to Mpad = round_up(2S, 16); each
+//   [Mpad][64] block is stored exactly as the 128-byte-swizzled K-major shared-memory image the
+//   tcgen05 descriptors expect: the 16-byte chunk q (8 spectra) of row m sits at chunk q ^ (m & 7)
+//   of that row.  One (channel, k-tile) is therefore one contiguous 2*Mpad*128-byte span that the
+//   X-stage fetches with plain bulk copies, no tensor map.  Spectra t >= n_t are written as zeros.
+// EXACT_FP32:  per subband  [C][M][n_t] float2.
+// ---------------------------------------------------------------------------------------------
+
+// One X-stage job = one set of rows of a (subband, channel) k-tile loaded to shared memory plus up
+// to kMaxMmaGroups accumulator groups computed from it (see xstage_tc.cu).
+struct XMmaGroup {
+    int a_row;      // first row of the A operand, relative to the first loaded row (128 rows used)
+    int b_row;      // first row of the B operand, relative to the first loaded row
+    int n;          // number of B rows = accumulator columns (multiple of 16, <= 256)
+    int tmem_col;   // first TMEM column of the Re accumulator; Im follows at tmem_col + n
+    int out_row;    // global input index of A row 0
+    int out_col;    // global input index of B row 0
+};
+struct XJob {
+    int ld_row[2];     // two row ranges of the [Mpad][64] block copied to smem back to back
+    int ld_nrows[2];   // (second may be empty)
+    int n_groups;
+    int tmem_cols;     // power of two >= 32 to allocate
+    XMmaGroup g[kMaxMmaGroups];
+};
+
+struct StageEvents {
+    cudaEvent_t f0 = nullptr, f1 = nullptr, x1 = nullptr;
+};
+
+}  // namespace cobalt
+
+struct cobalt_plan_s {
+    int S = 0, B = 0, C = 0, T = 0, bits = 0, mode = COBALT_MODE_TENSOR_FP16;
+    long long N = 0, n_t = 0, N_u = 0, n_bl = 0;
+    int M = 0, Mpad = 0, n_kt = 0;
+    int chunk = 1;
+    int device = 0, sm_count = 0;
+    double f_s = 195312.5;
+    std::vector<double> f_sb;
+    double *d_f_sb = nullptr;          // [B]
+    float *d_weights = nullptr;        // [16][C], tap k (0 = newest block), branch ph
+    std::vector<float> h_weights;
+    void *d_hist[2] = {nullptr, nullptr};   // raw integer samples [B][S][2][15 C][2]; ping-pong
+    int hist_cur = 0;
+    float2 *d_phase = nullptr;         // [chunk][S][C]  b[j] exp(-2 pi i frac(f tau))
+    void *d_z = nullptr;               // intermediate of one chunk (layout per mode)
+    size_t z_subband_bytes = 0;
+    std::vector<cobalt::XJob> jobs;    // X-stage jobs of one (subband, channel)
+    cobalt::XJob *d_jobs = nullptr;
+    size_t x_smem_bytes = 0;
+    int x_stages = 0;
+    size_t scratch_bytes = 0;
+    // host-buffer path
+    cudaStream_t hs[3] = {nullptr, nullptr, nullptr};
+    void *d_in[2] = {nullptr, nullptr};
+    void *d_out[2] = {nullptr, nullptr};
+    double *d_delays_h = nullptr;
+    float *d_bandpass_h = nullptr;
+    cudaEvent_t ev_in[2] = {nullptr, nullptr}, ev_cmp[2] = {nullptr, nullptr}, ev_out[2] = {nullptr, nullptr};
+    // timing
+    bool timing = false;
+    std::vector<cobalt::StageEvents> events;
+    int n_chunks_timed = 0;
+    int launches = 0;
+    mutable std::string err;
+};
+
+namespace cobalt {
+
+inline size_t sample_bytes(int bits) { return bits == 16 ? 4 : 2; }   // one complex sample
+
+// fstage.cu ---------------------------------------------------------------------------------
+cudaError_t launch_phase_table(const cobalt_plan_s *p, cudaStream_t st, const double *d_delays,
+                               const float *d_bandpass, int b0, int nb);
+// samples_b0 points at the first subband of the chunk [b0, b0 + nb)
+cudaError_t launch_fstage(const cobalt_plan_s *p, cudaStream_t st, const void *samples_b0, int b0, int nb);
+cudaError_t launch_history_update(const cobalt_plan_s *p, cudaStream_t st, const void *samples_b0, int b0, int nb);
+cudaError_t launch_unpack(cudaStream_t st, int bits, const void *d_in, long long n, float *d_out);
+// layout.cu ---------------------------------------------------------------------------------
+cudaError_t launch_z_to_float(const cobalt_plan_s *p, cudaStream_t st, const void *d_zsub, float2 *d_out);
+cudaError_t launch_float_to_z(const cobalt_plan_s *p, cudaStream_t st, const float2 *d_in, void *d_zsub);
+// xstage_simt.cu ----------------------------------------------------------------------------
+cudaError_t launch_xstage_simt(const cobalt_plan_s *p, cudaStream_t st, const void *d_z, int nb, float2 *d_vis);
+// xstage_tc.cu ------------------------------------------------------------------------------
+void build_xjobs(cobalt_plan_s *p);
+cudaError_t launch_xstage_tc(const cobalt_plan_s *p, cudaStream_t st, const void *d_z, int nb, float2 *d_vis);
+
+}  // namespace cobalt

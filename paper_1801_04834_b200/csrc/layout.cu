@@ -1,0 +1,78 @@
+// Conversions between the plan's internal channelised layout (cobalt_internal.h) and the plain
+// [C][2S][n_t] complex64 array of the debug taps cobalt_debug_channelised / cobalt_debug_correlate.
+// Test plumbing around step a7 ("transposes data on write-back"); not on the production path.
+#include "cobalt_internal.h"
+
+namespace cobalt {
+
+namespace {
+
+__device__ __forceinline__ size_t z16_offset(int c, int kt, int plane, int m, int tt, int n_kt, int Mpad) {
+    // byte offset of element (channel c, k-tile kt, plane, row m, spectrum tt of the tile)
+    return ((((size_t)c * n_kt + kt) * 2 + plane) * Mpad + m) * 128 + ((((tt >> 3) ^ (m & 7)) << 4) | ((tt & 7) << 1));
+}
+
+__global__ void z16_to_float_kernel(const unsigned char *__restrict__ z, float2 *__restrict__ out, int C, int M,
+                                    int Mpad, int n_kt, long long n_t) {
+    const long long total = (long long)C * M * n_t;
+    for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < total;
+         idx += (long long)gridDim.x * blockDim.x) {
+        const long long t = idx % n_t;
+        const int m = (int)((idx / n_t) % M);
+        const int c = (int)(idx / (n_t * M));
+        const int kt = (int)(t / kKTile), tt = (int)(t % kKTile);
+        const __half re = *reinterpret_cast<const __half *>(z + z16_offset(c, kt, 0, m, tt, n_kt, Mpad));
+        const __half im = *reinterpret_cast<const __half *>(z + z16_offset(c, kt, 1, m, tt, n_kt, Mpad));
+        out[idx] = make_float2(__half2float(re), __half2float(im));
+    }
+}
+
+// Writes every element of the [C][n_kt][2][Mpad][64] block, zeros in the padding rows / spectra.
+__global__ void float_to_z16_kernel(const float2 *__restrict__ in, unsigned char *__restrict__ z, int C, int M,
+                                    int Mpad, int n_kt, long long n_t) {
+    const long long total = (long long)C * n_kt * Mpad * kKTile;
+    for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < total;
+         idx += (long long)gridDim.x * blockDim.x) {
+        const int tt = (int)(idx % kKTile);
+        const int m = (int)((idx / kKTile) % Mpad);
+        const int kt = (int)((idx / ((long long)kKTile * Mpad)) % n_kt);
+        const int c = (int)(idx / ((long long)kKTile * Mpad * n_kt));
+        const long long t = (long long)kt * kKTile + tt;
+        float2 v = make_float2(0.f, 0.f);
+        if (m < M && t < n_t) v = in[((size_t)c * M + m) * n_t + t];
+        *reinterpret_cast<__half *>(z + z16_offset(c, kt, 0, m, tt, n_kt, Mpad)) = __float2half_rn(v.x);
+        *reinterpret_cast<__half *>(z + z16_offset(c, kt, 1, m, tt, n_kt, Mpad)) = __float2half_rn(v.y);
+    }
+}
+
+inline unsigned grid_for(long long total, int threads) {
+    long long blocks = (total + threads - 1) / threads;
+    if (blocks > 65535) blocks = 65535;
+    if (blocks < 1) blocks = 1;
+    return (unsigned)blocks;
+}
+
+}  // namespace
+
+cudaError_t launch_z_to_float(const cobalt_plan_s *p, cudaStream_t st, const void *d_zsub, float2 *d_out) {
+    const long long total = (long long)p->C * p->M * p->n_t;
+    if (p->mode == COBALT_MODE_TENSOR_FP16) {
+        z16_to_float_kernel<<<grid_for(total, 256), 256, 0, st>>>(static_cast<const unsigned char *>(d_zsub), d_out,
+                                                                  p->C, p->M, p->Mpad, p->n_kt, p->n_t);
+        return cudaGetLastError();
+    }
+    return cudaMemcpyAsync(d_out, d_zsub, (size_t)total * sizeof(float2), cudaMemcpyDeviceToDevice, st);
+}
+
+cudaError_t launch_float_to_z(const cobalt_plan_s *p, cudaStream_t st, const float2 *d_in, void *d_zsub) {
+    if (p->mode == COBALT_MODE_TENSOR_FP16) {
+        const long long total = (long long)p->C * p->n_kt * p->Mpad * kKTile;
+        float_to_z16_kernel<<<grid_for(total, 256), 256, 0, st>>>(d_in, static_cast<unsigned char *>(d_zsub), p->C,
+                                                                  p->M, p->Mpad, p->n_kt, p->n_t);
+        return cudaGetLastError();
+    }
+    const long long total = (long long)p->C * p->M * p->n_t;
+    return cudaMemcpyAsync(d_zsub, d_in, (size_t)total * sizeof(float2), cudaMemcpyDeviceToDevice, st);
+}
+
+}  // namespace cobalt

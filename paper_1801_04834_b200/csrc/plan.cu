@@ -1,0 +1,432 @@
+// Host side of the C ABI (include/cobalt.h): plan construction, the per-call launch sequence
+//   [phase table (fp64)] -> [unpack+FIR+FFT+rotate+bandpass+transpose] -> [history carry] -> [correlate]
+// per chunk of subbands (P:L360 step order; "a small number of buffers that the CUDA kernels
+// alternate between"), the host-buffer streaming variant, settings and the debug taps.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "cobalt_internal.h"
+
+using namespace cobalt;
+
+namespace {
+
+thread_local std::string g_err;   // failures before a plan exists
+
+int fail(const cobalt_plan_s *p, int code, const std::string &msg) {
+    if (p) p->err = msg;
+    g_err = msg;
+    return code;
+}
+
+#define CK(p, call)                                                                                        \
+    do {                                                                                                   \
+        cudaError_t e__ = (call);                                                                          \
+        if (e__ != cudaSuccess)                                                                            \
+            return fail(p, e__ == cudaErrorMemoryAllocation ? COBALT_ERR_NO_MEMORY : COBALT_ERR_CUDA,      \
+                        std::string(#call) + ": " + cudaGetErrorString(e__));                              \
+    } while (0)
+
+// Reading A1: Hann-windowed sinc, unit DC gain, double precision, rounded once to fp32.
+// weights[k][ph] = g[(15 - k) C + ph]  (reading A2: tap k = 0 multiplies the newest block).
+void build_weights(int C, std::vector<float> &w) {
+    const int L = kTaps * C;
+    const double pi = 3.141592653589793238462643383279502884;
+    std::vector<double> g(L);
+    double sum = 0.0;
+    for (int n = 0; n < L; ++n) {
+        const double u = ((double)n - 0.5 * (double)(L - 1)) / (double)C;
+        const double sinc = u == 0.0 ? 1.0 : std::sin(pi * u) / (pi * u);
+        const double hann = 0.5 - 0.5 * std::cos(2.0 * pi * (double)n / (double)(L - 1));
+        g[n] = sinc * hann;
+        sum += g[n];
+    }
+    w.resize(L);
+    for (int k = 0; k < kTaps; ++k)
+        for (int ph = 0; ph < C; ++ph) w[k * C + ph] = (float)(g[(kTaps - 1 - k) * C + ph] / sum);
+}
+
+size_t subband_input_bytes(const cobalt_plan_s *p) { return (size_t)p->M * (size_t)p->N * sample_bytes(p->bits); }
+size_t subband_output_bytes(const cobalt_plan_s *p) { return (size_t)p->C * (size_t)p->n_bl * 4 * sizeof(float2); }
+
+void free_scratch(cobalt_plan_s *p) {
+    cudaFree(p->d_z);
+    cudaFree(p->d_phase);
+    p->d_z = nullptr;
+    p->d_phase = nullptr;
+    for (int i = 0; i < 2; ++i) {
+        cudaFree(p->d_in[i]);
+        cudaFree(p->d_out[i]);
+        p->d_in[i] = p->d_out[i] = nullptr;
+    }
+}
+
+// (Re)allocate the per-chunk scratch for the current mode / chunk size.
+int alloc_scratch(cobalt_plan_s *p, int chunk_request) {
+    free_scratch(p);
+    if (p->mode == COBALT_MODE_TENSOR_FP16) p->z_subband_bytes = (size_t)p->C * p->n_kt * 2 * p->Mpad * 128;
+    else p->z_subband_bytes = (size_t)p->C * p->M * (size_t)p->n_t * sizeof(float2);
+    int chunk = chunk_request;
+    if (chunk <= 0) {   // default: about 1 GiB of intermediate per launch group
+        chunk = (int)(((size_t)1 << 30) / p->z_subband_bytes);
+        if (chunk < 1) chunk = 1;
+    }
+    if (chunk > p->B) chunk = p->B;
+    p->chunk = chunk;
+    CK(p, cudaMalloc(&p->d_z, (size_t)chunk * p->z_subband_bytes));
+    CK(p, cudaMemset(p->d_z, 0, (size_t)chunk * p->z_subband_bytes));   // zero rows 2S..Mpad stay zero forever
+    CK(p, cudaMalloc(&p->d_phase, (size_t)chunk * p->S * p->C * sizeof(float2)));
+    CK(p, cudaDeviceSynchronize());
+    const size_t hist = (size_t)p->B * p->M * (kTaps - 1) * p->C * sample_bytes(p->bits);
+    p->scratch_bytes = (size_t)chunk * p->z_subband_bytes + (size_t)chunk * p->S * p->C * sizeof(float2) + 2 * hist +
+                       (size_t)kTaps * p->C * sizeof(float) + (size_t)p->B * sizeof(double);
+    return COBALT_OK;
+}
+
+// One chunk of subbands [b0, b0 + nb): samples_b0 / vis_b0 point at subband b0.
+int enqueue_chunk(cobalt_plan_s *p, cudaStream_t st, const void *samples_b0, const double *d_delays,
+                  const float *d_bandpass, float2 *vis_b0, int b0, int nb, StageEvents *ev) {
+    if (ev) CK(p, cudaEventRecord(ev->f0, st));
+    CK(p, launch_phase_table(p, st, d_delays, d_bandpass, b0, nb));
+    CK(p, launch_fstage(p, st, samples_b0, b0, nb));
+    CK(p, launch_history_update(p, st, samples_b0, b0, nb));
+    if (ev) CK(p, cudaEventRecord(ev->f1, st));
+    if (p->mode == COBALT_MODE_TENSOR_FP16) CK(p, launch_xstage_tc(p, st, p->d_z, nb, vis_b0));
+    else CK(p, launch_xstage_simt(p, st, p->d_z, nb, vis_b0));
+    if (ev) CK(p, cudaEventRecord(ev->x1, st));
+    p->launches += 4;
+    return COBALT_OK;
+}
+
+int ensure_events(cobalt_plan_s *p, int n) {
+    while ((int)p->events.size() < n) {
+        StageEvents e;
+        CK(p, cudaEventCreate(&e.f0));
+        CK(p, cudaEventCreate(&e.f1));
+        CK(p, cudaEventCreate(&e.x1));
+        p->events.push_back(e);
+    }
+    return COBALT_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *cobalt_strerror(int status) {
+    switch (status) {
+        case COBALT_OK: return "ok";
+        case COBALT_ERR_BAD_ARG: return "bad argument";
+        case COBALT_ERR_NO_MEMORY: return "out of memory";
+        case COBALT_ERR_CUDA: return "CUDA error";
+        case COBALT_ERR_UNSUPPORTED_DEVICE: return "no CUDA device of compute capability 10.x (sm_100)";
+    }
+    return "unknown status";
+}
+
+const char *cobalt_last_error(const cobalt_plan_t *plan) { return plan ? plan->err.c_str() : g_err.c_str(); }
+
+int cobalt_plan(cobalt_plan_t **out, int stations, int subbands, int channels, int taps,
+                long long samples_per_integration, int input_bits) {
+    if (!out) return fail(nullptr, COBALT_ERR_BAD_ARG, "out is NULL");
+    *out = nullptr;
+    if (stations < 1 || stations > 16384) return fail(nullptr, COBALT_ERR_BAD_ARG, "stations must be in [1, 16384]");
+    if (subbands < 1) return fail(nullptr, COBALT_ERR_BAD_ARG, "subbands must be >= 1");
+    if (channels != 16 && channels != 64 && channels != 256)
+        return fail(nullptr, COBALT_ERR_BAD_ARG, "channels must be 16, 64 or 256");
+    if (taps != kTaps) return fail(nullptr, COBALT_ERR_BAD_ARG, "taps must be 16");
+    if (input_bits != 16 && input_bits != 8) return fail(nullptr, COBALT_ERR_BAD_ARG, "input_bits must be 16 or 8");
+    if (samples_per_integration < channels)
+        return fail(nullptr, COBALT_ERR_BAD_ARG, "samples_per_integration must be >= channels");
+    if (samples_per_integration / channels > (1ll << 30))
+        return fail(nullptr, COBALT_ERR_BAD_ARG, "samples_per_integration too large");
+
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+        cudaGetLastError();
+        return fail(nullptr, COBALT_ERR_UNSUPPORTED_DEVICE, "no CUDA device");
+    }
+    int dev = 0;
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess)
+        return fail(nullptr, COBALT_ERR_CUDA, "cudaGetDeviceProperties failed");
+    if (prop.major != 10)
+        return fail(nullptr, COBALT_ERR_UNSUPPORTED_DEVICE,
+                    std::string("device is sm_") + std::to_string(prop.major * 10 + prop.minor) + ", need sm_100");
+
+    cobalt_plan_s *p = new (std::nothrow) cobalt_plan_s();
+    if (!p) return fail(nullptr, COBALT_ERR_NO_MEMORY, "host allocation failed");
+    p->S = stations;
+    p->B = subbands;
+    p->C = channels;
+    p->T = taps;
+    p->bits = input_bits;
+    p->N = samples_per_integration;
+    p->n_t = p->N / p->C;
+    p->N_u = p->n_t * p->C;
+    p->n_bl = (long long)stations * (stations + 1) / 2;
+    p->M = 2 * stations;
+    p->Mpad = (p->M + 15) / 16 * 16;
+    p->n_kt = (int)((p->n_t + kKTile - 1) / kKTile);
+    p->device = dev;
+    p->sm_count = prop.multiProcessorCount;
+    p->f_sb.resize(subbands);
+    for (int s = 0; s < subbands; ++s) p->f_sb[s] = 100.0e6 + (12 + s) * p->f_s;   // reading A6
+    build_weights(p->C, p->h_weights);
+    build_xjobs(p);
+
+    int rc = COBALT_OK;
+    auto guard = [&](cudaError_t e, const char *what) {
+        if (e != cudaSuccess && rc == COBALT_OK)
+            rc = fail(p, e == cudaErrorMemoryAllocation ? COBALT_ERR_NO_MEMORY : COBALT_ERR_CUDA,
+                      std::string(what) + ": " + cudaGetErrorString(e));
+    };
+    const size_t hist = (size_t)p->B * p->M * (kTaps - 1) * p->C * sample_bytes(p->bits);
+    guard(cudaMalloc(&p->d_weights, p->h_weights.size() * sizeof(float)), "cudaMalloc weights");
+    guard(cudaMalloc(&p->d_f_sb, (size_t)p->B * sizeof(double)), "cudaMalloc f_sb");
+    guard(cudaMalloc(&p->d_hist[0], hist), "cudaMalloc history");
+    guard(cudaMalloc(&p->d_hist[1], hist), "cudaMalloc history");
+    guard(cudaMalloc(&p->d_jobs, p->jobs.size() * sizeof(XJob)), "cudaMalloc jobs");
+    if (rc == COBALT_OK) {
+        guard(cudaMemcpy(p->d_weights, p->h_weights.data(), p->h_weights.size() * sizeof(float), cudaMemcpyHostToDevice), "weights H2D");
+        guard(cudaMemcpy(p->d_f_sb, p->f_sb.data(), (size_t)p->B * sizeof(double), cudaMemcpyHostToDevice), "f_sb H2D");
+        guard(cudaMemcpy(p->d_jobs, p->jobs.data(), p->jobs.size() * sizeof(XJob), cudaMemcpyHostToDevice), "jobs H2D");
+        guard(cudaMemset(p->d_hist[0], 0, hist), "memset history");   // reading A3
+        guard(cudaMemset(p->d_hist[1], 0, hist), "memset history");
+    }
+    if (rc == COBALT_OK) rc = alloc_scratch(p, 0);
+    if (rc != COBALT_OK) {
+        g_err = p->err;
+        cobalt_destroy(p);
+        return rc;
+    }
+    *out = p;
+    return COBALT_OK;
+}
+
+int cobalt_destroy(cobalt_plan_t *p) {
+    if (!p) return COBALT_OK;
+    free_scratch(p);
+    cudaFree(p->d_weights);
+    cudaFree(p->d_f_sb);
+    cudaFree(p->d_hist[0]);
+    cudaFree(p->d_hist[1]);
+    cudaFree(p->d_jobs);
+    cudaFree(p->d_delays_h);
+    cudaFree(p->d_bandpass_h);
+    for (auto &e : p->events) {
+        cudaEventDestroy(e.f0);
+        cudaEventDestroy(e.f1);
+        cudaEventDestroy(e.x1);
+    }
+    for (int i = 0; i < 3; ++i)
+        if (p->hs[i]) cudaStreamDestroy(p->hs[i]);
+    for (int i = 0; i < 2; ++i) {
+        if (p->ev_in[i]) cudaEventDestroy(p->ev_in[i]);
+        if (p->ev_cmp[i]) cudaEventDestroy(p->ev_cmp[i]);
+        if (p->ev_out[i]) cudaEventDestroy(p->ev_out[i]);
+    }
+    delete p;
+    return COBALT_OK;
+}
+
+int cobalt_process(cobalt_plan_t *p, void *cuda_stream, const void *d_samples, const double *d_delays,
+                   const float *d_bandpass, void *d_visibilities) {
+    if (!p) return fail(nullptr, COBALT_ERR_BAD_ARG, "plan is NULL");
+    if (!d_samples || !d_delays || !d_bandpass || !d_visibilities) return fail(p, COBALT_ERR_BAD_ARG, "NULL buffer");
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const int n_chunks = (p->B + p->chunk - 1) / p->chunk;
+    if (p->timing) {
+        int rc = ensure_events(p, n_chunks);
+        if (rc != COBALT_OK) return rc;
+    }
+    p->launches = 0;
+    p->n_chunks_timed = 0;
+    for (int ci = 0; ci < n_chunks; ++ci) {
+        const int b0 = ci * p->chunk;
+        const int nb = (p->B - b0) < p->chunk ? (p->B - b0) : p->chunk;
+        const unsigned char *sm = static_cast<const unsigned char *>(d_samples) + (size_t)b0 * subband_input_bytes(p);
+        float2 *vis = reinterpret_cast<float2 *>(static_cast<unsigned char *>(d_visibilities) + (size_t)b0 * subband_output_bytes(p));
+        int rc = enqueue_chunk(p, st, sm, d_delays, d_bandpass, vis, b0, nb, p->timing ? &p->events[ci] : nullptr);
+        if (rc != COBALT_OK) return rc;
+    }
+    if (p->timing) p->n_chunks_timed = n_chunks;
+    p->hist_cur ^= 1;   // the history kernels of this call wrote the other buffer (stream ordered)
+    return COBALT_OK;
+}
+
+int cobalt_process_host(cobalt_plan_t *p, const void *h_samples, const double *h_delays, const float *h_bandpass,
+                        void *h_visibilities) {
+    if (!p) return fail(nullptr, COBALT_ERR_BAD_ARG, "plan is NULL");
+    if (!h_samples || !h_delays || !h_bandpass || !h_visibilities) return fail(p, COBALT_ERR_BAD_ARG, "NULL buffer");
+    const size_t in_b = subband_input_bytes(p), out_b = subband_output_bytes(p);
+    if (!p->hs[0]) {
+        for (int i = 0; i < 3; ++i) CK(p, cudaStreamCreateWithFlags(&p->hs[i], cudaStreamNonBlocking));
+        for (int i = 0; i < 2; ++i) {
+            CK(p, cudaEventCreateWithFlags(&p->ev_in[i], cudaEventDisableTiming));
+            CK(p, cudaEventCreateWithFlags(&p->ev_cmp[i], cudaEventDisableTiming));
+            CK(p, cudaEventCreateWithFlags(&p->ev_out[i], cudaEventDisableTiming));
+        }
+        CK(p, cudaMalloc(&p->d_delays_h, (size_t)p->S * sizeof(double)));
+        CK(p, cudaMalloc(&p->d_bandpass_h, (size_t)p->C * sizeof(float)));
+    }
+    if (!p->d_in[0]) {
+        for (int i = 0; i < 2; ++i) {
+            CK(p, cudaMalloc(&p->d_in[i], (size_t)p->chunk * in_b));
+            CK(p, cudaMalloc(&p->d_out[i], (size_t)p->chunk * out_b));
+        }
+    }
+    cudaStream_t s_in = p->hs[0], s_cmp = p->hs[1], s_out = p->hs[2];
+    CK(p, cudaMemcpyAsync(p->d_delays_h, h_delays, (size_t)p->S * sizeof(double), cudaMemcpyHostToDevice, s_cmp));
+    CK(p, cudaMemcpyAsync(p->d_bandpass_h, h_bandpass, (size_t)p->C * sizeof(float), cudaMemcpyHostToDevice, s_cmp));
+    const int n_chunks = (p->B + p->chunk - 1) / p->chunk;
+    p->launches = 0;
+    p->n_chunks_timed = 0;
+    for (int ci = 0; ci < n_chunks; ++ci) {
+        const int buf = ci & 1;
+        const int b0 = ci * p->chunk;
+        const int nb = (p->B - b0) < p->chunk ? (p->B - b0) : p->chunk;
+        if (ci >= 2) CK(p, cudaStreamWaitEvent(s_in, p->ev_cmp[buf], 0));     // d_in[buf] consumed
+        CK(p, cudaMemcpyAsync(p->d_in[buf], static_cast<const unsigned char *>(h_samples) + (size_t)b0 * in_b,
+                              (size_t)nb * in_b, cudaMemcpyHostToDevice, s_in));
+        CK(p, cudaEventRecord(p->ev_in[buf], s_in));
+        CK(p, cudaStreamWaitEvent(s_cmp, p->ev_in[buf], 0));
+        if (ci >= 2) CK(p, cudaStreamWaitEvent(s_cmp, p->ev_out[buf], 0));    // d_out[buf] drained
+        int rc = enqueue_chunk(p, s_cmp, p->d_in[buf], p->d_delays_h, p->d_bandpass_h,
+                               static_cast<float2 *>(p->d_out[buf]), b0, nb, nullptr);
+        if (rc != COBALT_OK) return rc;
+        CK(p, cudaEventRecord(p->ev_cmp[buf], s_cmp));
+        CK(p, cudaStreamWaitEvent(s_out, p->ev_cmp[buf], 0));
+        CK(p, cudaMemcpyAsync(static_cast<unsigned char *>(h_visibilities) + (size_t)b0 * out_b, p->d_out[buf],
+                              (size_t)nb * out_b, cudaMemcpyDeviceToHost, s_out));
+        CK(p, cudaEventRecord(p->ev_out[buf], s_out));
+    }
+    p->hist_cur ^= 1;
+    CK(p, cudaStreamSynchronize(s_in));
+    CK(p, cudaStreamSynchronize(s_cmp));
+    CK(p, cudaStreamSynchronize(s_out));
+    return COBALT_OK;
+}
+
+int cobalt_set_subband_frequencies(cobalt_plan_t *p, const double *h_hz) {
+    if (!p || !h_hz) return fail(p, COBALT_ERR_BAD_ARG, "NULL argument");
+    for (int s = 0; s < p->B; ++s)
+        if (!(h_hz[s] == h_hz[s]) || std::fabs(h_hz[s]) > 1e12) return fail(p, COBALT_ERR_BAD_ARG, "frequency not finite");
+    CK(p, cudaDeviceSynchronize());
+    p->f_sb.assign(h_hz, h_hz + p->B);
+    CK(p, cudaMemcpy(p->d_f_sb, p->f_sb.data(), (size_t)p->B * sizeof(double), cudaMemcpyHostToDevice));
+    return COBALT_OK;
+}
+
+int cobalt_set_sample_rate(cobalt_plan_t *p, double hz) {
+    if (!p || !(hz > 0.0) || hz > 1e12) return fail(p, COBALT_ERR_BAD_ARG, "sample rate must be positive and finite");
+    p->f_s = hz;
+    return COBALT_OK;
+}
+
+int cobalt_set_mode(cobalt_plan_t *p, int mode) {
+    if (!p || (mode != COBALT_MODE_TENSOR_FP16 && mode != COBALT_MODE_EXACT_FP32)) return fail(p, COBALT_ERR_BAD_ARG, "unknown mode");
+    if (mode == p->mode) return COBALT_OK;
+    CK(p, cudaDeviceSynchronize());
+    p->mode = mode;
+    return alloc_scratch(p, 0);
+}
+
+int cobalt_set_chunk_subbands(cobalt_plan_t *p, int chunk) {
+    if (!p || chunk < 1) return fail(p, COBALT_ERR_BAD_ARG, "chunk must be >= 1");
+    CK(p, cudaDeviceSynchronize());
+    return alloc_scratch(p, chunk);
+}
+
+int cobalt_reset(cobalt_plan_t *p) {
+    if (!p) return fail(nullptr, COBALT_ERR_BAD_ARG, "plan is NULL");
+    CK(p, cudaDeviceSynchronize());
+    const size_t hist = (size_t)p->B * p->M * (kTaps - 1) * p->C * sample_bytes(p->bits);
+    CK(p, cudaMemset(p->d_hist[0], 0, hist));
+    CK(p, cudaMemset(p->d_hist[1], 0, hist));
+    CK(p, cudaDeviceSynchronize());
+    return COBALT_OK;
+}
+
+int cobalt_info(const cobalt_plan_t *p, cobalt_info_t *info) {
+    if (!p || !info) return fail(p, COBALT_ERR_BAD_ARG, "NULL argument");
+    info->stations = p->S;
+    info->subbands = p->B;
+    info->channels = p->C;
+    info->taps = p->T;
+    info->input_bits = p->bits;
+    info->mode = p->mode;
+    info->samples_per_integration = p->N;
+    info->n_spectra = p->n_t;
+    info->n_consumed = p->N_u;
+    info->n_baselines = p->n_bl;
+    info->input_bytes = (long long)((size_t)p->B * subband_input_bytes(p));
+    info->output_bytes = (long long)((size_t)p->B * subband_output_bytes(p));
+    info->scratch_bytes = (long long)p->scratch_bytes;
+    info->chunk_subbands = p->chunk;
+    info->sm_count = p->sm_count;
+    info->sample_rate_hz = p->f_s;
+    return COBALT_OK;
+}
+
+int cobalt_set_timing(cobalt_plan_t *p, int enabled) {
+    if (!p) return fail(nullptr, COBALT_ERR_BAD_ARG, "plan is NULL");
+    p->timing = enabled != 0;
+    p->n_chunks_timed = 0;
+    return COBALT_OK;
+}
+
+int cobalt_get_timing(cobalt_plan_t *p, double *f_ms, double *x_ms, int *launches) {
+    if (!p) return fail(nullptr, COBALT_ERR_BAD_ARG, "plan is NULL");
+    double f = 0.0, x = 0.0;
+    for (int i = 0; i < p->n_chunks_timed; ++i) {
+        float a = 0.f, b = 0.f;
+        CK(p, cudaEventSynchronize(p->events[i].x1));
+        CK(p, cudaEventElapsedTime(&a, p->events[i].f0, p->events[i].f1));
+        CK(p, cudaEventElapsedTime(&b, p->events[i].f1, p->events[i].x1));
+        f += a;
+        x += b;
+    }
+    if (f_ms) *f_ms = f;
+    if (x_ms) *x_ms = x;
+    if (launches) *launches = p->launches;
+    return COBALT_OK;
+}
+
+int cobalt_debug_fir_weights(const cobalt_plan_t *p, float *h_weights) {
+    if (!p || !h_weights) return fail(p, COBALT_ERR_BAD_ARG, "NULL argument");
+    std::memcpy(h_weights, p->h_weights.data(), p->h_weights.size() * sizeof(float));
+    return COBALT_OK;
+}
+
+int cobalt_debug_unpack(void *cuda_stream, int input_bits, const void *d_in, long long n, float *d_out) {
+    if ((input_bits != 16 && input_bits != 8) || n < 0 || (n > 0 && (!d_in || !d_out)))
+        return fail(nullptr, COBALT_ERR_BAD_ARG, "bad unpack arguments");
+    CK(nullptr, launch_unpack(static_cast<cudaStream_t>(cuda_stream), input_bits, d_in, n, d_out));
+    return COBALT_OK;
+}
+
+int cobalt_debug_channelised(cobalt_plan_t *p, void *cuda_stream, const void *d_samples, const double *d_delays,
+                             const float *d_bandpass, int sb, void *d_z) {
+    if (!p || !d_samples || !d_delays || !d_bandpass || !d_z) return fail(p, COBALT_ERR_BAD_ARG, "NULL argument");
+    if (sb < 0 || sb >= p->B) return fail(p, COBALT_ERR_BAD_ARG, "subband out of range");
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const unsigned char *sm = static_cast<const unsigned char *>(d_samples) + (size_t)sb * subband_input_bytes(p);
+    CK(p, launch_phase_table(p, st, d_delays, d_bandpass, sb, 1));
+    CK(p, launch_fstage(p, st, sm, sb, 1));
+    CK(p, launch_z_to_float(p, st, p->d_z, static_cast<float2 *>(d_z)));
+    return COBALT_OK;
+}
+
+int cobalt_debug_correlate(cobalt_plan_t *p, void *cuda_stream, const void *d_z, void *d_vis) {
+    if (!p || !d_z || !d_vis) return fail(p, COBALT_ERR_BAD_ARG, "NULL argument");
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    CK(p, launch_float_to_z(p, st, static_cast<const float2 *>(d_z), p->d_z));
+    if (p->mode == COBALT_MODE_TENSOR_FP16) CK(p, launch_xstage_tc(p, st, p->d_z, 1, static_cast<float2 *>(d_vis)));
+    else CK(p, launch_xstage_simt(p, st, p->d_z, 1, static_cast<float2 *>(d_vis)));
+    return COBALT_OK;
+}
+
+}  // extern "C"

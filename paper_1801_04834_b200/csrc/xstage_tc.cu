@@ -1,0 +1,358 @@
+// X-stage, TENSOR_FP16 mode: the Hermitian contraction V = Z Z^H of one (subband, channel) on the
+// 5th-generation tensor cores (steps a8-a9 of SURVEY.md sec 8(a); "computes the correlations
+// of all pairs of antenna fields and averages in time"; BASELINE.json north_star (c)).
+//
+// Z is [2S inputs][n_t spectra] complex, held as two fp16 planes (re, im), K-major, already in the
+// 128-byte-swizzled shared-memory image (cobalt_internal.h), so operands arrive with plain bulk
+// copies (cp.async.bulk -> UBLKCP) signalled on mbarriers -- no tensor map, no register staging.
+//
+//   Re V = Zr Zr^T + Zi Zi^T        Im V = Zi Zr^T - Zr Zi^T
+//
+// is four tcgen05.mma (kind::f16, fp32 accumulate in TMEM) per 16-spectrum k-step into two
+// accumulators; the minus sign is the instruction descriptor's negate-A bit, so no negated plane is
+// ever stored.  Only tiles on or above the station diagonal are computed: an XJob (built once per
+// plan by build_xjobs) names the rows to load and up to two accumulator groups
+//   rows [0,128) x cols [0,Mpad)  and  rows [128,Mpad) x cols [128,Mpad)        (2S <= 192)
+// or, for large arrays, one (128-row block) x (<= 256-column chunk) tile per job.
+//
+// Warp roles (192 threads, persistent CTAs, one per SM): warp 0 = bulk-copy producer, warp 1 = TMEM
+// allocator + single-thread MMA issuer, warps 2-5 = epilogue (tcgen05.ld -> triangular baseline
+// index -> coalesced 16-byte stores of (re, im) pairs).
+#include "cobalt_internal.h"
+
+namespace cobalt {
+
+namespace {
+
+constexpr int kThreads = 192;
+constexpr int kSlackBytes = 128 * 128;   // A operands may over-read up to 128 rows of one plane
+constexpr int kBarrierBytes = 1024;
+
+struct XArgs {
+    const unsigned char *z;
+    float2 *vis;
+    const XJob *jobs;
+    size_t z_subband_bytes;
+    long long n_bl;
+    int C, M, Mpad, n_kt, jobs_per_channel, total_jobs, stages, stage_bytes;
+};
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    uint32_t done;
+    do {
+        asm volatile(
+            "{\n\t"
+            ".reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t"
+            "}"
+            : "=r"(done)
+            : "r"(bar), "r"(parity)
+            : "memory");
+    } while (!done);
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t bytes, uint32_t bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+                 "l"(src), "r"(bytes), "r"(bar)
+                 : "memory");
+}
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_commit(uint32_t bar) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+// D[tmem] (+)= A[smem] * B[smem]^T, 128 x N x 16, fp16 in, fp32 accumulate.
+__device__ __forceinline__ void tc_mma(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t acc) {
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t"
+        "}" ::"r"(d_tmem),
+        "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(acc)
+        : "memory");
+}
+// K-major, 128-byte swizzle: 8-row groups 1024 bytes apart (SBO), descriptor version 1 (sm_100).
+__device__ __forceinline__ uint64_t make_smem_desc(uint32_t addr) {
+    return (uint64_t)((addr >> 4) & 0x3FFFu) | (1ull << 16) | (64ull << 32) | (1ull << 46) | (2ull << 61);
+}
+// kind::f16 instruction descriptor: D = f32, A = B = f16, both K-major, M = 128.
+__device__ __forceinline__ uint32_t make_idesc(int n, int neg_a) {
+    return (1u << 4) | ((uint32_t)neg_a << 13) | ((uint32_t)(n >> 3) << 17) | ((128u >> 4) << 24);
+}
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&v)[16]) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, "
+        "[%16];"
+        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]),
+          "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+        : "r"(taddr));
+}
+__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+
+__global__ void __launch_bounds__(kThreads, 1) xstage_tc_kernel(const XArgs a) {
+    extern __shared__ __align__(1024) unsigned char smem_raw[];
+    // carve: [barriers 1 KB][stages ...][slack]; stage base must be 1024-byte aligned for the swizzle
+    const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    const uint32_t bar_base = smem_base;                       // full[s] at +8 s, empty[s] at +8 (16 + s)
+    const uint32_t tmem_full = bar_base + 8 * 32, tmem_empty = bar_base + 8 * 33;
+    const uint32_t tmem_slot = bar_base + 8 * 34;              // 4 bytes: TMEM base address
+    const uint32_t stage_base = smem_base + kBarrierBytes;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int stages = a.stages;
+
+    // every job of one plan allocates the same number of columns (max over jobs)
+    int tmem_cols = 32;
+    for (int j = 0; j < a.jobs_per_channel; ++j) tmem_cols = max(tmem_cols, a.jobs[j].tmem_cols);
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < stages; ++s) {
+            mbar_init(bar_base + 8 * s, 1);
+            mbar_init(bar_base + 8 * (16 + s), 1);
+        }
+        mbar_init(tmem_full, 1);
+        mbar_init(tmem_empty, 4);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 1) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tmem_slot), "r"(tmem_cols)
+                     : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    uint32_t tmem_base;
+    asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
+
+    if (warp == 0) {
+        // ------------------------------------------------------------------ producer
+        if (lane == 0) {
+            int s = 0;
+            uint32_t ph = 0;
+            for (int jid = blockIdx.x; jid < a.total_jobs; jid += gridDim.x) {
+                const int jl = jid % a.jobs_per_channel;
+                const int prob = jid / a.jobs_per_channel;           // subband-of-chunk * C + channel
+                const XJob &job = a.jobs[jl];
+                const int bl = prob / a.C, c = prob - bl * a.C;
+                const unsigned char *zc = a.z + (size_t)bl * a.z_subband_bytes + (size_t)c * a.n_kt * 2 * a.Mpad * 128;
+                const int n0 = job.ld_nrows[0], n1 = job.ld_nrows[1];
+                const uint32_t plane_bytes = (uint32_t)(n0 + n1) * 128;
+                for (int kt = 0; kt < a.n_kt; ++kt) {
+                    mbar_wait(bar_base + 8 * (16 + s), ph ^ 1);
+                    const uint32_t full = bar_base + 8 * s;
+                    const uint32_t dst = stage_base + (uint32_t)s * a.stage_bytes;
+                    mbar_expect_tx(full, 2 * plane_bytes);
+                    const unsigned char *src = zc + (size_t)kt * 2 * a.Mpad * 128;
+#pragma unroll
+                    for (int plane = 0; plane < 2; ++plane) {
+                        const unsigned char *sp = src + (size_t)plane * a.Mpad * 128;
+                        bulk_g2s(dst + plane * plane_bytes, sp + (size_t)job.ld_row[0] * 128, (uint32_t)n0 * 128, full);
+                        if (n1 > 0)
+                            bulk_g2s(dst + plane * plane_bytes + n0 * 128, sp + (size_t)job.ld_row[1] * 128,
+                                     (uint32_t)n1 * 128, full);
+                    }
+                    if (++s == stages) {
+                        s = 0;
+                        ph ^= 1;
+                    }
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ------------------------------------------------------------------ MMA issuer
+        if (lane == 0) {
+            int s = 0;
+            uint32_t ph = 0, it = 0;
+            for (int jid = blockIdx.x; jid < a.total_jobs; jid += gridDim.x, ++it) {
+                const XJob &job = a.jobs[jid % a.jobs_per_channel];
+                const uint32_t plane_bytes = (uint32_t)(job.ld_nrows[0] + job.ld_nrows[1]) * 128;
+                mbar_wait(tmem_empty, (it & 1) ^ 1);       // epilogue has drained the accumulators
+                tc_fence_after();
+                for (int kt = 0; kt < a.n_kt; ++kt) {
+                    mbar_wait(bar_base + 8 * s, ph);
+                    tc_fence_after();
+                    const uint32_t st = stage_base + (uint32_t)s * a.stage_bytes;
+                    for (int g = 0; g < job.n_groups; ++g) {
+                        const XMmaGroup &grp = job.g[g];
+                        const uint64_t ar = make_smem_desc(st + grp.a_row * 128);
+                        const uint64_t ai = make_smem_desc(st + plane_bytes + grp.a_row * 128);
+                        const uint64_t br = make_smem_desc(st + grp.b_row * 128);
+                        const uint64_t bi = make_smem_desc(st + plane_bytes + grp.b_row * 128);
+                        const uint32_t d_re = tmem_base + grp.tmem_col, d_im = d_re + grp.n;
+                        const uint32_t id_pos = make_idesc(grp.n, 0), id_neg = make_idesc(grp.n, 1);
+#pragma unroll
+                        for (int ks = 0; ks < kKTile / 16; ++ks) {
+                            const uint32_t acc = (kt | ks) ? 1u : 0u;
+                            const uint64_t ko = (uint64_t)(ks * 2);         // 32 bytes per k-step, >> 4
+                            tc_mma(d_re, ar + ko, br + ko, id_pos, acc);    // Re  = Zr Zr^T
+                            tc_mma(d_re, ai + ko, bi + ko, id_pos, 1u);     // Re += Zi Zi^T
+                            tc_mma(d_im, ai + ko, br + ko, id_pos, acc);    // Im  = Zi Zr^T
+                            tc_mma(d_im, ar + ko, bi + ko, id_neg, 1u);     // Im -= Zr Zi^T
+                        }
+                    }
+                    tc_commit(bar_base + 8 * (16 + s));    // stage free once these MMAs have read it
+                    if (++s == stages) {
+                        s = 0;
+                        ph ^= 1;
+                    }
+                }
+                tc_commit(tmem_full);                      // accumulators complete
+            }
+        }
+    } else {
+        // ------------------------------------------------------------------ epilogue
+        const int wq = warp & 3;                           // TMEM lane quarter this warp may access
+        uint32_t it = 0;
+        for (int jid = blockIdx.x; jid < a.total_jobs; jid += gridDim.x, ++it) {
+            const int jl = jid % a.jobs_per_channel;
+            const int prob = jid / a.jobs_per_channel;
+            const XJob &job = a.jobs[jl];
+            float4 *vc = reinterpret_cast<float4 *>(a.vis + (size_t)prob * a.n_bl * 4);
+            mbar_wait(tmem_full, it & 1);
+            tc_fence_after();
+            for (int g = 0; g < job.n_groups; ++g) {
+                const XMmaGroup &grp = job.g[g];
+                const int row0 = grp.out_row + wq * 32;    // first input index of this warp's lanes
+                const int arow = row0 + lane;
+                const int i = arow >> 1, p = arow & 1;
+                if (row0 >= a.M) continue;
+                for (int c0 = 0; c0 < grp.n; c0 += 16) {
+                    const int col0 = grp.out_col + c0;
+                    if (col0 >= a.M) break;
+                    if (((col0 + 15) >> 1) < (row0 >> 1)) continue;     // whole chunk below the diagonal
+                    uint32_t re[16], im[16];
+                    const uint32_t t = tmem_base + ((uint32_t)(wq * 32) << 16) + grp.tmem_col + c0;
+                    tmem_ld16(t, re);
+                    tmem_ld16(t + grp.n, im);
+                    tmem_ld_wait();
+#pragma unroll
+                    for (int e = 0; e < 16; e += 2) {
+                        const int b = col0 + e, k = b >> 1;
+                        if (arow < a.M && b < a.M && i <= k)
+                            vc[((size_t)k * (k + 1) / 2 + i) * 2 + p] =
+                                make_float4(__uint_as_float(re[e]), __uint_as_float(im[e]), __uint_as_float(re[e + 1]),
+                                            __uint_as_float(im[e + 1]));
+                    }
+                }
+            }
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(tmem_empty);
+        }
+    }
+
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 1) {
+        tc_fence_after();
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(tmem_cols) : "memory");
+    }
+}
+
+int round_up(int v, int m) { return (v + m - 1) / m * m; }
+int pow2_cols(int c) {
+    int p = 32;
+    while (p < c) p <<= 1;
+    return p;
+}
+
+}  // namespace
+
+// Tiling of the upper triangle of one channel's (2S x 2S) product into XJobs (see file header).
+void build_xjobs(cobalt_plan_s *p) {
+    p->jobs.clear();
+    const int Mpad = p->Mpad;
+    if (Mpad <= 192) {
+        XJob j{};
+        j.ld_row[0] = 0;
+        j.ld_nrows[0] = Mpad;
+        j.ld_row[1] = 0;
+        j.ld_nrows[1] = 0;
+        j.n_groups = 1;
+        j.g[0] = XMmaGroup{0, 0, Mpad, 0, 0, 0};
+        int cols = 2 * Mpad;
+        if (Mpad > 128) {
+            j.n_groups = 2;
+            j.g[1] = XMmaGroup{128, 128, Mpad - 128, 2 * Mpad, 128, 128};
+            cols += 2 * (Mpad - 128);
+        }
+        j.tmem_cols = pow2_cols(cols);
+        p->jobs.push_back(j);
+    } else {
+        const int nrb = (Mpad + 127) / 128;
+        for (int I = 0; I < nrb; ++I) {
+            const int r0 = 128 * I;
+            const int na = (Mpad - r0) < 128 ? (Mpad - r0) : 128;
+            const int width = Mpad - r0;
+            const int nchunks = (width + 255) / 256;
+            const int cw = round_up((width + nchunks - 1) / nchunks, 16);
+            for (int c0 = r0; c0 < Mpad; c0 += cw) {
+                const int n = (Mpad - c0) < cw ? (Mpad - c0) : cw;
+                XJob j{};
+                j.n_groups = 1;
+                if (c0 == r0) {   // diagonal chunk: B rows start at the A rows, load the union once
+                    j.ld_row[0] = r0;
+                    j.ld_nrows[0] = na > n ? na : n;
+                    j.ld_row[1] = 0;
+                    j.ld_nrows[1] = 0;
+                    j.g[0] = XMmaGroup{0, 0, n, 0, r0, c0};
+                } else {
+                    j.ld_row[0] = r0;
+                    j.ld_nrows[0] = na;
+                    j.ld_row[1] = c0;
+                    j.ld_nrows[1] = n;
+                    j.g[0] = XMmaGroup{0, na, n, 0, r0, c0};
+                }
+                j.tmem_cols = pow2_cols(2 * n);
+                p->jobs.push_back(j);
+            }
+        }
+    }
+    int max_rows = 0;
+    for (const XJob &j : p->jobs) max_rows = (j.ld_nrows[0] + j.ld_nrows[1]) > max_rows ? (j.ld_nrows[0] + j.ld_nrows[1]) : max_rows;
+    const size_t stage_bytes = (size_t)max_rows * 128 * 2;
+    const size_t budget = 227 * 1024 - 1024 /*alignment*/ - kBarrierBytes - kSlackBytes;
+    int stages = (int)(budget / stage_bytes);
+    if (stages > 8) stages = 8;
+    p->x_stages = stages;
+    p->x_smem_bytes = 1024 + kBarrierBytes + (size_t)stages * stage_bytes + kSlackBytes;
+}
+
+cudaError_t launch_xstage_tc(const cobalt_plan_s *p, cudaStream_t st, const void *d_z, int nb, float2 *d_vis) {
+    if (p->x_stages < 2) return cudaErrorInvalidConfiguration;
+    XArgs a;
+    a.z = static_cast<const unsigned char *>(d_z);
+    a.vis = d_vis;
+    a.jobs = p->d_jobs;
+    a.z_subband_bytes = p->z_subband_bytes;
+    a.n_bl = p->n_bl;
+    a.C = p->C;
+    a.M = p->M;
+    a.Mpad = p->Mpad;
+    a.n_kt = p->n_kt;
+    a.jobs_per_channel = (int)p->jobs.size();
+    a.total_jobs = nb * p->C * a.jobs_per_channel;
+    a.stages = p->x_stages;
+    int max_rows = 0;
+    for (const XJob &j : p->jobs) max_rows = (j.ld_nrows[0] + j.ld_nrows[1]) > max_rows ? (j.ld_nrows[0] + j.ld_nrows[1]) : max_rows;
+    a.stage_bytes = max_rows * 128 * 2;
+    cudaError_t e = cudaFuncSetAttribute(xstage_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->x_smem_bytes);
+    if (e != cudaSuccess) return e;
+    const int grid = a.total_jobs < p->sm_count ? a.total_jobs : p->sm_count;
+    xstage_tc_kernel<<<grid, kThreads, p->x_smem_bytes, st>>>(a);
+    return cudaGetLastError();
+}
+
+}  // namespace cobalt
