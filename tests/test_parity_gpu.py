@@ -1,0 +1,274 @@
+"""GPU parity: the CUDA path (through the C ABI, via the thin binding) against the float64 oracle,
+element by element on the same seeded integer inputs (SURVEY.md sec 8(c) pins P1, P10, P14, P15 and
+reading A17 for the error metrics).  Runs on the B200 box: `pytest -m gpu`.
+
+Tolerances (BASELINE.json north_star): fp32 mode max |dV| / sqrt(V_ii V_kk) <= 1e-4; tensor-core
+(fp16 operand) mode ||dV||_F / ||V||_F <= 2e-3 per (subband, channel); integer unpack and the
+channel / baseline / polarisation indexing bit-exact.
+"""
+import numpy as np
+import pytest
+
+from parity_util import TOL_FP32, TOL_TENSOR, err_fp32, err_frobenius
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def dev():
+    if not torch.cuda.is_available():
+        pytest.fail("gpu tests need a CUDA device (run through gpurun)")
+    return torch.device("cuda:0")
+
+
+def _synth():
+    from paper_1801_04834_b200 import synth
+
+    return synth
+
+
+def _run_gpu(cobalt, cfg, data, mode, dev, chunk=None, calls=1):
+    """Whole path through cobalt_process; returns the list of visibilities of each call."""
+    with cobalt.Correlator(cfg.S, cfg.B, cfg.C, cfg.N, cfg.bits, mode=mode) as cor:
+        if chunk is not None:
+            cor.set_chunk_subbands(chunk)
+        outs = []
+        for _ in range(calls):
+            vis = cor.process(data["samples"].to(dev), data["delays"].to(dev), data["bandpass"].to(dev))
+            torch.cuda.synchronize()
+            outs.append(vis.cpu().numpy())
+    return outs
+
+
+def _run_oracle(oracle, cfg, data, calls=1, subbands=None):
+    sb = range(cfg.B) if subbands is None else subbands
+    samples = data["samples"].cpu().numpy()
+    hist = {s: oracle.new_history(cfg.S, cfg.C) for s in sb}
+    outs = []
+    for _ in range(calls):
+        v = [oracle.process_subband(samples[s], cfg.C, data["delays"].cpu().numpy(), data["bandpass"].cpu().numpy().astype(np.float64),
+                                    oracle.default_subband_frequency(s), hist[s]) for s in sb]
+        outs.append(np.stack(v))
+    return outs
+
+
+def _assert_parity(vg, vo, mode_tensor, what):
+    assert np.all(np.isfinite(vg)), f"{what}: non-finite GPU output"
+    if mode_tensor:
+        e = err_frobenius(vg, vo)
+        assert e <= TOL_TENSOR, f"{what}: Frobenius error {e:.3e} > {TOL_TENSOR}"
+    else:
+        e = err_fp32(vg, vo)
+        assert e <= TOL_FP32, f"{what}: autocorrelation-normalised error {e:.3e} > {TOL_FP32}"
+    return e
+
+
+# ------------------------------------------------------------------ P1: unpack bit-exact
+@pytest.mark.parametrize("bits", [16, 8])
+def test_p1_unpack_every_value_bit_exact(cobalt, oracle, dev, bits):
+    if bits == 16:
+        x = np.arange(-32768, 32768, dtype=np.int64).astype(np.int16)
+    else:
+        x = np.arange(-128, 128, dtype=np.int64).astype(np.int8)
+    x = np.concatenate([x, x[::-1], x[: 37]])                      # ragged length
+    got = cobalt.unpack(torch.from_numpy(x).to(dev)).cpu().numpy()
+    want = oracle.unpack(x)
+    assert got.dtype == np.float32
+    assert np.array_equal(got.astype(np.float64), want)
+
+
+def test_unpack_empty(cobalt, dev):
+    out = cobalt.unpack(torch.empty(0, dtype=torch.int16, device=dev))
+    assert out.numel() == 0
+
+
+# ------------------------------------------------------------------ FIR weights (A1, A2)
+@pytest.mark.parametrize("C", [16, 64, 256])
+def test_fir_weights_are_the_rounded_prototype(cobalt, oracle, dev, C):
+    with cobalt.Correlator(2, 1, C, 4 * C) as cor:
+        w = cor.fir_weights()                                      # [k][ph], k = 0 newest block
+    g = oracle.fir_prototype(C)
+    want = g.reshape(16, C)[::-1].astype(np.float32)               # w[k][ph] = g[(15-k) C + ph]
+    assert np.array_equal(w, want)
+
+
+# ------------------------------------------------------------------ F-stage alone (steps a1-a7)
+@pytest.mark.parametrize("C,bits,S,n_t", [(16, 16, 3, 150), (64, 16, 2, 203), (256, 16, 2, 70), (64, 8, 3, 130), (256, 8, 1, 65), (16, 8, 2, 64)])
+@pytest.mark.parametrize("mode_tensor", [False, True])
+def test_channelised_matches_oracle(cobalt, oracle, dev, C, bits, S, n_t, mode_tensor):
+    """z (after rotation, bandpass, channel reorder) for one subband of a 2-subband input, ragged tail
+    (N not a multiple of C, n_t not a multiple of the 64-spectrum tile)."""
+    rng = np.random.default_rng(1000 + C + bits + S)
+    N = n_t * C + 7
+    lim = 3000 if bits == 16 else 100
+    samples = rng.integers(-lim, lim + 1, size=(2, S, 2, N, 2)).astype(np.int16 if bits == 16 else np.int8)
+    delays = rng.uniform(-50e-6, 50e-6, S)
+    bandpass = (1.0 + 0.1 * rng.uniform(-1, 1, C)).astype(np.float32)
+    mode = cobalt.COBALT_MODE_TENSOR_FP16 if mode_tensor else cobalt.COBALT_MODE_EXACT_FP32
+    with cobalt.Correlator(S, 2, C, N, bits, mode=mode) as cor:
+        z = cor.channelised(torch.from_numpy(samples).to(dev), torch.from_numpy(delays).to(dev),
+                            torch.from_numpy(bandpass).to(dev), sb=1)
+        torch.cuda.synchronize()
+        z = z.cpu().numpy()                                        # [C][2S][n_t]
+    _, zo = oracle.process_subband(samples[1], C, delays, bandpass.astype(np.float64),
+                                   oracle.default_subband_frequency(1), return_z=True)
+    zo = zo.reshape(2 * S, n_t, C).transpose(2, 0, 1)              # [S][2][n_t][C] -> [C][2S][n_t]
+    scale = np.sqrt(np.mean(np.abs(zo) ** 2))
+    err = np.max(np.abs(z - zo)) / scale
+    # fp32 arithmetic: 16 taps + log2(C) butterfly levels, ~1e-6; fp16 operands: 2^-11 relative rounding
+    assert err <= (2e-3 if mode_tensor else 2e-5), err
+
+
+# ------------------------------------------------------------------ P14: X-stage indexing, bit-exact
+@pytest.mark.parametrize("S,n_t", [(1, 5), (3, 64), (8, 100), (48, 130), (77, 70), (100, 64), (130, 65), (288, 40)])
+@pytest.mark.parametrize("mode_tensor", [False, True])
+def test_p14_correlate_small_integers_bit_exact(cobalt, oracle, dev, S, n_t, mode_tensor):
+    """Small integers are exact in fp16 and their sums exact in fp32, so the X-stage must equal integer
+    arithmetic bit for bit: pins the conjugation side, baseline order k(k+1)/2 + i and pol order."""
+    C = 16
+    rng = np.random.default_rng(77 + S)
+    zr = rng.integers(-8, 9, size=(C, 2 * S, n_t))
+    zi = rng.integers(-8, 9, size=(C, 2 * S, n_t))
+    z = (zr + 1j * zi).astype(np.complex64)
+    mode = cobalt.COBALT_MODE_TENSOR_FP16 if mode_tensor else cobalt.COBALT_MODE_EXACT_FP32
+    with cobalt.Correlator(S, 1, C, n_t * C, 16, mode=mode) as cor:
+        vis = cor.correlate(torch.from_numpy(z).to(dev))
+        torch.cuda.synchronize()
+        vis = vis.cpu().numpy()                                    # [C][n_bl][2][2]
+    zo = z.astype(np.complex128).reshape(C, S, 2, n_t).transpose(1, 2, 3, 0)   # -> [S][2][n_t][C]
+    want = oracle.correlate(np.ascontiguousarray(zo))
+    assert np.array_equal(vis.astype(np.complex128), want)
+
+
+# ------------------------------------------------------------------ whole path, configs 1 and 2 in full
+@pytest.mark.parametrize("mode_tensor", [False, True])
+def test_config1_tiny_full_parity(cobalt, oracle, dev, mode_tensor):
+    synth = _synth()
+    cfg = synth.CONFIGS[1]
+    data = synth.generate(cfg, device="cpu")
+    mode = cobalt.COBALT_MODE_TENSOR_FP16 if mode_tensor else cobalt.COBALT_MODE_EXACT_FP32
+    vg = _run_gpu(cobalt, cfg, data, mode, dev, calls=2)
+    vo = _run_oracle(oracle, cfg, data, calls=2)
+    for call in range(2):                                          # second call: carried history (P10)
+        _assert_parity(vg[call], vo[call], mode_tensor, f"config 1 call {call}")
+    # the tone of reading A16 sits in channel 5
+    p = np.abs(vo[0][0, :, 0, 0, 0])
+    assert int(np.argmax(p)) == 5
+
+
+@pytest.mark.parametrize("mode_tensor", [False, True])
+def test_config2_core_like_full_parity(cobalt, oracle, dev, mode_tensor):
+    synth = _synth()
+    cfg = synth.CONFIGS[2]
+    data = synth.generate(cfg, device=dev)
+    mode = cobalt.COBALT_MODE_TENSOR_FP16 if mode_tensor else cobalt.COBALT_MODE_EXACT_FP32
+    vg = _run_gpu(cobalt, cfg, data, mode, dev)
+    vo = _run_oracle(oracle, cfg, data)
+    _assert_parity(vg[0], vo[0], mode_tensor, "config 2")
+    # P13 / A15: 10 % common power => cross-correlation coefficient ~0.1 after delay compensation
+    v = vo[0][0]
+    auto0 = v[:, 0, 0, 0].real
+    auto1 = v[:, 2, 0, 0].real
+    rho = np.abs(v[8:-8, 1, 0, 0]) / np.sqrt(auto0[8:-8] * auto1[8:-8])
+    assert 0.06 < float(np.median(rho)) < 0.12
+
+
+# ------------------------------------------------------------------ chunking, history, ragged shapes
+@pytest.mark.parametrize("mode_tensor", [False, True])
+def test_subband_chunking_and_history_carry(cobalt, oracle, dev, mode_tensor):
+    """5 subbands processed 2 per launch group (ragged last chunk), two consecutive calls."""
+    synth = _synth()
+    cfg = synth.scaled(synth.CONFIGS[3], S=5, B=5, C=64, N=64 * 150 + 13)
+    data = synth.generate(cfg, device="cpu")
+    mode = cobalt.COBALT_MODE_TENSOR_FP16 if mode_tensor else cobalt.COBALT_MODE_EXACT_FP32
+    vg = _run_gpu(cobalt, cfg, data, mode, dev, chunk=2, calls=2)
+    vo = _run_oracle(oracle, cfg, data, calls=2)
+    for call in range(2):
+        _assert_parity(vg[call], vo[call], mode_tensor, f"chunked call {call}")
+
+
+def test_short_block_history_older_than_block(cobalt, oracle, dev):
+    """N = C (one spectrum per call): the new history is mostly the old one shifted (step a10)."""
+    synth = _synth()
+    cfg = synth.scaled(synth.CONFIGS[1], N=16)
+    data = synth.generate(synth.scaled(synth.CONFIGS[1], N=16 * 6), device="cpu")
+    full = data["samples"]
+    hist = oracle.new_history(cfg.S, cfg.C)
+    with cobalt.Correlator(cfg.S, 1, cfg.C, 16, 16, mode=cobalt.COBALT_MODE_EXACT_FP32) as cor:
+        for blk in range(6):
+            s = full[:, :, :, 16 * blk:16 * (blk + 1), :].contiguous()
+            vg = cor.process(s.to(dev), data["delays"].to(dev), data["bandpass"].to(dev)).cpu().numpy()
+            vo = oracle.process_subband(s[0].numpy(), cfg.C, data["delays"].numpy(), data["bandpass"].numpy().astype(np.float64),
+                                        oracle.default_subband_frequency(0), hist)
+            _assert_parity(vg[0], vo, False, f"block {blk}")
+
+
+@pytest.mark.parametrize("mode_tensor", [False, True])
+def test_reset_zeroes_history(cobalt, dev, mode_tensor):
+    synth = _synth()
+    cfg = synth.scaled(synth.CONFIGS[1], N=16 * 70)
+    data = synth.generate(cfg, device="cpu")
+    mode = cobalt.COBALT_MODE_TENSOR_FP16 if mode_tensor else cobalt.COBALT_MODE_EXACT_FP32
+    with cobalt.Correlator(cfg.S, 1, cfg.C, cfg.N, 16, mode=mode) as cor:
+        args = (data["samples"].to(dev), data["delays"].to(dev), data["bandpass"].to(dev))
+        a = cor.process(*args).cpu().numpy()
+        b = cor.process(*args).cpu().numpy()
+        cor.reset()
+        c = cor.process(*args).cpu().numpy()
+    assert np.array_equal(a, c)
+    assert not np.array_equal(a, b)
+
+
+# ------------------------------------------------------------------ extreme integers (A12)
+@pytest.mark.parametrize("bits", [16, 8])
+def test_extreme_sample_values(cobalt, oracle, dev, bits):
+    """Full-scale input incl. -32768 / -128: no overflow of the fp16 intermediate, parity holds."""
+    synth = _synth()
+    C, S, n_t = 64, 2, 80
+    rng = np.random.default_rng(5)
+    lo, hi = (-32768, 32767) if bits == 16 else (-128, 127)
+    samples = rng.choice(np.array([lo, hi, 0, -1, 1]), size=(1, S, 2, n_t * C, 2)).astype(np.int16 if bits == 16 else np.int8)
+    data = {"samples": torch.from_numpy(samples), "delays": torch.zeros(S, dtype=torch.float64),
+            "bandpass": torch.ones(C, dtype=torch.float32)}
+    cfg = synth.scaled(synth.CONFIGS[1], S=S, C=C, N=n_t * C, bits=bits)
+    for mode_tensor in (False, True):
+        mode = cobalt.COBALT_MODE_TENSOR_FP16 if mode_tensor else cobalt.COBALT_MODE_EXACT_FP32
+        vg = _run_gpu(cobalt, cfg, data, mode, dev)
+        vo = _run_oracle(oracle, cfg, data)
+        _assert_parity(vg[0], vo[0], mode_tensor, f"extreme values, tensor={mode_tensor}")
+
+
+# ------------------------------------------------------------------ P15: fp64 phase
+def test_p15_large_delay_phase_needs_fp64(cobalt, oracle, dev):
+    """tau = 50 us at ~100 MHz is ~5000 cycles: the rotation must agree with float64 to ~1e-6 rad
+    (fp32 phase arithmetic would be off by ~3e-3).  Checked through z of a DC input."""
+    C, S, n_t = 64, 2, 80
+    samples = np.zeros((1, S, 2, n_t * C, 2), dtype=np.int16)
+    samples[..., 0] = 1000                                          # DC -> centre channel C/2
+    delays = np.array([50e-6, -37.123456e-6])
+    bandpass = np.ones(C, dtype=np.float32)
+    with cobalt.Correlator(S, 1, C, n_t * C, 16, mode=cobalt.COBALT_MODE_EXACT_FP32) as cor:
+        z = cor.channelised(torch.from_numpy(samples).to(dev), torch.from_numpy(delays).to(dev),
+                            torch.from_numpy(bandpass).to(dev)).cpu().numpy()
+    f = oracle.default_subband_frequency(0)                         # channel C/2 is the subband centre
+    for a in range(S):
+        want = -2 * np.pi * ((f * delays[a]) % 1.0)
+        got = np.angle(z[C // 2, 2 * a, 40])
+        d = np.angle(np.exp(1j * (got - want)))
+        assert abs(d) < 2e-6, (a, d)
+
+
+# ------------------------------------------------------------------ host-buffer entry (e2e path)
+def test_process_host_matches_device_path(cobalt, dev):
+    synth = _synth()
+    cfg = synth.scaled(synth.CONFIGS[3], S=6, B=5, C=64, N=64 * 100)
+    data = synth.generate(cfg, device="cpu")
+    with cobalt.Correlator(cfg.S, cfg.B, cfg.C, cfg.N, cfg.bits) as cor:
+        cor.set_chunk_subbands(2)
+        a = cor.process(data["samples"].to(dev), data["delays"].to(dev), data["bandpass"].to(dev)).cpu().numpy()
+        cor.reset()
+        out = torch.empty(cor.vis_shape(), dtype=torch.complex64).pin_memory()
+        cor.process_host(data["samples"].pin_memory(), data["delays"], data["bandpass"], out)
+    assert np.array_equal(a, out.numpy())
