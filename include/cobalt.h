@@ -50,7 +50,9 @@ typedef enum {
 
 typedef enum {
     /* X-stage on tcgen05 tensor cores, fp16 operands, fp32 accumulation in TMEM.
-     * Tolerance vs the float64 oracle: ||dV||_F / ||V||_F <= 2e-3 per (subband, channel). */
+     * Tolerance vs the float64 oracle: ||dV||_F / ||V||_F <= 2e-3 per (subband, channel).
+     * The fp16 operands carry a power-of-two scale chosen per call from max|bandpass| so that
+     * full-scale input cannot overflow (undone exactly in the X-stage epilogue). */
     COBALT_MODE_TENSOR_FP16 = 0,
     /* Everything in fp32 (SIMT FMA correlator).  Tolerance: max |dV| / sqrt(V_ii V_kk) <= 1e-4. */
     COBALT_MODE_EXACT_FP32 = 1
@@ -145,6 +147,10 @@ const char *cobalt_last_error(const cobalt_plan_t *plan);
  * the number of kernels the call launched.  Any output pointer may be NULL. */
 int cobalt_set_timing(cobalt_plan_t *plan, int enabled);
 int cobalt_get_timing(cobalt_plan_t *plan, double *f_stage_ms, double *x_stage_ms, int *kernel_launches);
+/* The same, per kernel: ms4[0..3] = summed device time over the call's chunks of the phase-table kernel,
+ * the fused F-stage kernel (unpack+FIR+FFT+rotate+bandpass+transpose), the history-carry kernel and
+ * the X-stage kernel; the roofline figures of bench.py divide by ms4[1] and ms4[3]. */
+int cobalt_get_kernel_timing(cobalt_plan_t *plan, double *ms4, int *kernel_launches);
 
 /* --------------------------------------------------------------------------- debug taps */
 /* (used by the parity tests to pin individual steps; not needed in production)           */

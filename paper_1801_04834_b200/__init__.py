@@ -31,7 +31,7 @@ ABI_SYMBOLS = (
     "cobalt_plan", "cobalt_process", "cobalt_process_host", "cobalt_destroy",
     "cobalt_set_subband_frequencies", "cobalt_set_sample_rate", "cobalt_set_mode",
     "cobalt_set_chunk_subbands", "cobalt_reset", "cobalt_info", "cobalt_strerror", "cobalt_last_error",
-    "cobalt_set_timing", "cobalt_get_timing",
+    "cobalt_set_timing", "cobalt_get_timing", "cobalt_get_kernel_timing",
     "cobalt_debug_fir_weights", "cobalt_debug_unpack", "cobalt_debug_channelised", "cobalt_debug_correlate",
 )
 
@@ -85,6 +85,7 @@ def load(path: str | None = None):
     lib.cobalt_set_timing.argtypes = [_vp, ctypes.c_int]
     lib.cobalt_get_timing.argtypes = [_vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double),
                                       ctypes.POINTER(ctypes.c_int)]
+    lib.cobalt_get_kernel_timing.argtypes = [_vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_int)]
     lib.cobalt_debug_fir_weights.argtypes = [_vp, _vp]
     lib.cobalt_debug_unpack.argtypes = [_vp, ctypes.c_int, _vp, ctypes.c_longlong, _vp]
     lib.cobalt_debug_channelised.argtypes = [_vp, _vp, _vp, _vp, _vp, ctypes.c_int, _vp]
@@ -218,6 +219,12 @@ class Correlator:
         f, x, n = ctypes.c_double(), ctypes.c_double(), ctypes.c_int()
         _check(load().cobalt_get_timing(self._h, ctypes.byref(f), ctypes.byref(x), ctypes.byref(n)), self._h)
         return f.value, x.value, n.value
+
+    def get_kernel_timing(self):
+        """(phase-table ms, F-stage ms, history ms, X-stage ms, kernel launches) of the last process() call."""
+        ms, n = (ctypes.c_double * 4)(), ctypes.c_int()
+        _check(load().cobalt_get_kernel_timing(self._h, ms, ctypes.byref(n)), self._h)
+        return ms[0], ms[1], ms[2], ms[3], n.value
 
     # -- the hot path
     def vis_shape(self):

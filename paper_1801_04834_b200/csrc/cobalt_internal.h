@@ -48,8 +48,9 @@ struct XJob {
     XMmaGroup g[kMaxMmaGroups];
 };
 
+// Events bracketing the four kernels of one chunk: e[0] | phase table | e[1] | F-stage | e[2] | history | e[3] | X-stage | e[4]
 struct StageEvents {
-    cudaEvent_t f0 = nullptr, f1 = nullptr, x1 = nullptr;
+    cudaEvent_t e[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
 };
 
 }  // namespace cobalt
@@ -67,7 +68,9 @@ struct cobalt_plan_s {
     std::vector<float> h_weights;
     void *d_hist[2] = {nullptr, nullptr};   // raw integer samples [B][S][2][15 C][2]; ping-pong
     int hist_cur = 0;
-    float2 *d_phase = nullptr;         // [chunk][S][C]  b[j] exp(-2 pi i frac(f tau))
+    float2 *d_phase = nullptr;         // [chunk][S][C]  s b[j] exp(-2 pi i frac(f tau))
+    float *d_scale = nullptr;          // {s, 1/s, 1/s^2}: power-of-two scale of the fp16 intermediate (1 in EXACT mode)
+    float amp_max = 0.f;               // worst-case |F| for full-scale input: sum|g| * sqrt(2) * 2^(bits-1)
     void *d_z = nullptr;               // intermediate of one chunk (layout per mode)
     size_t z_subband_bytes = 0;
     std::vector<cobalt::XJob> jobs;    // X-stage jobs of one (subband, channel)
@@ -102,6 +105,7 @@ cudaError_t launch_fstage(const cobalt_plan_s *p, cudaStream_t st, const void *s
 cudaError_t launch_history_update(const cobalt_plan_s *p, cudaStream_t st, const void *samples_b0, int b0, int nb);
 cudaError_t launch_unpack(cudaStream_t st, int bits, const void *d_in, long long n, float *d_out);
 // layout.cu ---------------------------------------------------------------------------------
+cudaError_t launch_set_unit_scale(const cobalt_plan_s *p, cudaStream_t st);
 cudaError_t launch_z_to_float(const cobalt_plan_s *p, cudaStream_t st, const void *d_zsub, float2 *d_out);
 cudaError_t launch_float_to_z(const cobalt_plan_s *p, cudaStream_t st, const float2 *d_in, void *d_zsub);
 // xstage_simt.cu ----------------------------------------------------------------------------

@@ -269,10 +269,42 @@ __global__ void __launch_bounds__(FShape<C>::NT) fstage_kernel(FArgs a) {
 }
 
 // "we compute the channel-dependent phase angles in double precision".  One entry per
-// (subband of the chunk, station, channel): b[j] exp(-2 pi i frac(f[s][j] tau_a)), f per reading A6.
+// (subband of the chunk, station, channel): s b[j] exp(-2 pi i frac(f[s][j] tau_a)), f per reading A6.
+//
+// s is the power-of-two scale of the fp16 intermediate (TENSOR mode; 1 otherwise): with
+// e = ceil(log2(max_j |b_j| * amp_max / 32768)) and s = 2^-e, full-scale input cannot overflow fp16
+// (|z s| <= 32768) and tiny bandpass weights cannot push z into the fp16 subnormals.  The X-stage
+// epilogue multiplies the visibilities by 1/s^2; both factors are exact.  Every block derives the
+// same s from the same C weights; block 0 publishes {s, 1/s, 1/s^2} for the X-stage.
 __global__ void phase_table_kernel(const double *__restrict__ delays, const float *__restrict__ bandpass,
                                    const double *__restrict__ f_sb, int b0, int nb, int S, int C, double f_s,
+                                   float amp_max, int tensor, float *__restrict__ scale_out,
                                    float2 *__restrict__ out) {
+    __shared__ float s_max[32];
+    __shared__ float s_scale;
+    float bm = 0.f;
+    for (int j = threadIdx.x; j < C; j += blockDim.x) bm = fmaxf(bm, fabsf(bandpass[j]));
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) bm = fmaxf(bm, __shfl_xor_sync(0xffffffffu, bm, o));
+    if ((threadIdx.x & 31) == 0) s_max[threadIdx.x >> 5] = bm;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        float m = 0.f;
+        for (int w = 0; w < (int)((blockDim.x + 31) >> 5); ++w) m = fmaxf(m, s_max[w]);
+        int e = 0;
+        if (tensor && m > 0.f && m < 3.0e38f) {
+            e = (int)ceilf(log2f(m * amp_max / 32768.f));
+            e = max(-40, min(40, e));
+        }
+        s_scale = scalbnf(1.f, -e);
+        if (blockIdx.x == 0) {
+            scale_out[0] = scalbnf(1.f, -e);
+            scale_out[1] = scalbnf(1.f, e);
+            scale_out[2] = scalbnf(1.f, 2 * e);
+        }
+    }
+    __syncthreads();
+    const double sc = (double)s_scale;
     const long long total = (long long)nb * S * C;
     for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < total;
          idx += (long long)gridDim.x * blockDim.x) {
@@ -284,9 +316,13 @@ __global__ void phase_table_kernel(const double *__restrict__ delays, const floa
         const double frac = cyc - floor(cyc);
         double sn, cs;
         sincospi(-2.0 * frac, &sn, &cs);
-        const double b = (double)bandpass[j];
+        const double b = (double)bandpass[j] * sc;
         out[idx] = make_float2((float)(b * cs), (float)(b * sn));
     }
+}
+
+__global__ void unit_scale_kernel(float *scale_out) {
+    if (threadIdx.x < 3) scale_out[threadIdx.x] = 1.f;
 }
 
 // P:L360 "We carry FIR filter history samples across to the next block": new history = the last
@@ -349,7 +385,13 @@ cudaError_t launch_phase_table(const cobalt_plan_s *p, cudaStream_t st, const do
     long long blocks = (total + threads - 1) / threads;
     if (blocks > 4096) blocks = 4096;
     phase_table_kernel<<<(unsigned)blocks, threads, 0, st>>>(d_delays, d_bandpass, p->d_f_sb, b0, nb, p->S, p->C,
-                                                             p->f_s, p->d_phase);
+                                                             p->f_s, p->amp_max, p->mode == COBALT_MODE_TENSOR_FP16 ? 1 : 0,
+                                                             p->d_scale, p->d_phase);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_set_unit_scale(const cobalt_plan_s *p, cudaStream_t st) {
+    unit_scale_kernel<<<1, 32, 0, st>>>(p->d_scale);
     return cudaGetLastError();
 }
 

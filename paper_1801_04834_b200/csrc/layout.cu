@@ -12,9 +12,10 @@ __device__ __forceinline__ size_t z16_offset(int c, int kt, int plane, int m, in
     return ((((size_t)c * n_kt + kt) * 2 + plane) * Mpad + m) * 128 + ((((tt >> 3) ^ (m & 7)) << 4) | ((tt & 7) << 1));
 }
 
-__global__ void z16_to_float_kernel(const unsigned char *__restrict__ z, float2 *__restrict__ out, int C, int M,
-                                    int Mpad, int n_kt, long long n_t) {
+__global__ void z16_to_float_kernel(const unsigned char *__restrict__ z, const float *__restrict__ scale,
+                                    float2 *__restrict__ out, int C, int M, int Mpad, int n_kt, long long n_t) {
     const long long total = (long long)C * M * n_t;
+    const float inv_s = scale[1];   // the operands carry the power-of-two scale s (fstage.cu)
     for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < total;
          idx += (long long)gridDim.x * blockDim.x) {
         const long long t = idx % n_t;
@@ -23,7 +24,7 @@ __global__ void z16_to_float_kernel(const unsigned char *__restrict__ z, float2 
         const int kt = (int)(t / kKTile), tt = (int)(t % kKTile);
         const __half re = *reinterpret_cast<const __half *>(z + z16_offset(c, kt, 0, m, tt, n_kt, Mpad));
         const __half im = *reinterpret_cast<const __half *>(z + z16_offset(c, kt, 1, m, tt, n_kt, Mpad));
-        out[idx] = make_float2(__half2float(re), __half2float(im));
+        out[idx] = make_float2(__half2float(re) * inv_s, __half2float(im) * inv_s);
     }
 }
 
@@ -57,8 +58,8 @@ inline unsigned grid_for(long long total, int threads) {
 cudaError_t launch_z_to_float(const cobalt_plan_s *p, cudaStream_t st, const void *d_zsub, float2 *d_out) {
     const long long total = (long long)p->C * p->M * p->n_t;
     if (p->mode == COBALT_MODE_TENSOR_FP16) {
-        z16_to_float_kernel<<<grid_for(total, 256), 256, 0, st>>>(static_cast<const unsigned char *>(d_zsub), d_out,
-                                                                  p->C, p->M, p->Mpad, p->n_kt, p->n_t);
+        z16_to_float_kernel<<<grid_for(total, 256), 256, 0, st>>>(static_cast<const unsigned char *>(d_zsub), p->d_scale,
+                                                                  d_out, p->C, p->M, p->Mpad, p->n_kt, p->n_t);
         return cudaGetLastError();
     }
     return cudaMemcpyAsync(d_out, d_zsub, (size_t)total * sizeof(float2), cudaMemcpyDeviceToDevice, st);

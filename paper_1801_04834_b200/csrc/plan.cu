@@ -31,7 +31,7 @@ int fail(const cobalt_plan_s *p, int code, const std::string &msg) {
 
 // Reading A1: Hann-windowed sinc, unit DC gain, double precision, rounded once to fp32.
 // weights[k][ph] = g[(15 - k) C + ph]  (reading A2: tap k = 0 multiplies the newest block).
-void build_weights(int C, std::vector<float> &w) {
+void build_weights(int C, std::vector<float> &w, double &sum_abs) {
     const int L = kTaps * C;
     const double pi = 3.141592653589793238462643383279502884;
     std::vector<double> g(L);
@@ -46,6 +46,8 @@ void build_weights(int C, std::vector<float> &w) {
     w.resize(L);
     for (int k = 0; k < kTaps; ++k)
         for (int ph = 0; ph < C; ++ph) w[k * C + ph] = (float)(g[(kTaps - 1 - k) * C + ph] / sum);
+    sum_abs = 0.0;
+    for (float v : w) sum_abs += std::fabs((double)v);
 }
 
 size_t subband_input_bytes(const cobalt_plan_s *p) { return (size_t)p->M * (size_t)p->N * sample_bytes(p->bits); }
@@ -88,14 +90,16 @@ int alloc_scratch(cobalt_plan_s *p, int chunk_request) {
 // One chunk of subbands [b0, b0 + nb): samples_b0 / vis_b0 point at subband b0.
 int enqueue_chunk(cobalt_plan_s *p, cudaStream_t st, const void *samples_b0, const double *d_delays,
                   const float *d_bandpass, float2 *vis_b0, int b0, int nb, StageEvents *ev) {
-    if (ev) CK(p, cudaEventRecord(ev->f0, st));
+    if (ev) CK(p, cudaEventRecord(ev->e[0], st));
     CK(p, launch_phase_table(p, st, d_delays, d_bandpass, b0, nb));
+    if (ev) CK(p, cudaEventRecord(ev->e[1], st));
     CK(p, launch_fstage(p, st, samples_b0, b0, nb));
+    if (ev) CK(p, cudaEventRecord(ev->e[2], st));
     CK(p, launch_history_update(p, st, samples_b0, b0, nb));
-    if (ev) CK(p, cudaEventRecord(ev->f1, st));
+    if (ev) CK(p, cudaEventRecord(ev->e[3], st));
     if (p->mode == COBALT_MODE_TENSOR_FP16) CK(p, launch_xstage_tc(p, st, p->d_z, nb, vis_b0));
     else CK(p, launch_xstage_simt(p, st, p->d_z, nb, vis_b0));
-    if (ev) CK(p, cudaEventRecord(ev->x1, st));
+    if (ev) CK(p, cudaEventRecord(ev->e[4], st));
     p->launches += 4;
     return COBALT_OK;
 }
@@ -103,9 +107,7 @@ int enqueue_chunk(cobalt_plan_s *p, cudaStream_t st, const void *samples_b0, con
 int ensure_events(cobalt_plan_s *p, int n) {
     while ((int)p->events.size() < n) {
         StageEvents e;
-        CK(p, cudaEventCreate(&e.f0));
-        CK(p, cudaEventCreate(&e.f1));
-        CK(p, cudaEventCreate(&e.x1));
+        for (auto &ev : e.e) CK(p, cudaEventCreate(&ev));
         p->events.push_back(e);
     }
     return COBALT_OK;
@@ -174,7 +176,10 @@ int cobalt_plan(cobalt_plan_t **out, int stations, int subbands, int channels, i
     p->sm_count = prop.multiProcessorCount;
     p->f_sb.resize(subbands);
     for (int s = 0; s < subbands; ++s) p->f_sb[s] = 100.0e6 + (12 + s) * p->f_s;   // reading A6
-    build_weights(p->C, p->h_weights);
+    double sum_abs_g = 0.0;
+    build_weights(p->C, p->h_weights, sum_abs_g);
+    // worst-case modulus of a channelised sample for full-scale input: sum|g| sqrt(2) 2^(bits-1)
+    p->amp_max = (float)(sum_abs_g * 1.4142135623730951 * (input_bits == 16 ? 32768.0 : 128.0));
     build_xjobs(p);
 
     int rc = COBALT_OK;
@@ -189,6 +194,7 @@ int cobalt_plan(cobalt_plan_t **out, int stations, int subbands, int channels, i
     guard(cudaMalloc(&p->d_hist[0], hist), "cudaMalloc history");
     guard(cudaMalloc(&p->d_hist[1], hist), "cudaMalloc history");
     guard(cudaMalloc(&p->d_jobs, p->jobs.size() * sizeof(XJob)), "cudaMalloc jobs");
+    guard(cudaMalloc(&p->d_scale, 4 * sizeof(float)), "cudaMalloc scale");
     if (rc == COBALT_OK) {
         guard(cudaMemcpy(p->d_weights, p->h_weights.data(), p->h_weights.size() * sizeof(float), cudaMemcpyHostToDevice), "weights H2D");
         guard(cudaMemcpy(p->d_f_sb, p->f_sb.data(), (size_t)p->B * sizeof(double), cudaMemcpyHostToDevice), "f_sb H2D");
@@ -214,13 +220,11 @@ int cobalt_destroy(cobalt_plan_t *p) {
     cudaFree(p->d_hist[0]);
     cudaFree(p->d_hist[1]);
     cudaFree(p->d_jobs);
+    cudaFree(p->d_scale);
     cudaFree(p->d_delays_h);
     cudaFree(p->d_bandpass_h);
-    for (auto &e : p->events) {
-        cudaEventDestroy(e.f0);
-        cudaEventDestroy(e.f1);
-        cudaEventDestroy(e.x1);
-    }
+    for (auto &e : p->events)
+        for (auto &ev : e.e) cudaEventDestroy(ev);
     for (int i = 0; i < 3; ++i)
         if (p->hs[i]) cudaStreamDestroy(p->hs[i]);
     for (int i = 0; i < 2; ++i) {
@@ -378,20 +382,29 @@ int cobalt_set_timing(cobalt_plan_t *p, int enabled) {
     return COBALT_OK;
 }
 
-int cobalt_get_timing(cobalt_plan_t *p, double *f_ms, double *x_ms, int *launches) {
+int cobalt_get_kernel_timing(cobalt_plan_t *p, double *ms4, int *launches) {
     if (!p) return fail(nullptr, COBALT_ERR_BAD_ARG, "plan is NULL");
-    double f = 0.0, x = 0.0;
+    double acc[4] = {0.0, 0.0, 0.0, 0.0};
     for (int i = 0; i < p->n_chunks_timed; ++i) {
-        float a = 0.f, b = 0.f;
-        CK(p, cudaEventSynchronize(p->events[i].x1));
-        CK(p, cudaEventElapsedTime(&a, p->events[i].f0, p->events[i].f1));
-        CK(p, cudaEventElapsedTime(&b, p->events[i].f1, p->events[i].x1));
-        f += a;
-        x += b;
+        CK(p, cudaEventSynchronize(p->events[i].e[4]));
+        for (int k = 0; k < 4; ++k) {
+            float t = 0.f;
+            CK(p, cudaEventElapsedTime(&t, p->events[i].e[k], p->events[i].e[k + 1]));
+            acc[k] += t;
+        }
     }
-    if (f_ms) *f_ms = f;
-    if (x_ms) *x_ms = x;
+    if (ms4)
+        for (int k = 0; k < 4; ++k) ms4[k] = acc[k];
     if (launches) *launches = p->launches;
+    return COBALT_OK;
+}
+
+int cobalt_get_timing(cobalt_plan_t *p, double *f_ms, double *x_ms, int *launches) {
+    double ms[4];
+    int rc = cobalt_get_kernel_timing(p, ms, launches);
+    if (rc != COBALT_OK) return rc;
+    if (f_ms) *f_ms = ms[0] + ms[1] + ms[2];
+    if (x_ms) *x_ms = ms[3];
     return COBALT_OK;
 }
 
@@ -423,6 +436,7 @@ int cobalt_debug_channelised(cobalt_plan_t *p, void *cuda_stream, const void *d_
 int cobalt_debug_correlate(cobalt_plan_t *p, void *cuda_stream, const void *d_z, void *d_vis) {
     if (!p || !d_z || !d_vis) return fail(p, COBALT_ERR_BAD_ARG, "NULL argument");
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    CK(p, launch_set_unit_scale(p, st));   // caller-supplied operands are taken as they are
     CK(p, launch_float_to_z(p, st, static_cast<const float2 *>(d_z), p->d_z));
     if (p->mode == COBALT_MODE_TENSOR_FP16) CK(p, launch_xstage_tc(p, st, p->d_z, 1, static_cast<float2 *>(d_vis)));
     else CK(p, launch_xstage_simt(p, st, p->d_z, 1, static_cast<float2 *>(d_vis)));

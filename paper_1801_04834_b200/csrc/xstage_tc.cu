@@ -32,6 +32,7 @@ struct XArgs {
     const unsigned char *z;
     float2 *vis;
     const XJob *jobs;
+    const float *scale;     // {s, 1/s, 1/s^2} of the fp16 intermediate (fstage.cu)
     size_t z_subband_bytes;
     long long n_bl;
     int C, M, Mpad, n_kt, jobs_per_channel, total_jobs, stages, stage_bytes;
@@ -214,6 +215,7 @@ __global__ void __launch_bounds__(kThreads, 1) xstage_tc_kernel(const XArgs a) {
     } else {
         // ------------------------------------------------------------------ epilogue
         const int wq = warp & 3;                           // TMEM lane quarter this warp may access
+        const float inv_s2 = __ldg(a.scale + 2);           // undo the power-of-two operand scale (exact)
         uint32_t it = 0;
         for (int jid = blockIdx.x; jid < a.total_jobs; jid += gridDim.x, ++it) {
             const int jl = jid % a.jobs_per_channel;
@@ -242,8 +244,8 @@ __global__ void __launch_bounds__(kThreads, 1) xstage_tc_kernel(const XArgs a) {
                         const int b = col0 + e, k = b >> 1;
                         if (arow < a.M && b < a.M && i <= k)
                             vc[((size_t)k * (k + 1) / 2 + i) * 2 + p] =
-                                make_float4(__uint_as_float(re[e]), __uint_as_float(im[e]), __uint_as_float(re[e + 1]),
-                                            __uint_as_float(im[e + 1]));
+                                make_float4(__uint_as_float(re[e]) * inv_s2, __uint_as_float(im[e]) * inv_s2,
+                                            __uint_as_float(re[e + 1]) * inv_s2, __uint_as_float(im[e + 1]) * inv_s2);
                     }
                 }
             }
@@ -336,6 +338,7 @@ cudaError_t launch_xstage_tc(const cobalt_plan_s *p, cudaStream_t st, const void
     a.z = static_cast<const unsigned char *>(d_z);
     a.vis = d_vis;
     a.jobs = p->d_jobs;
+    a.scale = p->d_scale;
     a.z_subband_bytes = p->z_subband_bytes;
     a.n_bl = p->n_bl;
     a.C = p->C;

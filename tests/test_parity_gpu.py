@@ -272,3 +272,37 @@ def test_process_host_matches_device_path(cobalt, dev):
         out = torch.empty(cor.vis_shape(), dtype=torch.complex64).pin_memory()
         cor.process_host(data["samples"].pin_memory(), data["delays"], data["bandpass"], out)
     assert np.array_equal(a, out.numpy())
+
+
+# ------------------------------------------------------------------ fp16 operand scale
+def test_fp16_scale_worst_case_amplitude(cobalt, oracle, dev):
+    """Sign-matched full-scale input rotated by 45 degrees drives one component of z to
+    sum|g| * sqrt(2) * 32767 ~ 7.8e4 > 65504: without the power-of-two operand scale fp16 overflows."""
+    C, S, n_t, t0 = 64, 2, 64, 40
+    g = oracle.fir_prototype(C)
+    samples = np.zeros((1, S, 2, n_t * C, 2), dtype=np.int16)
+    seg = (32767 * np.sign(g)).astype(np.int16)                     # window of spectrum t0, natural order
+    samples[0, :, :, (t0 - 15) * C:(t0 + 1) * C, 0] = seg
+    samples[0, :, :, (t0 - 15) * C:(t0 + 1) * C, 1] = seg
+    f = oracle.default_subband_frequency(0)
+    tau = (np.floor(f * 1e-6) + 0.125) / f                          # frac(f tau) = 1/8 at the centre channel
+    delays = np.array([tau, 0.0])
+    bandpass = np.ones(C, dtype=np.float32)
+    _, zo = oracle.process_subband(samples[0], C, delays, bandpass.astype(np.float64), f, return_z=True)
+    assert np.max(np.abs(zo[0].real)) > 65504                       # the case really is out of fp16 range
+    with cobalt.Correlator(S, 1, C, n_t * C, 16) as cor:
+        vg = cor.process(torch.from_numpy(samples).to(dev), torch.from_numpy(delays).to(dev),
+                         torch.from_numpy(bandpass).to(dev)).cpu().numpy()
+    vo = oracle.process_subband(samples[0], C, delays, bandpass.astype(np.float64), f)
+    _assert_parity(vg[0], vo, True, "worst-case amplitude")
+
+
+@pytest.mark.parametrize("gain", [1e-4, 300.0])
+def test_fp16_scale_follows_bandpass_gain(cobalt, oracle, dev, gain):
+    synth = _synth()
+    cfg = synth.scaled(synth.CONFIGS[2], S=4, N=64 * 200)
+    data = synth.generate(cfg, device="cpu")
+    data["bandpass"] = (data["bandpass"] * gain * (1 + 0.2 * torch.rand(cfg.C))).to(torch.float32)
+    vg = _run_gpu(cobalt, cfg, data, cobalt.COBALT_MODE_TENSOR_FP16, dev)
+    vo = _run_oracle(oracle, cfg, data)
+    _assert_parity(vg[0], vo[0], True, f"bandpass gain {gain}")
