@@ -19,6 +19,7 @@
 // allocator + single-thread MMA issuer, warps 2-5 = epilogue (tcgen05.ld -> triangular baseline
 // index -> coalesced 16-byte stores of (re, im) pairs).
 #include "cobalt_internal.h"
+#include <cstdlib>
 
 namespace cobalt {
 
@@ -36,6 +37,7 @@ struct XArgs {
     size_t z_subband_bytes;
     long long n_bl;
     int C, M, Mpad, n_kt, jobs_per_channel, total_jobs, stages, stage_bytes;
+    int dbg;   // TEMP experiment knobs
 };
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -154,6 +156,7 @@ __global__ void __launch_bounds__(kThreads, 1) xstage_tc_kernel(const XArgs a) {
                     mbar_wait(bar_base + 8 * (16 + s), ph ^ 1);
                     const uint32_t full = bar_base + 8 * s;
                     const uint32_t dst = stage_base + (uint32_t)s * a.stage_bytes;
+                    if (a.dbg & 2) { mbar_arrive(full); if (++s == stages) { s = 0; ph ^= 1; } continue; }
                     mbar_expect_tx(full, 2 * plane_bytes);
                     const unsigned char *src = zc + (size_t)kt * 2 * a.Mpad * 128;
 #pragma unroll
@@ -185,7 +188,7 @@ __global__ void __launch_bounds__(kThreads, 1) xstage_tc_kernel(const XArgs a) {
                     mbar_wait(bar_base + 8 * s, ph);
                     tc_fence_after();
                     const uint32_t st = stage_base + (uint32_t)s * a.stage_bytes;
-                    for (int g = 0; g < job.n_groups; ++g) {
+                    for (int g = 0; g < ((a.dbg & 1) ? 0 : ((a.dbg & 8) ? 1 : job.n_groups)); ++g) {
                         const XMmaGroup &grp = job.g[g];
                         const uint64_t ar = make_smem_desc(st + grp.a_row * 128);
                         const uint64_t ai = make_smem_desc(st + plane_bytes + grp.a_row * 128);
@@ -242,7 +245,7 @@ __global__ void __launch_bounds__(kThreads, 1) xstage_tc_kernel(const XArgs a) {
 #pragma unroll
                     for (int e = 0; e < 16; e += 2) {
                         const int b = col0 + e, k = b >> 1;
-                        if (arow < a.M && b < a.M && i <= k)
+                        if (arow < a.M && b < a.M && i <= k && !(a.dbg & 4))
                             vc[((size_t)k * (k + 1) / 2 + i) * 2 + p] =
                                 make_float4(__uint_as_float(re[e]) * inv_s2, __uint_as_float(im[e]) * inv_s2,
                                             __uint_as_float(re[e + 1]) * inv_s2, __uint_as_float(im[e + 1]) * inv_s2);
@@ -351,6 +354,7 @@ cudaError_t launch_xstage_tc(const cobalt_plan_s *p, cudaStream_t st, const void
     int max_rows = 0;
     for (const XJob &j : p->jobs) max_rows = (j.ld_nrows[0] + j.ld_nrows[1]) > max_rows ? (j.ld_nrows[0] + j.ld_nrows[1]) : max_rows;
     a.stage_bytes = max_rows * 128 * 2;
+    a.dbg = getenv("COBALT_X_DBG") ? atoi(getenv("COBALT_X_DBG")) : 0;
     cudaError_t e = cudaFuncSetAttribute(xstage_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->x_smem_bytes);
     if (e != cudaSuccess) return e;
     const int grid = a.total_jobs < p->sm_count ? a.total_jobs : p->sm_count;
