@@ -7,17 +7,23 @@
 // builds the per-(station, channel) rotation table first (phase angles in double precision),
 // and a copy kernel carries the FIR history to the next call.
 //
-// Work decomposition of fstage_kernel<C, BITS, TENSOR>:
-//   CTA  = one stream (subband, station, pol) x a run of 64-spectrum k-tiles.
-//   FIR  : thread ph owns polyphase branch ph; its 16 weights and a 15-sample sliding window stay
-//          in registers while the CTA marches through time, so every input sample is loaded from
-//          global memory once per CTA (4-byte coalesced loads: a warp reads 128 contiguous bytes).
-//   FFT  : every 16 spectra the FIR outputs cross shared memory once; C = 16 R points are done as a
-//          radix-16 pass in registers, a twiddle, a conflict-free shared-memory exchange and a
-//          radix-R pass, R threads per spectrum.  The (-1)^ph needed for the ascending-frequency
-//          channel order (D[(j + C/2) mod C]) is folded into the FIR weights, so the reorder is free.
-//   out  : rotation*bandpass from a per-CTA table, fp16 (or fp32) conversion, staged in shared
-//          memory for 64 spectra and flushed as whole 128-byte lines (TENSOR) / 128-byte runs (EXACT).
+// fstage_kernel<C, BITS, TENSOR> is warp specialised (17 warps, one CTA per SM):
+//   CTA      = 256 / C consecutive streams (subband, station, pol) x a run of 64-spectrum k-tiles,
+//              walked in sub-tiles of 16 spectra.
+//   warp 16  = producer: the raw integer rows of the next sub-tiles (time-contiguous, so one bulk
+//              copy -- cp.async.bulk, SASS UBLKCP -- per stream and sub-tile) land in a 4-deep
+//              shared-memory ring signalled on mbarriers; the first sub-tile of a CTA is the 16-row
+//              warm-up taken from the carried history (or from the preceding samples).
+//   warps 0-7  = FIR: thread = polyphase branch.  Transposed-form filter: every new sample is
+//              converted once and added, scaled by its 16 weights, to the 16 pending outputs held
+//              in registers as (re, im) pairs (packed fma.rn.f32x2: one issue slot per two FMAs);
+//              the completed output goes to a double-buffered shared-memory tile.
+//   warps 8-15 = FFT + rotate + transpose: thread = (spectrum, 1/16 of its channels): radix-16 pass
+//              in registers, twiddle, warp-local shared-memory exchange, radix-R pass (C = 16 R),
+//              rotation * bandpass from a per-CTA table, fp16 (or fp32) conversion, staged
+//              transposed in shared memory and flushed as whole 32-byte sectors (TENSOR) /
+//              128-byte runs (EXACT).  The (-1)^ph needed for the ascending-frequency channel order
+//              (D[(j + C/2) mod C]) is folded into the FIR weights, so the reorder is free.
 #include "cobalt_internal.h"
 
 namespace cobalt {
@@ -32,7 +38,7 @@ struct FArgs {
     unsigned char *z;               // chunk intermediate
     long long N, n_t;
     size_t z_subband_bytes;
-    int S, M, Mpad, n_kt, b0, tiles_per_seg;
+    int S, M, Mpad, n_kt, b0, tiles_per_seg, groups_per_subband;
 };
 
 __device__ __forceinline__ float2 cmul(float2 a, float2 b) {
@@ -73,197 +79,336 @@ __device__ __forceinline__ void dft16(float2 (&a)[16]) {
     for (int k1 = 0; k1 < 4; ++k1) dft4(a[4 * k1], a[4 * k1 + 1], a[4 * k1 + 2], a[4 * k1 + 3]);   // -> a[4 k1 + k2]
 }
 
-// Step a1: the integer value as a float, bit-exact; `t` may address the carried history
-// (t < 0), the block (0 <= t < n_t) or the zero padding beyond the consumed samples.
-template <int BITS>
-__device__ __forceinline__ float2 load_sample(const unsigned char *xs, const unsigned char *hs, long long t, int ph,
-                                              int C, long long n_t) {
-    constexpr int SB = BITS == 16 ? 4 : 2;
-    const unsigned char *p;
-    if (t < 0) p = hs + ((long long)(kTaps - 1 + t) * C + ph) * SB;
-    else if (t < n_t) p = xs + (t * C + ph) * SB;
-    else return make_float2(0.f, 0.f);
-    if (BITS == 16) {
-        unsigned int w = __ldg(reinterpret_cast<const unsigned int *>(p));
-        return make_float2((float)(short)(w & 0xffffu), (float)(short)(w >> 16));
-    } else {
-        unsigned short w = __ldg(reinterpret_cast<const unsigned short *>(p));
-        return make_float2((float)(signed char)(w & 0xffu), (float)(signed char)(w >> 8));
-    }
+// ------------------------------------------------------------------ mbarrier / bulk-copy helpers
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    uint32_t done;
+    do {
+        asm volatile(
+            "{\n\t"
+            ".reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t"
+            "}"
+            : "=r"(done)
+            : "r"(bar), "r"(parity)
+            : "memory");
+    } while (!done);
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t bytes, uint32_t bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+                 "l"(src), "r"(bytes), "r"(bar)
+                 : "memory");
+}
+__device__ __forceinline__ void bar_sync_named(int id, int threads) {
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(threads) : "memory");
 }
 
-template <int C>
-struct FShape {
-    static constexpr int NT = C < 32 ? 32 : C;     // threads per CTA
-    static constexpr int R = C / 16;               // threads per spectrum in the FFT
-    static constexpr int EX_T = R == 16 ? 272 : (R == 4 ? 68 : 16);   // exchange elements per spectrum
-    static constexpr int XCH = (kSubTile * C > kSubTile * EX_T) ? kSubTile * C : kSubTile * EX_T;   // float2
-    static constexpr int STG16 = 264;              // bytes per channel of the fp16 staging (2 x 128 + pad)
-    static constexpr int STG32 = 17;               // float2 per channel of the fp32 staging (16 + pad)
-    static constexpr size_t smem(bool tensor) {
-        return (size_t)XCH * 8 + (size_t)C * 8 * 2 + (tensor ? (size_t)C * STG16 : (size_t)C * STG32 * 8);
-    }
-};
+constexpr int kFirThreads = 256, kFftThreads = 256, kFThreads = kFirThreads + kFftThreads + 32;
+constexpr int kRawStages = 4;
 
 template <int C, int BITS, bool TENSOR>
-__global__ void __launch_bounds__(FShape<C>::NT) fstage_kernel(FArgs a) {
-    using Sh = FShape<C>;
-    constexpr int NT = Sh::NT, R = Sh::R, SB = BITS == 16 ? 4 : 2;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    float2 *xch = reinterpret_cast<float2 *>(smem_raw);            // FIR->FFT tile, reused as exchange
-    float2 *tw = xch + Sh::XCH;                                    // W_C^m
-    float2 *wtab = tw + C;                                         // rotation * bandpass of this station
-    unsigned char *stg = reinterpret_cast<unsigned char *>(wtab + C);
+struct FShape {
+    static constexpr int SB = BITS == 16 ? 4 : 2;          // bytes per complex sample
+    static constexpr int SPC = 256 / C;                    // streams per CTA
+    static constexpr int R = C / 16;                       // threads per spectrum in the FFT
+    static constexpr int YS = C + R;                       // float2 per stream row of the FIR->FFT tile (padded)
+    static constexpr int RAW_STAGE = kSubTile * 256 * SB;  // bytes: [SPC][16 rows][C] samples
+    static constexpr int Y_BUF = kSubTile * SPC * YS * 8;  // bytes
+    static constexpr int XCH_GROUP = 272;                  // float2 per 16-lane group (16 x 17 / 4 x 68)
+    static constexpr int XCH = R > 1 ? 16 * XCH_GROUP * 8 : 0;
+    static constexpr int STG_ROW = TENSOR ? 18 * 4 : 17 * 8;   // bytes per (stream, channel) row of the staging
+    static constexpr int STG = 256 * STG_ROW;
+    static constexpr int OFF_BAR = 0;                      // 2*kRawStages + 4 mbarriers
+    static constexpr int OFF_RAW = 128;
+    static constexpr int OFF_Y = OFF_RAW + kRawStages * RAW_STAGE;
+    static constexpr int OFF_XCH = OFF_Y + 2 * Y_BUF;
+    static constexpr int OFF_STG = OFF_XCH + XCH;
+    static constexpr int OFF_WTAB = OFF_STG + STG;         // [SPC][C] float2
+    static constexpr int TOTAL = OFF_WTAB + 256 * 8;
+};
 
-    const int tid = threadIdx.x;
-    const bool active = tid < C;
-    const int stream = blockIdx.x;                 // within the chunk: bl * M + m
-    const int bl = stream / a.M, m = stream - bl * a.M;
+template <int BITS>
+__device__ __forceinline__ float2 unpack_sample(uint32_t raw) {
+    // Step a1: the two's-complement integer value as a float, exact.
+    if (BITS == 16) return make_float2((float)(short)(raw & 0xffffu), (float)(short)(raw >> 16));
+    return make_float2((float)(signed char)(raw & 0xffu), (float)(signed char)((raw >> 8) & 0xffu));
+}
+
+template <int C, int BITS, bool TENSOR>
+__global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a) {
+    using Sh = FShape<C, BITS, TENSOR>;
+    constexpr int SB = Sh::SB, SPC = Sh::SPC, R = Sh::R, YS = Sh::YS;
+    extern __shared__ __align__(128) unsigned char smem[];
+    const uint32_t sbase = smem_u32(smem);
+    const uint32_t bar_raw_full = sbase + Sh::OFF_BAR;                 // [kRawStages]
+    const uint32_t bar_raw_empty = bar_raw_full + 8 * kRawStages;      // [kRawStages]
+    const uint32_t bar_y_full = bar_raw_empty + 8 * kRawStages;        // [2]
+    const uint32_t bar_y_empty = bar_y_full + 16;                      // [2]
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int grp = blockIdx.x;                          // stream group within the chunk
+    const int bl = grp / a.groups_per_subband;
+    const int m0 = (grp - bl * a.groups_per_subband) * SPC;
+    const int n_valid = min(SPC, a.M - m0);              // streams of this CTA that exist
     const int kt0 = blockIdx.y * a.tiles_per_seg;
     const int kt1 = min(kt0 + a.tiles_per_seg, a.n_kt);
-    const unsigned char *xs = a.samples + ((size_t)bl * a.M + m) * (size_t)a.N * SB;
-    const unsigned char *hs = a.hist + ((size_t)(a.b0 + bl) * a.M + m) * (size_t)(kTaps - 1) * C * SB;
-    unsigned char *zsub = a.z + (size_t)bl * a.z_subband_bytes;
+    const int n_sub = (kt1 - kt0) * (kKTile / kSubTile);
+    const long long t0 = (long long)kt0 * kKTile;
 
-    for (int i = tid; i < C; i += NT) {
-        float sn, cs;
-        sincospif(-2.0f * (float)i / (float)C, &sn, &cs);
-        tw[i] = make_float2(cs, sn);
-        wtab[i] = a.phase[((size_t)bl * a.S + (m >> 1)) * C + i];
+    if (tid == 0) {
+        for (int s = 0; s < kRawStages; ++s) {
+            mbar_init(bar_raw_full + 8 * s, 1);
+            mbar_init(bar_raw_empty + 8 * s, kFirThreads / 32);
+        }
+        for (int b = 0; b < 2; ++b) {
+            mbar_init(bar_y_full + 8 * b, kFirThreads / 32);
+            mbar_init(bar_y_empty + 8 * b, kFftThreads / 32);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-
-    // FIR state: weights of branch ph = tid (with the (-1)^ph of the channel reorder) and the window.
-    float wk[kTaps];
-    float2 win[kTaps - 1];
-    if (active) {
-        const float sgn = (tid & 1) ? -1.f : 1.f;
-#pragma unroll
-        for (int k = 0; k < kTaps; ++k) wk[k] = a.weights[k * C + tid] * sgn;
-#pragma unroll
-        for (int i = 0; i < kTaps - 1; ++i)
-            win[i] = load_sample<BITS>(xs, hs, (long long)kt0 * kKTile - (kTaps - 1) + i, tid, C, a.n_t);
+    {   // rotation * bandpass of the CTA's streams (station = m >> 1)
+        float2 *wtab = reinterpret_cast<float2 *>(smem + Sh::OFF_WTAB);
+        for (int i = tid; i < 256; i += kFThreads) {
+            const int sl = i / C, j = i - sl * C;
+            const int m = min(m0 + sl, a.M - 1);
+            wtab[i] = a.phase[((size_t)bl * a.S + (m >> 1)) * C + j];
+        }
     }
     __syncthreads();
 
-    for (int kt = kt0; kt < kt1; ++kt) {
-#pragma unroll 1
-        for (int sub = 0; sub < kKTile / kSubTile; ++sub) {
-            const long long t_base = (long long)kt * kKTile + sub * kSubTile;
-            if (active) {
-                float2 xn[kSubTile];
+    if (warp == 16) {
+        // ------------------------------------------------------------------ producer
+        for (int j = 0; j <= n_sub; ++j) {
+            const int s = j % kRawStages;
+            const uint32_t ph = (uint32_t)(j / kRawStages) & 1u;
+            mbar_wait(bar_raw_empty + 8 * s, ph ^ 1u);
+            const long long tb = t0 - kSubTile + (long long)j * kSubTile;     // first row of the sub-tile
+            const uint32_t full = bar_raw_full + 8 * s;
+            uint32_t tx = 0;
+            for (int sl = 0; sl < n_valid; ++sl) {
+                const size_t stream = (size_t)bl * a.M + (m0 + sl);
+                const uint32_t dst0 = sbase + Sh::OFF_RAW + s * Sh::RAW_STAGE + sl * (kSubTile * C * SB);
 #pragma unroll
-                for (int i = 0; i < kSubTile; ++i) xn[i] = load_sample<BITS>(xs, hs, t_base + i, tid, C, a.n_t);
-#pragma unroll
-                for (int i = 0; i < kSubTile; ++i) {
-                    float re = 0.f, im = 0.f;
-#pragma unroll
-                    for (int k = 0; k < kTaps; ++k) {       // y[t] = sum_k w[k] x[t - k]
-                        const int src = i - k;
-                        const float2 v = src >= 0 ? xn[src] : win[kTaps - 1 + src];
-                        re = fmaf(wk[k], v.x, re);
-                        im = fmaf(wk[k], v.y, im);
-                    }
-                    if (t_base + i >= a.n_t) re = im = 0.f;  // padding spectra are exact zeros
-                    xch[i * C + tid] = make_float2(re, im);
-                }
-#pragma unroll
-                for (int i = 0; i < kTaps - 1; ++i) win[i] = xn[i + 1];
-            }
-            __syncthreads();   // (A) FIR tile complete
-
-            float2 o[16];      // 16 channels of spectrum tl
-            const int tl = tid / R, r = tid % R;
-            if (active) {
-                float2 v[16];
-#pragma unroll
-                for (int q = 0; q < 16; ++q) v[q] = xch[tl * C + r + R * q];
-                dft16(v);
-                if (R == 1) {
-#pragma unroll
-                    for (int k = 0; k < 16; ++k) o[k] = v[dft16_pos(k)];
-                } else {
-#pragma unroll
-                    for (int k = 1; k < 16; ++k) v[dft16_pos(k)] = cmul(v[dft16_pos(k)], tw[r * k]);
-#pragma unroll
-                    for (int k = 0; k < 16; ++k) o[k] = v[dft16_pos(k)];   // o[k1] = A[r][k1] W_C^{r k1}
-                }
-            }
-            if (R > 1) {
-                __syncthreads();   // (B) everyone has read the FIR tile; reuse it as the exchange
-                if (active) {
-                    if (R == 16) {
-#pragma unroll
-                        for (int k = 0; k < 16; ++k) xch[tl * Sh::EX_T + r * 17 + k] = o[k];
+                for (int part = 0; part < 2; ++part) {
+                    // part 0: rows from the carried history (t < 0); part 1: rows of this call's block
+                    long long lo, hi;
+                    const unsigned char *src;
+                    if (part == 0) {
+                        lo = max(tb, -(long long)(kTaps - 1));
+                        hi = min(tb + kSubTile, 0ll);
+                        src = a.hist + (((size_t)(a.b0 + bl) * a.M + (m0 + sl)) * (kTaps - 1) + (size_t)(lo + kTaps - 1)) * C * SB;
                     } else {
-#pragma unroll
-                        for (int k = 0; k < 16; ++k) xch[tl * Sh::EX_T + k * 4 + r + (k >> 2)] = o[k];
+                        lo = max(tb, 0ll);
+                        hi = min(tb + kSubTile, a.n_t);
+                        src = a.samples + (stream * (size_t)a.N + (size_t)lo * C) * SB;
                     }
-                }
-                __syncthreads();   // (C)
-                if (active) {
-                    if (R == 16) {
-                        float2 v[16];
-#pragma unroll
-                        for (int r2 = 0; r2 < 16; ++r2) v[r2] = xch[tl * Sh::EX_T + r2 * 17 + r];
-                        dft16(v);
-#pragma unroll
-                        for (int k2 = 0; k2 < 16; ++k2) o[k2] = v[dft16_pos(k2)];   // channel r + 16 k2
-                    } else {
-#pragma unroll
-                        for (int a4 = 0; a4 < 4; ++a4) {
-                            const int k1 = 4 * r + a4;
-                            float2 c0 = xch[tl * Sh::EX_T + k1 * 4 + 0 + r];
-                            float2 c1 = xch[tl * Sh::EX_T + k1 * 4 + 1 + r];
-                            float2 c2 = xch[tl * Sh::EX_T + k1 * 4 + 2 + r];
-                            float2 c3 = xch[tl * Sh::EX_T + k1 * 4 + 3 + r];
-                            dft4(c0, c1, c2, c3);
-                            o[a4 * 4 + 0] = c0;   // channel k1 + 16 k2
-                            o[a4 * 4 + 1] = c1;
-                            o[a4 * 4 + 2] = c2;
-                            o[a4 * 4 + 3] = c3;
+                    if (hi <= lo) continue;
+                    const uint32_t bytes = (uint32_t)(hi - lo) * C * SB;
+                    const uint32_t dst = dst0 + (uint32_t)(lo - tb) * C * SB;
+                    if ((reinterpret_cast<uintptr_t>(src) & 15u) == 0) {
+                        if (lane == 0) bulk_g2s(dst, src, bytes, full);
+                        tx += bytes;
+                    } else {   // stream not 16-byte aligned (odd N): element-wise copy by the warp
+                        for (uint32_t e = lane * SB; e < bytes; e += 32 * SB) {
+                            if (SB == 4) {
+                                const uint32_t v = __ldg(reinterpret_cast<const uint32_t *>(src + e));
+                                asm volatile("st.shared.b32 [%0], %1;" ::"r"(dst + e), "r"(v) : "memory");
+                            } else {
+                                const unsigned short v = __ldg(reinterpret_cast<const unsigned short *>(src + e));
+                                asm volatile("st.shared.b16 [%0], %1;" ::"r"(dst + e), "h"(v) : "memory");
+                            }
                         }
                     }
                 }
             }
-            // steps a5-a7: rotate * bandpass, convert, stage transposed
-            if (active) {
+            __syncwarp();
+            if (lane == 0) mbar_arrive_expect_tx(full, tx);
+        }
+    } else if (warp < kFirThreads / 32) {
+        // ------------------------------------------------------------------ FIR (steps a1, a2)
+        const int sl = tid / C, ph = tid - sl * C;
+        float wk[kTaps];
+        {
+            const float sgn = (ph & 1) ? -1.f : 1.f;      // (-1)^ph: channel j <- DFT bin (j + C/2) mod C
 #pragma unroll
-                for (int i = 0; i < 16; ++i) {
-                    int j;
-                    if (R == 16) j = r + 16 * i;
-                    else if (R == 4) j = 4 * r + (i >> 2) + 16 * (i & 3);
-                    else j = i;
-                    const float2 zz = cmul(o[i], wtab[j]);
-                    if (TENSOR) {
-                        const int tt = sub * kSubTile + tl;
-                        *reinterpret_cast<__half *>(stg + j * Sh::STG16 + tt * 2) = __float2half_rn(zz.x);
-                        *reinterpret_cast<__half *>(stg + j * Sh::STG16 + 128 + tt * 2) = __float2half_rn(zz.y);
-                    } else {
-                        reinterpret_cast<float2 *>(stg)[j * Sh::STG32 + tl] = zz;
-                    }
+            for (int k = 0; k < kTaps; ++k) wk[k] = a.weights[k * C + ph] * sgn;
+        }
+        float2 acc[kTaps];
+#pragma unroll
+        for (int k = 0; k < kTaps; ++k) acc[k] = make_float2(0.f, 0.f);
+        const uint32_t raw_thread = sbase + Sh::OFF_RAW + sl * (kSubTile * C * SB) + ph * SB;
+        float2 *ybuf = reinterpret_cast<float2 *>(smem + Sh::OFF_Y);
+
+        for (int j = 0; j <= n_sub; ++j) {
+            const int s = j % kRawStages;
+            mbar_wait(bar_raw_full + 8 * s, (uint32_t)(j / kRawStages) & 1u);
+            const int jj = j - 1;                         // real sub-tile index (j = 0 is the warm-up)
+            const int yb = jj & 1;
+            if (jj >= 0) mbar_wait(bar_y_empty + 8 * yb, ((uint32_t)(jj >> 1) & 1u) ^ 1u);
+            float2 *yrow = ybuf + (size_t)yb * (Sh::Y_BUF / 8) + sl * YS + ph;
+            const uint32_t raw = raw_thread + s * Sh::RAW_STAGE;
+#pragma unroll
+            for (int i = 0; i < kSubTile; ++i) {
+                uint32_t w;
+                if (SB == 4) asm volatile("ld.shared.b32 %0, [%1];" : "=r"(w) : "r"(raw + i * C * SB));
+                else {
+                    unsigned short h;
+                    asm volatile("ld.shared.b16 %0, [%1];" : "=h"(h) : "r"(raw + i * C * SB));
+                    w = h;
+                }
+                const float2 x = unpack_sample<BITS>(w);
+                // sample u contributes w[k] x[u] to output u + k (slot (u + k) mod 16); output u is then complete
+#pragma unroll
+                for (int k = 0; k < kTaps; ++k)
+                    acc[(i + k) & 15] = __ffma2_rn(make_float2(wk[k], wk[k]), x, acc[(i + k) & 15]);
+                if (jj >= 0) yrow[i * (SPC * YS)] = acc[i];
+                acc[i] = make_float2(0.f, 0.f);
+            }
+            __syncwarp();
+            if (lane == 0) {
+                mbar_arrive(bar_raw_empty + 8 * s);
+                if (jj >= 0) mbar_arrive(bar_y_full + 8 * yb);
+            }
+        }
+    } else {
+        // ------------------------------------------------------------------ FFT, rotate, transpose (steps a3-a7)
+        const int ft = tid - kFirThreads;                 // 0..255
+        const int tl = ft >> 4;                           // spectrum of the sub-tile
+        const int sl = (ft & 15) / R, r = (ft & 15) % R;  // stream of the CTA, residue of the channel index
+        float2 twr[16];                                   // W_C^{r k1}
+        if (R > 1) {
+#pragma unroll
+            for (int k = 0; k < 16; ++k) {
+                float sn, cs;
+                sincospif(-2.0f * (float)(r * k) / (float)C, &sn, &cs);
+                twr[k] = make_float2(cs, sn);
+            }
+        }
+        const float2 *ybuf = reinterpret_cast<const float2 *>(smem + Sh::OFF_Y);
+        float2 *xch = reinterpret_cast<float2 *>(smem + Sh::OFF_XCH) + (ft >> 4) * Sh::XCH_GROUP;
+        const float2 *wtab = reinterpret_cast<const float2 *>(smem + Sh::OFF_WTAB) + sl * C;
+        unsigned char *stg = smem + Sh::OFF_STG;
+        unsigned char *zsub = a.z + (size_t)bl * a.z_subband_bytes;
+        // flush role: this thread owns staging row ft = (stream fsl, channel fc)
+        const int fsl = ft / C, fc = ft - fsl * C;
+        const int fm = m0 + fsl;
+
+        for (int jj = 0; jj < n_sub; ++jj) {
+            const int yb = jj & 1;
+            const int kt = kt0 + (jj >> 2), sub = jj & 3;
+            const long long t_base = (long long)kt * kKTile + sub * kSubTile;
+            mbar_wait(bar_y_full + 8 * yb, (uint32_t)(jj >> 1) & 1u);
+            float2 o[16];
+            {
+                float2 v[16];
+                const float2 *yrow = ybuf + (size_t)yb * (Sh::Y_BUF / 8) + (tl * SPC + sl) * YS + r;
+#pragma unroll
+                for (int q = 0; q < 16; ++q) v[q] = yrow[R * q];
+                dft16(v);
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar_y_empty + 8 * yb);
+                if (R == 1) {
+#pragma unroll
+                    for (int k = 0; k < 16; ++k) o[k] = v[dft16_pos(k)];
+                } else {
+                    o[0] = v[0];
+#pragma unroll
+                    for (int k = 1; k < 16; ++k) o[k] = cmul(v[dft16_pos(k)], twr[k]);   // A[r][k1] W_C^{r k1}
                 }
             }
-            __syncthreads();   // (D) staging written, exchange reads done
-            if (TENSOR) {
-                if (sub == kKTile / kSubTile - 1) {
-                    // whole 128-byte lines: (channel, plane) rows of this stream, chunks pre-swizzled
-                    for (int idx = tid; idx < C * 16; idx += NT) {
-                        const int q = idx & 7, plane = (idx >> 3) & 1, c = idx >> 4;
-                        const uint2 lo = *reinterpret_cast<const uint2 *>(stg + c * Sh::STG16 + plane * 128 + q * 16);
-                        const uint2 hi = *reinterpret_cast<const uint2 *>(stg + c * Sh::STG16 + plane * 128 + q * 16 + 8);
-                        unsigned char *dst = zsub + ((((size_t)c * a.n_kt + kt) * 2 + plane) * a.Mpad + m) * 128 +
-                                             ((q ^ (m & 7)) << 4);
-                        *reinterpret_cast<uint4 *>(dst) = make_uint4(lo.x, lo.y, hi.x, hi.y);
-                    }
+            if (R == 16) {
+#pragma unroll
+                for (int k = 0; k < 16; ++k) xch[r * 17 + k] = o[k];
+                __syncwarp();
+                float2 v[16];
+#pragma unroll
+                for (int r2 = 0; r2 < 16; ++r2) v[r2] = xch[r2 * 17 + r];
+                dft16(v);
+#pragma unroll
+                for (int k2 = 0; k2 < 16; ++k2) o[k2] = v[dft16_pos(k2)];   // channel r + 16 k2
+                __syncwarp();
+            } else if (R == 4) {
+                float2 *xg = xch + sl * 68;
+#pragma unroll
+                for (int k = 0; k < 16; ++k) xg[k * 4 + r + (k >> 2)] = o[k];
+                __syncwarp();
+#pragma unroll
+                for (int a4 = 0; a4 < 4; ++a4) {
+                    const int k1 = 4 * r + a4;
+                    float2 c0 = xg[k1 * 4 + 0 + r];
+                    float2 c1 = xg[k1 * 4 + 1 + r];
+                    float2 c2 = xg[k1 * 4 + 2 + r];
+                    float2 c3 = xg[k1 * 4 + 3 + r];
+                    dft4(c0, c1, c2, c3);
+                    o[a4 * 4 + 0] = c0;   // channel k1 + 16 k2
+                    o[a4 * 4 + 1] = c1;
+                    o[a4 * 4 + 2] = c2;
+                    o[a4 * 4 + 3] = c3;
                 }
-            } else {
-                float2 *z32 = reinterpret_cast<float2 *>(zsub);
-                for (int idx = tid; idx < C * kSubTile; idx += NT) {
-                    const int t16 = idx & 15, c = idx >> 4;
-                    const long long t = t_base + t16;
-                    if (t < a.n_t) z32[((size_t)c * a.M + m) * a.n_t + t] = reinterpret_cast<float2 *>(stg)[c * Sh::STG32 + t16];
+                __syncwarp();
+            }
+            // steps a5-a7: rotate * bandpass, convert, stage transposed
+            const bool live = t_base + tl < a.n_t;        // padding spectra of the last k-tile are exact zeros
+#pragma unroll
+            for (int i = 0; i < 16; ++i) {
+                int j;
+                if (R == 16) j = r + 16 * i;
+                else if (R == 4) j = 4 * r + (i >> 2) + 16 * (i & 3);
+                else j = i;
+                float2 zz = cmul(o[i], wtab[j]);
+                if (!live) zz = make_float2(0.f, 0.f);
+                if (TENSOR) {
+                    const __half2 h = __floats2half2_rn(zz.x, zz.y);
+                    *reinterpret_cast<__half2 *>(stg + (sl * C + j) * Sh::STG_ROW + tl * 4) = h;
+                } else {
+                    *reinterpret_cast<float2 *>(stg + (sl * C + j) * Sh::STG_ROW + tl * 8) = zz;
                 }
             }
+            bar_sync_named(1, kFftThreads);               // staging complete
+            if (fm < a.M) {
+                if (TENSOR) {
+                    // 16 spectra of (stream, channel): words (re | im << 16) -> one 16-byte chunk per plane and 8 spectra
+                    uint32_t w[16];
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) {
+                        const uint2 v = *reinterpret_cast<const uint2 *>(stg + ft * Sh::STG_ROW + i * 8);
+                        w[2 * i] = v.x;
+                        w[2 * i + 1] = v.y;
+                    }
+                    unsigned char *row = zsub + (((size_t)fc * a.n_kt + kt) * 2 * a.Mpad + fm) * 128;
+#pragma unroll
+                    for (int half = 0; half < 2; ++half) {
+                        uint4 re, im;
+                        re.x = __byte_perm(w[8 * half + 0], w[8 * half + 1], 0x5410);
+                        re.y = __byte_perm(w[8 * half + 2], w[8 * half + 3], 0x5410);
+                        re.z = __byte_perm(w[8 * half + 4], w[8 * half + 5], 0x5410);
+                        re.w = __byte_perm(w[8 * half + 6], w[8 * half + 7], 0x5410);
+                        im.x = __byte_perm(w[8 * half + 0], w[8 * half + 1], 0x7632);
+                        im.y = __byte_perm(w[8 * half + 2], w[8 * half + 3], 0x7632);
+                        im.z = __byte_perm(w[8 * half + 4], w[8 * half + 5], 0x7632);
+                        im.w = __byte_perm(w[8 * half + 6], w[8 * half + 7], 0x7632);
+                        const int q = ((2 * sub + half) ^ (fm & 7)) << 4;      // pre-swizzled chunk (cobalt_internal.h)
+                        *reinterpret_cast<uint4 *>(row + q) = re;
+                        *reinterpret_cast<uint4 *>(row + (size_t)a.Mpad * 128 + q) = im;
+                    }
+                } else {
+                    float2 *dst = reinterpret_cast<float2 *>(zsub) + ((size_t)fc * a.M + fm) * a.n_t + t_base;
+#pragma unroll
+                    for (int i = 0; i < 16; ++i)
+                        if (t_base + i < a.n_t) dst[i] = *reinterpret_cast<const float2 *>(stg + ft * Sh::STG_ROW + i * 8);
+                }
+            }
+            bar_sync_named(1, kFftThreads);               // staging drained
         }
     }
 }
@@ -350,22 +495,25 @@ __global__ void unpack_kernel(const I *__restrict__ in, long long n, float *__re
 
 template <int C, int BITS, bool TENSOR>
 cudaError_t launch_f(const cobalt_plan_s *p, cudaStream_t st, const FArgs &a, int nb) {
-    using Sh = FShape<C>;
+    using Sh = FShape<C, BITS, TENSOR>;
     auto kern = fstage_kernel<C, BITS, TENSOR>;
-    const size_t smem = Sh::smem(TENSOR);
+    const size_t smem = Sh::TOTAL;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     FArgs args = a;
-    // Enough CTAs for several waves, as few segments as possible (each segment re-reads 15 rows).
-    const long long streams = (long long)nb * p->M;
-    const long long want = (long long)p->sm_count * 16;
-    int n_seg = (int)((want + streams - 1) / streams);
+    // One CTA per SM: enough CTAs for >= 8 waves when the chunk allows, as few time segments as
+    // possible (each segment re-reads its 16 warm-up rows).
+    args.groups_per_subband = (p->M + Sh::SPC - 1) / Sh::SPC;
+    const long long groups = (long long)nb * args.groups_per_subband;
+    const long long want = (long long)p->sm_count * 8;
+    int n_seg = (int)((want + groups - 1) / groups);
     if (n_seg < 1) n_seg = 1;
-    if (n_seg > p->n_kt) n_seg = p->n_kt;
+    const int max_seg = (p->n_kt + 3) / 4;            // at least 4 k-tiles (256 spectra) per segment
+    if (n_seg > max_seg) n_seg = max_seg;
     args.tiles_per_seg = (p->n_kt + n_seg - 1) / n_seg;
     n_seg = (p->n_kt + args.tiles_per_seg - 1) / args.tiles_per_seg;
-    dim3 grid((unsigned)streams, (unsigned)n_seg);
-    kern<<<grid, Sh::NT, smem, st>>>(args);
+    dim3 grid((unsigned)groups, (unsigned)n_seg);
+    kern<<<grid, kFThreads, smem, st>>>(args);
     return cudaGetLastError();
 }
 
