@@ -41,20 +41,25 @@ struct FArgs {
     int S, M, Mpad, n_kt, b0, tiles_per_seg, groups_per_subband;
 };
 
-__device__ __forceinline__ float2 cmul(float2 a, float2 b) {
-    return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+// Packed fp32 pairs (fma.rn.f32x2 family, SASS FFMA2/FADD2/FMUL2): a complex value is one 64-bit
+// register pair, so a complex add or a real-times-complex FMA costs one issue slot instead of two.
+__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return __fadd2_rn(a, b); }
+__device__ __forceinline__ float2 csub(float2 a, float2 b) { return __ffma2_rn(b, make_float2(-1.f, -1.f), a); }
+// v * W, W = (t.x + i t.y):  v.x (W.re, W.im) + v.y (-W.im, W.re).  The swapped, half-negated operand is a
+// register-read modifier of FFMA2 (SASS .F32x2.LO_HI.NP), so a complex multiply is two issue slots.
+__device__ __forceinline__ float2 cmul_tab2(float2 v, float2 t) {
+    const float2 p = __fmul2_rn(make_float2(v.x, v.x), t);
+    return __ffma2_rn(make_float2(-t.y, t.x), make_float2(v.y, v.y), p);
 }
 
 // Forward 4-point DFT in place: X[k] = sum_n a[n] (-i)^{nk}.
 __device__ __forceinline__ void dft4(float2 &a0, float2 &a1, float2 &a2, float2 &a3) {
-    float2 t0 = make_float2(a0.x + a2.x, a0.y + a2.y);
-    float2 t1 = make_float2(a0.x - a2.x, a0.y - a2.y);
-    float2 t2 = make_float2(a1.x + a3.x, a1.y + a3.y);
-    float2 t3 = make_float2(a1.x - a3.x, a1.y - a3.y);
-    a0 = make_float2(t0.x + t2.x, t0.y + t2.y);
-    a2 = make_float2(t0.x - t2.x, t0.y - t2.y);
-    a1 = make_float2(t1.x + t3.y, t1.y - t3.x);   // t1 - i t3
-    a3 = make_float2(t1.x - t3.y, t1.y + t3.x);   // t1 + i t3
+    const float2 t0 = cadd(a0, a2), t1 = csub(a0, a2), t2 = cadd(a1, a3), t3 = csub(a1, a3);
+    a0 = cadd(t0, t2);
+    a2 = csub(t0, t2);
+    const float2 t3s = make_float2(t3.y, t3.x);
+    a1 = __ffma2_rn(t3s, make_float2(1.f, -1.f), t1);   // t1 - i t3
+    a3 = __ffma2_rn(t3s, make_float2(-1.f, 1.f), t1);   // t1 + i t3
 }
 
 // Forward 16-point DFT in place (radix 4 x 4).  On return X[k] is at a[dft16_pos(k)].
@@ -66,15 +71,15 @@ __device__ __forceinline__ void dft16(float2 (&a)[16]) {
     for (int n2 = 0; n2 < 4; ++n2) dft4(a[n2], a[4 + n2], a[8 + n2], a[12 + n2]);   // -> a[4 k1 + n2]
     constexpr float c1 = 0.92387953251128674f, s1 = 0.38268343236508977f, h = 0.70710678118654752f;
     // W16^m = (cos(2 pi m/16), -sin(2 pi m/16)) for m = n2 k1
-    a[4 * 1 + 1] = cmul(a[4 * 1 + 1], make_float2(c1, -s1));    // m = 1
-    a[4 * 1 + 2] = cmul(a[4 * 1 + 2], make_float2(h, -h));      // m = 2
-    a[4 * 1 + 3] = cmul(a[4 * 1 + 3], make_float2(s1, -c1));    // m = 3
-    a[4 * 2 + 1] = cmul(a[4 * 2 + 1], make_float2(h, -h));      // m = 2
+    a[4 * 1 + 1] = cmul_tab2(a[4 * 1 + 1], make_float2(c1, -s1));    // m = 1
+    a[4 * 1 + 2] = cmul_tab2(a[4 * 1 + 2], make_float2(h, -h));      // m = 2
+    a[4 * 1 + 3] = cmul_tab2(a[4 * 1 + 3], make_float2(s1, -c1));    // m = 3
+    a[4 * 2 + 1] = cmul_tab2(a[4 * 2 + 1], make_float2(h, -h));      // m = 2
     a[4 * 2 + 2] = make_float2(a[4 * 2 + 2].y, -a[4 * 2 + 2].x);   // m = 4: -i
-    a[4 * 2 + 3] = cmul(a[4 * 2 + 3], make_float2(-h, -h));     // m = 6
-    a[4 * 3 + 1] = cmul(a[4 * 3 + 1], make_float2(s1, -c1));    // m = 3
-    a[4 * 3 + 2] = cmul(a[4 * 3 + 2], make_float2(-h, -h));     // m = 6
-    a[4 * 3 + 3] = cmul(a[4 * 3 + 3], make_float2(-c1, s1));    // m = 9
+    a[4 * 2 + 3] = cmul_tab2(a[4 * 2 + 3], make_float2(-h, -h));     // m = 6
+    a[4 * 3 + 1] = cmul_tab2(a[4 * 3 + 1], make_float2(s1, -c1));    // m = 3
+    a[4 * 3 + 2] = cmul_tab2(a[4 * 3 + 2], make_float2(-h, -h));     // m = 6
+    a[4 * 3 + 3] = cmul_tab2(a[4 * 3 + 3], make_float2(-c1, s1));    // m = 9
 #pragma unroll
     for (int k1 = 0; k1 < 4; ++k1) dft4(a[4 * k1], a[4 * k1 + 1], a[4 * k1 + 2], a[4 * k1 + 3]);   // -> a[4 k1 + k2]
 }
@@ -113,28 +118,35 @@ __device__ __forceinline__ void bar_sync_named(int id, int threads) {
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(threads) : "memory");
 }
 
-constexpr int kFirThreads = 256, kFftThreads = 256, kFThreads = kFirThreads + kFftThreads + 32;
-constexpr int kRawStages = 4;
+// Thread roles: warps 0-7 FIR, warps 8-15 / 16-23 the two FFT groups, warp 24 the producer.
+constexpr int kFirThreads = 256, kFftGroup = 256, kFftGroups = 2;
+constexpr int kProducerWarp = (kFirThreads + kFftGroups * kFftGroup) / 32;
+constexpr int kFThreads = kFirThreads + kFftGroups * kFftGroup + 32;
+constexpr int kRawStages = 3;      // ring of raw sub-tiles (bulk copies in flight)
+constexpr int kYBufs = 3;          // ring of FIR-output sub-tiles
 
 template <int C, int BITS, bool TENSOR>
 struct FShape {
     static constexpr int SB = BITS == 16 ? 4 : 2;          // bytes per complex sample
     static constexpr int SPC = 256 / C;                    // streams per CTA
     static constexpr int R = C / 16;                       // threads per spectrum in the FFT
-    static constexpr int YS = C + R;                       // float2 per stream row of the FIR->FFT tile (padded)
+    // FIR-output tile [16 spectra][SPC streams][YS] float2; branch ph sits at ph + (ph >> 4) so that the
+    // radix-16 pass, the in-place exchange and the radix-R pass are all free of bank conflicts
+    static constexpr int YS = C + R;
     static constexpr int RAW_STAGE = kSubTile * 256 * SB;  // bytes: [SPC][16 rows][C] samples
     static constexpr int Y_BUF = kSubTile * SPC * YS * 8;  // bytes
-    static constexpr int XCH_GROUP = 272;                  // float2 per 16-lane group (16 x 17 / 4 x 68)
-    static constexpr int XCH = R > 1 ? 16 * XCH_GROUP * 8 : 0;
-    static constexpr int STG_ROW = TENSOR ? 18 * 4 : 17 * 8;   // bytes per (stream, channel) row of the staging
+    // staging of the transposed output, one per FFT group: TENSOR: 32 spectra of (re | im << 16) words
+    // + 2 pad words per (stream, channel) row; EXACT: 16 spectra of float2 + 1 pad
+    static constexpr int STG_ROW = TENSOR ? 34 * 4 : 17 * 8;
     static constexpr int STG = 256 * STG_ROW;
-    static constexpr int OFF_BAR = 0;                      // 2*kRawStages + 4 mbarriers
+    static constexpr int OFF_BAR = 0;                      // 2 kRawStages + 2 kYBufs mbarriers
     static constexpr int OFF_RAW = 128;
     static constexpr int OFF_Y = OFF_RAW + kRawStages * RAW_STAGE;
-    static constexpr int OFF_XCH = OFF_Y + 2 * Y_BUF;
-    static constexpr int OFF_STG = OFF_XCH + XCH;
-    static constexpr int OFF_WTAB = OFF_STG + STG;         // [SPC][C] float2
-    static constexpr int TOTAL = OFF_WTAB + 256 * 8;
+    static constexpr int OFF_STG = OFF_Y + kYBufs * Y_BUF;
+    static constexpr int OFF_WTAB = OFF_STG + kFftGroups * STG;   // [SPC][C] float2: rotation * bandpass
+    static constexpr int OFF_TW = OFF_WTAB + 256 * 8;      // [16][R] float2 W_C^{r k1}
+    static constexpr int TOTAL = OFF_TW + (R > 1 ? R * 16 * 8 : 0);
+    static_assert(TOTAL <= 227 * 1024, "shared memory budget");
 };
 
 template <int BITS>
@@ -152,8 +164,8 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a) {
     const uint32_t sbase = smem_u32(smem);
     const uint32_t bar_raw_full = sbase + Sh::OFF_BAR;                 // [kRawStages]
     const uint32_t bar_raw_empty = bar_raw_full + 8 * kRawStages;      // [kRawStages]
-    const uint32_t bar_y_full = bar_raw_empty + 8 * kRawStages;        // [2]
-    const uint32_t bar_y_empty = bar_y_full + 16;                      // [2]
+    const uint32_t bar_y_full = bar_raw_empty + 8 * kRawStages;        // [kYBufs]
+    const uint32_t bar_y_empty = bar_y_full + 8 * kYBufs;              // [kYBufs]
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int grp = blockIdx.x;                          // stream group within the chunk
@@ -170,23 +182,31 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a) {
             mbar_init(bar_raw_full + 8 * s, 1);
             mbar_init(bar_raw_empty + 8 * s, kFirThreads / 32);
         }
-        for (int b = 0; b < 2; ++b) {
+        for (int b = 0; b < kYBufs; ++b) {
             mbar_init(bar_y_full + 8 * b, kFirThreads / 32);
-            mbar_init(bar_y_empty + 8 * b, kFftThreads / 32);
+            mbar_init(bar_y_empty + 8 * b, kFftGroup / 32);
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    {   // rotation * bandpass of the CTA's streams (station = m >> 1)
+    {   // rotation * bandpass of the CTA's streams (station = m >> 1) and the inter-pass twiddles
         float2 *wtab = reinterpret_cast<float2 *>(smem + Sh::OFF_WTAB);
         for (int i = tid; i < 256; i += kFThreads) {
             const int sl = i / C, j = i - sl * C;
             const int m = min(m0 + sl, a.M - 1);
             wtab[i] = a.phase[((size_t)bl * a.S + (m >> 1)) * C + j];
         }
+        if (R > 1) {
+            float2 *tw = reinterpret_cast<float2 *>(smem + Sh::OFF_TW);
+            for (int i = tid; i < R * 16; i += kFThreads) {
+                float sn, cs;
+                sincospif(-2.0f * (float)((i / R) * (i % R)) / (float)C, &sn, &cs);   // entry [k1][r]
+                tw[i] = make_float2(cs, sn);
+            }
+        }
     }
     __syncthreads();
 
-    if (warp == 16) {
+    if (warp == kProducerWarp) {
         // ------------------------------------------------------------------ producer
         for (int j = 0; j <= n_sub; ++j) {
             const int s = j % kRawStages;
@@ -243,36 +263,46 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a) {
 #pragma unroll
             for (int k = 0; k < kTaps; ++k) wk[k] = a.weights[k * C + ph] * sgn;
         }
-        float2 acc[kTaps];
+        float2 acc[kTaps];                                // outputs still collecting taps (garbage until warmed up)
 #pragma unroll
         for (int k = 0; k < kTaps; ++k) acc[k] = make_float2(0.f, 0.f);
         const uint32_t raw_thread = sbase + Sh::OFF_RAW + sl * (kSubTile * C * SB) + ph * SB;
-        float2 *ybuf = reinterpret_cast<float2 *>(smem + Sh::OFF_Y);
+        float2 *ybuf = reinterpret_cast<float2 *>(smem + Sh::OFF_Y) + sl * YS + ph + (ph >> 4);
 
         for (int j = 0; j <= n_sub; ++j) {
             const int s = j % kRawStages;
             mbar_wait(bar_raw_full + 8 * s, (uint32_t)(j / kRawStages) & 1u);
             const int jj = j - 1;                         // real sub-tile index (j = 0 is the warm-up)
-            const int yb = jj & 1;
-            if (jj >= 0) mbar_wait(bar_y_empty + 8 * yb, ((uint32_t)(jj >> 1) & 1u) ^ 1u);
-            float2 *yrow = ybuf + (size_t)yb * (Sh::Y_BUF / 8) + sl * YS + ph;
+            const int yb = jj % kYBufs;
             const uint32_t raw = raw_thread + s * Sh::RAW_STAGE;
+            // The warm-up sub-tile (jj < 0) also stores: into buffer 0, which nobody reads before the first real
+            // sub-tile has overwritten it and signalled y_full.
+            if (jj >= 0) mbar_wait(bar_y_empty + 8 * yb, ((uint32_t)(jj / kYBufs) & 1u) ^ 1u);
+            float2 *yrow = ybuf + (size_t)(jj >= 0 ? yb : 0) * (Sh::Y_BUF / 8);
 #pragma unroll
-            for (int i = 0; i < kSubTile; ++i) {
-                uint32_t w;
-                if (SB == 4) asm volatile("ld.shared.b32 %0, [%1];" : "=r"(w) : "r"(raw + i * C * SB));
-                else {
-                    unsigned short h;
-                    asm volatile("ld.shared.b16 %0, [%1];" : "=h"(h) : "r"(raw + i * C * SB));
-                    w = h;
+            for (int half = 0; half < 2; ++half) {
+                uint32_t rw[kSubTile / 2];                // 8 raw words per batch: one shared-memory latency, not 8
+#pragma unroll
+                for (int i = 0; i < kSubTile / 2; ++i) {
+                    const uint32_t addr = raw + (half * 8 + i) * C * SB;
+                    if (SB == 4) asm volatile("ld.shared.b32 %0, [%1];" : "=r"(rw[i]) : "r"(addr));
+                    else {
+                        unsigned short h;
+                        asm volatile("ld.shared.b16 %0, [%1];" : "=h"(h) : "r"(addr));
+                        rw[i] = h;
+                    }
                 }
-                const float2 x = unpack_sample<BITS>(w);
-                // sample u contributes w[k] x[u] to output u + k (slot (u + k) mod 16); output u is then complete
 #pragma unroll
-                for (int k = 0; k < kTaps; ++k)
-                    acc[(i + k) & 15] = __ffma2_rn(make_float2(wk[k], wk[k]), x, acc[(i + k) & 15]);
-                if (jj >= 0) yrow[i * (SPC * YS)] = acc[i];
-                acc[i] = make_float2(0.f, 0.f);
+                for (int ii = 0; ii < kSubTile / 2; ++ii) {
+                    const int i = half * 8 + ii;
+                    const float2 x = unpack_sample<BITS>(rw[ii]);
+                    // sample u contributes w[k] x[u] to output u + k (slot (u + k) mod 16); output u is then complete
+#pragma unroll
+                    for (int k = 0; k < kTaps - 1; ++k)
+                        acc[(i + k) & 15] = __ffma2_rn(make_float2(wk[k], wk[k]), x, acc[(i + k) & 15]);
+                    yrow[i * (SPC * YS)] = acc[i];
+                    acc[(i + 15) & 15] = __fmul2_rn(make_float2(wk[15], wk[15]), x);   // first tap of output u + 15
+                }
             }
             __syncwarp();
             if (lane == 0) {
@@ -282,133 +312,140 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a) {
         }
     } else {
         // ------------------------------------------------------------------ FFT, rotate, transpose (steps a3-a7)
-        const int ft = tid - kFirThreads;                 // 0..255
+        // Group g takes the pairs of sub-tiles (32 spectra = half a k-tile) pp = g, g + 2, ...
+        const int g = (tid - kFirThreads) / kFftGroup;
+        const int ft = (tid - kFirThreads) % kFftGroup;   // 0..255
         const int tl = ft >> 4;                           // spectrum of the sub-tile
         const int sl = (ft & 15) / R, r = (ft & 15) % R;  // stream of the CTA, residue of the channel index
-        float2 twr[16];                                   // W_C^{r k1}
-        if (R > 1) {
-#pragma unroll
-            for (int k = 0; k < 16; ++k) {
-                float sn, cs;
-                sincospif(-2.0f * (float)(r * k) / (float)C, &sn, &cs);
-                twr[k] = make_float2(cs, sn);
-            }
-        }
-        const float2 *ybuf = reinterpret_cast<const float2 *>(smem + Sh::OFF_Y);
-        float2 *xch = reinterpret_cast<float2 *>(smem + Sh::OFF_XCH) + (ft >> 4) * Sh::XCH_GROUP;
+        float2 *ybase = reinterpret_cast<float2 *>(smem + Sh::OFF_Y) + (tl * SPC + sl) * YS;
         const float2 *wtab = reinterpret_cast<const float2 *>(smem + Sh::OFF_WTAB) + sl * C;
-        unsigned char *stg = smem + Sh::OFF_STG;
+        const float2 *twr = reinterpret_cast<const float2 *>(smem + Sh::OFF_TW) + r;   // W_C^{r k1} at [k1 * R]
+        unsigned char *stg = smem + Sh::OFF_STG + g * Sh::STG;
         unsigned char *zsub = a.z + (size_t)bl * a.z_subband_bytes;
-        // flush role: this thread owns staging row ft = (stream fsl, channel fc)
-        const int fsl = ft / C, fc = ft - fsl * C;
-        const int fm = m0 + fsl;
+        // flush items of this thread (TENSOR): staging row it * 64 + (ft >> 2) = (stream, channel), 8 spectra
+        // tg = ft & 3.  Row (channel c, k-tile kt, plane, input m) of z starts at ((c n_kt + kt) 2 Mpad + m) 128;
+        // the 16-byte chunk q of that row sits at q ^ (m & 7) (cobalt_internal.h), q = 4 (sub >> 1) + tg.
+        const size_t plane_stride = (size_t)a.Mpad * 128;
+        size_t fl_off[4];
+        bool fl_ok[4];
+#pragma unroll
+        for (int it = 0; it < 4; ++it) {
+            const int row = it * (kFftGroup / 4) + (ft >> 2);
+            const int fsl = row / C, fc = row - fsl * C, fm = m0 + fsl;
+            fl_ok[it] = fm < a.M;
+            fl_off[it] = ((size_t)fc * a.n_kt * 2 * a.Mpad + fm) * 128 + ((((ft & 3) ^ (fm & 3)) << 4) | (fm & 4) << 4);
+        }
 
-        for (int jj = 0; jj < n_sub; ++jj) {
-            const int yb = jj & 1;
-            const int kt = kt0 + (jj >> 2), sub = jj & 3;
-            const long long t_base = (long long)kt * kKTile + sub * kSubTile;
-            mbar_wait(bar_y_full + 8 * yb, (uint32_t)(jj >> 1) & 1u);
-            float2 o[16];
-            {
-                float2 v[16];
-                const float2 *yrow = ybuf + (size_t)yb * (Sh::Y_BUF / 8) + (tl * SPC + sl) * YS + r;
+        for (int pp = g; pp < n_sub / 2; pp += kFftGroups) {
+#pragma unroll 1
+            for (int h = 0; h < 2; ++h) {
+                const int jj = 2 * pp + h;
+                const int yb = jj % kYBufs;
+                const int kt = kt0 + (jj >> 2), sub = jj & 3;
+                const long long t_base = (long long)kt * kKTile + sub * kSubTile;
+                float2 *y = ybase + (size_t)yb * (Sh::Y_BUF / 8);
+                mbar_wait(bar_y_full + 8 * yb, (uint32_t)(jj / kYBufs) & 1u);
+                float2 o[16];
 #pragma unroll
-                for (int q = 0; q < 16; ++q) v[q] = yrow[R * q];
-                dft16(v);
-                __syncwarp();
-                if (lane == 0) mbar_arrive(bar_y_empty + 8 * yb);
-                if (R == 1) {
+                for (int q = 0; q < 16; ++q) o[q] = y[r + R * q + ((r + R * q) >> 4)];
+                dft16(o);                                 // X[k] at o[dft16_pos(k)]
+                if (R == 16) {
+                    // twiddle, exchange in place (each thread rewrites the 16 slots it read), radix-16 pass
 #pragma unroll
-                    for (int k = 0; k < 16; ++k) o[k] = v[dft16_pos(k)];
-                } else {
-                    o[0] = v[0];
+                    for (int k = 0; k < 16; ++k)
+                        y[r + 17 * k] = k ? cmul_tab2(o[dft16_pos(k)], twr[k * R]) : o[0];   // A[r][k1] W_C^{r k1}
+                    __syncwarp();
 #pragma unroll
-                    for (int k = 1; k < 16; ++k) o[k] = cmul(v[dft16_pos(k)], twr[k]);   // A[r][k1] W_C^{r k1}
-                }
-            }
-            if (R == 16) {
+                    for (int r2 = 0; r2 < 16; ++r2) o[r2] = y[r2 + 17 * r];
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(bar_y_empty + 8 * yb);
+                    dft16(o);                             // channel r + 16 k2 at o[dft16_pos(k2)]
+                } else if (R == 4) {
 #pragma unroll
-                for (int k = 0; k < 16; ++k) xch[r * 17 + k] = o[k];
-                __syncwarp();
-                float2 v[16];
+                    for (int k = 0; k < 16; ++k)
+                        y[r + 4 * k + (k >> 2)] = k ? cmul_tab2(o[dft16_pos(k)], twr[k * R]) : o[0];
+                    __syncwarp();
 #pragma unroll
-                for (int r2 = 0; r2 < 16; ++r2) v[r2] = xch[r2 * 17 + r];
-                dft16(v);
+                    for (int a4 = 0; a4 < 4; ++a4) {
+                        const int k1 = 4 * r + a4;         // channel k1 + 16 k2 at o[4 a4 + k2]
 #pragma unroll
-                for (int k2 = 0; k2 < 16; ++k2) o[k2] = v[dft16_pos(k2)];   // channel r + 16 k2
-                __syncwarp();
-            } else if (R == 4) {
-                float2 *xg = xch + sl * 68;
-#pragma unroll
-                for (int k = 0; k < 16; ++k) xg[k * 4 + r + (k >> 2)] = o[k];
-                __syncwarp();
-#pragma unroll
-                for (int a4 = 0; a4 < 4; ++a4) {
-                    const int k1 = 4 * r + a4;
-                    float2 c0 = xg[k1 * 4 + 0 + r];
-                    float2 c1 = xg[k1 * 4 + 1 + r];
-                    float2 c2 = xg[k1 * 4 + 2 + r];
-                    float2 c3 = xg[k1 * 4 + 3 + r];
-                    dft4(c0, c1, c2, c3);
-                    o[a4 * 4 + 0] = c0;   // channel k1 + 16 k2
-                    o[a4 * 4 + 1] = c1;
-                    o[a4 * 4 + 2] = c2;
-                    o[a4 * 4 + 3] = c3;
-                }
-                __syncwarp();
-            }
-            // steps a5-a7: rotate * bandpass, convert, stage transposed
-            const bool live = t_base + tl < a.n_t;        // padding spectra of the last k-tile are exact zeros
-#pragma unroll
-            for (int i = 0; i < 16; ++i) {
-                int j;
-                if (R == 16) j = r + 16 * i;
-                else if (R == 4) j = 4 * r + (i >> 2) + 16 * (i & 3);
-                else j = i;
-                float2 zz = cmul(o[i], wtab[j]);
-                if (!live) zz = make_float2(0.f, 0.f);
-                if (TENSOR) {
-                    const __half2 h = __floats2half2_rn(zz.x, zz.y);
-                    *reinterpret_cast<__half2 *>(stg + (sl * C + j) * Sh::STG_ROW + tl * 4) = h;
-                } else {
-                    *reinterpret_cast<float2 *>(stg + (sl * C + j) * Sh::STG_ROW + tl * 8) = zz;
-                }
-            }
-            bar_sync_named(1, kFftThreads);               // staging complete
-            if (fm < a.M) {
-                if (TENSOR) {
-                    // 16 spectra of (stream, channel): words (re | im << 16) -> one 16-byte chunk per plane and 8 spectra
-                    uint32_t w[16];
-#pragma unroll
-                    for (int i = 0; i < 8; ++i) {
-                        const uint2 v = *reinterpret_cast<const uint2 *>(stg + ft * Sh::STG_ROW + i * 8);
-                        w[2 * i] = v.x;
-                        w[2 * i + 1] = v.y;
+                        for (int r2 = 0; r2 < 4; ++r2) o[4 * a4 + r2] = y[4 * k1 + r2 + r];
                     }
-                    unsigned char *row = zsub + (((size_t)fc * a.n_kt + kt) * 2 * a.Mpad + fm) * 128;
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(bar_y_empty + 8 * yb);
 #pragma unroll
-                    for (int half = 0; half < 2; ++half) {
+                    for (int a4 = 0; a4 < 4; ++a4) dft4(o[4 * a4], o[4 * a4 + 1], o[4 * a4 + 2], o[4 * a4 + 3]);
+                } else {
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(bar_y_empty + 8 * yb);
+                }
+                // steps a5-a7: rotate * bandpass, convert, stage transposed.  Spectra t >= n_t (padding of
+                // the last k-tile) are staged as exact zeros: the rotation table is replaced by zero.
+                const bool live = t_base + tl < a.n_t;
+                const int ts = TENSOR ? h * kSubTile + tl : tl;   // spectrum slot in the staging row
+#pragma unroll
+                for (int i = 0; i < 16; ++i) {
+                    int j, oi;                            // channel index, register holding it
+                    if (R == 16) { j = r + 16 * i; oi = dft16_pos(i); }
+                    else if (R == 4) { j = 4 * r + (i >> 2) + 16 * (i & 3); oi = i; }
+                    else { j = i; oi = dft16_pos(i); }
+                    float2 zz = cmul_tab2(o[oi], wtab[j]);
+                    if (TENSOR) {
+                        uint32_t hv;
+                        {
+                            const __half2 t2 = __floats2half2_rn(zz.x, zz.y);
+                            hv = *reinterpret_cast<const uint32_t *>(&t2);
+                        }
+                        if (!live) hv = 0u;
+                        *reinterpret_cast<uint32_t *>(stg + (sl * C + j) * Sh::STG_ROW + ts * 4) = hv;
+                    } else {
+                        if (!live) zz = make_float2(0.f, 0.f);
+                        *reinterpret_cast<float2 *>(stg + (sl * C + j) * Sh::STG_ROW + ts * 8) = zz;
+                    }
+                }
+                if (TENSOR && h == 0) continue;           // flush every 32 spectra
+                bar_sync_named(1 + g, kFftGroup);         // staging complete
+                if (TENSOR) {
+                    // item = (row = (stream, channel), tg = 8 spectra): 8 words (re | im << 16) -> one 16-byte
+                    // chunk per plane; 4 consecutive lanes write one 64-byte run of a 128-byte row
+                    unsigned char *zkt = zsub + (size_t)kt * 2 * plane_stride;
+                    const size_t half = (size_t)(sub >> 1) << 6;   // which 64 bytes of the row these 32 spectra are
+#pragma unroll
+                    for (int it = 0; it < 4; ++it) {
+                        if (!fl_ok[it]) continue;
+                        const unsigned char *src = stg + (it * (kFftGroup / 4) + (ft >> 2)) * Sh::STG_ROW + (ft & 3) * 32;
+                        uint32_t w[8];
+#pragma unroll
+                        for (int i = 0; i < 4; ++i) {
+                            const uint2 v = *reinterpret_cast<const uint2 *>(src + i * 8);
+                            w[2 * i] = v.x;
+                            w[2 * i + 1] = v.y;
+                        }
                         uint4 re, im;
-                        re.x = __byte_perm(w[8 * half + 0], w[8 * half + 1], 0x5410);
-                        re.y = __byte_perm(w[8 * half + 2], w[8 * half + 3], 0x5410);
-                        re.z = __byte_perm(w[8 * half + 4], w[8 * half + 5], 0x5410);
-                        re.w = __byte_perm(w[8 * half + 6], w[8 * half + 7], 0x5410);
-                        im.x = __byte_perm(w[8 * half + 0], w[8 * half + 1], 0x7632);
-                        im.y = __byte_perm(w[8 * half + 2], w[8 * half + 3], 0x7632);
-                        im.z = __byte_perm(w[8 * half + 4], w[8 * half + 5], 0x7632);
-                        im.w = __byte_perm(w[8 * half + 6], w[8 * half + 7], 0x7632);
-                        const int q = ((2 * sub + half) ^ (fm & 7)) << 4;      // pre-swizzled chunk (cobalt_internal.h)
-                        *reinterpret_cast<uint4 *>(row + q) = re;
-                        *reinterpret_cast<uint4 *>(row + (size_t)a.Mpad * 128 + q) = im;
+                        re.x = __byte_perm(w[0], w[1], 0x5410);
+                        re.y = __byte_perm(w[2], w[3], 0x5410);
+                        re.z = __byte_perm(w[4], w[5], 0x5410);
+                        re.w = __byte_perm(w[6], w[7], 0x5410);
+                        im.x = __byte_perm(w[0], w[1], 0x7632);
+                        im.y = __byte_perm(w[2], w[3], 0x7632);
+                        im.z = __byte_perm(w[4], w[5], 0x7632);
+                        im.w = __byte_perm(w[6], w[7], 0x7632);
+                        unsigned char *rowp = zkt + (fl_off[it] ^ half);
+                        *reinterpret_cast<uint4 *>(rowp) = re;
+                        *reinterpret_cast<uint4 *>(rowp + plane_stride) = im;
                     }
                 } else {
-                    float2 *dst = reinterpret_cast<float2 *>(zsub) + ((size_t)fc * a.M + fm) * a.n_t + t_base;
+                    const int fsl = ft / C, fc = ft - fsl * C;    // this thread owns staging row ft = (stream, channel)
+                    const int fm = m0 + fsl;
+                    if (fm < a.M) {
+                        float2 *dst = reinterpret_cast<float2 *>(zsub) + ((size_t)fc * a.M + fm) * a.n_t + t_base;
 #pragma unroll
-                    for (int i = 0; i < 16; ++i)
-                        if (t_base + i < a.n_t) dst[i] = *reinterpret_cast<const float2 *>(stg + ft * Sh::STG_ROW + i * 8);
+                        for (int i = 0; i < 16; ++i)
+                            if (t_base + i < a.n_t) dst[i] = *reinterpret_cast<const float2 *>(stg + ft * Sh::STG_ROW + i * 8);
+                    }
                 }
+                bar_sync_named(1 + g, kFftGroup);         // staging drained
             }
-            bar_sync_named(1, kFftThreads);               // staging drained
         }
     }
 }
