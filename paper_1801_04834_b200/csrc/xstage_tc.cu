@@ -19,7 +19,6 @@
 // allocator + single-thread MMA issuer, warps 2-5 = epilogue (tcgen05.ld -> triangular baseline
 // index -> coalesced 16-byte stores of (re, im) pairs).
 #include "cobalt_internal.h"
-#include <cstdlib>
 
 namespace cobalt {
 
@@ -37,7 +36,6 @@ struct XArgs {
     size_t z_subband_bytes;
     long long n_bl;
     int C, M, Mpad, n_kt, jobs_per_channel, total_jobs, stages, stage_bytes;
-    int dbg;   // TEMP experiment knobs
 };
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -102,6 +100,19 @@ __device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&v)[16]) {
           "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
         : "r"(taddr));
 }
+// One lane of a fully converged warp; ptxas then treats the guarded region as single-threaded and emits the
+// UTCHMMA / UBLKCP sequence without a per-instruction ELECT loop.
+__device__ __forceinline__ bool elect_one() {
+    uint32_t pred;
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "elect.sync _|p, 0xffffffff;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t"
+        "}"
+        : "=r"(pred));
+    return pred != 0;
+}
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 
 __global__ void __launch_bounds__(kThreads, 1) xstage_tc_kernel(const XArgs a) {
@@ -141,31 +152,28 @@ __global__ void __launch_bounds__(kThreads, 1) xstage_tc_kernel(const XArgs a) {
 
     if (warp == 0) {
         // ------------------------------------------------------------------ producer
-        if (lane == 0) {
+        if (elect_one()) {
             int s = 0;
             uint32_t ph = 0;
+            const size_t kt_bytes = (size_t)2 * a.Mpad * 128, pl_bytes = (size_t)a.Mpad * 128;
             for (int jid = blockIdx.x; jid < a.total_jobs; jid += gridDim.x) {
                 const int jl = jid % a.jobs_per_channel;
                 const int prob = jid / a.jobs_per_channel;           // subband-of-chunk * C + channel
-                const XJob &job = a.jobs[jl];
                 const int bl = prob / a.C, c = prob - bl * a.C;
-                const unsigned char *zc = a.z + (size_t)bl * a.z_subband_bytes + (size_t)c * a.n_kt * 2 * a.Mpad * 128;
-                const int n0 = job.ld_nrows[0], n1 = job.ld_nrows[1];
-                const uint32_t plane_bytes = (uint32_t)(n0 + n1) * 128;
-                for (int kt = 0; kt < a.n_kt; ++kt) {
+                const int r0 = a.jobs[jl].ld_row[0], r1 = a.jobs[jl].ld_row[1];
+                const uint32_t b0 = (uint32_t)a.jobs[jl].ld_nrows[0] * 128, b1 = (uint32_t)a.jobs[jl].ld_nrows[1] * 128;
+                const unsigned char *src = a.z + (size_t)bl * a.z_subband_bytes + (size_t)c * a.n_kt * kt_bytes;
+                const uint32_t plane_bytes = b0 + b1;
+                for (int kt = 0; kt < a.n_kt; ++kt, src += kt_bytes) {
                     mbar_wait(bar_base + 8 * (16 + s), ph ^ 1);
                     const uint32_t full = bar_base + 8 * s;
                     const uint32_t dst = stage_base + (uint32_t)s * a.stage_bytes;
-                    if (a.dbg & 2) { mbar_arrive(full); if (++s == stages) { s = 0; ph ^= 1; } continue; }
                     mbar_expect_tx(full, 2 * plane_bytes);
-                    const unsigned char *src = zc + (size_t)kt * 2 * a.Mpad * 128;
 #pragma unroll
                     for (int plane = 0; plane < 2; ++plane) {
-                        const unsigned char *sp = src + (size_t)plane * a.Mpad * 128;
-                        bulk_g2s(dst + plane * plane_bytes, sp + (size_t)job.ld_row[0] * 128, (uint32_t)n0 * 128, full);
-                        if (n1 > 0)
-                            bulk_g2s(dst + plane * plane_bytes + n0 * 128, sp + (size_t)job.ld_row[1] * 128,
-                                     (uint32_t)n1 * 128, full);
+                        const unsigned char *sp = src + (size_t)plane * pl_bytes;
+                        bulk_g2s(dst + plane * plane_bytes, sp + (size_t)r0 * 128, b0, full);
+                        if (b1 > 0) bulk_g2s(dst + plane * plane_bytes + b0, sp + (size_t)r1 * 128, b1, full);
                     }
                     if (++s == stages) {
                         s = 0;
@@ -176,34 +184,50 @@ __global__ void __launch_bounds__(kThreads, 1) xstage_tc_kernel(const XArgs a) {
         }
     } else if (warp == 1) {
         // ------------------------------------------------------------------ MMA issuer
-        if (lane == 0) {
+        if (elect_one()) {
             int s = 0;
             uint32_t ph = 0, it = 0;
+            // shared-memory descriptor of byte offset 0 of stage 0; rows / stages / k-steps only add to the
+            // 14-bit start-address field (units of 16 bytes; shared memory is < 256 KB, so it cannot carry out)
+            const uint64_t desc0 = make_smem_desc(stage_base);
+            const uint32_t stage_units = (uint32_t)a.stage_bytes >> 4;
             for (int jid = blockIdx.x; jid < a.total_jobs; jid += gridDim.x, ++it) {
-                const XJob &job = a.jobs[jid % a.jobs_per_channel];
-                const uint32_t plane_bytes = (uint32_t)(job.ld_nrows[0] + job.ld_nrows[1]) * 128;
+                const XJob *job = a.jobs + jid % a.jobs_per_channel;
+                const int n_groups = job->n_groups;
+                const uint32_t plane_units = (uint32_t)(job->ld_nrows[0] + job->ld_nrows[1]) * 8;
+                uint32_t g_a[kMaxMmaGroups], g_b[kMaxMmaGroups], g_d[kMaxMmaGroups], g_n[kMaxMmaGroups];
+                uint32_t g_pos[kMaxMmaGroups], g_neg[kMaxMmaGroups];
+#pragma unroll
+                for (int g = 0; g < kMaxMmaGroups; ++g) {
+                    const XMmaGroup &grp = job->g[g < n_groups ? g : 0];
+                    g_a[g] = (uint32_t)grp.a_row * 8;
+                    g_b[g] = (uint32_t)grp.b_row * 8;
+                    g_n[g] = (uint32_t)grp.n;
+                    g_d[g] = tmem_base + (uint32_t)grp.tmem_col;
+                    g_pos[g] = make_idesc(grp.n, 0);
+                    g_neg[g] = make_idesc(grp.n, 1);
+                }
                 mbar_wait(tmem_empty, (it & 1) ^ 1);       // epilogue has drained the accumulators
                 tc_fence_after();
                 for (int kt = 0; kt < a.n_kt; ++kt) {
                     mbar_wait(bar_base + 8 * s, ph);
                     tc_fence_after();
-                    const uint32_t st = stage_base + (uint32_t)s * a.stage_bytes;
-                    for (int g = 0; g < ((a.dbg & 1) ? 0 : ((a.dbg & 8) ? 1 : job.n_groups)); ++g) {
-                        const XMmaGroup &grp = job.g[g];
-                        const uint64_t ar = make_smem_desc(st + grp.a_row * 128);
-                        const uint64_t ai = make_smem_desc(st + plane_bytes + grp.a_row * 128);
-                        const uint64_t br = make_smem_desc(st + grp.b_row * 128);
-                        const uint64_t bi = make_smem_desc(st + plane_bytes + grp.b_row * 128);
-                        const uint32_t d_re = tmem_base + grp.tmem_col, d_im = d_re + grp.n;
-                        const uint32_t id_pos = make_idesc(grp.n, 0), id_neg = make_idesc(grp.n, 1);
+                    const uint64_t st = desc0 + (uint64_t)((uint32_t)s * stage_units);
 #pragma unroll
-                        for (int ks = 0; ks < kKTile / 16; ++ks) {
-                            const uint32_t acc = (kt | ks) ? 1u : 0u;
-                            const uint64_t ko = (uint64_t)(ks * 2);         // 32 bytes per k-step, >> 4
-                            tc_mma(d_re, ar + ko, br + ko, id_pos, acc);    // Re  = Zr Zr^T
-                            tc_mma(d_re, ai + ko, bi + ko, id_pos, 1u);     // Re += Zi Zi^T
-                            tc_mma(d_im, ai + ko, br + ko, id_pos, acc);    // Im  = Zi Zr^T
-                            tc_mma(d_im, ar + ko, bi + ko, id_neg, 1u);     // Im -= Zr Zi^T
+                    for (int g = 0; g < kMaxMmaGroups; ++g) {
+                        if (g < n_groups) {
+                            const uint64_t ar = st + g_a[g], ai = ar + plane_units;
+                            const uint64_t br = st + g_b[g], bi = br + plane_units;
+                            const uint32_t d_re = g_d[g], d_im = d_re + g_n[g];
+#pragma unroll
+                            for (int ks = 0; ks < kKTile / 16; ++ks) {
+                                const uint32_t acc = (kt | ks) ? 1u : 0u;
+                                const uint64_t ko = (uint64_t)(ks * 2);         // 32 bytes per k-step, >> 4
+                                tc_mma(d_re, ar + ko, br + ko, g_pos[g], acc);    // Re  = Zr Zr^T
+                                tc_mma(d_re, ai + ko, bi + ko, g_pos[g], 1u);     // Re += Zi Zi^T
+                                tc_mma(d_im, ai + ko, br + ko, g_pos[g], acc);    // Im  = Zi Zr^T
+                                tc_mma(d_im, ar + ko, bi + ko, g_neg[g], 1u);     // Im -= Zr Zi^T
+                            }
                         }
                     }
                     tc_commit(bar_base + 8 * (16 + s));    // stage free once these MMAs have read it
@@ -245,7 +269,7 @@ __global__ void __launch_bounds__(kThreads, 1) xstage_tc_kernel(const XArgs a) {
 #pragma unroll
                     for (int e = 0; e < 16; e += 2) {
                         const int b = col0 + e, k = b >> 1;
-                        if (arow < a.M && b < a.M && i <= k && !(a.dbg & 4))
+                        if (arow < a.M && b < a.M && i <= k)
                             vc[((size_t)k * (k + 1) / 2 + i) * 2 + p] =
                                 make_float4(__uint_as_float(re[e]) * inv_s2, __uint_as_float(im[e]) * inv_s2,
                                             __uint_as_float(re[e + 1]) * inv_s2, __uint_as_float(im[e + 1]) * inv_s2);
@@ -354,7 +378,6 @@ cudaError_t launch_xstage_tc(const cobalt_plan_s *p, cudaStream_t st, const void
     int max_rows = 0;
     for (const XJob &j : p->jobs) max_rows = (j.ld_nrows[0] + j.ld_nrows[1]) > max_rows ? (j.ld_nrows[0] + j.ld_nrows[1]) : max_rows;
     a.stage_bytes = max_rows * 128 * 2;
-    a.dbg = getenv("COBALT_X_DBG") ? atoi(getenv("COBALT_X_DBG")) : 0;
     cudaError_t e = cudaFuncSetAttribute(xstage_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->x_smem_bytes);
     if (e != cudaSuccess) return e;
     const int grid = a.total_jobs < p->sm_count ? a.total_jobs : p->sm_count;
