@@ -33,12 +33,14 @@ constexpr int kMaxMmaGroups = 2;   // MMA groups per X-stage job
 // One X-stage job = one set of rows of a (subband, channel) k-tile loaded to shared memory plus up
 // to kMaxMmaGroups accumulator groups computed from it (see xstage_tc.cu).
 struct XMmaGroup {
-    int a_row;      // first row of the A operand, relative to the first loaded row (128 rows used)
+    int a_row;      // first row of the A operand, relative to the first loaded row (m rows used)
     int b_row;      // first row of the B operand, relative to the first loaded row
     int n;          // number of B rows = accumulator columns (multiple of 16, <= 256)
     int tmem_col;   // first TMEM column of the Re accumulator; Im follows at tmem_col + n
     int out_row;    // global input index of A row 0
     int out_col;    // global input index of B row 0
+    int m;          // instruction M: 128, or 64 (accumulator row r then sits in TMEM lane 32 (r / 16) + r % 16)
+    int row_min;    // rows (global input index) below this are another group's job and are not stored
 };
 struct XJob {
     int ld_row[2];     // two row ranges of the [Mpad][64] block copied to smem back to back

@@ -12,11 +12,12 @@
 // accumulators; the minus sign is the instruction descriptor's negate-A bit, so no negated plane is
 // ever stored.  Only tiles on or above the station diagonal are computed: an XJob (built once per
 // plan by build_xjobs) names the rows to load and up to two accumulator groups
-//   rows [0,128) x cols [0,Mpad)  and  rows [128,Mpad) x cols [128,Mpad)        (2S <= 192)
+//   rows [0,128) x cols [0,Mpad)  (M = 128)  and  rows [Mpad-64,Mpad) x cols [128,Mpad)  (M = 64; only its
+//   rows >= 128 are stored)                                                      (2S <= 192)
 // or, for large arrays, one (128-row block) x (<= 256-column chunk) tile per job.
 //
-// Warp roles (192 threads, persistent CTAs, one per SM): warp 0 = bulk-copy producer, warp 1 = TMEM
-// allocator + single-thread MMA issuer, warps 2-5 = epilogue (tcgen05.ld -> triangular baseline
+// Warp roles (320 threads, persistent CTAs, one per SM): warp 0 = bulk-copy producer, warp 1 = TMEM
+// allocator + single-thread MMA issuer, warps 2-9 = epilogue (tcgen05.ld -> triangular baseline
 // index -> coalesced 16-byte stores of (re, im) pairs).
 #include "cobalt_internal.h"
 
@@ -24,7 +25,8 @@ namespace cobalt {
 
 namespace {
 
-constexpr int kThreads = 192;
+constexpr int kEpiWarps = 8;            // two per TMEM lane quarter, alternating 16-column chunks
+constexpr int kThreads = 64 + 32 * kEpiWarps;
 constexpr int kSlackBytes = 128 * 128;   // A operands may over-read up to 128 rows of one plane
 constexpr int kBarrierBytes = 1024;
 
@@ -55,11 +57,11 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
         asm volatile(
             "{\n\t"
             ".reg .pred p;\n\t"
-            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\t"
             "selp.u32 %0, 1, 0, p;\n\t"
             "}"
             : "=r"(done)
-            : "r"(bar), "r"(parity)
+            : "r"(bar), "r"(parity), "r"(20000u)
             : "memory");
     } while (!done);
 }
@@ -88,9 +90,9 @@ __device__ __forceinline__ void tc_mma(uint32_t d_tmem, uint64_t a_desc, uint64_
 __device__ __forceinline__ uint64_t make_smem_desc(uint32_t addr) {
     return (uint64_t)((addr >> 4) & 0x3FFFu) | (1ull << 16) | (64ull << 32) | (1ull << 46) | (2ull << 61);
 }
-// kind::f16 instruction descriptor: D = f32, A = B = f16, both K-major, M = 128.
-__device__ __forceinline__ uint32_t make_idesc(int n, int neg_a) {
-    return (1u << 4) | ((uint32_t)neg_a << 13) | ((uint32_t)(n >> 3) << 17) | ((128u >> 4) << 24);
+// kind::f16 instruction descriptor: D = f32, A = B = f16, both K-major.
+__device__ __forceinline__ uint32_t make_idesc(int m, int n, int neg_a) {
+    return (1u << 4) | ((uint32_t)neg_a << 13) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(m >> 4) << 24);
 }
 __device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&v)[16]) {
     asm volatile(
@@ -136,7 +138,7 @@ __global__ void __launch_bounds__(kThreads, 1) xstage_tc_kernel(const XArgs a) {
             mbar_init(bar_base + 8 * (16 + s), 1);
         }
         mbar_init(tmem_full, 1);
-        mbar_init(tmem_empty, 4);
+        mbar_init(tmem_empty, kEpiWarps);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == 1) {
@@ -204,8 +206,8 @@ __global__ void __launch_bounds__(kThreads, 1) xstage_tc_kernel(const XArgs a) {
                     g_b[g] = (uint32_t)grp.b_row * 8;
                     g_n[g] = (uint32_t)grp.n;
                     g_d[g] = tmem_base + (uint32_t)grp.tmem_col;
-                    g_pos[g] = make_idesc(grp.n, 0);
-                    g_neg[g] = make_idesc(grp.n, 1);
+                    g_pos[g] = make_idesc(grp.m, grp.n, 0);
+                    g_neg[g] = make_idesc(grp.m, grp.n, 1);
                 }
                 mbar_wait(tmem_empty, (it & 1) ^ 1);       // epilogue has drained the accumulators
                 tc_fence_after();
@@ -241,38 +243,57 @@ __global__ void __launch_bounds__(kThreads, 1) xstage_tc_kernel(const XArgs a) {
         }
     } else {
         // ------------------------------------------------------------------ epilogue
-        const int wq = warp & 3;                           // TMEM lane quarter this warp may access
+        // Warps 2..9: warp w reads TMEM lane quarter w % 4 (the only one it may access); the two warps of a quarter
+        // take alternate 16-column chunks.  The TMEM load of a warp's next chunk is in flight while it stores the
+        // current one.
+        const int wq = warp & 3;
+        const int half = (warp - 2) >> 2;
         const float inv_s2 = __ldg(a.scale + 2);           // undo the power-of-two operand scale (exact)
         uint32_t it = 0;
         for (int jid = blockIdx.x; jid < a.total_jobs; jid += gridDim.x, ++it) {
             const int jl = jid % a.jobs_per_channel;
             const int prob = jid / a.jobs_per_channel;
-            const XJob &job = a.jobs[jl];
+            const XJob *job = a.jobs + jl;
+            const int n_groups = job->n_groups;
             float4 *vc = reinterpret_cast<float4 *>(a.vis + (size_t)prob * a.n_bl * 4);
             mbar_wait(tmem_full, it & 1);
             tc_fence_after();
-            for (int g = 0; g < job.n_groups; ++g) {
-                const XMmaGroup &grp = job.g[g];
-                const int row0 = grp.out_row + wq * 32;    // first input index of this warp's lanes
-                const int arow = row0 + lane;
+            for (int g = 0; g < n_groups; ++g) {
+                const int gm = job->g[g].m, gn = job->g[g].n, row_min = job->g[g].row_min;
+                const int out_col = job->g[g].out_col;
+                // M = 128: accumulator row = TMEM lane; M = 64: row r in lane 32 (r / 16) + r % 16
+                const int rows_w = gm == 128 ? 32 : 16;
+                const int row0 = job->g[g].out_row + wq * rows_w;      // first input index of this warp's lanes
+                const int arow = row0 + (lane & (rows_w - 1));
+                const bool lane_ok = lane < rows_w && arow >= row_min && arow < a.M;
                 const int i = arow >> 1, p = arow & 1;
-                if (row0 >= a.M) continue;
-                for (int c0 = 0; c0 < grp.n; c0 += 16) {
-                    const int col0 = grp.out_col + c0;
-                    if (col0 >= a.M) break;
-                    if (((col0 + 15) >> 1) < (row0 >> 1)) continue;     // whole chunk below the diagonal
-                    uint32_t re[16], im[16];
-                    const uint32_t t = tmem_base + ((uint32_t)(wq * 32) << 16) + grp.tmem_col + c0;
-                    tmem_ld16(t, re);
-                    tmem_ld16(t + grp.n, im);
+                if (row0 >= a.M || row0 + rows_w <= row_min) continue;
+                const uint32_t t0 = tmem_base + ((uint32_t)(wq * 32) << 16) + job->g[g].tmem_col;
+                // chunks of this warp: c0 = 16 (2 q + half), on or above the diagonal, inside the matrix
+                int c_first = max(0, (max(row0, row_min) & ~1) - out_col) >> 4;     // first chunk touching k >= i
+                if ((c_first & 1) != half) ++c_first;
+                int c_end = (min(gn, a.M - out_col) + 15) >> 4;
+                uint32_t re[16], im[16];
+                if (c_first < c_end) {
+                    tmem_ld16(t0 + c_first * 16, re);
+                    tmem_ld16(t0 + gn + c_first * 16, im);
+                }
+                for (int c = c_first; c < c_end; c += 2) {
                     tmem_ld_wait();
+                    float4 v[8];
 #pragma unroll
-                    for (int e = 0; e < 16; e += 2) {
-                        const int b = col0 + e, k = b >> 1;
-                        if (arow < a.M && b < a.M && i <= k)
-                            vc[((size_t)k * (k + 1) / 2 + i) * 2 + p] =
-                                make_float4(__uint_as_float(re[e]) * inv_s2, __uint_as_float(im[e]) * inv_s2,
-                                            __uint_as_float(re[e + 1]) * inv_s2, __uint_as_float(im[e + 1]) * inv_s2);
+                    for (int e = 0; e < 8; ++e)
+                        v[e] = make_float4(__uint_as_float(re[2 * e]) * inv_s2, __uint_as_float(im[2 * e]) * inv_s2,
+                                           __uint_as_float(re[2 * e + 1]) * inv_s2, __uint_as_float(im[2 * e + 1]) * inv_s2);
+                    if (c + 2 < c_end) {
+                        tmem_ld16(t0 + (c + 2) * 16, re);
+                        tmem_ld16(t0 + gn + (c + 2) * 16, im);
+                    }
+                    const int col0 = out_col + c * 16;
+#pragma unroll
+                    for (int e = 0; e < 8; ++e) {
+                        const int b = col0 + 2 * e, k = b >> 1;
+                        if (lane_ok && b < a.M && i <= k) vc[((size_t)k * (k + 1) / 2 + i) * 2 + p] = v[e];
                     }
                 }
             }
@@ -310,11 +331,13 @@ void build_xjobs(cobalt_plan_s *p) {
         j.ld_row[1] = 0;
         j.ld_nrows[1] = 0;
         j.n_groups = 1;
-        j.g[0] = XMmaGroup{0, 0, Mpad, 0, 0, 0};
+        j.g[0] = XMmaGroup{0, 0, Mpad, 0, 0, 0, 128, 0};
         int cols = 2 * Mpad;
         if (Mpad > 128) {
             j.n_groups = 2;
-            j.g[1] = XMmaGroup{128, 128, Mpad - 128, 2 * Mpad, 128, 128};
+            // rows [128, Mpad) x columns [128, Mpad) as an M = 64 instruction over the last 64 rows (an M = 128
+            // instruction with N <= 64 is bound by its 4 KB A-operand read, M = 64 reads half of that)
+            j.g[1] = XMmaGroup{Mpad - 64, 128, Mpad - 128, 2 * Mpad, Mpad - 64, 128, 64, 128};
             cols += 2 * (Mpad - 128);
         }
         j.tmem_cols = pow2_cols(cols);
@@ -336,13 +359,13 @@ void build_xjobs(cobalt_plan_s *p) {
                     j.ld_nrows[0] = na > n ? na : n;
                     j.ld_row[1] = 0;
                     j.ld_nrows[1] = 0;
-                    j.g[0] = XMmaGroup{0, 0, n, 0, r0, c0};
+                    j.g[0] = XMmaGroup{0, 0, n, 0, r0, c0, na <= 64 ? 64 : 128, r0};
                 } else {
                     j.ld_row[0] = r0;
                     j.ld_nrows[0] = na;
                     j.ld_row[1] = c0;
                     j.ld_nrows[1] = n;
-                    j.g[0] = XMmaGroup{0, na, n, 0, r0, c0};
+                    j.g[0] = XMmaGroup{0, na, n, 0, r0, c0, na <= 64 ? 64 : 128, r0};
                 }
                 j.tmem_cols = pow2_cols(2 * n);
                 p->jobs.push_back(j);
