@@ -343,3 +343,20 @@ def test_p13_noise_power_and_correlation_coefficient(oracle):
         assert np.all(np.abs(rho - 0.1) < 4.0 / np.sqrt(n_t))
         rho_xy = np.abs(v[:, 0, 1]) / np.sqrt(aii[:, 0, 0].real * akk[:, 1, 1].real)
         assert np.all(rho_xy < 4.5 / np.sqrt(n_t))                   # independent pols: only noise
+
+
+# ------------------------------------------------------------------ frozen tiny case (tests/golden/)
+def test_golden_tiny_case_is_reproduced(oracle):
+    """The oracle still gives the values frozen by tests/golden/make_golden.py (which calls only the oracle)."""
+    import os
+    import sys
+
+    here = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+    sys.path.insert(0, here)
+    import make_golden as mg
+
+    x = np.loadtxt(os.path.join(here, "tiny_fx_input.txt"), dtype=np.int64).astype(np.int16).reshape(mg.S, 2, mg.N, 2)
+    assert np.array_equal(x, mg.inputs())
+    exp = np.loadtxt(os.path.join(here, "tiny_fx_expected.txt")).view(np.complex128).reshape(mg.C, 3, 2, 2)
+    vis = oracle.process_subband(x, mg.C, mg.DELAYS, mg.BANDPASS, oracle.default_subband_frequency(0))
+    assert np.max(np.abs(vis - exp)) <= 1e-9 * np.max(np.abs(exp))

@@ -306,3 +306,22 @@ def test_fp16_scale_follows_bandpass_gain(cobalt, oracle, dev, gain):
     vg = _run_gpu(cobalt, cfg, data, cobalt.COBALT_MODE_TENSOR_FP16, dev)
     vo = _run_oracle(oracle, cfg, data)
     _assert_parity(vg[0], vo[0], True, f"bandpass gain {gain}")
+
+
+def test_golden_tiny_case_on_gpu(cobalt, dev):
+    """The frozen oracle values of tests/golden/ (written by the oracle alone) against both GPU modes."""
+    import os
+    import sys
+
+    here = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+    sys.path.insert(0, here)
+    import make_golden as mg
+
+    x = np.loadtxt(os.path.join(here, "tiny_fx_input.txt"), dtype=np.int64).astype(np.int16).reshape(1, mg.S, 2, mg.N, 2)
+    exp = np.loadtxt(os.path.join(here, "tiny_fx_expected.txt")).view(np.complex128).reshape(1, mg.C, 3, 2, 2)
+    for mode, tensor in ((cobalt.COBALT_MODE_EXACT_FP32, False), (cobalt.COBALT_MODE_TENSOR_FP16, True)):
+        with cobalt.Correlator(mg.S, 1, mg.C, mg.N, 16, mode=mode) as cor:
+            vis = cor.process(torch.from_numpy(x).to(dev), torch.from_numpy(mg.DELAYS).to(dev),
+                              torch.from_numpy(mg.BANDPASS.astype(np.float32)).to(dev))
+            torch.cuda.synchronize()
+        _assert_parity(vis.cpu().numpy(), exp, tensor, f"golden tiny case, tensor={tensor}")
