@@ -2,6 +2,7 @@
 // Nothing here is part of the ABI (see include/cobalt.h) and nothing here is shared with oracle/.
 #pragma once
 
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <cuda_fp16.h>
 
@@ -17,6 +18,9 @@ constexpr int kTaps = 16;          // P:L360 FIR filter; BASELINE.json: 16-tap
 constexpr int kSubTile = 16;       // spectra per FIR->FFT hand-over
 constexpr int kKTile = 64;         // spectra per X-stage K tile (= one 128-byte fp16 row)
 constexpr int kMaxMmaGroups = 2;   // MMA groups per X-stage job
+constexpr int kStoreTile = 32;     // spectra per F-stage tensor store (half a k-tile row)
+// streams (rows m) per F-stage tensor-store box: the CTA's 256 / C streams, at most 4 (all with the same m >> 2)
+constexpr int kStoreBoxStreams(int C) { return 256 / C < 4 ? 256 / C : 4; }
 
 // ---------------------------------------------------------------------------------------------
 // Layout of the channelised intermediate ("z", step a7, "transposes data on write-back").
@@ -74,6 +78,7 @@ struct cobalt_plan_s {
     float *d_scale = nullptr;          // {s, 1/s, 1/s^2}: power-of-two scale of the fp16 intermediate (1 in EXACT mode)
     float amp_max = 0.f;               // worst-case |F| for full-scale input: sum|g| * sqrt(2) * 2^(bits-1)
     void *d_z = nullptr;               // intermediate of one chunk (layout per mode)
+    CUtensorMap zmap;                  // TENSOR mode: d_z as (spectrum-in-k-tile, chunk subband * C + channel, plane, row m, k-tile)
     size_t z_subband_bytes = 0;
     std::vector<cobalt::XJob> jobs;    // X-stage jobs of one (subband, channel)
     cobalt::XJob *d_jobs = nullptr;

@@ -121,34 +121,47 @@ __device__ __forceinline__ void bar_sync_named(int id, int threads) {
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(threads) : "memory");
 }
 
-// Thread roles: warps 0-7 FIR, warps 8-15 / 16-23 the two FFT groups, warp 24 the producer.
-constexpr int kFirThreads = 256, kFftGroup = 256, kFftGroups = 2;
-constexpr int kProducerWarp = (kFirThreads + kFftGroups * kFftGroup) / 32;
-constexpr int kFThreads = kFirThreads + kFftGroups * kFftGroup + 32;
+// Thread roles: warps 0-7 FIR, warps 8-15 FFT (two teams of four warps taking alternate sub-tiles), warp 16 the
+// bulk-copy producer, warp 17 the tensor-store issuer.
+constexpr int kFirThreads = 256, kFftThreads = 256, kFftTeam = 128, kFftTeams = 2;
+constexpr int kProducerWarp = (kFirThreads + kFftThreads) / 32;
+constexpr int kStoreWarp = kProducerWarp + 1;
+constexpr int kFThreads = kFirThreads + kFftThreads + 64;
 constexpr int kRawStages = 3;      // ring of raw sub-tiles (bulk copies in flight)
 constexpr int kYBufs = 3;          // ring of FIR-output sub-tiles
+constexpr int kStgTile = 32;       // spectra per staged output tile (= one tensor store per box)
+constexpr int kStgBufs = 2;
 
 template <int C, int BITS, bool TENSOR>
 struct FShape {
     static constexpr int SB = BITS == 16 ? 4 : 2;          // bytes per complex sample
     static constexpr int SPC = 256 / C;                    // streams per CTA
     static constexpr int R = C / 16;                       // threads per spectrum in the FFT
-    // FIR-output tile [16 spectra][SPC streams][YS] float2; branch ph sits at ph + (ph >> 4) so that the
-    // radix-16 pass, the in-place exchange and the radix-R pass are all free of bank conflicts
-    static constexpr int YS = C + R;
+    // FIR-output tile [16 spectra][SPC streams][YS] float2.
+    //   C = 256: branch ph = r + 16 q sits at 18 r + q, so that the FFT thread r reads its 16 inputs, and rewrites
+    //            them in the in-place exchange, as 16-byte pairs, conflict free; the FIR lanes are permuted to match.
+    //   C < 256: branch ph sits at ph + (ph >> 4).
+    static constexpr int YS = R == 16 ? 16 * 18 : C + R;
     static constexpr int RAW_STAGE = kSubTile * 256 * SB;  // bytes: [SPC][16 rows][C] samples
     static constexpr int Y_BUF = kSubTile * SPC * YS * 8;  // bytes
-    // staging of the transposed output, one per FFT group: TENSOR: 32 spectra of (re | im << 16) words
-    // + 2 pad words per (stream, channel) row; EXACT: 16 spectra of float2 + 1 pad
-    static constexpr int STG_ROW = TENSOR ? 34 * 4 : 17 * 8;
-    static constexpr int STG = 256 * STG_ROW;
-    static constexpr int OFF_BAR = 0;                      // 2 kRawStages + 2 kYBufs mbarriers
-    static constexpr int OFF_RAW = 128;
+    // TENSOR: staged output tile = kStgTile spectra of every (stream, channel) of the CTA as fp16 planes, laid out
+    // as the shared-memory side of the tensor store: boxes of [SPB streams][2 planes][C channels][32 spectra]
+    // (64-byte rows), 64-byte swizzled.
+    static constexpr int SPB = SPC < 4 ? SPC : 4;          // streams per store box
+    static constexpr int BOXES = SPC / SPB;
+    static constexpr int BOX_BYTES = SPB * 2 * C * kStgTile * 2;
+    static constexpr int STG = TENSOR ? BOXES * BOX_BYTES : 0;   // 32 KB
+    static constexpr int OFF_BAR = 0;                      // mbarriers
+    static constexpr int OFF_STG = 1024;                   // 1024-byte aligned (swizzle pattern)
+    static constexpr int OFF_RAW = OFF_STG + kStgBufs * STG;
     static constexpr int OFF_Y = OFF_RAW + kRawStages * RAW_STAGE;
-    static constexpr int OFF_STG = OFF_Y + kYBufs * Y_BUF;
-    static constexpr int OFF_WTAB = OFF_STG + kFftGroups * STG;   // [SPC][C] float2: rotation * bandpass
-    static constexpr int OFF_TW = OFF_WTAB + 256 * 8;      // [16][R] float2 W_C^{r k1}
-    static constexpr int TOTAL = OFF_TW + (R > 1 ? R * 16 * 8 : 0);
+    // per-thread tables, one row of 16 float2 per (stream, residue r) at a pitch of 144 bytes (16-byte loads of
+    // consecutive rows then hit distinct banks)
+    static constexpr int TAB_ROW = 144;
+    static constexpr int OFF_WTAB = OFF_Y + kYBufs * Y_BUF;      // [SPC][R] rows: rotation * bandpass, in register order
+    static constexpr int OFF_ZERO = OFF_WTAB + 16 * TAB_ROW;     // 16 float2 of zeros (spectra beyond n_t)
+    static constexpr int OFF_TW = OFF_ZERO + 128;                // [R] rows: W_C^{r k1}
+    static constexpr int TOTAL = OFF_TW + (R > 1 ? R * TAB_ROW : 0);
     static_assert(TOTAL <= 227 * 1024, "shared memory budget");
 };
 
@@ -159,16 +172,45 @@ __device__ __forceinline__ float2 unpack_sample(uint32_t raw) {
     return make_float2((float)(signed char)(raw & 0xffu), (float)(signed char)((raw >> 8) & 0xffu));
 }
 
+__device__ __forceinline__ bool elect_one() {
+    uint32_t pred;
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "elect.sync _|p, 0xffffffff;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t"
+        "}"
+        : "=r"(pred));
+    return pred != 0;
+}
+
+__device__ __forceinline__ uint32_t pack_half2(float lo, float hi) {
+    const __half2 t = __floats2half2_rn(lo, hi);
+    return *reinterpret_cast<const uint32_t *>(&t);
+}
+
+// channel index held in register slot i of FFT thread r after the last pass, and the register holding it
+template <int R>
+__device__ __forceinline__ constexpr int out_channel(int r, int i) {
+    return R == 16 ? r + 16 * i : R == 4 ? 4 * r + (i >> 2) + 16 * (i & 3) : i;
+}
+template <int R>
+__device__ __forceinline__ constexpr int out_reg(int i) {
+    return R == 4 ? i : dft16_pos(i);
+}
+
 template <int C, int BITS, bool TENSOR>
-__global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a) {
+__global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, const __grid_constant__ CUtensorMap zmap) {
     using Sh = FShape<C, BITS, TENSOR>;
     constexpr int SB = Sh::SB, SPC = Sh::SPC, R = Sh::R, YS = Sh::YS;
-    extern __shared__ __align__(128) unsigned char smem[];
+    extern __shared__ __align__(1024) unsigned char smem[];
     const uint32_t sbase = smem_u32(smem);
     const uint32_t bar_raw_full = sbase + Sh::OFF_BAR;                 // [kRawStages]
     const uint32_t bar_raw_empty = bar_raw_full + 8 * kRawStages;      // [kRawStages]
     const uint32_t bar_y_full = bar_raw_empty + 8 * kRawStages;        // [kYBufs]
     const uint32_t bar_y_empty = bar_y_full + 8 * kYBufs;              // [kYBufs]
+    const uint32_t bar_stg_full = bar_y_empty + 8 * kYBufs;            // [kStgBufs]
+    const uint32_t bar_stg_empty = bar_stg_full + 8 * kStgBufs;        // [kStgBufs]
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int grp = blockIdx.x;                          // stream group within the chunk
@@ -187,23 +229,28 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a) {
         }
         for (int b = 0; b < kYBufs; ++b) {
             mbar_init(bar_y_full + 8 * b, kFirThreads / 32);
-            mbar_init(bar_y_empty + 8 * b, kFftGroup / 32);
+            mbar_init(bar_y_empty + 8 * b, kFftTeam / 32);
+        }
+        for (int b = 0; b < kStgBufs; ++b) {
+            mbar_init(bar_stg_full + 8 * b, kFftThreads / 32);
+            mbar_init(bar_stg_empty + 8 * b, 1);
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    {   // rotation * bandpass of the CTA's streams (station = m >> 1) and the inter-pass twiddles
-        float2 *wtab = reinterpret_cast<float2 *>(smem + Sh::OFF_WTAB);
-        for (int i = tid; i < 256; i += kFThreads) {
-            const int sl = i / C, j = i - sl * C;
-            const int m = min(m0 + sl, a.M - 1);
-            wtab[i] = a.phase[((size_t)bl * a.S + (m >> 1)) * C + j];
+    {   // rotation * bandpass of the CTA's streams (station = m >> 1) in the FFT threads' register order, zeros for
+        // streams that do not exist (their staged rows are then exact zeros), and the inter-pass twiddles
+        for (int idx = tid; idx < 256; idx += kFThreads) {
+            const int sl = idx / C, rr = (idx % C) / 16, i = idx % 16;
+            const int m = m0 + sl;
+            reinterpret_cast<float2 *>(smem + Sh::OFF_WTAB + (idx >> 4) * Sh::TAB_ROW)[i] =
+                m < a.M ? a.phase[((size_t)bl * a.S + (m >> 1)) * C + out_channel<R>(rr, i)] : make_float2(0.f, 0.f);
         }
+        if (tid < 16) reinterpret_cast<float2 *>(smem + Sh::OFF_ZERO)[tid] = make_float2(0.f, 0.f);
         if (R > 1) {
-            float2 *tw = reinterpret_cast<float2 *>(smem + Sh::OFF_TW);
-            for (int i = tid; i < R * 16; i += kFThreads) {
+            for (int idx = tid; idx < R * 16; idx += kFThreads) {
                 float sn, cs;
-                sincospif(-2.0f * (float)((i / R) * (i % R)) / (float)C, &sn, &cs);   // entry [k1][r]
-                tw[i] = make_float2(cs, sn);
+                sincospif(-2.0f * (float)((idx / 16) * (idx % 16)) / (float)C, &sn, &cs);   // entry [r][k1]
+                reinterpret_cast<float2 *>(smem + Sh::OFF_TW + (idx >> 4) * Sh::TAB_ROW)[idx & 15] = make_float2(cs, sn);
             }
         }
     }
@@ -257,9 +304,43 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a) {
             __syncwarp();
             if (lane == 0) mbar_arrive_expect_tx(full, tx);
         }
+    } else if (warp == kStoreWarp) {
+        // ------------------------------------------------------------------ tensor-store issuer (step a7)
+        // One staged tile = 32 spectra of every (stream, channel) of the CTA.  Row (channel c, k-tile kt, plane,
+        // input m) of z is 128 bytes = 64 spectra whose 16-byte chunk q sits at q ^ (m & 7) (cobalt_internal.h):
+        // the 32 spectra of a tile are therefore the 64-byte half (tile & 1) ^ ((m >> 2) & 1) of the row, permuted
+        // inside by m & 3 (done by the FFT threads); m >> 2 is the same for the <= 4 streams of a box.
+        if (TENSOR && elect_one()) {
+            for (int tile = 0; tile < n_sub / 2; ++tile) {
+                const int sbuf = tile & 1;
+                mbar_wait(bar_stg_full + 8 * sbuf, (uint32_t)(tile >> 1) & 1u);
+                const int kt = kt0 + (tile >> 1);
+#pragma unroll
+                for (int b = 0; b < Sh::BOXES; ++b) {
+                    const int mb = m0 + b * Sh::SPB;
+                    if (mb >= a.Mpad) break;
+                    const int c0 = 32 * ((tile & 1) ^ ((mb >> 2) & 1));
+                    asm volatile(
+                        "cp.async.bulk.tensor.5d.global.shared::cta.bulk_group [%0, {%2, %3, %4, %5, %6}], [%1];" ::"l"(&zmap),
+                        "r"(sbase + Sh::OFF_STG + sbuf * Sh::STG + b * Sh::BOX_BYTES), "r"(c0), "r"(bl * C), "r"(0), "r"(mb), "r"(kt)
+                        : "memory");
+                }
+                asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+                asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // shared memory has been read
+                mbar_arrive(bar_stg_empty + 8 * sbuf);
+            }
+            asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+        }
     } else if (warp < kFirThreads / 32) {
         // ------------------------------------------------------------------ FIR (steps a1, a2)
-        const int sl = tid / C, ph = tid - sl * C;
+        int sl, ph;
+        if (R == 16) {   // lane permutation matching the 18 r + q tile (see FShape)
+            sl = 0;
+            ph = (lane >> 1) + 16 * (2 * warp + (lane & 1));
+        } else {
+            sl = tid / C;
+            ph = tid - sl * C;
+        }
         float wk[kTaps];
         {
             const float sgn = (ph & 1) ? -1.f : 1.f;      // (-1)^ph: channel j <- DFT bin (j + C/2) mod C
@@ -270,7 +351,7 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a) {
 #pragma unroll
         for (int k = 0; k < kTaps; ++k) acc[k] = make_float2(0.f, 0.f);
         const uint32_t raw_thread = sbase + Sh::OFF_RAW + sl * (kSubTile * C * SB) + ph * SB;
-        float2 *ybuf = reinterpret_cast<float2 *>(smem + Sh::OFF_Y) + sl * YS + ph + (ph >> 4);
+        float2 *ybuf = reinterpret_cast<float2 *>(smem + Sh::OFF_Y) + sl * YS + (R == 16 ? 18 * (ph & 15) + (ph >> 4) : ph + (ph >> 4));
 
         for (int j = 0; j <= n_sub; ++j) {
             const int s = j % kRawStages;
@@ -315,139 +396,161 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a) {
         }
     } else {
         // ------------------------------------------------------------------ FFT, rotate, transpose (steps a3-a7)
-        // Group g takes the pairs of sub-tiles (32 spectra = half a k-tile) pp = g, g + 2, ...
-        const int g = (tid - kFirThreads) / kFftGroup;
-        const int ft = (tid - kFirThreads) % kFftGroup;   // 0..255
-        const int tl = ft >> 4;                           // spectrum of the sub-tile
-        const int sl = (ft & 15) / R, r = (ft & 15) % R;  // stream of the CTA, residue of the channel index
-        float2 *ybase = reinterpret_cast<float2 *>(smem + Sh::OFF_Y) + (tl * SPC + sl) * YS;
-        const float2 *wtab = reinterpret_cast<const float2 *>(smem + Sh::OFF_WTAB) + sl * C;
-        const float2 *twr = reinterpret_cast<const float2 *>(smem + Sh::OFF_TW) + r;   // W_C^{r k1} at [k1 * R]
-        unsigned char *stg = smem + Sh::OFF_STG + g * Sh::STG;
-        unsigned char *zsub = a.z + (size_t)bl * a.z_subband_bytes;
-        // flush items of this thread (TENSOR): staging row it * 64 + (ft >> 2) = (stream, channel), 8 spectra
-        // tg = ft & 3.  Row (channel c, k-tile kt, plane, input m) of z starts at ((c n_kt + kt) 2 Mpad + m) 128;
-        // the 16-byte chunk q of that row sits at q ^ (m & 7) (cobalt_internal.h), q = 4 (sub >> 1) + tg.
-        const size_t plane_stride = (size_t)a.Mpad * 128;
-        size_t fl_off[4];
-        bool fl_ok[4];
-#pragma unroll
-        for (int it = 0; it < 4; ++it) {
-            const int row = it * (kFftGroup / 4) + (ft >> 2);
-            const int fsl = row / C, fc = row - fsl * C, fm = m0 + fsl;
-            fl_ok[it] = fm < a.M;
-            fl_off[it] = ((size_t)fc * a.n_kt * 2 * a.Mpad + fm) * 128 + ((((ft & 3) ^ (fm & 3)) << 4) | (fm & 4) << 4);
+        // Team tm takes the sub-tiles jj = tm, tm + 2, ...; a thread owns TWO consecutive spectra (so that the fp16
+        // values of spectra t, t + 1 leave as one 32-bit word and every table load serves both) and 16 channels.
+        const int tm = (tid - kFirThreads) / kFftTeam;
+        const int ft = (tid - kFirThreads) % kFftTeam;    // 0..127
+        int tp, sl, r;                                    // spectrum pair of the sub-tile, stream of the CTA, channel residue
+        if (R == 4) {   // warp = 8 pairs x 1 stream x 4 residues: conflict-free staging (see FShape / store issuer)
+            tp = (ft & 31) >> 2;
+            sl = ft >> 5;
+            r = ft & 3;
+        } else {
+            tp = ft >> 4;
+            sl = (ft & 15) / R;
+            r = (ft & 15) % R;
         }
+        float2 *ybase = reinterpret_cast<float2 *>(smem + Sh::OFF_Y) + (2 * tp * SPC + sl) * YS;
+        const float4 *wtab4 = reinterpret_cast<const float4 *>(smem + Sh::OFF_WTAB + (sl * R + r) * Sh::TAB_ROW);
+        const float4 *zero4 = reinterpret_cast<const float4 *>(smem + Sh::OFF_ZERO);
+        const float4 *tw4 = reinterpret_cast<const float4 *>(smem + Sh::OFF_TW + r * Sh::TAB_ROW);
+        const int m = m0 + sl;
+        // staging word of (channel c, plane, pair p of the tile): box b = sl / SPB, then [stream][plane][channel][64 B],
+        // the 16-byte chunk (p >> 2) stored at (p >> 2) ^ (m & 3), 64-byte swizzled like the tensor store reads it
+        const uint32_t stg_thread = (uint32_t)((sl / Sh::SPB) * Sh::BOX_BYTES + (sl % Sh::SPB) * (2 * C * 64));
+        unsigned char *zsub = a.z + (size_t)bl * a.z_subband_bytes;
 
-        for (int pp = g; pp < n_sub / 2; pp += kFftGroups) {
-#pragma unroll 1
-            for (int h = 0; h < 2; ++h) {
-                const int jj = 2 * pp + h;
-                const int yb = jj % kYBufs;
-                const int kt = kt0 + (jj >> 2), sub = jj & 3;
-                const long long t_base = (long long)kt * kKTile + sub * kSubTile;
-                float2 *y = ybase + (size_t)yb * (Sh::Y_BUF / 8);
-                mbar_wait(bar_y_full + 8 * yb, (uint32_t)(jj / kYBufs) & 1u);
-                float2 o[16];
+        for (int jj = tm; jj < n_sub; jj += kFftTeams) {
+            const int yb = jj % kYBufs;
+            const int kt = kt0 + (jj >> 2), sub = jj & 3;
+            const long long t_spec = (long long)kt * kKTile + sub * kSubTile + 2 * tp;   // first of the two spectra
+            float2 *y0 = ybase + (size_t)yb * (Sh::Y_BUF / 8);
+            float2 *y1 = y0 + SPC * YS;
+            mbar_wait(bar_y_full + 8 * yb, (uint32_t)(jj / kYBufs) & 1u);
+            float2 o0[16], o1[16];
+            if (R == 16) {
 #pragma unroll
-                for (int q = 0; q < 16; ++q) o[q] = y[r + R * q + ((r + R * q) >> 4)];
-                dft16(o);                                 // X[k] at o[dft16_pos(k)]
-                if (R == 16) {
-                    // twiddle, exchange in place (each thread rewrites the 16 slots it read), radix-16 pass
-#pragma unroll
-                    for (int k = 0; k < 16; ++k)
-                        y[r + 17 * k] = k ? cmul_tab2(o[dft16_pos(k)], twr[k * R]) : o[0];   // A[r][k1] W_C^{r k1}
-                    __syncwarp();
-#pragma unroll
-                    for (int r2 = 0; r2 < 16; ++r2) o[r2] = y[r2 + 17 * r];
-                    __syncwarp();
-                    if (lane == 0) mbar_arrive(bar_y_empty + 8 * yb);
-                    dft16(o);                             // channel r + 16 k2 at o[dft16_pos(k2)]
-                } else if (R == 4) {
-#pragma unroll
-                    for (int k = 0; k < 16; ++k)
-                        y[r + 4 * k + (k >> 2)] = k ? cmul_tab2(o[dft16_pos(k)], twr[k * R]) : o[0];
-                    __syncwarp();
-#pragma unroll
-                    for (int a4 = 0; a4 < 4; ++a4) {
-                        const int k1 = 4 * r + a4;         // channel k1 + 16 k2 at o[4 a4 + k2]
-#pragma unroll
-                        for (int r2 = 0; r2 < 4; ++r2) o[4 * a4 + r2] = y[4 * k1 + r2 + r];
-                    }
-                    __syncwarp();
-                    if (lane == 0) mbar_arrive(bar_y_empty + 8 * yb);
-#pragma unroll
-                    for (int a4 = 0; a4 < 4; ++a4) dft4(o[4 * a4], o[4 * a4 + 1], o[4 * a4 + 2], o[4 * a4 + 3]);
-                } else {
-                    __syncwarp();
-                    if (lane == 0) mbar_arrive(bar_y_empty + 8 * yb);
+                for (int q = 0; q < 16; q += 2) {
+                    const float4 v0 = *reinterpret_cast<const float4 *>(y0 + 18 * r + q);
+                    const float4 v1 = *reinterpret_cast<const float4 *>(y1 + 18 * r + q);
+                    o0[q] = make_float2(v0.x, v0.y);
+                    o0[q + 1] = make_float2(v0.z, v0.w);
+                    o1[q] = make_float2(v1.x, v1.y);
+                    o1[q + 1] = make_float2(v1.z, v1.w);
                 }
-                // steps a5-a7: rotate * bandpass, convert, stage transposed.  Spectra t >= n_t (padding of
-                // the last k-tile) are staged as exact zeros: the rotation table is replaced by zero.
-                const bool live = t_base + tl < a.n_t;
-                const int ts = TENSOR ? h * kSubTile + tl : tl;   // spectrum slot in the staging row
+            } else {
 #pragma unroll
-                for (int i = 0; i < 16; ++i) {
-                    int j, oi;                            // channel index, register holding it
-                    if (R == 16) { j = r + 16 * i; oi = dft16_pos(i); }
-                    else if (R == 4) { j = 4 * r + (i >> 2) + 16 * (i & 3); oi = i; }
-                    else { j = i; oi = dft16_pos(i); }
-                    float2 zz = cmul_tab2(o[oi], wtab[j]);
-                    if (TENSOR) {
-                        uint32_t hv;
-                        {
-                            const __half2 t2 = __floats2half2_rn(zz.x, zz.y);
-                            hv = *reinterpret_cast<const uint32_t *>(&t2);
+                for (int q = 0; q < 16; ++q) {
+                    o0[q] = y0[r + R * q + ((r + R * q) >> 4)];
+                    o1[q] = y1[r + R * q + ((r + R * q) >> 4)];
+                }
+            }
+            dft16(o0);                                    // X[k] at o[dft16_pos(k)]
+            dft16(o1);
+            if (R == 16) {
+                // twiddle, exchange in place (each thread rewrites the 16 slots it read), radix-16 pass
+#pragma unroll
+                for (int k = 0; k < 16; k += 2) {
+                    const float4 w = tw4[k >> 1];           // W_C^{r k}, W_C^{r (k + 1)}
+                    const float2 a0 = k ? cmul_tab2(o0[dft16_pos(k)], make_float2(w.x, w.y)) : o0[0];
+                    const float2 a1 = k ? cmul_tab2(o1[dft16_pos(k)], make_float2(w.x, w.y)) : o1[0];
+                    const float2 b0 = cmul_tab2(o0[dft16_pos(k + 1)], make_float2(w.z, w.w));
+                    const float2 b1 = cmul_tab2(o1[dft16_pos(k + 1)], make_float2(w.z, w.w));
+                    *reinterpret_cast<float4 *>(y0 + 18 * r + k) = make_float4(a0.x, a0.y, b0.x, b0.y);
+                    *reinterpret_cast<float4 *>(y1 + 18 * r + k) = make_float4(a1.x, a1.y, b1.x, b1.y);
+                }
+                __syncwarp();
+#pragma unroll
+                for (int r2 = 0; r2 < 16; ++r2) {
+                    o0[r2] = y0[18 * r2 + r];
+                    o1[r2] = y1[18 * r2 + r];
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar_y_empty + 8 * yb);
+                dft16(o0);                                // channel r + 16 k2 at o[dft16_pos(k2)]
+                dft16(o1);
+            } else if (R == 4) {
+#pragma unroll
+                for (int k = 0; k < 16; k += 2) {
+                    const float4 w = tw4[k >> 1];
+                    y0[r + 4 * k + (k >> 2)] = k ? cmul_tab2(o0[dft16_pos(k)], make_float2(w.x, w.y)) : o0[0];
+                    y1[r + 4 * k + (k >> 2)] = k ? cmul_tab2(o1[dft16_pos(k)], make_float2(w.x, w.y)) : o1[0];
+                    y0[r + 4 * (k + 1) + ((k + 1) >> 2)] = cmul_tab2(o0[dft16_pos(k + 1)], make_float2(w.z, w.w));
+                    y1[r + 4 * (k + 1) + ((k + 1) >> 2)] = cmul_tab2(o1[dft16_pos(k + 1)], make_float2(w.z, w.w));
+                }
+                __syncwarp();
+#pragma unroll
+                for (int a4 = 0; a4 < 4; ++a4) {
+                    const int k1 = 4 * r + a4;             // channel k1 + 16 k2 at o[4 a4 + k2]
+#pragma unroll
+                    for (int r2 = 0; r2 < 4; ++r2) {
+                        o0[4 * a4 + r2] = y0[4 * k1 + r2 + r];
+                        o1[4 * a4 + r2] = y1[4 * k1 + r2 + r];
+                    }
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar_y_empty + 8 * yb);
+#pragma unroll
+                for (int a4 = 0; a4 < 4; ++a4) {
+                    dft4(o0[4 * a4], o0[4 * a4 + 1], o0[4 * a4 + 2], o0[4 * a4 + 3]);
+                    dft4(o1[4 * a4], o1[4 * a4 + 1], o1[4 * a4 + 2], o1[4 * a4 + 3]);
+                }
+            } else {
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar_y_empty + 8 * yb);
+            }
+            // steps a5-a7: rotate * bandpass, convert, stage transposed.  Spectra t >= n_t (padding of the last
+            // k-tile) leave as exact zeros: the rotation table is replaced by zeros.
+            const bool live0 = t_spec < a.n_t, live1 = t_spec + 1 < a.n_t;
+            const float4 *wt = live0 ? wtab4 : zero4;
+            if (TENSOR) {
+                const int tile = jj >> 1, sbuf = tile & 1;
+                const int p = 8 * (jj & 1) + tp;          // pair of spectra within the 32-spectrum tile
+                const uint32_t msk = live1 || !live0 ? 0xffffffffu : 0x0000ffffu;   // n_t odd: last pair is half live
+                mbar_wait(bar_stg_empty + 8 * sbuf, ((uint32_t)(tile >> 1) & 1u) ^ 1u);
+                unsigned char *stg = smem + Sh::OFF_STG + sbuf * Sh::STG + stg_thread;
+                // byte offset of (channel j, plane re, this pair) in the box: 64 j + 16 ((p >> 2) ^ (m & 3)) + 4 (p & 3), then
+                // the store's 64-byte swizzle (bits 4-5 ^= bits 7-8).  Bits 7-8 come from 64 j only, and j = (part fixed by
+                // r) + (part fixed by the register slot i), so the r part is folded in once and the i part is a constant.
+                const uint32_t rbits = R == 16 ? (uint32_t)(r >> 1) & 3u : R == 4 ? (uint32_t)(r & 1) << 1 : 0u;
+                const uint32_t base = (uint32_t)out_channel<R>(r, 0) * 64 + (uint32_t)(((((p >> 2) ^ (m & 3)) << 4) | ((p & 3) << 2)) ^ (rbits << 4));
+                // the slot part of the swizzle flips bits 4-5 by a compile-time constant: one base address per value
+                unsigned char *stg_v[4];
+#pragma unroll
+                for (int v = 0; v < 4; ++v) stg_v[v] = stg + (base ^ (uint32_t)(v << 4));
+#pragma unroll
+                for (int i = 0; i < 16; i += 2) {
+                    const float4 w = wt[i >> 1];
+#pragma unroll
+                    for (int e = 0; e < 2; ++e) {
+                        const int oi = out_reg<R>(i + e);
+                        const int dj = out_channel<R>(0, i + e);                 // compile-time part of the channel index
+                        const int ibits = R == 16 ? 0 : R == 4 ? ((i + e) >> 3) & 1 : ((i + e) >> 1) & 3;
+                        const float2 ww = e ? make_float2(w.z, w.w) : make_float2(w.x, w.y);
+                        const float2 z0 = cmul_tab2(o0[oi], ww), z1 = cmul_tab2(o1[oi], ww);
+                        *reinterpret_cast<uint32_t *>(stg_v[ibits] + dj * 64) = pack_half2(z0.x, z1.x) & msk;
+                        *reinterpret_cast<uint32_t *>(stg_v[ibits] + dj * 64 + C * 64) = pack_half2(z0.y, z1.y) & msk;
+                    }
+                }
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy writes -> visible to the store
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar_stg_full + 8 * sbuf);
+            } else {
+                // EXACT mode (parity instrument): fp32 values straight to z [C][M][n_t]
+                if (m < a.M) {
+#pragma unroll
+                    for (int i = 0; i < 16; i += 2) {
+                        const float4 w = wt[i >> 1];
+#pragma unroll
+                        for (int e = 0; e < 2; ++e) {
+                            const int j = out_channel<R>(r, i + e), oi = out_reg<R>(i + e);
+                            const float2 ww = e ? make_float2(w.z, w.w) : make_float2(w.x, w.y);
+                            float2 *dst = reinterpret_cast<float2 *>(zsub) + ((size_t)j * a.M + m) * a.n_t + t_spec;
+                            if (live0) dst[0] = cmul_tab2(o0[oi], ww);
+                            if (live1) dst[1] = cmul_tab2(o1[oi], ww);
                         }
-                        if (!live) hv = 0u;
-                        *reinterpret_cast<uint32_t *>(stg + (sl * C + j) * Sh::STG_ROW + ts * 4) = hv;
-                    } else {
-                        if (!live) zz = make_float2(0.f, 0.f);
-                        *reinterpret_cast<float2 *>(stg + (sl * C + j) * Sh::STG_ROW + ts * 8) = zz;
                     }
                 }
-                if (TENSOR && h == 0) continue;           // flush every 32 spectra
-                bar_sync_named(1 + g, kFftGroup);         // staging complete
-                if (TENSOR) {
-                    // item = (row = (stream, channel), tg = 8 spectra): 8 words (re | im << 16) -> one 16-byte
-                    // chunk per plane; 4 consecutive lanes write one 64-byte run of a 128-byte row
-                    unsigned char *zkt = zsub + (size_t)kt * 2 * plane_stride;
-                    const size_t half = (size_t)(sub >> 1) << 6;   // which 64 bytes of the row these 32 spectra are
-#pragma unroll
-                    for (int it = 0; it < 4; ++it) {
-                        if (!fl_ok[it]) continue;
-                        const unsigned char *src = stg + (it * (kFftGroup / 4) + (ft >> 2)) * Sh::STG_ROW + (ft & 3) * 32;
-                        uint32_t w[8];
-#pragma unroll
-                        for (int i = 0; i < 4; ++i) {
-                            const uint2 v = *reinterpret_cast<const uint2 *>(src + i * 8);
-                            w[2 * i] = v.x;
-                            w[2 * i + 1] = v.y;
-                        }
-                        uint4 re, im;
-                        re.x = __byte_perm(w[0], w[1], 0x5410);
-                        re.y = __byte_perm(w[2], w[3], 0x5410);
-                        re.z = __byte_perm(w[4], w[5], 0x5410);
-                        re.w = __byte_perm(w[6], w[7], 0x5410);
-                        im.x = __byte_perm(w[0], w[1], 0x7632);
-                        im.y = __byte_perm(w[2], w[3], 0x7632);
-                        im.z = __byte_perm(w[4], w[5], 0x7632);
-                        im.w = __byte_perm(w[6], w[7], 0x7632);
-                        unsigned char *rowp = zkt + (fl_off[it] ^ half);
-                        *reinterpret_cast<uint4 *>(rowp) = re;
-                        *reinterpret_cast<uint4 *>(rowp + plane_stride) = im;
-                    }
-                } else {
-                    const int fsl = ft / C, fc = ft - fsl * C;    // this thread owns staging row ft = (stream, channel)
-                    const int fm = m0 + fsl;
-                    if (fm < a.M) {
-                        float2 *dst = reinterpret_cast<float2 *>(zsub) + ((size_t)fc * a.M + fm) * a.n_t + t_base;
-#pragma unroll
-                        for (int i = 0; i < 16; ++i)
-                            if (t_base + i < a.n_t) dst[i] = *reinterpret_cast<const float2 *>(stg + ft * Sh::STG_ROW + i * 8);
-                    }
-                }
-                bar_sync_named(1 + g, kFftGroup);         // staging drained
             }
         }
     }
@@ -538,6 +641,7 @@ cudaError_t launch_f(const cobalt_plan_s *p, cudaStream_t st, const FArgs &a, in
     using Sh = FShape<C, BITS, TENSOR>;
     auto kern = fstage_kernel<C, BITS, TENSOR>;
     const size_t smem = Sh::TOTAL;
+    static_assert(Sh::SPB == kStoreBoxStreams(C), "plan.cu builds the tensor map with the same box");
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     FArgs args = a;
@@ -553,7 +657,7 @@ cudaError_t launch_f(const cobalt_plan_s *p, cudaStream_t st, const FArgs &a, in
     args.tiles_per_seg = (p->n_kt + n_seg - 1) / n_seg;
     n_seg = (p->n_kt + args.tiles_per_seg - 1) / args.tiles_per_seg;
     dim3 grid((unsigned)groups, (unsigned)n_seg);
-    kern<<<grid, kFThreads, smem, st>>>(args);
+    kern<<<grid, kFThreads, smem, st>>>(args, p->zmap);
     return cudaGetLastError();
 }
 

@@ -65,6 +65,31 @@ void free_scratch(cobalt_plan_s *p) {
     }
 }
 
+// Tensor map of the fp16 intermediate of one chunk for the F-stage's tensor stores (fstage.cu, store issuer).
+// Dimensions, innermost first: spectrum within the k-tile (64 fp16 = one 128-byte row), chunk subband * C + channel,
+// plane (re, im), row m (input), k-tile; the box is half a row of every (stream of the CTA, plane, channel).
+int build_zmap(cobalt_plan_s *p) {
+    std::memset(&p->zmap, 0, sizeof(p->zmap));
+    if (p->mode != COBALT_MODE_TENSOR_FP16) return COBALT_OK;
+    typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                                  const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    void *fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    CK(p, cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres));
+    if (!fn || qres != cudaDriverEntryPointSuccess) return fail(p, COBALT_ERR_CUDA, "cuTensorMapEncodeTiled is not available");
+    const cuuint64_t row = 128, plane = (cuuint64_t)p->Mpad * row, kt = 2 * plane, chan = (cuuint64_t)p->n_kt * kt;
+    const cuuint64_t dims[5] = {(cuuint64_t)kKTile, (cuuint64_t)p->chunk * p->C, 2, (cuuint64_t)p->Mpad, (cuuint64_t)p->n_kt};
+    const cuuint64_t strides[4] = {chan, plane, row, kt};   // bytes, dimensions 1..4
+    const cuuint32_t box[5] = {(cuuint32_t)kStoreTile, (cuuint32_t)p->C, 2, (cuuint32_t)kStoreBoxStreams(p->C), 1};
+    const cuuint32_t estr[5] = {1, 1, 1, 1, 1};
+    const CUresult r = reinterpret_cast<encode_fn>(fn)(&p->zmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 5, p->d_z, dims, strides, box, estr,
+                                                       CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_64B,
+                                                       CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(p, COBALT_ERR_CUDA, "cuTensorMapEncodeTiled failed with CUresult " + std::to_string((int)r));
+    return COBALT_OK;
+}
+
 // (Re)allocate the per-chunk scratch for the current mode / chunk size.
 int alloc_scratch(cobalt_plan_s *p, int chunk_request) {
     free_scratch(p);
@@ -81,6 +106,10 @@ int alloc_scratch(cobalt_plan_s *p, int chunk_request) {
     CK(p, cudaMemset(p->d_z, 0, (size_t)chunk * p->z_subband_bytes));   // zero rows 2S..Mpad stay zero forever
     CK(p, cudaMalloc(&p->d_phase, (size_t)chunk * p->S * p->C * sizeof(float2)));
     CK(p, cudaDeviceSynchronize());
+    {
+        const int rc = build_zmap(p);
+        if (rc != COBALT_OK) return rc;
+    }
     const size_t hist = (size_t)p->B * p->M * (kTaps - 1) * p->C * sample_bytes(p->bits);
     p->scratch_bytes = (size_t)chunk * p->z_subband_bytes + (size_t)chunk * p->S * p->C * sizeof(float2) + 2 * hist +
                        (size_t)kTaps * p->C * sizeof(float) + (size_t)p->B * sizeof(double);
