@@ -25,12 +25,16 @@ constexpr int kStoreBoxStreams(int C) { return 256 / C < 4 ? 256 / C : 4; }
 // ---------------------------------------------------------------------------------------------
 // Layout of the channelised intermediate ("z", step a7, "transposes data on write-back").
 //
-// TENSOR_FP16: per subband  [C][n_kt][2 planes (re, im)][Mpad rows][64 t] fp16,
-//   rows = inputs (2*station + pol) padded with zero rows to Mpad = round_up(2S, 16); each
-//   [Mpad][64] block is stored exactly as the 128-byte-swizzled K-major shared-memory image the
-//   tcgen05 descriptors expect: the 16-byte chunk q (8 spectra) of row m sits at chunk q ^ (m & 7)
-//   of that row.  One (channel, k-tile) is therefore one contiguous 2*Mpad*128-byte span that the
-//   X-stage fetches with plain bulk copies, no tensor map.  Spectra t >= n_t are written as zeros.
+// TENSOR_FP16: per subband  [C][n_kt][Mpad/8 row groups][2 planes (re, im)][8 rows][64 t] fp16,
+//   rows = inputs (2*station + pol) padded with zero rows to Mpad = round_up(2S, 16).  A row is 128 bytes
+//   (64 spectra); the 16-byte chunk q (8 spectra) of row m sits at chunk q ^ (m & 7) of that row, i.e. every
+//   [8 rows][128 B] block is one atom of the 128-byte-swizzled K-major shared-memory image the tcgen05
+//   descriptors expect.  The two planes alternate atom by atom, so the same bytes can be read two ways:
+//     one plane   = atoms 2048 bytes apart (descriptor SBO = 2048; the im plane starts 1024 bytes in);
+//     both planes = atoms 1024 bytes apart (SBO = 1024): rows in the order re 0-7, im 0-7, re 8-15, ...
+//   (the X-stage uses the second view for the small block the 128-row instruction cannot reach).
+//   One (channel, k-tile) is one contiguous Mpad*256-byte span that the X-stage fetches with one plain
+//   bulk copy, no tensor map.  Spectra t >= n_t are written as zeros.
 // EXACT_FP32:  per subband  [C][M][n_t] float2.
 // ---------------------------------------------------------------------------------------------
 
@@ -45,6 +49,9 @@ struct XMmaGroup {
     int out_col;    // global input index of B row 0
     int m;          // instruction M: 128, or 64 (accumulator row r then sits in TMEM lane 32 (r / 16) + r % 16)
     int row_min;    // rows (global input index) below this are another group's job and are not stored
+    int kind;       // 0: four single-plane products into Re | Im accumulators (2 n columns);
+                    // 1: one both-plane product [Zr; Zi] [Zr; Zi]^T of the rows a_row.. (n = 2 x rows per plane,
+                    //    n columns), combined into Re / Im by the epilogue
 };
 struct XJob {
     int ld_row[2];     // two row ranges of the [Mpad][64] block copied to smem back to back

@@ -306,8 +306,9 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, con
         }
     } else if (warp == kStoreWarp) {
         // ------------------------------------------------------------------ tensor-store issuer (step a7)
-        // One staged tile = 32 spectra of every (stream, channel) of the CTA.  Row (channel c, k-tile kt, plane,
-        // input m) of z is 128 bytes = 64 spectra whose 16-byte chunk q sits at q ^ (m & 7) (cobalt_internal.h):
+        // One staged tile = 32 spectra of every (stream, channel) of the CTA.  Row (channel c, k-tile kt, row group
+        // m / 8, plane, m % 8) of z is 128 bytes = 64 spectra whose 16-byte chunk q sits at q ^ (m & 7) (cobalt_internal.h;
+        // tensor-map coordinates: spectrum, channel, 2 (m / 8) + plane, m % 8, k-tile):
         // the 32 spectra of a tile are therefore the 64-byte half (tile & 1) ^ ((m >> 2) & 1) of the row, permuted
         // inside by m & 3 (done by the FFT threads); m >> 2 is the same for the <= 4 streams of a box.
         if (TENSOR && elect_one()) {
@@ -322,7 +323,7 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, con
                     const int c0 = 32 * ((tile & 1) ^ ((mb >> 2) & 1));
                     asm volatile(
                         "cp.async.bulk.tensor.5d.global.shared::cta.bulk_group [%0, {%2, %3, %4, %5, %6}], [%1];" ::"l"(&zmap),
-                        "r"(sbase + Sh::OFF_STG + sbuf * Sh::STG + b * Sh::BOX_BYTES), "r"(c0), "r"(bl * C), "r"(0), "r"(mb), "r"(kt)
+                        "r"(sbase + Sh::OFF_STG + sbuf * Sh::STG + b * Sh::BOX_BYTES), "r"(c0), "r"(bl * C), "r"(2 * (mb >> 3)), "r"(mb & 7), "r"(kt)
                         : "memory");
                 }
                 asm volatile("cp.async.bulk.commit_group;" ::: "memory");

@@ -9,7 +9,8 @@ namespace {
 
 __device__ __forceinline__ size_t z16_offset(int c, int kt, int plane, int m, int tt, int n_kt, int Mpad) {
     // byte offset of element (channel c, k-tile kt, plane, row m, spectrum tt of the tile)
-    return ((((size_t)c * n_kt + kt) * 2 + plane) * Mpad + m) * 128 + ((((tt >> 3) ^ (m & 7)) << 4) | ((tt & 7) << 1));
+    return ((((size_t)c * n_kt + kt) * (Mpad >> 3) + (m >> 3)) * 2 + plane) * 1024 + (size_t)(m & 7) * 128 +
+           ((((tt >> 3) ^ (m & 7)) << 4) | ((tt & 7) << 1));
 }
 
 __global__ void z16_to_float_kernel(const unsigned char *__restrict__ z, const float *__restrict__ scale,
@@ -28,7 +29,7 @@ __global__ void z16_to_float_kernel(const unsigned char *__restrict__ z, const f
     }
 }
 
-// Writes every element of the [C][n_kt][2][Mpad][64] block, zeros in the padding rows / spectra.
+// Writes every element of the [C][n_kt][Mpad/8][2][8][64] block, zeros in the padding rows / spectra.
 __global__ void float_to_z16_kernel(const float2 *__restrict__ in, unsigned char *__restrict__ z, int C, int M,
                                     int Mpad, int n_kt, long long n_t) {
     const long long total = (long long)C * n_kt * Mpad * kKTile;

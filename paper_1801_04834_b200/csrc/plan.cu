@@ -67,7 +67,8 @@ void free_scratch(cobalt_plan_s *p) {
 
 // Tensor map of the fp16 intermediate of one chunk for the F-stage's tensor stores (fstage.cu, store issuer).
 // Dimensions, innermost first: spectrum within the k-tile (64 fp16 = one 128-byte row), chunk subband * C + channel,
-// plane (re, im), row m (input), k-tile; the box is half a row of every (stream of the CTA, plane, channel).
+// u = 2 * (row group m / 8) + plane (1024-byte atoms, cobalt_internal.h), row within the group m % 8, k-tile; the box is
+// half a row of every (stream of the CTA, plane, channel) -- the CTA's streams share one row group.
 int build_zmap(cobalt_plan_s *p) {
     std::memset(&p->zmap, 0, sizeof(p->zmap));
     if (p->mode != COBALT_MODE_TENSOR_FP16) return COBALT_OK;
@@ -78,9 +79,9 @@ int build_zmap(cobalt_plan_s *p) {
     cudaDriverEntryPointQueryResult qres;
     CK(p, cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres));
     if (!fn || qres != cudaDriverEntryPointSuccess) return fail(p, COBALT_ERR_CUDA, "cuTensorMapEncodeTiled is not available");
-    const cuuint64_t row = 128, plane = (cuuint64_t)p->Mpad * row, kt = 2 * plane, chan = (cuuint64_t)p->n_kt * kt;
-    const cuuint64_t dims[5] = {(cuuint64_t)kKTile, (cuuint64_t)p->chunk * p->C, 2, (cuuint64_t)p->Mpad, (cuuint64_t)p->n_kt};
-    const cuuint64_t strides[4] = {chan, plane, row, kt};   // bytes, dimensions 1..4
+    const cuuint64_t row = 128, atom = 8 * row, kt = (cuuint64_t)p->Mpad * 2 * row, chan = (cuuint64_t)p->n_kt * kt;
+    const cuuint64_t dims[5] = {(cuuint64_t)kKTile, (cuuint64_t)p->chunk * p->C, (cuuint64_t)(p->Mpad / 8) * 2, 8, (cuuint64_t)p->n_kt};
+    const cuuint64_t strides[4] = {chan, atom, row, kt};   // bytes, dimensions 1..4
     const cuuint32_t box[5] = {(cuuint32_t)kStoreTile, (cuuint32_t)p->C, 2, (cuuint32_t)kStoreBoxStreams(p->C), 1};
     const cuuint32_t estr[5] = {1, 1, 1, 1, 1};
     const CUresult r = reinterpret_cast<encode_fn>(fn)(&p->zmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 5, p->d_z, dims, strides, box, estr,

@@ -3,8 +3,10 @@
 // of all pairs of antenna fields and averages in time"; BASELINE.json north_star (c)).
 //
 // Z is [2S inputs][n_t spectra] complex, held as two fp16 planes (re, im), K-major, already in the
-// 128-byte-swizzled shared-memory image (cobalt_internal.h), so operands arrive with plain bulk
-// copies (cp.async.bulk -> UBLKCP) signalled on mbarriers -- no tensor map, no register staging.
+// 128-byte-swizzled shared-memory image with the planes alternating every 8 rows (cobalt_internal.h),
+// so one (channel, k-tile) arrives with one plain bulk copy (cp.async.bulk -> UBLKCP) signalled on an
+// mbarrier -- no tensor map, no register staging -- and can be read plane by plane (descriptor
+// stride 2048) or as the stacked matrix [Zr; Zi] (stride 1024).
 //
 //   Re V = Zr Zr^T + Zi Zi^T        Im V = Zi Zr^T - Zr Zi^T
 //
@@ -12,8 +14,9 @@
 // accumulators; the minus sign is the instruction descriptor's negate-A bit, so no negated plane is
 // ever stored.  Only tiles on or above the station diagonal are computed: an XJob (built once per
 // plan by build_xjobs) names the rows to load and up to two accumulator groups
-//   rows [0,128) x cols [0,Mpad)  (M = 128)  and  rows [Mpad-64,Mpad) x cols [128,Mpad)  (M = 64; only its
-//   rows >= 128 are stored)                                                      (2S <= 192)
+//   rows [0,128) x cols [0,Mpad)  (M = 128, four products)  and, for the rows the 128-row instruction
+//   cannot reach, ONE product W W^T of the stacked rows W = [Zr; Zi][128, Mpad) per k-step (all four
+//   real products at once; the epilogue adds / subtracts its quadrants)            (2S <= 192)
 // or, for large arrays, one (128-row block) x (<= 256-column chunk) tile per job.
 //
 // Warp roles (320 threads, persistent CTAs, one per SM): warp 0 = bulk-copy producer, warp 1 = TMEM
@@ -27,7 +30,6 @@ namespace {
 
 constexpr int kEpiWarps = 8;            // two per TMEM lane quarter, alternating 16-column chunks
 constexpr int kThreads = 64 + 32 * kEpiWarps;
-constexpr int kSlackBytes = 128 * 128;   // A operands may over-read up to 128 rows of one plane
 constexpr int kBarrierBytes = 1024;
 
 struct XArgs {
@@ -86,9 +88,9 @@ __device__ __forceinline__ void tc_mma(uint32_t d_tmem, uint64_t a_desc, uint64_
         "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(acc)
         : "memory");
 }
-// K-major, 128-byte swizzle: 8-row groups 1024 bytes apart (SBO), descriptor version 1 (sm_100).
-__device__ __forceinline__ uint64_t make_smem_desc(uint32_t addr) {
-    return (uint64_t)((addr >> 4) & 0x3FFFu) | (1ull << 16) | (64ull << 32) | (1ull << 46) | (2ull << 61);
+// K-major, 128-byte swizzle: 8-row groups sbo bytes apart (SBO), descriptor version 1 (sm_100).
+__device__ __forceinline__ uint64_t make_smem_desc(uint32_t addr, uint32_t sbo) {
+    return (uint64_t)((addr >> 4) & 0x3FFFu) | (1ull << 16) | ((uint64_t)(sbo >> 4) << 32) | (1ull << 46) | (2ull << 61);
 }
 // kind::f16 instruction descriptor: D = f32, A = B = f16, both K-major.
 __device__ __forceinline__ uint32_t make_idesc(int m, int n, int neg_a) {
@@ -157,26 +159,21 @@ __global__ void __launch_bounds__(kThreads, 1) xstage_tc_kernel(const XArgs a) {
         if (elect_one()) {
             int s = 0;
             uint32_t ph = 0;
-            const size_t kt_bytes = (size_t)2 * a.Mpad * 128, pl_bytes = (size_t)a.Mpad * 128;
+            const size_t kt_bytes = (size_t)a.Mpad * 256;     // [Mpad / 8][2 planes][8 rows][128 B]
             for (int jid = blockIdx.x; jid < a.total_jobs; jid += gridDim.x) {
                 const int jl = jid % a.jobs_per_channel;
                 const int prob = jid / a.jobs_per_channel;           // subband-of-chunk * C + channel
                 const int bl = prob / a.C, c = prob - bl * a.C;
                 const int r0 = a.jobs[jl].ld_row[0], r1 = a.jobs[jl].ld_row[1];
-                const uint32_t b0 = (uint32_t)a.jobs[jl].ld_nrows[0] * 128, b1 = (uint32_t)a.jobs[jl].ld_nrows[1] * 128;
+                const uint32_t b0 = (uint32_t)a.jobs[jl].ld_nrows[0] * 256, b1 = (uint32_t)a.jobs[jl].ld_nrows[1] * 256;
                 const unsigned char *src = a.z + (size_t)bl * a.z_subband_bytes + (size_t)c * a.n_kt * kt_bytes;
-                const uint32_t plane_bytes = b0 + b1;
                 for (int kt = 0; kt < a.n_kt; ++kt, src += kt_bytes) {
                     mbar_wait(bar_base + 8 * (16 + s), ph ^ 1);
                     const uint32_t full = bar_base + 8 * s;
                     const uint32_t dst = stage_base + (uint32_t)s * a.stage_bytes;
-                    mbar_expect_tx(full, 2 * plane_bytes);
-#pragma unroll
-                    for (int plane = 0; plane < 2; ++plane) {
-                        const unsigned char *sp = src + (size_t)plane * pl_bytes;
-                        bulk_g2s(dst + plane * plane_bytes, sp + (size_t)r0 * 128, b0, full);
-                        if (b1 > 0) bulk_g2s(dst + plane * plane_bytes + b0, sp + (size_t)r1 * 128, b1, full);
-                    }
+                    mbar_expect_tx(full, b0 + b1);
+                    bulk_g2s(dst, src + (size_t)r0 * 256, b0, full);
+                    if (b1 > 0) bulk_g2s(dst + b0, src + (size_t)r1 * 256, b1, full);
                     if (++s == stages) {
                         s = 0;
                         ph ^= 1;
@@ -191,19 +188,20 @@ __global__ void __launch_bounds__(kThreads, 1) xstage_tc_kernel(const XArgs a) {
             uint32_t ph = 0, it = 0;
             // shared-memory descriptor of byte offset 0 of stage 0; rows / stages / k-steps only add to the
             // 14-bit start-address field (units of 16 bytes; shared memory is < 256 KB, so it cannot carry out)
-            const uint64_t desc0 = make_smem_desc(stage_base);
+            const uint64_t desc_plane = make_smem_desc(stage_base, 2048);   // one plane: atoms 2048 bytes apart
+            const uint64_t desc_both = make_smem_desc(stage_base, 1024);    // [Zr; Zi] stacked 8 rows at a time
             const uint32_t stage_units = (uint32_t)a.stage_bytes >> 4;
             for (int jid = blockIdx.x; jid < a.total_jobs; jid += gridDim.x, ++it) {
                 const XJob *job = a.jobs + jid % a.jobs_per_channel;
                 const int n_groups = job->n_groups;
-                const uint32_t plane_units = (uint32_t)(job->ld_nrows[0] + job->ld_nrows[1]) * 8;
                 uint32_t g_a[kMaxMmaGroups], g_b[kMaxMmaGroups], g_d[kMaxMmaGroups], g_n[kMaxMmaGroups];
-                uint32_t g_pos[kMaxMmaGroups], g_neg[kMaxMmaGroups];
+                uint32_t g_pos[kMaxMmaGroups], g_neg[kMaxMmaGroups], g_kind[kMaxMmaGroups];
 #pragma unroll
                 for (int g = 0; g < kMaxMmaGroups; ++g) {
                     const XMmaGroup &grp = job->g[g < n_groups ? g : 0];
-                    g_a[g] = (uint32_t)grp.a_row * 8;
-                    g_b[g] = (uint32_t)grp.b_row * 8;
+                    g_a[g] = (uint32_t)grp.a_row * 16;             // 256 bytes per row of both planes, >> 4
+                    g_b[g] = (uint32_t)grp.b_row * 16;
+                    g_kind[g] = (uint32_t)grp.kind;
                     g_n[g] = (uint32_t)grp.n;
                     g_d[g] = tmem_base + (uint32_t)grp.tmem_col;
                     g_pos[g] = make_idesc(grp.m, grp.n, 0);
@@ -214,12 +212,17 @@ __global__ void __launch_bounds__(kThreads, 1) xstage_tc_kernel(const XArgs a) {
                 for (int kt = 0; kt < a.n_kt; ++kt) {
                     mbar_wait(bar_base + 8 * s, ph);
                     tc_fence_after();
-                    const uint64_t st = desc0 + (uint64_t)((uint32_t)s * stage_units);
+                    const uint64_t so = (uint64_t)((uint32_t)s * stage_units);
 #pragma unroll
                     for (int g = 0; g < kMaxMmaGroups; ++g) {
-                        if (g < n_groups) {
-                            const uint64_t ar = st + g_a[g], ai = ar + plane_units;
-                            const uint64_t br = st + g_b[g], bi = br + plane_units;
+                        if (g < n_groups && g_kind[g] == 1) {
+                            const uint64_t aw = desc_both + so + g_a[g], bw = desc_both + so + g_b[g];
+#pragma unroll
+                            for (int ks = 0; ks < kKTile / 16; ++ks)
+                                tc_mma(g_d[g], aw + (uint64_t)(ks * 2), bw + (uint64_t)(ks * 2), g_pos[g], (kt | ks) ? 1u : 0u);
+                        } else if (g < n_groups) {
+                            const uint64_t ar = desc_plane + so + g_a[g], ai = ar + 64;   // im plane: 1024 bytes in
+                            const uint64_t br = desc_plane + so + g_b[g], bi = br + 64;
                             const uint32_t d_re = g_d[g], d_im = d_re + g_n[g];
 #pragma unroll
                             for (int ks = 0; ks < kKTile / 16; ++ks) {
@@ -263,6 +266,48 @@ __global__ void __launch_bounds__(kThreads, 1) xstage_tc_kernel(const XArgs a) {
                 const int out_col = job->g[g].out_col;
                 // M = 128: accumulator row = TMEM lane; M = 64: row r in lane 32 (r / 16) + r % 16
                 const int rows_w = gm == 128 ? 32 : 16;
+                if (job->g[g].kind == 1) {
+                    // Stacked product D = W W^T, W = [Zr; Zi] 8 rows at a time: accumulator row (and column)
+                    // a = 16 q + 8 plane + r is input out_row + 8 q + r.  A lane and its partner lane ^ 8 hold the
+                    // re-plane and im-plane rows of one input; a 16-column chunk is 8 inputs, re columns then im.
+                    //   Re V = D[re][re] + D[im][im]        Im V = D[im][re] - D[re][im]
+                    const int arow = wq * rows_w + (lane & (rows_w - 1));
+                    const int pl = (arow >> 3) & 1;
+                    const int mrow = job->g[g].out_row + ((arow >> 4) << 3) + (arow & 7);
+                    const bool row_ok = lane < rows_w && arow < gn && mrow < a.M;
+                    const int i = mrow >> 1, p = mrow & 1;
+                    const uint32_t t0 = tmem_base + ((uint32_t)(wq * 32) << 16) + job->g[g].tmem_col;
+                    if (wq * rows_w < gn) {                             // warp-uniform
+                        for (int c = half; c < (gn >> 4); c += 2) {
+                            uint32_t x[16];
+                            tmem_ld16(t0 + c * 16, x);
+                            tmem_ld_wait();
+                            float val[8];
+#pragma unroll
+                            for (int r = 0; r < 8; ++r) {
+                                const float o = __shfl_xor_sync(0xffffffffu, __uint_as_float(x[8 + r]), 8);
+                                val[r] = pl ? __uint_as_float(x[r]) - o : __uint_as_float(x[r]) + o;
+                            }
+                            // re-plane lanes finish columns 0-3 of the chunk, im-plane lanes columns 4-7
+                            float re[4], im[4];
+#pragma unroll
+                            for (int q = 0; q < 4; ++q) {
+                                const float got = __shfl_xor_sync(0xffffffffu, pl ? val[q] : val[4 + q], 8);
+                                re[q] = pl ? got : val[q];
+                                im[q] = pl ? val[4 + q] : got;
+                            }
+                            const int b0 = job->g[g].out_col + 8 * c + 4 * pl;      // input index of column q = 0
+#pragma unroll
+                            for (int e = 0; e < 2; ++e) {
+                                const int b = b0 + 2 * e, k = b >> 1;
+                                if (row_ok && b < a.M && i <= k)
+                                    vc[((size_t)k * (k + 1) / 2 + i) * 2 + p] =
+                                        make_float4(re[2 * e] * inv_s2, im[2 * e] * inv_s2, re[2 * e + 1] * inv_s2, im[2 * e + 1] * inv_s2);
+                            }
+                        }
+                    }
+                    continue;
+                }
                 const int row0 = job->g[g].out_row + wq * rows_w;      // first input index of this warp's lanes
                 const int arow = row0 + (lane & (rows_w - 1));
                 const bool lane_ok = lane < rows_w && arow >= row_min && arow < a.M;
@@ -331,14 +376,14 @@ void build_xjobs(cobalt_plan_s *p) {
         j.ld_row[1] = 0;
         j.ld_nrows[1] = 0;
         j.n_groups = 1;
-        j.g[0] = XMmaGroup{0, 0, Mpad, 0, 0, 0, 128, 0};
+        j.g[0] = XMmaGroup{0, 0, Mpad, 0, 0, 0, 128, 0, 0};
         int cols = 2 * Mpad;
         if (Mpad > 128) {
             j.n_groups = 2;
-            // rows [128, Mpad) x columns [128, Mpad) as an M = 64 instruction over the last 64 rows (an M = 128
-            // instruction with N <= 64 is bound by its 4 KB A-operand read, M = 64 reads half of that)
-            j.g[1] = XMmaGroup{Mpad - 64, 128, Mpad - 128, 2 * Mpad, Mpad - 64, 128, 64, 128};
-            cols += 2 * (Mpad - 128);
+            // rows and columns [128, Mpad): one stacked product per k-step (kind 1), 2 (Mpad - 128) rows and columns
+            const int nw = 2 * (Mpad - 128);
+            j.g[1] = XMmaGroup{128, 128, nw, 2 * Mpad, 128, 128, nw <= 64 ? 64 : 128, 128, 1};
+            cols += nw;
         }
         j.tmem_cols = pow2_cols(cols);
         p->jobs.push_back(j);
@@ -359,27 +404,36 @@ void build_xjobs(cobalt_plan_s *p) {
                     j.ld_nrows[0] = na > n ? na : n;
                     j.ld_row[1] = 0;
                     j.ld_nrows[1] = 0;
-                    j.g[0] = XMmaGroup{0, 0, n, 0, r0, c0, na <= 64 ? 64 : 128, r0};
+                    j.g[0] = XMmaGroup{0, 0, n, 0, r0, c0, na <= 64 ? 64 : 128, r0, 0};
                 } else {
                     j.ld_row[0] = r0;
                     j.ld_nrows[0] = na;
                     j.ld_row[1] = c0;
                     j.ld_nrows[1] = n;
-                    j.g[0] = XMmaGroup{0, na, n, 0, r0, c0, na <= 64 ? 64 : 128, r0};
+                    j.g[0] = XMmaGroup{0, na, n, 0, r0, c0, na <= 64 ? 64 : 128, r0, 0};
                 }
                 j.tmem_cols = pow2_cols(2 * n);
                 p->jobs.push_back(j);
             }
         }
     }
-    int max_rows = 0;
-    for (const XJob &j : p->jobs) max_rows = (j.ld_nrows[0] + j.ld_nrows[1]) > max_rows ? (j.ld_nrows[0] + j.ld_nrows[1]) : max_rows;
-    const size_t stage_bytes = (size_t)max_rows * 128 * 2;
-    const size_t budget = 227 * 1024 - 1024 /*alignment*/ - kBarrierBytes - kSlackBytes;
+    int max_rows = 0, slack_rows = 0;
+    for (const XJob &j : p->jobs) {
+        const int rows = j.ld_nrows[0] + j.ld_nrows[1];
+        max_rows = rows > max_rows ? rows : max_rows;
+    }
+    for (const XJob &j : p->jobs)      // an A operand always reads its instruction's M rows, loaded or not
+        for (int g = 0; g < j.n_groups; ++g) {
+            const int reach = j.g[g].a_row + (j.g[g].kind == 1 ? j.g[g].m / 2 : j.g[g].m);
+            slack_rows = reach - max_rows > slack_rows ? reach - max_rows : slack_rows;
+        }
+    const size_t stage_bytes = (size_t)max_rows * 256;
+    const size_t slack = (size_t)slack_rows * 256;
+    const size_t budget = 227 * 1024 - 1024 /*alignment*/ - kBarrierBytes - slack;
     int stages = (int)(budget / stage_bytes);
     if (stages > 8) stages = 8;
     p->x_stages = stages;
-    p->x_smem_bytes = 1024 + kBarrierBytes + (size_t)stages * stage_bytes + kSlackBytes;
+    p->x_smem_bytes = 1024 + kBarrierBytes + (size_t)stages * stage_bytes + slack;
 }
 
 cudaError_t launch_xstage_tc(const cobalt_plan_s *p, cudaStream_t st, const void *d_z, int nb, float2 *d_vis) {
@@ -400,7 +454,7 @@ cudaError_t launch_xstage_tc(const cobalt_plan_s *p, cudaStream_t st, const void
     a.stages = p->x_stages;
     int max_rows = 0;
     for (const XJob &j : p->jobs) max_rows = (j.ld_nrows[0] + j.ld_nrows[1]) > max_rows ? (j.ld_nrows[0] + j.ld_nrows[1]) : max_rows;
-    a.stage_bytes = max_rows * 128 * 2;
+    a.stage_bytes = max_rows * 256;
     cudaError_t e = cudaFuncSetAttribute(xstage_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->x_smem_bytes);
     if (e != cudaSuccess) return e;
     const int grid = a.total_jobs < p->sm_count ? a.total_jobs : p->sm_count;

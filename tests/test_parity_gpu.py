@@ -122,7 +122,7 @@ def test_channelised_matches_oracle(cobalt, oracle, dev, C, bits, S, n_t, mode_t
 
 
 # ------------------------------------------------------------------ P14: X-stage indexing, bit-exact
-@pytest.mark.parametrize("S,n_t", [(1, 5), (3, 64), (8, 100), (48, 130), (77, 70), (100, 64), (130, 65), (288, 40)])
+@pytest.mark.parametrize("S,n_t", [(1, 5), (3, 64), (8, 100), (48, 130), (64, 66), (70, 66), (77, 70), (81, 129), (88, 64), (96, 70), (100, 64), (130, 65), (288, 40)])
 @pytest.mark.parametrize("mode_tensor", [False, True])
 def test_p14_correlate_small_integers_bit_exact(cobalt, oracle, dev, S, n_t, mode_tensor):
     """Small integers are exact in fp16 and their sums exact in fp32, so the X-stage must equal integer
