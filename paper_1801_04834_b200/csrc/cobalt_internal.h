@@ -91,6 +91,8 @@ struct cobalt_plan_s {
     cobalt::XJob *d_jobs = nullptr;
     size_t x_smem_bytes = 0;
     int x_stages = 0;
+    bool x_staged = false;             // X-stage epilogue through a shared-memory image of the channel's output block
+    size_t x_out_off = 0;
     size_t scratch_bytes = 0;
     // host-buffer path
     cudaStream_t hs[3] = {nullptr, nullptr, nullptr};

@@ -28,9 +28,11 @@ namespace cobalt {
 
 namespace {
 
-constexpr int kEpiWarps = 8;            // two per TMEM lane quarter, alternating 16-column chunks
+constexpr int kEpiWarps = 16;           // four per TMEM lane quarter, taking every fourth 16-column chunk
+constexpr int kEpiSub = kEpiWarps / 4;
 constexpr int kThreads = 64 + 32 * kEpiWarps;
-constexpr int kBarrierBytes = 1024;
+constexpr int kBarrierBytes = 4096;       // mbarriers (first 512 bytes) + a copy of the job table
+constexpr int kMaxSmemJobs = (kBarrierBytes - 512) / (int)sizeof(XJob);
 
 struct XArgs {
     const unsigned char *z;
@@ -40,6 +42,7 @@ struct XArgs {
     size_t z_subband_bytes;
     long long n_bl;
     int C, M, Mpad, n_kt, jobs_per_channel, total_jobs, stages, stage_bytes;
+    uint32_t out_off;       // STAGED: byte offset of the visibility staging block from the 1024-aligned smem base
 };
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -66,6 +69,24 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
             : "r"(bar), "r"(parity), "r"(20000u)
             : "memory");
     } while (!done);
+}
+// Spin without a suspend hint: for the one wait whose wake-up latency is on the critical path.
+__device__ __forceinline__ void mbar_wait_spin(uint32_t bar, uint32_t parity) {
+    uint32_t done;
+    do {
+        asm volatile(
+            "{\n\t"
+            ".reg .pred p;\n\t"
+            "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t"
+            "}"
+            : "=r"(done)
+            : "r"(bar), "r"(parity)
+            : "memory");
+    } while (!done);
+}
+__device__ __forceinline__ void bulk_s2g(void *dst, uint32_t src, uint32_t bytes) {
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(src), "r"(bytes) : "memory");
 }
 __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t bytes, uint32_t bar) {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
@@ -119,6 +140,11 @@ __device__ __forceinline__ bool elect_one() {
 }
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 
+// STAGED (one job per channel and the channel's [n_bl][2][2] block fits in shared memory): the epilogue writes
+// the visibilities into a shared-memory image of the channel's output block and one thread sends it to global
+// memory with a single bulk copy (cp.async.bulk, SASS UBLKCP) that drains while the next job's MMAs run; the
+// accumulators are handed back as soon as the last TMEM load has landed.
+template <bool STAGED>
 __global__ void __launch_bounds__(kThreads, 1) xstage_tc_kernel(const XArgs a) {
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     // carve: [barriers 1 KB][stages ...][slack]; stage base must be 1024-byte aligned for the swizzle
@@ -130,6 +156,15 @@ __global__ void __launch_bounds__(kThreads, 1) xstage_tc_kernel(const XArgs a) {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int stages = a.stages;
 
+    // the job table is read by every role for every job: keep it in shared memory (global-memory latency would sit
+    // on the epilogue's critical path)
+    const XJob *jobs = a.jobs;
+    if (a.jobs_per_channel <= kMaxSmemJobs) {
+        int *dst = reinterpret_cast<int *>(smem_raw + (smem_base - smem_u32(smem_raw)) + 512);
+        const int *src = reinterpret_cast<const int *>(a.jobs);
+        for (int w = threadIdx.x; w < a.jobs_per_channel * (int)(sizeof(XJob) / 4); w += kThreads) dst[w] = src[w];
+        jobs = reinterpret_cast<const XJob *>(dst);
+    }
     // every job of one plan allocates the same number of columns (max over jobs)
     int tmem_cols = 32;
     for (int j = 0; j < a.jobs_per_channel; ++j) tmem_cols = max(tmem_cols, a.jobs[j].tmem_cols);
@@ -164,8 +199,8 @@ __global__ void __launch_bounds__(kThreads, 1) xstage_tc_kernel(const XArgs a) {
                 const int jl = jid % a.jobs_per_channel;
                 const int prob = jid / a.jobs_per_channel;           // subband-of-chunk * C + channel
                 const int bl = prob / a.C, c = prob - bl * a.C;
-                const int r0 = a.jobs[jl].ld_row[0], r1 = a.jobs[jl].ld_row[1];
-                const uint32_t b0 = (uint32_t)a.jobs[jl].ld_nrows[0] * 256, b1 = (uint32_t)a.jobs[jl].ld_nrows[1] * 256;
+                const int r0 = jobs[jl].ld_row[0], r1 = jobs[jl].ld_row[1];
+                const uint32_t b0 = (uint32_t)jobs[jl].ld_nrows[0] * 256, b1 = (uint32_t)jobs[jl].ld_nrows[1] * 256;
                 const unsigned char *src = a.z + (size_t)bl * a.z_subband_bytes + (size_t)c * a.n_kt * kt_bytes;
                 for (int kt = 0; kt < a.n_kt; ++kt, src += kt_bytes) {
                     mbar_wait(bar_base + 8 * (16 + s), ph ^ 1);
@@ -192,7 +227,7 @@ __global__ void __launch_bounds__(kThreads, 1) xstage_tc_kernel(const XArgs a) {
             const uint64_t desc_both = make_smem_desc(stage_base, 1024);    // [Zr; Zi] stacked 8 rows at a time
             const uint32_t stage_units = (uint32_t)a.stage_bytes >> 4;
             for (int jid = blockIdx.x; jid < a.total_jobs; jid += gridDim.x, ++it) {
-                const XJob *job = a.jobs + jid % a.jobs_per_channel;
+                const XJob *job = jobs + jid % a.jobs_per_channel;
                 const int n_groups = job->n_groups;
                 uint32_t g_a[kMaxMmaGroups], g_b[kMaxMmaGroups], g_d[kMaxMmaGroups], g_n[kMaxMmaGroups];
                 uint32_t g_pos[kMaxMmaGroups], g_neg[kMaxMmaGroups], g_kind[kMaxMmaGroups];
@@ -207,7 +242,7 @@ __global__ void __launch_bounds__(kThreads, 1) xstage_tc_kernel(const XArgs a) {
                     g_pos[g] = make_idesc(grp.m, grp.n, 0);
                     g_neg[g] = make_idesc(grp.m, grp.n, 1);
                 }
-                mbar_wait(tmem_empty, (it & 1) ^ 1);       // epilogue has drained the accumulators
+                mbar_wait_spin(tmem_empty, (it & 1) ^ 1);  // epilogue has drained the accumulators
                 tc_fence_after();
                 for (int kt = 0; kt < a.n_kt; ++kt) {
                     mbar_wait(bar_base + 8 * s, ph);
@@ -250,15 +285,21 @@ __global__ void __launch_bounds__(kThreads, 1) xstage_tc_kernel(const XArgs a) {
         // take alternate 16-column chunks.  The TMEM load of a warp's next chunk is in flight while it stores the
         // current one.
         const int wq = warp & 3;
-        const int half = (warp - 2) >> 2;
+        const int sub = (warp - 2) >> 2;
         const float inv_s2 = __ldg(a.scale + 2);           // undo the power-of-two operand scale (exact)
         uint32_t it = 0;
         for (int jid = blockIdx.x; jid < a.total_jobs; jid += gridDim.x, ++it) {
             const int jl = jid % a.jobs_per_channel;
             const int prob = jid / a.jobs_per_channel;
-            const XJob *job = a.jobs + jl;
+            const XJob *job = jobs + jl;
             const int n_groups = job->n_groups;
-            float4 *vc = reinterpret_cast<float4 *>(a.vis + (size_t)prob * a.n_bl * 4);
+            float4 *vg = reinterpret_cast<float4 *>(a.vis + (size_t)prob * a.n_bl * 4);
+            float4 *vc = STAGED ? reinterpret_cast<float4 *>(smem_raw + (smem_base - smem_u32(smem_raw)) + a.out_off) : vg;
+            if (STAGED && it > 0) {
+                // the previous job's bulk store must have read the staging block before it is overwritten
+                if (threadIdx.x == 64) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+                asm volatile("bar.sync 1, %0;" ::"n"(32 * kEpiWarps) : "memory");
+            }
             mbar_wait(tmem_full, it & 1);
             tc_fence_after();
             for (int g = 0; g < n_groups; ++g) {
@@ -278,7 +319,7 @@ __global__ void __launch_bounds__(kThreads, 1) xstage_tc_kernel(const XArgs a) {
                     const int i = mrow >> 1, p = mrow & 1;
                     const uint32_t t0 = tmem_base + ((uint32_t)(wq * 32) << 16) + job->g[g].tmem_col;
                     if (wq * rows_w < gn) {                             // warp-uniform
-                        for (int c = half; c < (gn >> 4); c += 2) {
+                        for (int c = sub; c < (gn >> 4); c += kEpiSub) {
                             uint32_t x[16];
                             tmem_ld16(t0 + c * 16, x);
                             tmem_ld_wait();
@@ -314,38 +355,60 @@ __global__ void __launch_bounds__(kThreads, 1) xstage_tc_kernel(const XArgs a) {
                 const int i = arow >> 1, p = arow & 1;
                 if (row0 >= a.M || row0 + rows_w <= row_min) continue;
                 const uint32_t t0 = tmem_base + ((uint32_t)(wq * 32) << 16) + job->g[g].tmem_col;
-                // chunks of this warp: c0 = 16 (2 q + half), on or above the diagonal, inside the matrix
-                int c_first = max(0, (max(row0, row_min) & ~1) - out_col) >> 4;     // first chunk touching k >= i
-                if ((c_first & 1) != half) ++c_first;
-                int c_end = (min(gn, a.M - out_col) + 15) >> 4;
+                // chunks of this warp: every kEpiSub-th chunk on or above the diagonal, inside the matrix
+                const int c_first = (max(0, (max(row0, row_min) & ~1) - out_col) >> 4) + sub;   // first chunk touching k >= i
+                const int c_end = (min(gn, a.M - out_col) + 15) >> 4;
+                const int i_max = (min(row0 + rows_w, a.M) - 1) >> 1;           // last station of this warp's rows
                 uint32_t re[16], im[16];
                 if (c_first < c_end) {
                     tmem_ld16(t0 + c_first * 16, re);
                     tmem_ld16(t0 + gn + c_first * 16, im);
                 }
-                for (int c = c_first; c < c_end; c += 2) {
+                for (int c = c_first; c < c_end; c += kEpiSub) {
                     tmem_ld_wait();
                     float4 v[8];
 #pragma unroll
                     for (int e = 0; e < 8; ++e)
                         v[e] = make_float4(__uint_as_float(re[2 * e]) * inv_s2, __uint_as_float(im[2 * e]) * inv_s2,
                                            __uint_as_float(re[2 * e + 1]) * inv_s2, __uint_as_float(im[2 * e + 1]) * inv_s2);
-                    if (c + 2 < c_end) {
-                        tmem_ld16(t0 + (c + 2) * 16, re);
-                        tmem_ld16(t0 + gn + (c + 2) * 16, im);
+                    if (c + kEpiSub < c_end) {
+                        tmem_ld16(t0 + (c + kEpiSub) * 16, re);
+                        tmem_ld16(t0 + gn + (c + kEpiSub) * 16, im);
                     }
                     const int col0 = out_col + c * 16;
+                    const int k0 = col0 >> 1;
+                    if (k0 >= i_max && col0 + 16 <= a.M) {
+                        // whole chunk above the diagonal for every row of the warp: baseline index of (i, k0 + e) steps by k
+                        if (lane_ok) {
+                            int idx = (k0 * (k0 + 1) / 2 + i) * 2 + p;
 #pragma unroll
-                    for (int e = 0; e < 8; ++e) {
-                        const int b = col0 + 2 * e, k = b >> 1;
-                        if (lane_ok && b < a.M && i <= k) vc[((size_t)k * (k + 1) / 2 + i) * 2 + p] = v[e];
+                            for (int e = 0; e < 8; ++e) {
+                                vc[idx] = v[e];
+                                idx += 2 * (k0 + e + 1);
+                            }
+                        }
+                    } else {
+#pragma unroll
+                        for (int e = 0; e < 8; ++e) {
+                            const int b = col0 + 2 * e, k = b >> 1;
+                            if (lane_ok && b < a.M && i <= k) vc[((size_t)k * (k + 1) / 2 + i) * 2 + p] = v[e];
+                        }
                     }
                 }
             }
             tc_fence_before();
             __syncwarp();
-            if (lane == 0) mbar_arrive(tmem_empty);
+            if (lane == 0) mbar_arrive(tmem_empty);        // every TMEM load of this warp has completed (wait::ld)
+            if (STAGED) {
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy writes -> visible to the bulk copy
+                asm volatile("bar.sync 2, %0;" ::"n"(32 * kEpiWarps) : "memory");
+                if (threadIdx.x == 64) {
+                    bulk_s2g(vg, smem_base + a.out_off, (uint32_t)(a.n_bl * 32));
+                    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+                }
+            }
         }
+        if (STAGED && threadIdx.x == 64) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
     }
 
     tc_fence_before();
@@ -429,11 +492,17 @@ void build_xjobs(cobalt_plan_s *p) {
         }
     const size_t stage_bytes = (size_t)max_rows * 256;
     const size_t slack = (size_t)slack_rows * 256;
-    const size_t budget = 227 * 1024 - 1024 /*alignment*/ - kBarrierBytes - slack;
+    // staged epilogue: the whole [n_bl][2][2] block of a channel, if that still leaves three load stages
+    size_t out_bytes = ((size_t)p->n_bl * 32 + 127) / 128 * 128;
+    const size_t fixed = 1024 /*alignment*/ + kBarrierBytes + slack;
+    p->x_staged = p->jobs.size() == 1 && fixed + out_bytes + 3 * stage_bytes <= (size_t)227 * 1024;
+    if (!p->x_staged) out_bytes = 0;
+    const size_t budget = 227 * 1024 - fixed - out_bytes;
     int stages = (int)(budget / stage_bytes);
     if (stages > 8) stages = 8;
     p->x_stages = stages;
-    p->x_smem_bytes = 1024 + kBarrierBytes + (size_t)stages * stage_bytes + slack;
+    p->x_out_off = kBarrierBytes + (size_t)stages * stage_bytes + slack;
+    p->x_smem_bytes = fixed + (size_t)stages * stage_bytes + out_bytes;
 }
 
 cudaError_t launch_xstage_tc(const cobalt_plan_s *p, cudaStream_t st, const void *d_z, int nb, float2 *d_vis) {
@@ -455,10 +524,12 @@ cudaError_t launch_xstage_tc(const cobalt_plan_s *p, cudaStream_t st, const void
     int max_rows = 0;
     for (const XJob &j : p->jobs) max_rows = (j.ld_nrows[0] + j.ld_nrows[1]) > max_rows ? (j.ld_nrows[0] + j.ld_nrows[1]) : max_rows;
     a.stage_bytes = max_rows * 256;
-    cudaError_t e = cudaFuncSetAttribute(xstage_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->x_smem_bytes);
+    a.out_off = (uint32_t)p->x_out_off;
+    auto kern = p->x_staged ? xstage_tc_kernel<true> : xstage_tc_kernel<false>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->x_smem_bytes);
     if (e != cudaSuccess) return e;
     const int grid = a.total_jobs < p->sm_count ? a.total_jobs : p->sm_count;
-    xstage_tc_kernel<<<grid, kThreads, p->x_smem_bytes, st>>>(a);
+    kern<<<grid, kThreads, p->x_smem_bytes, st>>>(a);
     return cudaGetLastError();
 }
 
