@@ -19,9 +19,10 @@
 //   real products at once; the epilogue adds / subtracts its quadrants)            (2S <= 192)
 // or, for large arrays, one (128-row block) x (<= 256-column chunk) tile per job.
 //
-// Warp roles (320 threads, persistent CTAs, one per SM): warp 0 = bulk-copy producer, warp 1 = TMEM
-// allocator + single-thread MMA issuer, warps 2-9 = epilogue (tcgen05.ld -> triangular baseline
-// index -> coalesced 16-byte stores of (re, im) pairs).
+// Warp roles (576 threads, persistent CTAs, one per SM): warp 0 = bulk-copy producer, warp 1 = TMEM
+// allocator + single-thread MMA issuer, warps 2-17 = epilogue (tcgen05.ld -> triangular baseline
+// index -> 16-byte stores of (re, im) pairs into a shared-memory image of the channel's output block,
+// which leaves with one bulk store; direct global stores when the block does not fit).
 #include "cobalt_internal.h"
 
 namespace cobalt {
