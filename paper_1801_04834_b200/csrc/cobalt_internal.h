@@ -118,6 +118,8 @@ cudaError_t launch_phase_table(const cobalt_plan_s *p, cudaStream_t st, const do
                                const float *d_bandpass, int b0, int nb);
 // samples_b0 points at the first subband of the chunk [b0, b0 + nb)
 cudaError_t launch_fstage(const cobalt_plan_s *p, cudaStream_t st, const void *samples_b0, int b0, int nb);
+// fstage_tc.cu (C = 256, TENSOR_FP16: DFT on the tensor cores) ------------------------------
+cudaError_t launch_fstage_tc(const cobalt_plan_s *p, cudaStream_t st, const void *samples_b0, int b0, int nb);
 cudaError_t launch_history_update(const cobalt_plan_s *p, cudaStream_t st, const void *samples_b0, int b0, int nb);
 cudaError_t launch_unpack(cudaStream_t st, int bits, const void *d_in, long long n, float *d_out);
 // layout.cu ---------------------------------------------------------------------------------

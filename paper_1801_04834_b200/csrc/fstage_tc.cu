@@ -1,0 +1,534 @@
+// F-stage for C = 256, TENSOR_FP16 mode, with the 256-point DFT on the 5th-generation tensor cores.
+//
+// Same steps a1-a7 as fstage.cu and the same inputs,
+// outputs and layouts; what differs is where the DFT runs.  fstage.cu does FIR and FFT on the FP32 pipe and is
+// bound by it (profiles/: sm__pipe_fma_cycles_active 71 %).  Here the DFT is the 16 x 16 Cooley-Tukey split
+//
+//   D[k1 + 16 k2] = sum_r W16^{r k2} ( W256^{r k1} ( sum_q W16^{q k1} y[r + 16 q] ) )
+//
+// and each 16-point pass is a real GEMM on tcgen05 (fp16 operands, fp32 accumulation in TMEM):
+//   [rows (spectrum t, r)] x [K = 32: (q, re/im)] x [N = 32: (k1, re/im)]   then
+//   [rows (spectrum t, k1)] x [K = 32: (r, re/im)] x [N = 32: (k2, re/im)]
+// with the same 32 x 32 matrix.  The FP32 pipe keeps the FIR (exact products of integers and fp32 weights),
+// the inter-pass twiddle W256^{r k1} and the rotation * bandpass; every intermediate that becomes an fp16
+// operand carries an exact power-of-two scale (a1 on the FIR output, a2 after the first pass) that the
+// rotation table undoes.
+//
+// Warp roles (19 warps, one CTA per SM, one stream per CTA):
+//   0-7   FIR: thread = polyphase branch, as in fstage.cu; output y as (re, im) fp16 pairs into operand tile A1
+//   8-15  pass epilogues: warp = (TMEM lane quarter, half of the 16 output columns).  For sub-tile i: D1 ->
+//         * W256^{r k1} -> fp16 -> operand tile A2; for sub-tile i - 1: D2 -> * rotation -> fp16 -> staging tile
+//         (spectra t, t + 1 paired through one shuffle), as the tensor store of fstage.cu expects it
+//   16    producer (bulk copies of raw samples), 17 tensor-store issuer, 18 TMEM allocator + MMA issuer
+#include "cobalt_internal.h"
+
+namespace cobalt {
+
+namespace {
+
+struct FArgsTC {
+    const unsigned char *samples;   // [nb][S][2][N] complex integers, first subband of the chunk
+    const unsigned char *hist;      // [B][S][2][15 C] complex integers
+    const float *weights;           // [16][C]
+    const float2 *phase;            // [nb][S][C]
+    long long N, n_t;
+    int S, M, Mpad, n_kt, b0, tiles_per_seg;
+    float a1, inv_a1a2;             // operand scales (powers of two)
+};
+
+constexpr int kC = 256;
+constexpr int kFirWarps = 8, kEpiWarps = 8;
+constexpr int kProducerWarp = kFirWarps + kEpiWarps, kStoreWarp = kProducerWarp + 1, kMmaWarp = kProducerWarp + 2;
+constexpr int kThreadsTC = (kMmaWarp + 1) * 32;
+constexpr int kRawStages = 3, kABufs = 2, kStgBufs = 2;
+constexpr float kA2 = 0.0625f;      // scale of the first-pass output (|X1| <= 16 |y|)
+// Operand tiles: K-major, no swizzle.  The 16-byte chunk kc (8 fp16 of K) of row rho sits at
+// (rho / 8) * kSBO + kc * kLBO + (rho % 8) * 16; the pads (144 instead of 128, 608 instead of 576) spread the
+// pass-epilogue stores over all banks.
+constexpr int kLBO = 144, kSBO = 608;
+constexpr int kATile = 32 * kSBO;   // 256 rows
+constexpr int kBTile = 4 * kSBO;    // 32 rows
+constexpr int kStgBytes = 2 * kC * 64;   // one stream: [2 planes][C channels][32 spectra] fp16
+
+template <int BITS>
+struct ShTC {
+    static constexpr int SB = BITS == 16 ? 4 : 2;
+    static constexpr int RAW_STAGE = kSubTile * kC * SB;
+    static constexpr int OFF_BAR = 0;
+    static constexpr int OFF_STG = 1024;
+    static constexpr int OFF_RAW = OFF_STG + kStgBufs * kStgBytes;
+    static constexpr int OFF_A1 = OFF_RAW + kRawStages * RAW_STAGE;
+    static constexpr int OFF_A2 = OFF_A1 + kABufs * kATile;
+    static constexpr int OFF_B = OFF_A2 + kABufs * kATile;
+    static constexpr int TOTAL = OFF_B + kBTile;
+    static_assert(TOTAL <= 227 * 1024, "shared memory budget");
+};
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    uint32_t done;
+    do {
+        asm volatile(
+            "{\n\t"
+            ".reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t"
+            "}"
+            : "=r"(done)
+            : "r"(bar), "r"(parity), "r"(20000u)
+            : "memory");
+    } while (!done);
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t bytes, uint32_t bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+                 "l"(src), "r"(bytes), "r"(bar)
+                 : "memory");
+}
+__device__ __forceinline__ bool elect_one() {
+    uint32_t pred;
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "elect.sync _|p, 0xffffffff;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t"
+        "}"
+        : "=r"(pred));
+    return pred != 0;
+}
+__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_commit(uint32_t bar) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void tc_mma(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t acc) {
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t"
+        "}" ::"r"(d_tmem),
+        "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(acc)
+        : "memory");
+}
+// K-major, no swizzle: chunks of K kLBO bytes apart, 8-row groups kSBO bytes apart, descriptor version 1 (sm_100).
+__device__ __forceinline__ uint64_t make_desc(uint32_t addr) {
+    return (uint64_t)((addr >> 4) & 0x3FFFu) | ((uint64_t)(kLBO >> 4) << 16) | ((uint64_t)(kSBO >> 4) << 32) | (1ull << 46);
+}
+// kind::f16 instruction descriptor: D = f32, A = B = f16, both K-major, M = 128, N = 32.
+constexpr uint32_t kIdesc = (1u << 4) | ((uint32_t)(32 >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&v)[16]) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, "
+        "[%16];"
+        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]),
+          "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+        : "r"(taddr));
+}
+__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+
+__device__ __forceinline__ uint32_t pack_half2(float lo, float hi) {
+    const __half2 t = __floats2half2_rn(lo, hi);
+    return *reinterpret_cast<const uint32_t *>(&t);
+}
+// v * (t.x + i t.y) with packed fp32 pairs (see fstage.cu)
+__device__ __forceinline__ float2 cmul(float2 v, float2 t) {
+    const float2 p = __fmul2_rn(make_float2(v.x, v.x), t);
+    return __ffma2_rn(make_float2(-t.y, t.x), make_float2(v.y, v.y), p);
+}
+template <int BITS>
+__device__ __forceinline__ float2 unpack_sample(uint32_t raw) {
+    // Step a1: the two's-complement integer value as a float, exact.
+    if (BITS == 16) return make_float2((float)(short)(raw & 0xffffu), (float)(short)(raw >> 16));
+    return make_float2((float)(signed char)(raw & 0xffu), (float)(signed char)((raw >> 8) & 0xffu));
+}
+
+template <int BITS>
+__global__ void __launch_bounds__(kThreadsTC, 1) fstage_tc_kernel(const FArgsTC a, const __grid_constant__ CUtensorMap zmap) {
+    using Sh = ShTC<BITS>;
+    constexpr int SB = Sh::SB, C = kC;
+    extern __shared__ __align__(1024) unsigned char smem[];
+    const uint32_t sbase = smem_u32(smem);
+    const uint32_t bar_raw_full = sbase + Sh::OFF_BAR;              // [kRawStages]
+    const uint32_t bar_raw_empty = bar_raw_full + 8 * kRawStages;   // [kRawStages]
+    const uint32_t bar_a1_full = bar_raw_empty + 8 * kRawStages;    // [2] FIR -> MMA
+    const uint32_t bar_a1_empty = bar_a1_full + 16;                 // [2] MMA (commit) -> FIR
+    const uint32_t bar_d1_full = bar_a1_empty + 16;                 // [2] MMA (commit) -> epilogue
+    const uint32_t bar_d1_empty = bar_d1_full + 16;                 // [2] epilogue -> MMA
+    const uint32_t bar_a2_full = bar_d1_empty + 16;                 // [2] epilogue -> MMA
+    const uint32_t bar_a2_empty = bar_a2_full + 16;                 // [2] MMA (commit) -> epilogue
+    const uint32_t bar_d2_full = bar_a2_empty + 16;                 // [2]
+    const uint32_t bar_d2_empty = bar_d2_full + 16;                 // [2]
+    const uint32_t bar_stg_full = bar_d2_empty + 16;                // [kStgBufs] epilogue -> store issuer
+    const uint32_t bar_stg_empty = bar_stg_full + 8 * kStgBufs;     // [kStgBufs]
+    const uint32_t tmem_slot = bar_stg_empty + 8 * kStgBufs;
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int bl = blockIdx.x / a.M;                     // subband of the chunk
+    const int m = blockIdx.x - bl * a.M;                 // input (2 station + pol) = stream of the subband
+    const int kt0 = blockIdx.y * a.tiles_per_seg;
+    const int kt1 = min(kt0 + a.tiles_per_seg, a.n_kt);
+    const int n_sub = (kt1 - kt0) * (kKTile / kSubTile);
+    const long long t0 = (long long)kt0 * kKTile;
+
+    if (tid == 0) {
+        for (int s = 0; s < kRawStages; ++s) {
+            mbar_init(bar_raw_full + 8 * s, 1);
+            mbar_init(bar_raw_empty + 8 * s, kFirWarps);
+        }
+        for (int b = 0; b < 2; ++b) {
+            mbar_init(bar_a1_full + 8 * b, kFirWarps);
+            mbar_init(bar_a1_empty + 8 * b, 1);
+            mbar_init(bar_d1_full + 8 * b, 1);
+            mbar_init(bar_d1_empty + 8 * b, kEpiWarps);
+            mbar_init(bar_a2_full + 8 * b, kEpiWarps);
+            mbar_init(bar_a2_empty + 8 * b, 1);
+            mbar_init(bar_d2_full + 8 * b, 1);
+            mbar_init(bar_d2_empty + 8 * b, kEpiWarps);
+        }
+        for (int b = 0; b < kStgBufs; ++b) {
+            mbar_init(bar_stg_full + 8 * b, 2 * kEpiWarps);      // two sub-tiles of 16 spectra per staged tile
+            mbar_init(bar_stg_empty + 8 * b, 1);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    {   // The 16-point DFT as a real 32 x 32 matrix, B[n = 2 k + c][kk = 2 q + c'] (K-major rows n):
+        // out_re(k) = sum_q yr Wr - yi Wi, out_im(k) = sum_q yr Wi + yi Wr, W = exp(-2 pi i q k / 16).
+        for (int idx = tid; idx < 32 * 32; idx += kThreadsTC) {
+            const int n = idx >> 5, kk = idx & 31;
+            const int k = n >> 1, c = n & 1, q = kk >> 1, cc = kk & 1;
+            float sn, cs;
+            sincospif(-2.0f * (float)((q * k) & 15) / 16.0f, &sn, &cs);      // W = cs + i sn
+            const float v = c == cc ? cs : (c ? sn : -sn);
+            *reinterpret_cast<__half *>(smem + Sh::OFF_B + (n >> 3) * kSBO + (kk >> 3) * kLBO + (n & 7) * 16 + (kk & 7) * 2) =
+                __float2half_rn(v);
+        }
+        fence_async_smem();
+    }
+    if (warp == kMmaWarp) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tmem_slot), "r"(256) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    uint32_t tmem_base;
+    asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
+
+    if (warp == kProducerWarp) {
+        // ------------------------------------------------------------------ producer (as in fstage.cu)
+        const size_t stream = (size_t)bl * a.M + m;
+        for (int j = 0; j <= n_sub; ++j) {
+            const int s = j % kRawStages;
+            mbar_wait(bar_raw_empty + 8 * s, ((uint32_t)(j / kRawStages) & 1u) ^ 1u);
+            const long long tb = t0 - kSubTile + (long long)j * kSubTile;     // first row of the sub-tile
+            const uint32_t full = bar_raw_full + 8 * s;
+            const uint32_t dst0 = sbase + Sh::OFF_RAW + s * Sh::RAW_STAGE;
+            uint32_t tx = 0;
+#pragma unroll
+            for (int part = 0; part < 2; ++part) {
+                // part 0: rows from the carried history (t < 0); part 1: rows of this call's block
+                long long lo, hi;
+                const unsigned char *src;
+                if (part == 0) {
+                    lo = max(tb, -(long long)(kTaps - 1));
+                    hi = min(tb + kSubTile, 0ll);
+                    src = a.hist + (((size_t)(a.b0 + bl) * a.M + m) * (kTaps - 1) + (size_t)(lo + kTaps - 1)) * C * SB;
+                } else {
+                    lo = max(tb, 0ll);
+                    hi = min(tb + kSubTile, a.n_t);
+                    src = a.samples + (stream * (size_t)a.N + (size_t)lo * C) * SB;
+                }
+                if (hi <= lo) continue;
+                const uint32_t bytes = (uint32_t)(hi - lo) * C * SB;
+                const uint32_t dst = dst0 + (uint32_t)(lo - tb) * C * SB;
+                if ((reinterpret_cast<uintptr_t>(src) & 15u) == 0) {
+                    if (lane == 0) bulk_g2s(dst, src, bytes, full);
+                    tx += bytes;
+                } else {   // stream not 16-byte aligned (odd N): element-wise copy by the warp
+                    for (uint32_t e = lane * SB; e < bytes; e += 32 * SB) {
+                        if (SB == 4) {
+                            const uint32_t v = __ldg(reinterpret_cast<const uint32_t *>(src + e));
+                            asm volatile("st.shared.b32 [%0], %1;" ::"r"(dst + e), "r"(v) : "memory");
+                        } else {
+                            const unsigned short v = __ldg(reinterpret_cast<const unsigned short *>(src + e));
+                            asm volatile("st.shared.b16 [%0], %1;" ::"r"(dst + e), "h"(v) : "memory");
+                        }
+                    }
+                }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive_expect_tx(full, tx);
+        }
+    } else if (warp == kStoreWarp) {
+        // ------------------------------------------------------------------ tensor-store issuer (step a7, as in fstage.cu)
+        if (elect_one()) {
+            for (int tile = 0; tile < n_sub / 2; ++tile) {
+                const int sbuf = tile & 1;
+                mbar_wait(bar_stg_full + 8 * sbuf, (uint32_t)(tile >> 1) & 1u);
+                const int kt = kt0 + (tile >> 1);
+                const int c0 = 32 * ((tile & 1) ^ ((m >> 2) & 1));
+                asm volatile(
+                    "cp.async.bulk.tensor.5d.global.shared::cta.bulk_group [%0, {%2, %3, %4, %5, %6}], [%1];" ::"l"(&zmap),
+                    "r"(sbase + Sh::OFF_STG + sbuf * kStgBytes), "r"(c0), "r"(bl * C), "r"(2 * (m >> 3)), "r"(m & 7), "r"(kt)
+                    : "memory");
+                asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+                asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // shared memory has been read
+                mbar_arrive(bar_stg_empty + 8 * sbuf);
+            }
+            asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+        }
+    } else if (warp == kMmaWarp) {
+        // ------------------------------------------------------------------ MMA issuer
+        // Iteration i: first pass of sub-tile i (A1[i & 1] -> D1[i & 1]), then second pass of sub-tile i - 1.
+        // A tile = 256 rows = two M = 128 instructions; K = 32 = two k-steps of 16 (two 16-byte chunks each).
+        if (elect_one()) {
+            const uint64_t desc_b = make_desc(sbase + Sh::OFF_B);
+            for (int i = 0; i <= n_sub; ++i) {
+                if (i < n_sub) {
+                    const int b = i & 1;
+                    const uint32_t par = (uint32_t)(i >> 1) & 1u;
+                    mbar_wait(bar_a1_full + 8 * b, par);
+                    mbar_wait(bar_d1_empty + 8 * b, par ^ 1u);
+                    tc_fence_after();
+                    const uint64_t desc_a = make_desc(sbase + Sh::OFF_A1 + b * kATile);
+#pragma unroll
+                    for (int h = 0; h < 2; ++h)
+#pragma unroll
+                        for (int ks = 0; ks < 2; ++ks)
+                            tc_mma(tmem_base + (uint32_t)(b * 2 + h) * 32, desc_a + (uint64_t)((h * 16 * kSBO + ks * 2 * kLBO) >> 4),
+                                   desc_b + (uint64_t)((ks * 2 * kLBO) >> 4), kIdesc, (uint32_t)ks);
+                    tc_commit(bar_a1_empty + 8 * b);
+                    tc_commit(bar_d1_full + 8 * b);
+                }
+                if (i >= 1) {
+                    const int b = (i - 1) & 1;
+                    const uint32_t par = (uint32_t)((i - 1) >> 1) & 1u;
+                    mbar_wait(bar_a2_full + 8 * b, par);
+                    mbar_wait(bar_d2_empty + 8 * b, par ^ 1u);
+                    tc_fence_after();
+                    const uint64_t desc_a = make_desc(sbase + Sh::OFF_A2 + b * kATile);
+#pragma unroll
+                    for (int h = 0; h < 2; ++h)
+#pragma unroll
+                        for (int ks = 0; ks < 2; ++ks)
+                            tc_mma(tmem_base + 128 + (uint32_t)(b * 2 + h) * 32, desc_a + (uint64_t)((h * 16 * kSBO + ks * 2 * kLBO) >> 4),
+                                   desc_b + (uint64_t)((ks * 2 * kLBO) >> 4), kIdesc, (uint32_t)ks);
+                    tc_commit(bar_a2_empty + 8 * b);
+                    tc_commit(bar_d2_full + 8 * b);
+                }
+            }
+        }
+    } else if (warp < kFirWarps) {
+        // ------------------------------------------------------------------ FIR (steps a1, a2; as in fstage.cu)
+        // thread = branch ph = r + 16 q, r = lane / 2, q = 2 warp + lane % 2 (a warp reads 32 consecutive branches)
+        const int r = lane >> 1, q = 2 * warp + (lane & 1);
+        const int ph = r + 16 * q;
+        float wk[kTaps];
+        {
+            // (-1)^ph: channel j <- DFT bin (j + C/2) mod C; a1: power-of-two scale of the fp16 operand
+            const float sgn = (ph & 1) ? -a.a1 : a.a1;
+#pragma unroll
+            for (int k = 0; k < kTaps; ++k) wk[k] = a.weights[k * C + ph] * sgn;
+        }
+        float2 acc[kTaps];
+#pragma unroll
+        for (int k = 0; k < kTaps; ++k) acc[k] = make_float2(0.f, 0.f);
+        const uint32_t raw_thread = sbase + Sh::OFF_RAW + ph * SB;
+        // A1 element (row t * 16 + r, K position 2 q): (2 t + r / 8) kSBO + (q / 4) kLBO + (r % 8) 16 + (q % 4) 4
+        const uint32_t a1_thread = sbase + Sh::OFF_A1 + (r >> 3) * kSBO + (q >> 2) * kLBO + (r & 7) * 16 + (q & 3) * 4;
+
+        for (int j = 0; j <= n_sub; ++j) {
+            const int s = j % kRawStages;
+            mbar_wait(bar_raw_full + 8 * s, (uint32_t)(j / kRawStages) & 1u);
+            const int jj = j - 1;                         // real sub-tile index (j = 0 is the warm-up)
+            const int yb = jj & 1;
+            const uint32_t raw = raw_thread + s * Sh::RAW_STAGE;
+            if (jj >= 0) mbar_wait(bar_a1_empty + 8 * yb, ((uint32_t)(jj >> 1) & 1u) ^ 1u);
+            const uint32_t arow = a1_thread + (jj >= 0 ? yb : 0) * kATile;
+#pragma unroll
+            for (int half = 0; half < 2; ++half) {
+                uint32_t rw[kSubTile / 2];
+#pragma unroll
+                for (int i = 0; i < kSubTile / 2; ++i) {
+                    const uint32_t addr = raw + (half * 8 + i) * C * SB;
+                    if (SB == 4) asm volatile("ld.shared.b32 %0, [%1];" : "=r"(rw[i]) : "r"(addr));
+                    else {
+                        unsigned short hv;
+                        asm volatile("ld.shared.b16 %0, [%1];" : "=h"(hv) : "r"(addr));
+                        rw[i] = hv;
+                    }
+                }
+#pragma unroll
+                for (int ii = 0; ii < kSubTile / 2; ++ii) {
+                    const int i = half * 8 + ii;
+                    const float2 x = unpack_sample<BITS>(rw[ii]);
+                    // sample u contributes w[k] x[u] to output u + k (slot (u + k) mod 16); output u is then complete
+#pragma unroll
+                    for (int k = 0; k < kTaps - 1; ++k)
+                        acc[(i + k) & 15] = __ffma2_rn(make_float2(wk[k], wk[k]), x, acc[(i + k) & 15]);
+                    if (jj >= 0)
+                        asm volatile("st.shared.b32 [%0], %1;" ::"r"(arow + i * 2 * kSBO), "r"(pack_half2(acc[i].x, acc[i].y)) : "memory");
+                    acc[(i + 15) & 15] = __fmul2_rn(make_float2(wk[15], wk[15]), x);   // first tap of output u + 15
+                }
+            }
+            fence_async_smem();                           // generic-proxy writes -> visible to the tensor core
+            __syncwarp();
+            if (lane == 0) {
+                mbar_arrive(bar_raw_empty + 8 * s);
+                if (jj >= 0) mbar_arrive(bar_a1_full + 8 * yb);
+            }
+        }
+    } else {
+        // ------------------------------------------------------------------ pass epilogues (steps a3-a7)
+        // Accumulator row = TMEM lane = (t % 8) * 16 + x of half h = t / 8, where x = r (first pass) or k1 (second
+        // pass); accumulator column = 2 k + (re, im).  This warp owns lane quarter qd and output columns k = 8 ch .. 8 ch + 7.
+        const int e = warp - kFirWarps;
+        const int qd = e & 3, ch = e >> 2;
+        const int tl = lane >> 4, x = lane & 15;
+        const uint32_t tm_lane = tmem_base + ((uint32_t)(qd * 32) << 16) + (uint32_t)ch * 16;
+        float2 tw[8], rot[8];
+#pragma unroll
+        for (int i2 = 0; i2 < 8; ++i2) {
+            float sn, cs;
+            sincospif(-2.0f * (float)(x * (8 * ch + i2)) / 256.0f, &sn, &cs);      // W256^{r k1}, r = x
+            tw[i2] = make_float2(cs * kA2, sn * kA2);
+            const float2 w = a.phase[((size_t)bl * a.S + (m >> 1)) * C + x + 16 * (8 * ch + i2)];   // channel j = k1 + 16 k2, k1 = x
+            rot[i2] = make_float2(w.x * a.inv_a1a2, w.y * a.inv_a1a2);
+        }
+        // A2 element (row t * 16 + k1, K position 2 r): (2 t + k1 / 8) kSBO + (r / 4) kLBO + (k1 % 8) 16 + (r % 4) 4
+        const uint32_t a2_thread = sbase + Sh::OFF_A2 + (2 * (2 * qd + tl) + ch) * kSBO + (x >> 2) * kLBO + (x & 3) * 4;
+        // staging word of (plane, channel j, spectrum pair p): 64 j + 16 ((p >> 2) ^ (m & 3) ^ ((j >> 1) & 3)) + 4 (p & 3)
+        // (fstage.cu: the row's chunk permutation by m & 3, then the tensor store's 64-byte swizzle); j >> 1 & 3 = x >> 1 & 3
+        const uint32_t stg_thread = sbase + Sh::OFF_STG + tl * (C * 64) + (x + 128 * ch) * 64;
+        const uint32_t swz = (uint32_t)((m & 3) ^ ((x >> 1) & 3));
+
+        for (int i = 0; i <= n_sub; ++i) {
+            if (i < n_sub) {
+                // ---- first pass of sub-tile i: twiddle, fp16, into the second-pass operand tile
+                const int b = i & 1;
+                const uint32_t par = (uint32_t)(i >> 1) & 1u;
+                uint32_t v0[16], v1[16];
+                mbar_wait(bar_d1_full + 8 * b, par);
+                tc_fence_after();
+                tmem_ld16(tm_lane + (uint32_t)(b * 2) * 32, v0);
+                tmem_ld16(tm_lane + (uint32_t)(b * 2 + 1) * 32, v1);
+                tmem_ld_wait();
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar_d1_empty + 8 * b);
+                mbar_wait(bar_a2_empty + 8 * b, par ^ 1u);
+                const uint32_t dst = a2_thread + b * kATile;
+#pragma unroll
+                for (int i2 = 0; i2 < 8; ++i2) {
+                    const float2 y0 = cmul(make_float2(__uint_as_float(v0[2 * i2]), __uint_as_float(v0[2 * i2 + 1])), tw[i2]);
+                    const float2 y1 = cmul(make_float2(__uint_as_float(v1[2 * i2]), __uint_as_float(v1[2 * i2 + 1])), tw[i2]);
+                    asm volatile("st.shared.b32 [%0], %1;" ::"r"(dst + i2 * 16), "r"(pack_half2(y0.x, y0.y)) : "memory");
+                    asm volatile("st.shared.b32 [%0], %1;" ::"r"(dst + 16 * kSBO + i2 * 16), "r"(pack_half2(y1.x, y1.y)) : "memory");
+                }
+                fence_async_smem();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar_a2_full + 8 * b);
+            }
+            if (i >= 1) {
+                // ---- second pass of sub-tile i - 1: rotation * bandpass, fp16 pairs of spectra, into the staging tile
+                const int ip = i - 1, b = ip & 1;
+                const uint32_t par = (uint32_t)(ip >> 1) & 1u;
+                uint32_t v0[16], v1[16];
+                mbar_wait(bar_d2_full + 8 * b, par);
+                tc_fence_after();
+                tmem_ld16(tm_lane + 128 + (uint32_t)(b * 2) * 32, v0);
+                tmem_ld16(tm_lane + 128 + (uint32_t)(b * 2 + 1) * 32, v1);
+                tmem_ld_wait();
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar_d2_empty + 8 * b);
+                const int tile = ip >> 1, sbuf = tile & 1;
+                mbar_wait(bar_stg_empty + 8 * sbuf, ((uint32_t)(tile >> 1) & 1u) ^ 1u);
+                const long long t_sub = (long long)(kt0 + (ip >> 2)) * kKTile + (ip & 3) * kSubTile;
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    const long long t_even = t_sub + 8 * h + 2 * qd;              // the even spectrum of this lane pair
+                    const uint32_t msk = t_even + 1 < a.n_t ? 0xffffffffu : t_even < a.n_t ? 0x0000ffffu : 0u;
+                    const int p = 8 * (ip & 1) + 4 * h + qd;
+                    const uint32_t dst = stg_thread + sbuf * kStgBytes + ((((uint32_t)(p >> 2) ^ swz) << 4) | ((uint32_t)(p & 3) << 2));
+#pragma unroll
+                    for (int i2 = 0; i2 < 8; ++i2) {
+                        const uint32_t vr = h ? v1[2 * i2] : v0[2 * i2], vi = h ? v1[2 * i2 + 1] : v0[2 * i2 + 1];
+                        const float2 z = cmul(make_float2(__uint_as_float(vr), __uint_as_float(vi)), rot[i2]);
+                        // lanes l (spectrum t) and l + 16 (t + 1): the even one builds the re-plane word, the odd one the im-plane word
+                        const float o = __shfl_xor_sync(0xffffffffu, tl ? z.x : z.y, 16);
+                        const uint32_t word = tl ? pack_half2(o, z.y) : pack_half2(z.x, o);
+                        asm volatile("st.shared.b32 [%0], %1;" ::"r"(dst + i2 * (16 * 64)), "r"(word & msk) : "memory");
+                    }
+                }
+                fence_async_smem();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar_stg_full + 8 * sbuf);
+            }
+        }
+    }
+
+    tc_fence_before();
+    __syncthreads();
+    if (warp == kMmaWarp) {
+        tc_fence_after();
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(256) : "memory");
+    }
+}
+
+}  // namespace
+
+// C = 256, TENSOR_FP16 only; fstage.cu keeps every other case (and stays the reference for this one in the tests).
+cudaError_t launch_fstage_tc(const cobalt_plan_s *p, cudaStream_t st, const void *samples_b0, int b0, int nb) {
+    FArgsTC a;
+    a.samples = static_cast<const unsigned char *>(samples_b0);
+    a.hist = static_cast<const unsigned char *>(p->d_hist[p->hist_cur]);
+    a.weights = p->d_weights;
+    a.phase = p->d_phase;
+    a.N = p->N;
+    a.n_t = p->n_t;
+    a.S = p->S;
+    a.M = p->M;
+    a.Mpad = p->Mpad;
+    a.n_kt = p->n_kt;
+    a.b0 = b0;
+    // a1: |y| <= amp_max (full-scale input through the FIR) must stay below 32768 as an fp16 operand
+    int e1 = 0;
+    while (p->amp_max * (float)(1.0 / (double)(1 << e1)) > 32768.f) ++e1;
+    a.a1 = (float)(1.0 / (double)(1 << e1));
+    a.inv_a1a2 = (float)(1 << e1) / kA2;
+    // One CTA per SM and stream: as few time segments as possible (each re-reads its 16 warm-up rows) that still
+    // give >= 8 waves.
+    const long long groups = (long long)nb * p->M;
+    const long long want = (long long)p->sm_count * 8;
+    int n_seg = (int)((want + groups - 1) / groups);
+    if (n_seg < 1) n_seg = 1;
+    const int max_seg = (p->n_kt + 3) / 4;
+    if (n_seg > max_seg) n_seg = max_seg;
+    a.tiles_per_seg = (p->n_kt + n_seg - 1) / n_seg;
+    n_seg = (p->n_kt + a.tiles_per_seg - 1) / a.tiles_per_seg;
+    dim3 grid((unsigned)groups, (unsigned)n_seg);
+    cudaError_t e;
+    if (p->bits == 16) {
+        e = cudaFuncSetAttribute(fstage_tc_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, ShTC<16>::TOTAL);
+        if (e != cudaSuccess) return e;
+        fstage_tc_kernel<16><<<grid, kThreadsTC, ShTC<16>::TOTAL, st>>>(a, p->zmap);
+    } else {
+        e = cudaFuncSetAttribute(fstage_tc_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, ShTC<8>::TOTAL);
+        if (e != cudaSuccess) return e;
+        fstage_tc_kernel<8><<<grid, kThreadsTC, ShTC<8>::TOTAL, st>>>(a, p->zmap);
+    }
+    return cudaGetLastError();
+}
+
+}  // namespace cobalt
