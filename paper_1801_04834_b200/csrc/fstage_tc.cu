@@ -40,7 +40,8 @@ constexpr int kC = 256;
 constexpr int kFirWarps = 8, kEpiWarps = 8;
 constexpr int kProducerWarp = kFirWarps + kEpiWarps, kStoreWarp = kProducerWarp + 1, kMmaWarp = kProducerWarp + 2;
 constexpr int kThreadsTC = (kMmaWarp + 1) * 32;
-constexpr int kRawStages = 3, kABufs = 2, kStgBufs = 2;
+constexpr int kRawStages = 3, kA1Bufs = 3, kA2Bufs = 2, kStgBufs = 2;
+constexpr int kD2Col = kA1Bufs * 64;   // TMEM: D1[kA1Bufs][2 halves][32 columns], then D2[kA2Bufs][2][32]
 constexpr float kA2 = 0.0625f;      // scale of the first-pass output (|X1| <= 16 |y|)
 // Operand tiles: K-major, no swizzle.  The 16-byte chunk kc (8 fp16 of K) of row rho sits at
 // (rho / 8) * kSBO + kc * kLBO + (rho % 8) * 16; the pads (144 instead of 128, 608 instead of 576) spread the
@@ -58,8 +59,8 @@ struct ShTC {
     static constexpr int OFF_STG = 1024;
     static constexpr int OFF_RAW = OFF_STG + kStgBufs * kStgBytes;
     static constexpr int OFF_A1 = OFF_RAW + kRawStages * RAW_STAGE;
-    static constexpr int OFF_A2 = OFF_A1 + kABufs * kATile;
-    static constexpr int OFF_B = OFF_A2 + kABufs * kATile;
+    static constexpr int OFF_A2 = OFF_A1 + kA1Bufs * kATile;
+    static constexpr int OFF_B = OFF_A2 + kA2Bufs * kATile;
     static constexpr int TOTAL = OFF_B + kBTile;
     static_assert(TOTAL <= 227 * 1024, "shared memory budget");
 };
@@ -152,6 +153,21 @@ __device__ __forceinline__ float2 unpack_sample(uint32_t raw) {
     return make_float2((float)(signed char)(raw & 0xffu), (float)(signed char)((raw >> 8) & 0xffu));
 }
 
+// Second-pass epilogue of one half tile: 8 channels (k2 = 8 ch + i2) of this lane's (spectrum, k1) times
+// rotation * bandpass, spectra t (lanes 0-15) and t + 1 (lanes 16-31) paired into fp16x2 words -- the even lane
+// builds the re-plane word, the odd lane the im-plane word -- and stored 16 channels (16 * 64 bytes) apart.
+template <bool MASK>
+__device__ __forceinline__ void store_pass2(const uint32_t (&v)[16], const float2 (&rot)[8], int tl, uint32_t dst, uint32_t msk) {
+#pragma unroll
+    for (int i2 = 0; i2 < 8; ++i2) {
+        const float2 z = cmul(make_float2(__uint_as_float(v[2 * i2]), __uint_as_float(v[2 * i2 + 1])), rot[i2]);
+        const float o = __shfl_xor_sync(0xffffffffu, tl ? z.x : z.y, 16);
+        uint32_t word = pack_half2(tl ? o : z.x, tl ? z.y : o);
+        if (MASK) word &= msk;
+        asm volatile("st.shared.b32 [%0], %1;" ::"r"(dst + i2 * (16 * 64)), "r"(word) : "memory");
+    }
+}
+
 template <int BITS>
 __global__ void __launch_bounds__(kThreadsTC, 1) fstage_tc_kernel(const FArgsTC a, const __grid_constant__ CUtensorMap zmap) {
     using Sh = ShTC<BITS>;
@@ -160,11 +176,11 @@ __global__ void __launch_bounds__(kThreadsTC, 1) fstage_tc_kernel(const FArgsTC 
     const uint32_t sbase = smem_u32(smem);
     const uint32_t bar_raw_full = sbase + Sh::OFF_BAR;              // [kRawStages]
     const uint32_t bar_raw_empty = bar_raw_full + 8 * kRawStages;   // [kRawStages]
-    const uint32_t bar_a1_full = bar_raw_empty + 8 * kRawStages;    // [2] FIR -> MMA
-    const uint32_t bar_a1_empty = bar_a1_full + 16;                 // [2] MMA (commit) -> FIR
-    const uint32_t bar_d1_full = bar_a1_empty + 16;                 // [2] MMA (commit) -> epilogue
-    const uint32_t bar_d1_empty = bar_d1_full + 16;                 // [2] epilogue -> MMA
-    const uint32_t bar_a2_full = bar_d1_empty + 16;                 // [2] epilogue -> MMA
+    const uint32_t bar_a1_full = bar_raw_empty + 8 * kRawStages;    // [kA1Bufs] FIR -> MMA
+    const uint32_t bar_a1_empty = bar_a1_full + 8 * kA1Bufs;        // [kA1Bufs] MMA (commit) -> FIR
+    const uint32_t bar_d1_full = bar_a1_empty + 8 * kA1Bufs;        // [kA1Bufs] MMA (commit) -> epilogue
+    const uint32_t bar_d1_empty = bar_d1_full + 8 * kA1Bufs;        // [kA1Bufs] epilogue -> MMA
+    const uint32_t bar_a2_full = bar_d1_empty + 8 * kA1Bufs;        // [2] epilogue -> MMA
     const uint32_t bar_a2_empty = bar_a2_full + 16;                 // [2] MMA (commit) -> epilogue
     const uint32_t bar_d2_full = bar_a2_empty + 16;                 // [2]
     const uint32_t bar_d2_empty = bar_d2_full + 16;                 // [2]
@@ -185,11 +201,13 @@ __global__ void __launch_bounds__(kThreadsTC, 1) fstage_tc_kernel(const FArgsTC 
             mbar_init(bar_raw_full + 8 * s, 1);
             mbar_init(bar_raw_empty + 8 * s, kFirWarps);
         }
-        for (int b = 0; b < 2; ++b) {
+        for (int b = 0; b < kA1Bufs; ++b) {
             mbar_init(bar_a1_full + 8 * b, kFirWarps);
             mbar_init(bar_a1_empty + 8 * b, 1);
             mbar_init(bar_d1_full + 8 * b, 1);
             mbar_init(bar_d1_empty + 8 * b, kEpiWarps);
+        }
+        for (int b = 0; b < kA2Bufs; ++b) {
             mbar_init(bar_a2_full + 8 * b, kEpiWarps);
             mbar_init(bar_a2_empty + 8 * b, 1);
             mbar_init(bar_d2_full + 8 * b, 1);
@@ -215,7 +233,7 @@ __global__ void __launch_bounds__(kThreadsTC, 1) fstage_tc_kernel(const FArgsTC 
         fence_async_smem();
     }
     if (warp == kMmaWarp) {
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tmem_slot), "r"(256) : "memory");
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tmem_slot), "r"(512) : "memory");
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
     }
     tc_fence_before();
@@ -295,8 +313,8 @@ __global__ void __launch_bounds__(kThreadsTC, 1) fstage_tc_kernel(const FArgsTC 
             const uint64_t desc_b = make_desc(sbase + Sh::OFF_B);
             for (int i = 0; i <= n_sub; ++i) {
                 if (i < n_sub) {
-                    const int b = i & 1;
-                    const uint32_t par = (uint32_t)(i >> 1) & 1u;
+                    const int b = i % kA1Bufs;
+                    const uint32_t par = (uint32_t)(i / kA1Bufs) & 1u;
                     mbar_wait(bar_a1_full + 8 * b, par);
                     mbar_wait(bar_d1_empty + 8 * b, par ^ 1u);
                     tc_fence_after();
@@ -321,7 +339,7 @@ __global__ void __launch_bounds__(kThreadsTC, 1) fstage_tc_kernel(const FArgsTC 
                     for (int h = 0; h < 2; ++h)
 #pragma unroll
                         for (int ks = 0; ks < 2; ++ks)
-                            tc_mma(tmem_base + 128 + (uint32_t)(b * 2 + h) * 32, desc_a + (uint64_t)((h * 16 * kSBO + ks * 2 * kLBO) >> 4),
+                            tc_mma(tmem_base + kD2Col + (uint32_t)(b * 2 + h) * 32, desc_a + (uint64_t)((h * 16 * kSBO + ks * 2 * kLBO) >> 4),
                                    desc_b + (uint64_t)((ks * 2 * kLBO) >> 4), kIdesc, (uint32_t)ks);
                     tc_commit(bar_a2_empty + 8 * b);
                     tc_commit(bar_d2_full + 8 * b);
@@ -351,9 +369,9 @@ __global__ void __launch_bounds__(kThreadsTC, 1) fstage_tc_kernel(const FArgsTC 
             const int s = j % kRawStages;
             mbar_wait(bar_raw_full + 8 * s, (uint32_t)(j / kRawStages) & 1u);
             const int jj = j - 1;                         // real sub-tile index (j = 0 is the warm-up)
-            const int yb = jj & 1;
+            const int yb = jj % kA1Bufs;
             const uint32_t raw = raw_thread + s * Sh::RAW_STAGE;
-            if (jj >= 0) mbar_wait(bar_a1_empty + 8 * yb, ((uint32_t)(jj >> 1) & 1u) ^ 1u);
+            if (jj >= 0) mbar_wait(bar_a1_empty + 8 * yb, ((uint32_t)(jj / kA1Bufs) & 1u) ^ 1u);
             const uint32_t arow = a1_thread + (jj >= 0 ? yb : 0) * kATile;
 #pragma unroll
             for (int half = 0; half < 2; ++half) {
@@ -415,8 +433,8 @@ __global__ void __launch_bounds__(kThreadsTC, 1) fstage_tc_kernel(const FArgsTC 
         for (int i = 0; i <= n_sub; ++i) {
             if (i < n_sub) {
                 // ---- first pass of sub-tile i: twiddle, fp16, into the second-pass operand tile
-                const int b = i & 1;
-                const uint32_t par = (uint32_t)(i >> 1) & 1u;
+                const int b = i % kA1Bufs, b2 = i & 1;
+                const uint32_t par = (uint32_t)(i / kA1Bufs) & 1u, par2 = (uint32_t)(i >> 1) & 1u;
                 uint32_t v0[16], v1[16];
                 mbar_wait(bar_d1_full + 8 * b, par);
                 tc_fence_after();
@@ -426,8 +444,8 @@ __global__ void __launch_bounds__(kThreadsTC, 1) fstage_tc_kernel(const FArgsTC 
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive(bar_d1_empty + 8 * b);
-                mbar_wait(bar_a2_empty + 8 * b, par ^ 1u);
-                const uint32_t dst = a2_thread + b * kATile;
+                mbar_wait(bar_a2_empty + 8 * b2, par2 ^ 1u);
+                const uint32_t dst = a2_thread + b2 * kATile;
 #pragma unroll
                 for (int i2 = 0; i2 < 8; ++i2) {
                     const float2 y0 = cmul(make_float2(__uint_as_float(v0[2 * i2]), __uint_as_float(v0[2 * i2 + 1])), tw[i2]);
@@ -437,7 +455,7 @@ __global__ void __launch_bounds__(kThreadsTC, 1) fstage_tc_kernel(const FArgsTC 
                 }
                 fence_async_smem();
                 __syncwarp();
-                if (lane == 0) mbar_arrive(bar_a2_full + 8 * b);
+                if (lane == 0) mbar_arrive(bar_a2_full + 8 * b2);
             }
             if (i >= 1) {
                 // ---- second pass of sub-tile i - 1: rotation * bandpass, fp16 pairs of spectra, into the staging tile
@@ -446,8 +464,8 @@ __global__ void __launch_bounds__(kThreadsTC, 1) fstage_tc_kernel(const FArgsTC 
                 uint32_t v0[16], v1[16];
                 mbar_wait(bar_d2_full + 8 * b, par);
                 tc_fence_after();
-                tmem_ld16(tm_lane + 128 + (uint32_t)(b * 2) * 32, v0);
-                tmem_ld16(tm_lane + 128 + (uint32_t)(b * 2 + 1) * 32, v1);
+                tmem_ld16(tm_lane + kD2Col + (uint32_t)(b * 2) * 32, v0);
+                tmem_ld16(tm_lane + kD2Col + (uint32_t)(b * 2 + 1) * 32, v1);
                 tmem_ld_wait();
                 tc_fence_before();
                 __syncwarp();
@@ -455,20 +473,17 @@ __global__ void __launch_bounds__(kThreadsTC, 1) fstage_tc_kernel(const FArgsTC 
                 const int tile = ip >> 1, sbuf = tile & 1;
                 mbar_wait(bar_stg_empty + 8 * sbuf, ((uint32_t)(tile >> 1) & 1u) ^ 1u);
                 const long long t_sub = (long long)(kt0 + (ip >> 2)) * kKTile + (ip & 3) * kSubTile;
+                const uint32_t dst = stg_thread + sbuf * kStgBytes;
+                const uint32_t c0 = (uint32_t)(2 * (ip & 1));                       // p = 8 (ip & 1) + 4 h + qd: p >> 2 = c0 + h, p & 3 = qd
+                if (t_sub + kSubTile <= a.n_t) {
+                    store_pass2<false>(v0, rot, tl, dst + (((c0 ^ swz) << 4) | ((uint32_t)qd << 2)), 0xffffffffu);
+                    store_pass2<false>(v1, rot, tl, dst + ((((c0 + 1) ^ swz) << 4) | ((uint32_t)qd << 2)), 0xffffffffu);
+                } else {   // last k-tile: spectra t >= n_t leave as exact zeros
 #pragma unroll
-                for (int h = 0; h < 2; ++h) {
-                    const long long t_even = t_sub + 8 * h + 2 * qd;              // the even spectrum of this lane pair
-                    const uint32_t msk = t_even + 1 < a.n_t ? 0xffffffffu : t_even < a.n_t ? 0x0000ffffu : 0u;
-                    const int p = 8 * (ip & 1) + 4 * h + qd;
-                    const uint32_t dst = stg_thread + sbuf * kStgBytes + ((((uint32_t)(p >> 2) ^ swz) << 4) | ((uint32_t)(p & 3) << 2));
-#pragma unroll
-                    for (int i2 = 0; i2 < 8; ++i2) {
-                        const uint32_t vr = h ? v1[2 * i2] : v0[2 * i2], vi = h ? v1[2 * i2 + 1] : v0[2 * i2 + 1];
-                        const float2 z = cmul(make_float2(__uint_as_float(vr), __uint_as_float(vi)), rot[i2]);
-                        // lanes l (spectrum t) and l + 16 (t + 1): the even one builds the re-plane word, the odd one the im-plane word
-                        const float o = __shfl_xor_sync(0xffffffffu, tl ? z.x : z.y, 16);
-                        const uint32_t word = tl ? pack_half2(o, z.y) : pack_half2(z.x, o);
-                        asm volatile("st.shared.b32 [%0], %1;" ::"r"(dst + i2 * (16 * 64)), "r"(word & msk) : "memory");
+                    for (int h = 0; h < 2; ++h) {
+                        const long long t_even = t_sub + 8 * h + 2 * qd;          // the even spectrum of this lane pair
+                        const uint32_t msk = t_even + 1 < a.n_t ? 0xffffffffu : t_even < a.n_t ? 0x0000ffffu : 0u;
+                        store_pass2<true>(h ? v1 : v0, rot, tl, dst + ((((c0 + h) ^ swz) << 4) | ((uint32_t)qd << 2)), msk);
                     }
                 }
                 fence_async_smem();
@@ -482,7 +497,7 @@ __global__ void __launch_bounds__(kThreadsTC, 1) fstage_tc_kernel(const FArgsTC 
     __syncthreads();
     if (warp == kMmaWarp) {
         tc_fence_after();
-        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(256) : "memory");
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(512) : "memory");
     }
 }
 
