@@ -312,13 +312,16 @@ def run_ours(args, rank, world, local):
     n_samples = float(cfg.B) * 2 * cfg.S * (cfg.n_t * cfg.C)               # complex samples per pol-stream
     f_bytes = n_samples * F_BYTES_PER_SAMPLE[cfg.bits] if args.mode == "tensor" else n_samples * (cfg.bits // 4 + 8)
     x_flop = units * X_FLOP_PER_BASELINE_SAMPLE
-    roof_f = {"kernel": "fstage_kernel", "bound": "hbm", "achieved": f_bytes / t_f / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-              "frac": f_bytes / t_f / 1e9 / peaks["hbm_gbs"], "traffic": stored_traffic("fstage_kernel"),
+    # C = 256 in tensor mode runs the DFT on the tensor cores (csrc/fstage_tc.cu) unless COBALT_FSTAGE_SIMT is set
+    f_kernel = "fstage_tc_kernel" if (cfg.C == 256 and args.mode == "tensor" and "COBALT_FSTAGE_SIMT" not in os.environ) else "fstage_kernel"
+    roof_f = {"kernel": f_kernel, "bound": "hbm", "achieved": f_bytes / t_f / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+              "frac": f_bytes / t_f / 1e9 / peaks["hbm_gbs"], "traffic": stored_traffic(f_kernel) if cfg.name == "full-array-16bit" else None,
               "peak_source": peaks["source"], "ms_per_launch": t_f * 1e3 / n_chunks, "launches_per_step": n_chunks,
               "algorithmic_bytes_per_launch": f_bytes / n_chunks}
     roof_x = {"kernel": "xstage_tc_kernel" if args.mode == "tensor" else "xstage_simt_kernel", "bound": "tensor",
               "achieved": x_flop / t_x / 1e12, "peak": peaks["tensor_tflops_sustained"], "unit": "TFLOP/s",
-              "frac": x_flop / t_x / 1e12 / peaks["tensor_tflops_sustained"], "traffic": stored_traffic("xstage_tc_kernel"),
+              "frac": x_flop / t_x / 1e12 / peaks["tensor_tflops_sustained"],
+              "traffic": stored_traffic("xstage_tc_kernel") if cfg.name == "full-array-16bit" else None,
               "peak_source": peaks["source"] + " (sustained bf16; fp16 runs at the same rate)",
               "ms_per_launch": t_x * 1e3 / n_chunks, "launches_per_step": n_chunks,
               "algorithmic_flop_per_launch": x_flop / n_chunks,
