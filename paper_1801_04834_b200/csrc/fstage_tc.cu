@@ -154,15 +154,17 @@ __device__ __forceinline__ float2 unpack_sample(uint32_t raw) {
 }
 
 // Second-pass epilogue of one half tile: 8 channels (k2 = 8 ch + i2) of this lane's (spectrum, k1) times
-// rotation * bandpass, spectra t (lanes 0-15) and t + 1 (lanes 16-31) paired into fp16x2 words -- the even lane
-// builds the re-plane word, the odd lane the im-plane word -- and stored 16 channels (16 * 64 bytes) apart.
+// rotation * bandpass, converted to an fp16 (re, im) pair.  Lanes l (spectrum t) and l + 16 (t + 1) swap their pairs
+// with one shuffle and each picks two halves with one byte permute: the even lane builds the re-plane word
+// (re t, re t+1), the odd lane the im-plane word (im t, im t+1); stored 16 channels (16 * 64 bytes) apart.
 template <bool MASK>
-__device__ __forceinline__ void store_pass2(const uint32_t (&v)[16], const float2 (&rot)[8], int tl, uint32_t dst, uint32_t msk) {
+__device__ __forceinline__ void store_pass2(const uint32_t (&v)[16], const float2 (&rot)[8], uint32_t sel, uint32_t dst, uint32_t msk) {
 #pragma unroll
     for (int i2 = 0; i2 < 8; ++i2) {
         const float2 z = cmul(make_float2(__uint_as_float(v[2 * i2]), __uint_as_float(v[2 * i2 + 1])), rot[i2]);
-        const float o = __shfl_xor_sync(0xffffffffu, tl ? z.x : z.y, 16);
-        uint32_t word = pack_half2(tl ? o : z.x, tl ? z.y : o);
+        const uint32_t own = pack_half2(z.x, z.y);
+        const uint32_t other = __shfl_xor_sync(0xffffffffu, own, 16);
+        uint32_t word = __byte_perm(own, other, sel);
         if (MASK) word &= msk;
         asm volatile("st.shared.b32 [%0], %1;" ::"r"(dst + i2 * (16 * 64)), "r"(word) : "memory");
     }
@@ -429,6 +431,8 @@ __global__ void __launch_bounds__(kThreadsTC, 1) fstage_tc_kernel(const FArgsTC 
         // (fstage.cu: the row's chunk permutation by m & 3, then the tensor store's 64-byte swizzle); j >> 1 & 3 = x >> 1 & 3
         const uint32_t stg_thread = sbase + Sh::OFF_STG + tl * (C * 64) + (x + 128 * ch) * 64;
         const uint32_t swz = (uint32_t)((m & 3) ^ ((x >> 1) & 3));
+        // byte permute of (own pair, partner's pair): even spectrum -> (own re, partner re), odd -> (partner im, own im)
+        const uint32_t sel = tl ? 0x3276u : 0x5410u;
 
         for (int i = 0; i <= n_sub; ++i) {
             if (i < n_sub) {
@@ -476,14 +480,14 @@ __global__ void __launch_bounds__(kThreadsTC, 1) fstage_tc_kernel(const FArgsTC 
                 const uint32_t dst = stg_thread + sbuf * kStgBytes;
                 const uint32_t c0 = (uint32_t)(2 * (ip & 1));                       // p = 8 (ip & 1) + 4 h + qd: p >> 2 = c0 + h, p & 3 = qd
                 if (t_sub + kSubTile <= a.n_t) {
-                    store_pass2<false>(v0, rot, tl, dst + (((c0 ^ swz) << 4) | ((uint32_t)qd << 2)), 0xffffffffu);
-                    store_pass2<false>(v1, rot, tl, dst + ((((c0 + 1) ^ swz) << 4) | ((uint32_t)qd << 2)), 0xffffffffu);
+                    store_pass2<false>(v0, rot, sel, dst + (((c0 ^ swz) << 4) | ((uint32_t)qd << 2)), 0xffffffffu);
+                    store_pass2<false>(v1, rot, sel, dst + ((((c0 + 1) ^ swz) << 4) | ((uint32_t)qd << 2)), 0xffffffffu);
                 } else {   // last k-tile: spectra t >= n_t leave as exact zeros
 #pragma unroll
                     for (int h = 0; h < 2; ++h) {
                         const long long t_even = t_sub + 8 * h + 2 * qd;          // the even spectrum of this lane pair
                         const uint32_t msk = t_even + 1 < a.n_t ? 0xffffffffu : t_even < a.n_t ? 0x0000ffffu : 0u;
-                        store_pass2<true>(h ? v1 : v0, rot, tl, dst + ((((c0 + h) ^ swz) << 4) | ((uint32_t)qd << 2)), msk);
+                        store_pass2<true>(h ? v1 : v0, rot, sel, dst + ((((c0 + h) ^ swz) << 4) | ((uint32_t)qd << 2)), msk);
                     }
                 }
                 fence_async_smem();
