@@ -46,6 +46,8 @@ def parse_args(argv=None):
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json config index (1-5)")
     ap.add_argument("--subbands", type=int, default=0, help="override the number of subbands (debugging)")
     ap.add_argument("--mode", default="tensor", choices=["tensor", "exact"])
+    ap.add_argument("--dft", default="fp32", choices=["fp32", "tensor"],
+                    help="F-stage DFT engine (cobalt_set_dft_engine); tensor: C = 256 only")
     ap.add_argument("--chunk", type=int, default=0, help="subbands per launch group (0 = library default)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -275,6 +277,8 @@ def run_ours(args, rank, world, local):
     cor = pkg.Correlator(cfg.S, cfg.B, cfg.C, cfg.N, cfg.bits, mode=mode)
     if args.chunk > 0:
         cor.set_chunk_subbands(args.chunk)
+    if args.dft == "tensor":
+        cor.set_dft_engine(pkg.COBALT_DFT_TENSOR)
     info = cor.info
     vis = torch.empty(cor.vis_shape(), dtype=torch.complex64, device=dev)
     stream = torch.cuda.current_stream()
@@ -312,8 +316,8 @@ def run_ours(args, rank, world, local):
     n_samples = float(cfg.B) * 2 * cfg.S * (cfg.n_t * cfg.C)               # complex samples per pol-stream
     f_bytes = n_samples * F_BYTES_PER_SAMPLE[cfg.bits] if args.mode == "tensor" else n_samples * (cfg.bits // 4 + 8)
     x_flop = units * X_FLOP_PER_BASELINE_SAMPLE
-    # C = 256 in tensor mode runs the DFT on the tensor cores (csrc/fstage_tc.cu) unless COBALT_FSTAGE_SIMT is set
-    f_kernel = "fstage_tc_kernel" if (cfg.C == 256 and args.mode == "tensor" and "COBALT_FSTAGE_SIMT" not in os.environ) else "fstage_kernel"
+    # --dft tensor: C = 256 in tensor mode runs the DFT on the tensor cores (csrc/fstage_tc.cu)
+    f_kernel = "fstage_tc_kernel" if (cfg.C == 256 and args.mode == "tensor" and args.dft == "tensor") else "fstage_kernel"
     roof_f = {"kernel": f_kernel, "bound": "hbm", "achieved": f_bytes / t_f / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
               "frac": f_bytes / t_f / 1e9 / peaks["hbm_gbs"], "traffic": stored_traffic(f_kernel) if cfg.name == "full-array-16bit" else None,
               "peak_source": peaks["source"], "ms_per_launch": t_f * 1e3 / n_chunks, "launches_per_step": n_chunks,
@@ -346,7 +350,7 @@ def run_ours(args, rank, world, local):
             "dtype": "f32 (fp16 tensor-core operands, fp32 accumulate; fp64 phase angles)" if args.mode == "tensor" else "f32",
             "data": "synthetic",
             "config": {"workload": cfg.name, "stations": cfg.S, "subbands": cfg.B, "channels": cfg.C, "taps": 16,
-                       "samples_per_integration": cfg.N, "input_bits": cfg.bits, "baselines": cfg.n_bl, "mode": args.mode,
+                       "samples_per_integration": cfg.N, "input_bits": cfg.bits, "baselines": cfg.n_bl, "mode": args.mode, "dft": args.dft,
                        "chunk_subbands": info.chunk_subbands, "parallelism": "replicas" if world > 1 else "single-gpu",
                        "l2": f"inputs ({cfg.input_bytes / 1e9:.2f} GB per step) exceed the 126 MB L2; no flush needed"},
             "roofline": dominant, "roofline_other": other,

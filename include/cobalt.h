@@ -129,6 +129,17 @@ int cobalt_set_subband_frequencies(cobalt_plan_t *plan, const double *h_hz);
 int cobalt_set_sample_rate(cobalt_plan_t *plan, double hz);
 /* Switch COBALT_MODE_*; reallocates the intermediate scratch, keeps the history. */
 int cobalt_set_mode(cobalt_plan_t *plan, int mode);
+/* Where the F-stage computes the C-point DFT (step a3) in COBALT_MODE_TENSOR_FP16:
+ *   COBALT_DFT_FP32   (default) radix-16 FFT in fp32 on the FP32 pipe; only the final channelised value is
+ *                     rounded to fp16, so channel isolation is that of the fp32 filter bank;
+ *   COBALT_DFT_TENSOR two 16-point DFT passes as fp16 GEMMs on the tensor cores (C = 256 only; other C and
+ *                     EXACT mode silently keep COBALT_DFT_FP32).  1-4 % faster on config 3, but the FIR output
+ *                     is rounded to fp16 BEFORE the DFT: a channel holding 2^-11 or less of the amplitude of
+ *                     the strongest channel of the same spectrum is no longer within the 2e-3 tolerance.
+ * Takes effect at the next cobalt_process. */
+#define COBALT_DFT_FP32 0
+#define COBALT_DFT_TENSOR 1
+int cobalt_set_dft_engine(cobalt_plan_t *plan, int engine);
 /* Subbands per internal launch group (>= 1, clipped to B).  Reallocates scratch. */
 int cobalt_set_chunk_subbands(cobalt_plan_t *plan, int chunk);
 /* Zero the FIR history (as after cobalt_plan).  Enqueued on the legacy default stream and

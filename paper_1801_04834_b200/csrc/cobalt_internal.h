@@ -70,6 +70,7 @@ struct StageEvents {
 
 struct cobalt_plan_s {
     int S = 0, B = 0, C = 0, T = 0, bits = 0, mode = COBALT_MODE_TENSOR_FP16;
+    int dft_engine = COBALT_DFT_FP32;  // cobalt_set_dft_engine
     long long N = 0, n_t = 0, N_u = 0, n_bl = 0;
     int M = 0, Mpad = 0, n_kt = 0;
     int chunk = 1;

@@ -26,8 +26,6 @@
 //              (D[(j + C/2) mod C]) is folded into the FIR weights, so the reorder is free.
 #include "cobalt_internal.h"
 
-#include <cstdlib>
-
 namespace cobalt {
 
 namespace {
@@ -691,7 +689,7 @@ cudaError_t launch_set_unit_scale(const cobalt_plan_s *p, cudaStream_t st) {
 }
 
 cudaError_t launch_fstage(const cobalt_plan_s *p, cudaStream_t st, const void *samples_b0, int b0, int nb) {
-    if (p->C == 256 && p->mode == COBALT_MODE_TENSOR_FP16 && !getenv("COBALT_FSTAGE_SIMT"))
+    if (p->C == 256 && p->mode == COBALT_MODE_TENSOR_FP16 && p->dft_engine == COBALT_DFT_TENSOR)
         return launch_fstage_tc(p, st, samples_b0, b0, nb);      // DFT on the tensor cores (fstage_tc.cu)
     FArgs a;
     a.samples = static_cast<const unsigned char *>(samples_b0);

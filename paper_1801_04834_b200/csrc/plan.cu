@@ -368,6 +368,12 @@ int cobalt_set_mode(cobalt_plan_t *p, int mode) {
     return alloc_scratch(p, 0);
 }
 
+int cobalt_set_dft_engine(cobalt_plan_t *p, int engine) {
+    if (!p || (engine != COBALT_DFT_FP32 && engine != COBALT_DFT_TENSOR)) return fail(p, COBALT_ERR_BAD_ARG, "unknown DFT engine");
+    p->dft_engine = engine;
+    return COBALT_OK;
+}
+
 int cobalt_set_chunk_subbands(cobalt_plan_t *p, int chunk) {
     if (!p || chunk < 1) return fail(p, COBALT_ERR_BAD_ARG, "chunk must be >= 1");
     CK(p, cudaDeviceSynchronize());

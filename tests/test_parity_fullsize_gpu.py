@@ -68,13 +68,15 @@ def _check_sampled(oracle, cfg, data, vis, pairs, mode_tensor=True):
     return worst
 
 
-def _full_config(cobalt, oracle, dev, index, n_random):
+def _full_config(cobalt, oracle, dev, index, n_random, subbands=0, dft_engine=None):
     from paper_1801_04834_b200 import synth
 
-    cfg = synth.CONFIGS[index]
+    cfg = synth.CONFIGS[index] if subbands == 0 else synth.scaled(synth.CONFIGS[index], B=subbands)
     data = synth.generate(cfg, device=dev)
     with cobalt.Correlator(cfg.S, cfg.B, cfg.C, cfg.N, cfg.bits, mode=cobalt.COBALT_MODE_TENSOR_FP16) as cor:
         assert cor.info.n_baselines == cfg.n_bl and cor.info.n_spectra == cfg.n_t
+        if dft_engine is not None:
+            cor.set_dft_engine(dft_engine)
         vis = cor.process(data["samples"], data["delays"], data["bandpass"])
         torch.cuda.synchronize()
     _invariants(vis, cfg.S)
@@ -87,6 +89,12 @@ def _full_config(cobalt, oracle, dev, index, n_random):
 def test_config3_full_array_16bit_sampled(cobalt, oracle, dev):
     """77 stations, 244 subbands, 256 channels, 195312 int16 samples: 29.4 GB in, 6.0 GB out."""
     _full_config(cobalt, oracle, dev, 3, n_random=5)
+
+
+def test_config3_tensor_dft_engine_sampled(cobalt, oracle, dev):
+    """Config 3's per-subband size (16 subbands = two launch groups) with the DFT on the tensor cores
+    (cobalt_set_dft_engine(COBALT_DFT_TENSOR), csrc/fstage_tc.cu): same tolerance on LOFAR-shaped noise."""
+    _full_config(cobalt, oracle, dev, 3, n_random=5, subbands=16, dft_engine=cobalt.COBALT_DFT_TENSOR)
 
 
 def test_config4_full_array_8bit_sampled(cobalt, oracle, dev):

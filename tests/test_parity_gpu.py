@@ -222,11 +222,13 @@ def test_reset_zeroes_history(cobalt, dev, mode_tensor):
 
 
 # ------------------------------------------------------------------ extreme integers (A12)
+@pytest.mark.parametrize("C,n_t", [(64, 80), (256, 48)])
 @pytest.mark.parametrize("bits", [16, 8])
-def test_extreme_sample_values(cobalt, oracle, dev, bits):
-    """Full-scale input incl. -32768 / -128: no overflow of the fp16 intermediate, parity holds."""
+def test_extreme_sample_values(cobalt, oracle, dev, bits, C, n_t):
+    """Full-scale input incl. -32768 / -128: no overflow of the fp16 intermediate (C = 256: nor of the fp16
+    operands of the tensor-core DFT passes), parity holds."""
     synth = _synth()
-    C, S, n_t = 64, 2, 80
+    S = 2
     rng = np.random.default_rng(5)
     lo, hi = (-32768, 32767) if bits == 16 else (-128, 127)
     samples = rng.choice(np.array([lo, hi, 0, -1, 1]), size=(1, S, 2, n_t * C, 2)).astype(np.int16 if bits == 16 else np.int8)
@@ -275,10 +277,12 @@ def test_process_host_matches_device_path(cobalt, dev):
 
 
 # ------------------------------------------------------------------ fp16 operand scale
-def test_fp16_scale_worst_case_amplitude(cobalt, oracle, dev):
+@pytest.mark.parametrize("C,n_t,t0", [(64, 64, 40), (256, 32, 20)])
+def test_fp16_scale_worst_case_amplitude(cobalt, oracle, dev, C, n_t, t0):
     """Sign-matched full-scale input rotated by 45 degrees drives one component of z to
-    sum|g| * sqrt(2) * 32767 ~ 7.8e4 > 65504: without the power-of-two operand scale fp16 overflows."""
-    C, S, n_t, t0 = 64, 2, 64, 40
+    sum|g| * sqrt(2) * 32767 ~ 7.8e4 > 65504: without the power-of-two operand scales fp16 overflows
+    (C = 256 also exercises the operands of the tensor-core DFT: FIR output at its maximum in every branch)."""
+    S = 2
     g = oracle.fir_prototype(C)
     samples = np.zeros((1, S, 2, n_t * C, 2), dtype=np.int16)
     seg = (32767 * np.sign(g)).astype(np.int16)                     # window of spectrum t0, natural order
@@ -306,6 +310,33 @@ def test_fp16_scale_follows_bandpass_gain(cobalt, oracle, dev, gain):
     vg = _run_gpu(cobalt, cfg, data, cobalt.COBALT_MODE_TENSOR_FP16, dev)
     vo = _run_oracle(oracle, cfg, data)
     _assert_parity(vg[0], vo[0], True, f"bandpass gain {gain}")
+
+
+@pytest.mark.parametrize("bits,S,n_t", [(16, 3, 70), (8, 2, 129), (16, 1, 16)])
+def test_tensor_dft_engine_matches_oracle_and_differs_from_fp32(cobalt, oracle, dev, bits, S, n_t):
+    """cobalt_set_dft_engine(COBALT_DFT_TENSOR) (C = 256: two fp16 GEMM passes on tcgen05, csrc/fstage_tc.cu):
+    within the 2e-3 tolerance on noise-like input incl. a ragged last k-tile, and really a different code path."""
+    synth = _synth()
+    cfg = synth.scaled(synth.CONFIGS[3 if bits == 16 else 4], S=S, B=2, C=256, N=256 * n_t + 7)
+    data = synth.generate(cfg, device="cpu")
+    vo = _run_oracle(oracle, cfg, data)[0]                          # [B][C][n_bl][2][2]
+    out = {}
+    for engine in (cobalt.COBALT_DFT_FP32, cobalt.COBALT_DFT_TENSOR):
+        with cobalt.Correlator(cfg.S, cfg.B, cfg.C, cfg.N, cfg.bits) as cor:
+            cor.set_dft_engine(engine)
+            vg = cor.process(data["samples"].to(dev), data["delays"].to(dev), data["bandpass"].to(dev))
+            torch.cuda.synchronize()
+            out[engine] = vg.cpu().numpy()
+        for b in range(cfg.B):
+            _assert_parity(out[engine][b], vo[b], True, f"dft engine {engine}, subband {b}")
+    assert not np.array_equal(out[cobalt.COBALT_DFT_FP32], out[cobalt.COBALT_DFT_TENSOR])
+
+
+def test_dft_engine_rejects_unknown_value(cobalt, dev):
+    with cobalt.Correlator(2, 1, 64, 64 * 20, 16) as cor:
+        with pytest.raises(Exception):
+            cor.set_dft_engine(7)
+        cor.set_dft_engine(cobalt.COBALT_DFT_TENSOR)      # accepted for any C; C != 256 keeps the fp32 FFT
 
 
 def test_golden_tiny_case_on_gpu(cobalt, dev):
