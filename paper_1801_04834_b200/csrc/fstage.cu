@@ -143,7 +143,11 @@ struct FShape {
     //   C < 256: branch ph sits at ph + (ph >> 4).
     static constexpr int YS = R == 16 ? 16 * 18 : C + R;
     static constexpr int RAW_STAGE = kSubTile * 256 * SB;  // bytes: [SPC][16 rows][C] samples
-    static constexpr int Y_BUF = kSubTile * SPC * YS * 8;  // bytes
+    // One spectrum of the tile = SPC * YS float2; for C = 64 two pad elements make the stride of a spectrum PAIR
+    // 4 (mod 16) eight-byte words, so that the four pairs of an FFT half-warp (lane = (pair, residue r)) hit
+    // distinct banks in every load and store of the exchange (without them: 4-way conflicts, LSU pipe 91 % busy).
+    static constexpr int TS = SPC * YS + (R == 4 ? 2 : 0);
+    static constexpr int Y_BUF = kSubTile * TS * 8;        // bytes
     // TENSOR: staged output tile = kStgTile spectra of every (stream, channel) of the CTA as fp16 planes, laid out
     // as the shared-memory side of the tensor store: boxes of [SPB streams][2 planes][C channels][32 spectra]
     // (64-byte rows), 64-byte swizzled.
@@ -385,7 +389,7 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, con
 #pragma unroll
                     for (int k = 0; k < kTaps - 1; ++k)
                         acc[(i + k) & 15] = __ffma2_rn(make_float2(wk[k], wk[k]), x, acc[(i + k) & 15]);
-                    yrow[i * (SPC * YS)] = acc[i];
+                    yrow[i * Sh::TS] = acc[i];
                     acc[(i + 15) & 15] = __fmul2_rn(make_float2(wk[15], wk[15]), x);   // first tap of output u + 15
                 }
             }
@@ -411,7 +415,7 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, con
             sl = (ft & 15) / R;
             r = (ft & 15) % R;
         }
-        float2 *ybase = reinterpret_cast<float2 *>(smem + Sh::OFF_Y) + (2 * tp * SPC + sl) * YS;
+        float2 *ybase = reinterpret_cast<float2 *>(smem + Sh::OFF_Y) + 2 * tp * Sh::TS + sl * YS;
         const float4 *wtab4 = reinterpret_cast<const float4 *>(smem + Sh::OFF_WTAB + (sl * R + r) * Sh::TAB_ROW);
         const float4 *zero4 = reinterpret_cast<const float4 *>(smem + Sh::OFF_ZERO);
         const float4 *tw4 = reinterpret_cast<const float4 *>(smem + Sh::OFF_TW + r * Sh::TAB_ROW);
@@ -426,7 +430,7 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, con
             const int kt = kt0 + (jj >> 2), sub = jj & 3;
             const long long t_spec = (long long)kt * kKTile + sub * kSubTile + 2 * tp;   // first of the two spectra
             float2 *y0 = ybase + (size_t)yb * (Sh::Y_BUF / 8);
-            float2 *y1 = y0 + SPC * YS;
+            float2 *y1 = y0 + Sh::TS;
             mbar_wait(bar_y_full + 8 * yb, (uint32_t)(jj / kYBufs) & 1u);
             float2 o0[16], o1[16];
             if (R == 16) {
