@@ -634,6 +634,18 @@ __global__ void history_kernel(const W *__restrict__ samples, const W *__restric
     }
 }
 
+// Same carry for the common case (block at least 15 C samples long, every stream 16-byte aligned): 16-byte copies.
+__global__ void history_vec_kernel(const uint4 *__restrict__ samples, uint4 *__restrict__ hist_new, long long streams,
+                                   long long stream0, long long stream_vecs, long long first_vec, int hist_vecs) {
+    const long long total = streams * hist_vecs;
+    for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < total;
+         idx += (long long)gridDim.x * blockDim.x) {
+        const long long st = idx / hist_vecs;
+        const int i = (int)(idx - st * hist_vecs);
+        hist_new[(stream0 + st) * hist_vecs + i] = __ldg(samples + st * stream_vecs + first_vec + i);
+    }
+}
+
 template <typename I>
 __global__ void unpack_kernel(const I *__restrict__ in, long long n, float *__restrict__ out) {
     for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < n;
@@ -727,6 +739,16 @@ cudaError_t launch_history_update(const cobalt_plan_s *p, cudaStream_t st, const
     if (blocks > 65535) blocks = 65535;
     const void *ho = p->d_hist[p->hist_cur];
     void *hn = p->d_hist[p->hist_cur ^ 1];
+    const size_t sb = sample_bytes(p->bits);
+    if (p->N_u >= HC && (p->N * sb) % 16 == 0 && ((p->N_u - HC) * sb) % 16 == 0 && (HC * sb) % 16 == 0 &&
+        (reinterpret_cast<uintptr_t>(samples_b0) & 15u) == 0) {
+        const int hist_vecs = (int)(HC * sb / 16);
+        long long vb = (streams * hist_vecs + threads - 1) / threads;
+        if (vb > 65535) vb = 65535;
+        history_vec_kernel<<<(unsigned)vb, threads, 0, st>>>(static_cast<const uint4 *>(samples_b0), static_cast<uint4 *>(hn), streams,
+                                                          stream0, (long long)(p->N * sb / 16), (long long)((p->N_u - HC) * sb / 16), hist_vecs);
+        return cudaGetLastError();
+    }
     if (p->bits == 16)
         history_kernel<unsigned int><<<(unsigned)blocks, threads, 0, st>>>(
             static_cast<const unsigned int *>(samples_b0), static_cast<const unsigned int *>(ho),
