@@ -48,6 +48,8 @@ def parse_args(argv=None):
     ap.add_argument("--mode", default="tensor", choices=["tensor", "exact"])
     ap.add_argument("--dft", default="fp32", choices=["fp32", "tensor"],
                     help="F-stage DFT engine (cobalt_set_dft_engine); tensor: C = 256 only")
+    ap.add_argument("--interp", action="store_true",
+                    help="time cobalt_process_interp (delay running linearly over the block, SURVEY.md sec 8(f) row 1)")
     ap.add_argument("--chunk", type=int, default=0, help="subbands per launch group (0 = library default)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -284,8 +286,10 @@ def run_ours(args, rank, world, local):
     stream = torch.cuda.current_stream()
     cor.set_timing(True)
 
+    # --interp: a LOFAR-like drift of 0.15 cycles of the first subband's centre frequency over the block
+    delays_end = (delays + 0.15 / 1.0e8) if args.interp else None
     for _ in range(args.warmup):
-        cor.process(samples, delays, bandpass, out=vis)
+        cor.process(samples, delays, bandpass, out=vis, delays_end=delays_end)
     torch.cuda.synchronize()
 
     sampler = ClockSampler(physical_gpu_index(local))
@@ -297,7 +301,7 @@ def run_ours(args, rank, world, local):
     sampler.start()
     ev[0].record(stream)
     for i in range(args.steps):
-        cor.process(samples, delays, bandpass, out=vis)
+        cor.process(samples, delays, bandpass, out=vis, delays_end=delays_end)
         ev[i + 1].record(stream)
         ms = cor.get_kernel_timing()          # waits for this step's events (device time per kernel)
         for k in range(4):
@@ -342,7 +346,7 @@ def run_ours(args, rank, world, local):
 
     # ---- end to end through the public host-buffer call (pinned host memory, H2D + D2H inside the timed region)
     e2e = None
-    if not args.no_e2e:
+    if not args.no_e2e and not args.interp:
         e2e = run_e2e(args, cfg, cor, samples, delays, bandpass, world, dev)
 
     cpu = None
@@ -359,6 +363,7 @@ def run_ours(args, rank, world, local):
             "data": "synthetic",
             "config": {"workload": cfg.name, "stations": cfg.S, "subbands": cfg.B, "channels": cfg.C, "taps": 16,
                        "samples_per_integration": cfg.N, "input_bits": cfg.bits, "baselines": cfg.n_bl, "mode": args.mode, "dft": args.dft,
+                       "call": "cobalt_process_interp" if args.interp else "cobalt_process",
                        "chunk_subbands": info.chunk_subbands, "parallelism": "replicas" if world > 1 else "single-gpu",
                        "l2": f"inputs ({cfg.input_bytes / 1e9:.2f} GB per step) exceed the 126 MB L2; no flush needed"},
             "roofline": dominant, "roofline_other": other, "roofline_alu": roof_alu,

@@ -119,6 +119,20 @@ int cobalt_process(cobalt_plan_t *plan, void *cuda_stream, const void *d_samples
 int cobalt_process_host(cobalt_plan_t *plan, const void *h_samples, const double *h_delays,
                         const float *h_bandpass, void *h_visibilities);
 
+/* cobalt_process with a delay that varies over the block ("we compute the
+ * channel-dependent phase angles [from the residual delay at the start and the end of the block] in double
+ * precision ... interpolated linearly ... sin/cos and complex multiplication in single precision").  Reading A21
+ * (DESIGN.md): spectrum t (0 <= t < n_t) of station a is rotated with
+ *     tau_a(t) = delays_begin[a] + (delays_end[a] - delays_begin[a]) * t / n_t,
+ * z = F * b[j] * exp(-2 pi i f[s][j] tau_a(t)).  The phase at t = 0 and the phase step per spectrum
+ * f (tau_e - tau_b) / n_t are computed in fp64; the per-spectrum factor in fp32, accurate while
+ * |f (tau_e - tau_b)| stays below about 100 cycles per block.  d_delays_end: device [S] doubles; everything else as
+ * cobalt_process (same buffers, asynchrony, history carry, errors).  delays_end == delays_begin gives
+ * cobalt_process to rounding.  The F-stage always uses COBALT_DFT_FP32 in this call. */
+int cobalt_process_interp(cobalt_plan_t *plan, void *cuda_stream, const void *d_samples,
+                          const double *d_delays_begin, const double *d_delays_end, const float *d_bandpass,
+                          void *d_visibilities);
+
 /* Frees all plan state.  cobalt_destroy(NULL) is a no-op returning COBALT_OK.  The caller must
  * have synchronised every stream that still runs work of this plan. */
 int cobalt_destroy(cobalt_plan_t *plan);

@@ -61,6 +61,13 @@ def _load():
                                                ctypes.c_int, ctypes.c_void_p, _D, _D, _D, ctypes.c_double,
                                                ctypes.c_double, _D, _D]
         lib.oracle_process_subband.restype = ctypes.c_int
+        lib.oracle_fstage_interp_f64.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_longlong, _D, _D, _D,
+                                                 _D, _D, _D, ctypes.c_double, ctypes.c_double, _D]
+        lib.oracle_fstage_interp_f64.restype = ctypes.c_int
+        lib.oracle_process_subband_interp.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_longlong,
+                                                      ctypes.c_int, ctypes.c_void_p, _D, _D, _D, _D, ctypes.c_double,
+                                                      ctypes.c_double, _D, _D]
+        lib.oracle_process_subband_interp.restype = ctypes.c_int
         lib.oracle_channel_direct.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_longlong, _D, _D,
                                               _D, _D, _D, ctypes.c_double, ctypes.c_double, ctypes.c_int, _D, _D]
         lib.oracle_channel_direct.restype = ctypes.c_int
@@ -161,7 +168,7 @@ def new_history(S: int, C: int, T: int = TAPS) -> np.ndarray:
 
 
 def fstage(x: np.ndarray, C: int, hist: np.ndarray | None = None, delays=None, bandpass=None,
-           f_sb: float = 0.0, f_s: float = F_S, g: np.ndarray | None = None, T: int = TAPS) -> np.ndarray:
+           f_sb: float = 0.0, f_s: float = F_S, g: np.ndarray | None = None, T: int = TAPS, delays_end=None) -> np.ndarray:
     """Float entry of the F-stage (steps 2-7, 9): x complex [S][2][N] -> z complex [S][2][n_t][C].
 
     ``hist`` (complex [S][2][(T-1)*C]) is updated in place when given.  ``g`` overrides the
@@ -179,15 +186,17 @@ def fstage(x: np.ndarray, C: int, hist: np.ndarray | None = None, delays=None, b
     z = np.empty((S, 2, n_t, C, 2), dtype=np.float64)
     d = None if delays is None else _f64(delays, (S,))
     b = _f64(np.ones(C) if bandpass is None else bandpass, (C,))
-    rc = _load().oracle_fstage_f64(S, C, T, N, _p(xr), _p(_f64(g, (T * C,))), _p(hr), _p(d), _p(b), f_sb, f_s, _p(z))
+    de = None if delays_end is None else _f64(delays_end, (S,))
+    rc = _load().oracle_fstage_interp_f64(S, C, T, N, _p(xr), _p(_f64(g, (T * C,))), _p(hr), _p(d), _p(de), _p(b), f_sb, f_s, _p(z))
     if rc:
-        raise MemoryError("oracle_fstage_f64")
+        raise MemoryError("oracle_fstage_interp_f64")
     return _r2c(z)
 
 
 def process_subband(samples: np.ndarray, C: int, delays, bandpass, f_sb: float, hist: np.ndarray | None = None,
-                    f_s: float = F_S, T: int = TAPS, return_z: bool = False):
-    """One subband, steps 1-9.  samples int16/int8 [S][2][N][2] -> vis complex [C][n_bl][2][2]."""
+                    f_s: float = F_S, T: int = TAPS, return_z: bool = False, delays_end=None):
+    """One subband, steps 1-9.  samples int16/int8 [S][2][N][2] -> vis complex [C][n_bl][2][2].
+    ``delays_end`` given: the delay of spectrum t is delays + (delays_end - delays) t / n_t (reading A21)."""
     s = np.ascontiguousarray(samples)
     S, two, N, ri = s.shape
     assert two == 2 and ri == 2 and s.dtype in (np.int16, np.int8)
@@ -198,8 +207,9 @@ def process_subband(samples: np.ndarray, C: int, delays, bandpass, f_sb: float, 
     n_t = N // C
     vis = np.empty((C, n_baselines(S), 2, 2, 2), dtype=np.float64)
     z = np.empty((S, 2, n_t, C, 2), dtype=np.float64) if return_z else None
-    rc = _load().oracle_process_subband(S, C, T, N, bits, s.ctypes.data, _p(hist.view(np.float64)),
-                                        _p(_f64(delays, (S,))), _p(_f64(bandpass, (C,))), f_sb, f_s, _p(vis), _p(z))
+    de = None if delays_end is None else _f64(delays_end, (S,))
+    rc = _load().oracle_process_subband_interp(S, C, T, N, bits, s.ctypes.data, _p(hist.view(np.float64)),
+                                               _p(_f64(delays, (S,))), _p(de), _p(_f64(bandpass, (C,))), f_sb, f_s, _p(vis), _p(z))
     if rc:
         raise MemoryError("oracle_process_subband")
     return (_r2c(vis), _r2c(z)) if return_z else _r2c(vis)

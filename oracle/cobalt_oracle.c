@@ -155,6 +155,28 @@ void oracle_rotate(int C, double f_sb, double f_s, double tau, const double *ban
     }
 }
 
+/* "the phase angles [are computed] from the residual delay at the start and
+ * the end of the block ... in double precision [and] interpolated linearly over the block".  Reading A21
+ * (DESIGN.md): spectrum t of an n_t-spectrum block is rotated with the delay
+ *   tau(t) = tau_b + (tau_e - tau_b) t / n_t,          t = 0 .. n_t - 1,
+ * i.e. z[t][j] = F[t][j] b[j] exp(-2 pi i frac(f[j] tau(t))); tau_e = tau_b is oracle_rotate. */
+void oracle_rotate_interp(int C, double f_sb, double f_s, double tau_b, double tau_e, const double *bandpass /*[C]*/,
+                          long long n_t, double *F /*[n_t][C][2] in/out*/) {
+    for (int j = 0; j < C; ++j) {
+        const double f = oracle_channel_frequency(C, f_sb, f_s, j);
+        for (long long t = 0; t < n_t; ++t) {
+            double tau = tau_b + (tau_e - tau_b) * ((double)t / (double)n_t);
+            double cyc = f * tau;
+            double frac = cyc - floor(cyc);
+            double wr = bandpass[j] * cos(-2.0 * ORACLE_PI * frac);
+            double wi = bandpass[j] * sin(-2.0 * ORACLE_PI * frac);
+            double a = F[2 * (t * C + j)], b = F[2 * (t * C + j) + 1];
+            F[2 * (t * C + j)] = a * wr - b * wi;
+            F[2 * (t * C + j) + 1] = a * wi + b * wr;
+        }
+    }
+}
+
 /* ------------------------------------------------------------------ step 8 */
 /* P:L360.  V[j][bl(i,k)][p][q] = sum_t z[i][p][t][j] conj(z[k][q][t][j]), i <= k
  * (readings A9, A10: plain sum, no division, autos keep all four products). */
@@ -193,10 +215,21 @@ void oracle_correlate(int S, int C, long long n_t, const double *z /*[S][2][n_t]
  * quantisation, directly from the test).  hist is read, then replaced by the
  * last (T-1)*C consumed samples (step 9, "carry FIR filter history").
  * delays may be NULL (no rotation, no bandpass: z = F). */
+int oracle_fstage_interp_f64(int S, int C, int T, long long N, const double *x /*[S][2][N][2]*/,
+                             const double *g /*[T*C]*/, double *hist /*[S][2][(T-1)*C][2]*/,
+                             const double *delays /*[S] or NULL*/, const double *delays_end /*[S] or NULL*/,
+                             const double *bandpass /*[C]*/, double f_sb, double f_s, double *z /*[S][2][n_t][C][2]*/);
 int oracle_fstage_f64(int S, int C, int T, long long N, const double *x /*[S][2][N][2]*/,
                       const double *g /*[T*C]*/, double *hist /*[S][2][(T-1)*C][2]*/,
                       const double *delays /*[S] or NULL*/, const double *bandpass /*[C]*/,
                       double f_sb, double f_s, double *z /*[S][2][n_t][C][2]*/) {
+    return oracle_fstage_interp_f64(S, C, T, N, x, g, hist, delays, NULL, bandpass, f_sb, f_s, z);
+}
+/* delays_end != NULL: time-varying delay of reading A21 (oracle_rotate_interp). */
+int oracle_fstage_interp_f64(int S, int C, int T, long long N, const double *x /*[S][2][N][2]*/,
+                             const double *g /*[T*C]*/, double *hist /*[S][2][(T-1)*C][2]*/,
+                             const double *delays /*[S] or NULL*/, const double *delays_end /*[S] or NULL*/,
+                             const double *bandpass /*[C]*/, double f_sb, double f_s, double *z /*[S][2][n_t][C][2]*/) {
     const long long n_t = N / C;          /* reading A11: trailing N - n_t*C samples unused */
     const long long nu = n_t * C;
     const long long nh = (long long)(T - 1) * C;
@@ -217,7 +250,8 @@ int oracle_fstage_f64(int S, int C, int T, long long N, const double *x /*[S][2]
         double *zz = z + 2 * (long long)sp * nu;
         oracle_fir(C, T, g, xh, n_t, y);
         oracle_dft(C, y, n_t, zz);
-        if (delays) oracle_rotate(C, f_sb, f_s, delays[sp / 2], bandpass, n_t, zz);
+        if (delays && delays_end) oracle_rotate_interp(C, f_sb, f_s, delays[sp / 2], delays_end[sp / 2], bandpass, n_t, zz);
+        else if (delays) oracle_rotate(C, f_sb, f_s, delays[sp / 2], bandpass, n_t, zz);
         memcpy(h, xh + 2 * nu, sizeof(double) * 2 * (size_t)nh);   /* last nh of hist||block */
         free(xh);
         free(y);
@@ -229,9 +263,18 @@ int oracle_fstage_f64(int S, int C, int T, long long N, const double *x /*[S][2]
 /* One subband through steps 1-9 from integer samples.  bits = 16 or 8.
  * z_out may be NULL; otherwise receives z [S][2][n_t][C][2].
  * Returns 0, or 1 on allocation failure / bad bits. */
+int oracle_process_subband_interp(int S, int C, int T, long long N, int bits, const void *samples,
+                                  double *hist, const double *delays, const double *delays_end, const double *bandpass,
+                                  double f_sb, double f_s, double *vis, double *z_out);
 int oracle_process_subband(int S, int C, int T, long long N, int bits, const void *samples,
                            double *hist, const double *delays, const double *bandpass,
                            double f_sb, double f_s, double *vis, double *z_out) {
+    return oracle_process_subband_interp(S, C, T, N, bits, samples, hist, delays, NULL, bandpass, f_sb, f_s, vis, z_out);
+}
+/* delays_end != NULL: time-varying delay of reading A21. */
+int oracle_process_subband_interp(int S, int C, int T, long long N, int bits, const void *samples,
+                                  double *hist, const double *delays, const double *delays_end, const double *bandpass,
+                                  double f_sb, double f_s, double *vis, double *z_out) {
     const long long n_t = N / C;
     const long long n_in = (long long)S * 2 * N * 2;
     if (bits != 16 && bits != 8) return 1;
@@ -247,7 +290,7 @@ int oracle_process_subband(int S, int C, int T, long long N, int bits, const voi
     if (bits == 16) oracle_unpack_i16((const int16_t *)samples, n_in, x);
     else oracle_unpack_i8((const int8_t *)samples, n_in, x);
     oracle_fir_prototype(C, T, g);
-    int rc = oracle_fstage_f64(S, C, T, N, x, g, hist, delays, bandpass, f_sb, f_s, z);
+    int rc = oracle_fstage_interp_f64(S, C, T, N, x, g, hist, delays, delays_end, bandpass, f_sb, f_s, z);
     if (!rc) oracle_correlate(S, C, n_t, z, vis);
     free(x);
     free(g);

@@ -30,7 +30,7 @@ F_S = 195312.5
 
 # every symbol include/cobalt.h declares (tests check the library exports exactly these)
 ABI_SYMBOLS = (
-    "cobalt_plan", "cobalt_process", "cobalt_process_host", "cobalt_destroy",
+    "cobalt_plan", "cobalt_process", "cobalt_process_interp", "cobalt_process_host", "cobalt_destroy",
     "cobalt_set_subband_frequencies", "cobalt_set_sample_rate", "cobalt_set_mode",
     "cobalt_set_dft_engine", "cobalt_set_chunk_subbands", "cobalt_reset", "cobalt_info", "cobalt_strerror", "cobalt_last_error",
     "cobalt_set_timing", "cobalt_get_timing", "cobalt_get_kernel_timing",
@@ -72,6 +72,7 @@ def load(path: str | None = None):
     lib.cobalt_plan.argtypes = [ctypes.POINTER(_vp), ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int,
                                 ctypes.c_longlong, ctypes.c_int]
     lib.cobalt_process.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp]
+    lib.cobalt_process_interp.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp, _vp]
     lib.cobalt_process_host.argtypes = [_vp, _vp, _vp, _vp, _vp]
     lib.cobalt_destroy.argtypes = [_vp]
     lib.cobalt_set_subband_frequencies.argtypes = [_vp, _vp]
@@ -147,6 +148,11 @@ def cobalt_plan(stations, subbands, channels, taps, samples_per_integration, inp
 def cobalt_process(plan, stream, d_samples, d_delays, d_bandpass, d_visibilities):
     _check(load().cobalt_process(plan, _stream_ptr(stream), _ptr(d_samples), _ptr(d_delays), _ptr(d_bandpass),
                                  _ptr(d_visibilities)), plan)
+
+
+def cobalt_process_interp(plan, stream, d_samples, d_delays_begin, d_delays_end, d_bandpass, d_visibilities):
+    _check(load().cobalt_process_interp(plan, _stream_ptr(stream), _ptr(d_samples), _ptr(d_delays_begin), _ptr(d_delays_end),
+                                        _ptr(d_bandpass), _ptr(d_visibilities)), plan)
 
 
 def cobalt_process_host(plan, h_samples, h_delays, h_bandpass, h_visibilities):
@@ -237,9 +243,11 @@ class Correlator:
         i = self.info
         return (i.subbands, i.channels, i.n_baselines, 2, 2)
 
-    def process(self, samples, delays, bandpass, out=None, stream=None):
+    def process(self, samples, delays, bandpass, out=None, stream=None, delays_end=None):
         """samples int16/int8 [B][S][2][N][2], delays float64 [S], bandpass float32 [C] (CUDA tensors)
-        -> complex64 [B][C][n_bl][2][2].  Enqueues on ``stream`` (default: torch's current stream)."""
+        -> complex64 [B][C][n_bl][2][2].  Enqueues on ``stream`` (default: torch's current stream).
+        ``delays_end`` (float64 [S]) selects cobalt_process_interp: the delay runs linearly from ``delays`` at the first
+        spectrum to ``delays_end`` at the end of the block."""
         import torch
 
         i = self.info
@@ -251,7 +259,11 @@ class Correlator:
         if out is None:
             out = torch.empty(self.vis_shape(), dtype=torch.complex64, device=samples.device)
         assert out.is_cuda and out.is_contiguous() and out.dtype == torch.complex64 and tuple(out.shape) == self.vis_shape()
-        cobalt_process(self._h, stream, samples, delays, bandpass, out)
+        if delays_end is None:
+            cobalt_process(self._h, stream, samples, delays, bandpass, out)
+        else:
+            assert delays_end.is_cuda and delays_end.dtype == torch.float64 and delays_end.is_contiguous() and delays_end.numel() == i.stations
+            cobalt_process_interp(self._h, stream, samples, delays, delays_end, bandpass, out)
         return out
 
     def process_host(self, samples, delays, bandpass, out):

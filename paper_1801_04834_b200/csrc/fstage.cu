@@ -35,6 +35,7 @@ struct FArgs {
     const unsigned char *hist;      // [B][S][2][15 C] complex integers
     const float *weights;           // [16][C]
     const float2 *phase;            // [nb][S][C]
+    const float *dstep;             // [nb][S][C] phase step per spectrum in cycles (time-varying delay), or nullptr
     unsigned char *z;               // chunk intermediate
     long long N, n_t;
     size_t z_subband_bytes;
@@ -50,6 +51,20 @@ __device__ __forceinline__ float2 csub(float2 a, float2 b) { return __ffma2_rn(b
 __device__ __forceinline__ float2 cmul_tab2(float2 v, float2 t) {
     const float2 p = __fmul2_rn(make_float2(v.x, v.x), t);
     return __ffma2_rn(make_float2(-t.y, t.x), make_float2(v.y, v.y), p);
+}
+
+// Time-varying delay: rotation w (for the delay at the start of the block) times exp(-2 pi i frac(t step)) for the
+// spectra t and t + 1; step in cycles per spectrum.  fp32 throughout.
+__device__ __forceinline__ void interp_factors(float step, long long t, float2 w, float2 &w0, float2 &w1) {
+    float p0 = step * (float)t;
+    p0 -= rintf(p0);
+    float p1 = p0 + step;
+    p1 -= rintf(p1);
+    float s0, c0, s1, c1;
+    __sincosf(-6.283185307179586f * p0, &s0, &c0);
+    __sincosf(-6.283185307179586f * p1, &s1, &c1);
+    w0 = cmul_tab2(w, make_float2(c0, s0));
+    w1 = cmul_tab2(w, make_float2(c1, s1));
 }
 
 // Forward 4-point DFT in place: X[k] = sum_n a[n] (-i)^{nk}.
@@ -132,7 +147,7 @@ constexpr int kYBufs = 3;          // ring of FIR-output sub-tiles
 constexpr int kStgTile = 32;       // spectra per staged output tile (= one tensor store per box)
 constexpr int kStgBufs = 2;
 
-template <int C, int BITS, bool TENSOR>
+template <int C, int BITS, bool TENSOR, bool INTERP = false>
 struct FShape {
     static constexpr int SB = BITS == 16 ? 4 : 2;          // bytes per complex sample
     static constexpr int SPC = 256 / C;                    // streams per CTA
@@ -165,7 +180,9 @@ struct FShape {
     static constexpr int OFF_WTAB = OFF_Y + kYBufs * Y_BUF;      // [SPC][R] rows: rotation * bandpass, in register order
     static constexpr int OFF_ZERO = OFF_WTAB + 16 * TAB_ROW;     // 16 float2 of zeros (spectra beyond n_t)
     static constexpr int OFF_TW = OFF_ZERO + 128;                // [R] rows: W_C^{r k1}
-    static constexpr int TOTAL = OFF_TW + (R > 1 ? R * TAB_ROW : 0);
+    static constexpr int OFF_STEP = OFF_TW + (R > 1 ? R * TAB_ROW : 0);   // INTERP: [SPC][R] rows of 16 floats, pitch 80 bytes
+    static constexpr int STEP_ROW = 80;
+    static constexpr int TOTAL = OFF_STEP + (INTERP ? 16 * STEP_ROW : 0);
     static_assert(TOTAL <= 227 * 1024, "shared memory budget");
 };
 
@@ -203,9 +220,13 @@ __device__ __forceinline__ constexpr int out_reg(int i) {
     return R == 4 ? i : dft16_pos(i);
 }
 
-template <int C, int BITS, bool TENSOR>
+// INTERP (reading A21): the delay of spectrum t is tau_b + (tau_e - tau_b) t / n_t.
+// The table holds the rotation for tau_b; a second table holds the phase step per spectrum f (tau_e - tau_b) / n_t in
+// cycles (computed in fp64), and the per-spectrum factor exp(-2 pi i frac(t step)) is formed in fp32 ("sin/cos and
+// complex multiply in single precision").
+template <int C, int BITS, bool TENSOR, bool INTERP>
 __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, const __grid_constant__ CUtensorMap zmap) {
-    using Sh = FShape<C, BITS, TENSOR>;
+    using Sh = FShape<C, BITS, TENSOR, INTERP>;
     constexpr int SB = Sh::SB, SPC = Sh::SPC, R = Sh::R, YS = Sh::YS;
     extern __shared__ __align__(1024) unsigned char smem[];
     const uint32_t sbase = smem_u32(smem);
@@ -248,6 +269,14 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, con
             const int m = m0 + sl;
             reinterpret_cast<float2 *>(smem + Sh::OFF_WTAB + (idx >> 4) * Sh::TAB_ROW)[i] =
                 m < a.M ? a.phase[((size_t)bl * a.S + (m >> 1)) * C + out_channel<R>(rr, i)] : make_float2(0.f, 0.f);
+        }
+        if (INTERP) {
+            for (int idx = tid; idx < 256; idx += kFThreads) {
+                const int sl = idx / C, rr = (idx % C) / 16, i = idx % 16;
+                const int m = m0 + sl;
+                reinterpret_cast<float *>(smem + Sh::OFF_STEP + (idx >> 4) * Sh::STEP_ROW)[i] =
+                    m < a.M ? a.dstep[((size_t)bl * a.S + (m >> 1)) * C + out_channel<R>(rr, i)] : 0.f;
+            }
         }
         if (tid < 16) reinterpret_cast<float2 *>(smem + Sh::OFF_ZERO)[tid] = make_float2(0.f, 0.f);
         if (R > 1) {
@@ -418,6 +447,7 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, con
         float2 *ybase = reinterpret_cast<float2 *>(smem + Sh::OFF_Y) + 2 * tp * Sh::TS + sl * YS;
         const float4 *wtab4 = reinterpret_cast<const float4 *>(smem + Sh::OFF_WTAB + (sl * R + r) * Sh::TAB_ROW);
         const float4 *zero4 = reinterpret_cast<const float4 *>(smem + Sh::OFF_ZERO);
+        const float *steps = reinterpret_cast<const float *>(smem + Sh::OFF_STEP + (sl * R + r) * Sh::STEP_ROW);
         const float4 *tw4 = reinterpret_cast<const float4 *>(smem + Sh::OFF_TW + r * Sh::TAB_ROW);
         const int m = m0 + sl;
         // staging word of (channel c, plane, pair p of the tile): box b = sl / SPB, then [stream][plane][channel][64 B],
@@ -532,7 +562,9 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, con
                         const int dj = out_channel<R>(0, i + e);                 // compile-time part of the channel index
                         const int ibits = R == 16 ? 0 : R == 4 ? ((i + e) >> 3) & 1 : ((i + e) >> 1) & 3;
                         const float2 ww = e ? make_float2(w.z, w.w) : make_float2(w.x, w.y);
-                        const float2 z0 = cmul_tab2(o0[oi], ww), z1 = cmul_tab2(o1[oi], ww);
+                        float2 ww0 = ww, ww1 = ww;
+                        if (INTERP) interp_factors(steps[i + e], t_spec, ww, ww0, ww1);
+                        const float2 z0 = cmul_tab2(o0[oi], ww0), z1 = cmul_tab2(o1[oi], ww1);
                         *reinterpret_cast<uint32_t *>(stg_v[ibits] + dj * 64) = pack_half2(z0.x, z1.x) & msk;
                         *reinterpret_cast<uint32_t *>(stg_v[ibits] + dj * 64 + C * 64) = pack_half2(z0.y, z1.y) & msk;
                     }
@@ -550,9 +582,11 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, con
                         for (int e = 0; e < 2; ++e) {
                             const int j = out_channel<R>(r, i + e), oi = out_reg<R>(i + e);
                             const float2 ww = e ? make_float2(w.z, w.w) : make_float2(w.x, w.y);
+                            float2 ww0 = ww, ww1 = ww;
+                            if (INTERP) interp_factors(steps[i + e], t_spec, ww, ww0, ww1);
                             float2 *dst = reinterpret_cast<float2 *>(zsub) + ((size_t)j * a.M + m) * a.n_t + t_spec;
-                            if (live0) dst[0] = cmul_tab2(o0[oi], ww);
-                            if (live1) dst[1] = cmul_tab2(o1[oi], ww);
+                            if (live0) dst[0] = cmul_tab2(o0[oi], ww0);
+                            if (live1) dst[1] = cmul_tab2(o1[oi], ww1);
                         }
                     }
                 }
@@ -572,7 +606,8 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, con
 __global__ void phase_table_kernel(const double *__restrict__ delays, const float *__restrict__ bandpass,
                                    const double *__restrict__ f_sb, int b0, int nb, int S, int C, double f_s,
                                    float amp_max, int tensor, float *__restrict__ scale_out,
-                                   float2 *__restrict__ out) {
+                                   float2 *__restrict__ out, const double *__restrict__ delays_end, double inv_n_t,
+                                   float *__restrict__ step_out) {
     __shared__ float s_max[32];
     __shared__ float s_scale;
     float bm = 0.f;
@@ -611,6 +646,8 @@ __global__ void phase_table_kernel(const double *__restrict__ delays, const floa
         sincospi(-2.0 * frac, &sn, &cs);
         const double b = (double)bandpass[j] * sc;
         out[idx] = make_float2((float)(b * cs), (float)(b * sn));
+        // time-varying delay (reading A21): phase step per spectrum, in cycles, from the fp64 delays
+        if (delays_end) step_out[idx] = (float)(f * (delays_end[s] - delays[s]) * inv_n_t);
     }
 }
 
@@ -653,10 +690,10 @@ __global__ void unpack_kernel(const I *__restrict__ in, long long n, float *__re
         out[idx] = (float)in[idx];
 }
 
-template <int C, int BITS, bool TENSOR>
+template <int C, int BITS, bool TENSOR, bool INTERP>
 cudaError_t launch_f(const cobalt_plan_s *p, cudaStream_t st, const FArgs &a, int nb) {
-    using Sh = FShape<C, BITS, TENSOR>;
-    auto kern = fstage_kernel<C, BITS, TENSOR>;
+    using Sh = FShape<C, BITS, TENSOR, INTERP>;
+    auto kern = fstage_kernel<C, BITS, TENSOR, INTERP>;
     const size_t smem = Sh::TOTAL;
     static_assert(Sh::SPB == kStoreBoxStreams(C), "plan.cu builds the tensor map with the same box");
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -681,8 +718,12 @@ cudaError_t launch_f(const cobalt_plan_s *p, cudaStream_t st, const FArgs &a, in
 template <int C>
 cudaError_t launch_f_c(const cobalt_plan_s *p, cudaStream_t st, const FArgs &a, int nb) {
     const bool tensor = p->mode == COBALT_MODE_TENSOR_FP16;
-    if (p->bits == 16) return tensor ? launch_f<C, 16, true>(p, st, a, nb) : launch_f<C, 16, false>(p, st, a, nb);
-    return tensor ? launch_f<C, 8, true>(p, st, a, nb) : launch_f<C, 8, false>(p, st, a, nb);
+    if (a.dstep) {
+        if (p->bits == 16) return tensor ? launch_f<C, 16, true, true>(p, st, a, nb) : launch_f<C, 16, false, true>(p, st, a, nb);
+        return tensor ? launch_f<C, 8, true, true>(p, st, a, nb) : launch_f<C, 8, false, true>(p, st, a, nb);
+    }
+    if (p->bits == 16) return tensor ? launch_f<C, 16, true, false>(p, st, a, nb) : launch_f<C, 16, false, false>(p, st, a, nb);
+    return tensor ? launch_f<C, 8, true, false>(p, st, a, nb) : launch_f<C, 8, false, false>(p, st, a, nb);
 }
 
 }  // namespace
@@ -695,7 +736,8 @@ cudaError_t launch_phase_table(const cobalt_plan_s *p, cudaStream_t st, const do
     if (blocks > 4096) blocks = 4096;
     phase_table_kernel<<<(unsigned)blocks, threads, 0, st>>>(d_delays, d_bandpass, p->d_f_sb, b0, nb, p->S, p->C,
                                                              p->f_s, p->amp_max, p->mode == COBALT_MODE_TENSOR_FP16 ? 1 : 0,
-                                                             p->d_scale, p->d_phase);
+                                                             p->d_scale, p->d_phase, p->cur_delays_end, 1.0 / (double)p->n_t,
+                                                             p->d_dstep);
     return cudaGetLastError();
 }
 
@@ -705,13 +747,14 @@ cudaError_t launch_set_unit_scale(const cobalt_plan_s *p, cudaStream_t st) {
 }
 
 cudaError_t launch_fstage(const cobalt_plan_s *p, cudaStream_t st, const void *samples_b0, int b0, int nb) {
-    if (p->C == 256 && p->mode == COBALT_MODE_TENSOR_FP16 && p->dft_engine == COBALT_DFT_TENSOR)
+    if (p->C == 256 && p->mode == COBALT_MODE_TENSOR_FP16 && p->dft_engine == COBALT_DFT_TENSOR && !p->cur_delays_end)
         return launch_fstage_tc(p, st, samples_b0, b0, nb);      // DFT on the tensor cores (fstage_tc.cu)
     FArgs a;
     a.samples = static_cast<const unsigned char *>(samples_b0);
     a.hist = static_cast<const unsigned char *>(p->d_hist[p->hist_cur]);
     a.weights = p->d_weights;
     a.phase = p->d_phase;
+    a.dstep = p->cur_delays_end ? p->d_dstep : nullptr;
     a.z = static_cast<unsigned char *>(p->d_z);
     a.N = p->N;
     a.n_t = p->n_t;

@@ -55,6 +55,8 @@ size_t subband_output_bytes(const cobalt_plan_s *p) { return (size_t)p->C * (siz
 
 void free_scratch(cobalt_plan_s *p) {
     cudaFree(p->d_z);
+    cudaFree(p->d_dstep);
+    p->d_dstep = nullptr;
     cudaFree(p->d_phase);
     p->d_z = nullptr;
     p->d_phase = nullptr;
@@ -106,6 +108,7 @@ int alloc_scratch(cobalt_plan_s *p, int chunk_request) {
     CK(p, cudaMalloc(&p->d_z, (size_t)chunk * p->z_subband_bytes));
     CK(p, cudaMemset(p->d_z, 0, (size_t)chunk * p->z_subband_bytes));   // zero rows 2S..Mpad stay zero forever
     CK(p, cudaMalloc(&p->d_phase, (size_t)chunk * p->S * p->C * sizeof(float2)));
+    CK(p, cudaMalloc(&p->d_dstep, (size_t)chunk * p->S * p->C * sizeof(float)));
     CK(p, cudaDeviceSynchronize());
     {
         const int rc = build_zmap(p);
@@ -289,6 +292,16 @@ int cobalt_process(cobalt_plan_t *p, void *cuda_stream, const void *d_samples, c
     if (p->timing) p->n_chunks_timed = n_chunks;
     p->hist_cur ^= 1;   // the history kernels of this call wrote the other buffer (stream ordered)
     return COBALT_OK;
+}
+
+int cobalt_process_interp(cobalt_plan_t *p, void *cuda_stream, const void *d_samples, const double *d_delays_begin,
+                          const double *d_delays_end, const float *d_bandpass, void *d_visibilities) {
+    if (!p) return fail(nullptr, COBALT_ERR_BAD_ARG, "plan is NULL");
+    if (!d_delays_end) return fail(p, COBALT_ERR_BAD_ARG, "NULL buffer");
+    p->cur_delays_end = d_delays_end;      // read by the launch helpers of this call only
+    const int rc = cobalt_process(p, cuda_stream, d_samples, d_delays_begin, d_bandpass, d_visibilities);
+    p->cur_delays_end = nullptr;
+    return rc;
 }
 
 int cobalt_process_host(cobalt_plan_t *p, const void *h_samples, const double *h_delays, const float *h_bandpass,

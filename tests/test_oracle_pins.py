@@ -360,3 +360,42 @@ def test_golden_tiny_case_is_reproduced(oracle):
     exp = np.loadtxt(os.path.join(here, "tiny_fx_expected.txt")).view(np.complex128).reshape(mg.C, 3, 2, 2)
     vis = oracle.process_subband(x, mg.C, mg.DELAYS, mg.BANDPASS, oracle.default_subband_frequency(0))
     assert np.max(np.abs(vis - exp)) <= 1e-9 * np.max(np.abs(exp))
+
+
+# ------------------------------------------------------------------ P16: time-varying delay (reading A21)
+def test_p16_equal_begin_and_end_delays_are_the_static_rotation(oracle):
+    rng = np.random.default_rng(16)
+    C, S, n_t = 16, 3, 37
+    x = rng.integers(-300, 300, size=(S, 2, n_t * C + 5, 2)).astype(np.int16)
+    tau = rng.uniform(0, 2e-6, S)
+    b = 1.0 + 0.1 * rng.uniform(-1, 1, C)
+    f = 1.2e8
+    v0 = oracle.process_subband(x, C, tau, b, f)
+    v1 = oracle.process_subband(x, C, tau, b, f, delays_end=tau.copy())
+    assert np.array_equal(v0, v1)
+
+
+@pytest.mark.parametrize("drift_cycles", [0.15, -3.7])
+def test_p16_linear_delay_drift_is_a_geometric_series(oracle, drift_cycles):
+    """Warmed-up DC input puts F[t][C/2] = A in every spectrum, so with station 1 drifting from tau_b to tau_e the
+    cross-correlation of the centre channel is a geometric series with a closed form:
+      V01 = |A|^2 sum_t exp(+2 pi i f_c (tau_b + (tau_e - tau_b) t / n_t)) = |A|^2 e^{2 pi i f_c tau_b} (1 - r^n_t) / (1 - r),
+    r = exp(2 pi i f_c (tau_e - tau_b) / n_t).  Fixes the interpolation end points (t = 0 is tau_b, t = n_t would be
+    tau_e), the sign and that the phase is linear in t."""
+    C, n_t = 16, 200
+    A = 2.0 - 1.5j
+    f_c = 1.0e8                                                 # channel C/2 sits at f_sb
+    tau_b = 0.3 / f_c
+    tau_e = tau_b + drift_cycles / f_c
+    x = np.full((2, 2, n_t * C), A, dtype=np.complex128)
+    hist = np.full((2, 2, (T - 1) * C), A, dtype=np.complex128)  # filter already warmed up
+    z = oracle.fstage(x, C, hist=hist, delays=np.array([0.0, tau_b]), bandpass=np.ones(C), f_sb=f_c,
+                      delays_end=np.array([0.0, tau_e]))
+    np.testing.assert_allclose(z[0, 0, :, C // 2], A, rtol=0, atol=1e-12)          # station 0: not rotated
+    v = oracle.correlate(z)                                     # [C][n_bl][2][2]
+    r = np.exp(2j * np.pi * drift_cycles / n_t)
+    want = abs(A) ** 2 * np.exp(2j * np.pi * 0.3) * (1 - r ** n_t) / (1 - r)
+    got = v[C // 2, oracle.baseline_index(0, 1), 0, 0]
+    assert abs(got - want) <= 1e-9 * abs(A) ** 2 * n_t
+    # autocorrelation of the drifting station is unaffected (a pure phase)
+    assert abs(v[C // 2, oracle.baseline_index(1, 1), 0, 0] - abs(A) ** 2 * n_t) <= 1e-9 * abs(A) ** 2 * n_t

@@ -339,6 +339,53 @@ def test_dft_engine_rejects_unknown_value(cobalt, dev):
         cor.set_dft_engine(cobalt.COBALT_DFT_TENSOR)      # accepted for any C; C != 256 keeps the fp32 FFT
 
 
+# ------------------------------------------------------------------ time-varying delay (reading A21)
+@pytest.mark.parametrize("C,bits,S,n_t,drift", [(16, 16, 3, 150, 0.15), (64, 16, 2, 203, -2.5), (256, 16, 2, 70, 0.15),
+                                                (64, 8, 3, 130, 30.0), (256, 8, 1, 65, -0.4)])
+@pytest.mark.parametrize("mode_tensor", [False, True])
+def test_time_varying_delay_matches_oracle(cobalt, oracle, dev, C, bits, S, n_t, drift, mode_tensor):
+    """cobalt_process_interp: the delay runs linearly from delays to delays_end over the block; drift =
+    phase change of the subband centre over the block in cycles (LOFAR rates give ~0.15; 30 stresses the fp32 step)."""
+    synth = _synth()
+    cfg = synth.scaled(synth.CONFIGS[2 if bits == 16 else 4], S=S, B=2, C=C, N=n_t * C + 3, bits=bits)
+    data = synth.generate(cfg, device="cpu")
+    rng = np.random.default_rng(21)
+    tau_b = data["delays"].numpy()
+    tau_e = tau_b + drift / oracle.default_subband_frequency(0) * rng.uniform(0.5, 1.0, S)
+    bp = data["bandpass"].numpy().astype(np.float64)
+    samples = data["samples"].numpy()
+    mode = cobalt.COBALT_MODE_TENSOR_FP16 if mode_tensor else cobalt.COBALT_MODE_EXACT_FP32
+    with cobalt.Correlator(cfg.S, cfg.B, cfg.C, cfg.N, cfg.bits, mode=mode) as cor:
+        cor.set_dft_engine(cobalt.COBALT_DFT_TENSOR)            # ignored by this call: it always uses the fp32 FFT
+        vg = cor.process(data["samples"].to(dev), data["delays"].to(dev), data["bandpass"].to(dev),
+                         delays_end=torch.from_numpy(tau_e).to(dev))
+        vs = cor.process(data["samples"].to(dev), data["delays"].to(dev), data["bandpass"].to(dev))   # second call: history carried
+        torch.cuda.synchronize()
+        vg = vg.cpu().numpy()
+    for b in range(cfg.B):
+        vo = oracle.process_subband(samples[b], C, tau_b, bp, oracle.default_subband_frequency(b), delays_end=tau_e)
+        _assert_parity(vg[b], vo, mode_tensor, f"time-varying delay, subband {b}")
+        if S > 1:
+            static = oracle.process_subband(samples[b], C, tau_b, bp, oracle.default_subband_frequency(b))
+            assert np.max(np.abs(static - vo)) > 1e-3 * np.max(np.abs(vo))      # the drift really changes the result
+    assert np.all(np.isfinite(vs.cpu().numpy()))
+
+
+def test_time_varying_delay_with_equal_ends_is_the_static_call(cobalt, dev):
+    synth = _synth()
+    cfg = synth.scaled(synth.CONFIGS[2], S=4, B=1, C=64, N=64 * 90)
+    data = synth.generate(cfg, device="cpu")
+    out = []
+    for interp in (False, True):
+        with cobalt.Correlator(cfg.S, cfg.B, cfg.C, cfg.N, cfg.bits, mode=cobalt.COBALT_MODE_EXACT_FP32) as cor:
+            d = data["delays"].to(dev)
+            v = cor.process(data["samples"].to(dev), d, data["bandpass"].to(dev), delays_end=d.clone() if interp else None)
+            torch.cuda.synchronize()
+            out.append(v.cpu().numpy())
+    scale = np.max(np.abs(out[0]))
+    assert np.max(np.abs(out[0] - out[1])) <= 2e-6 * scale
+
+
 def test_golden_tiny_case_on_gpu(cobalt, dev):
     """The frozen oracle values of tests/golden/ (written by the oracle alone) against both GPU modes."""
     import os
