@@ -13,6 +13,8 @@
  *                      samples across to the next block."                          -> oracle_fir, oracle_dft
  *   P:L360, P:L368    "fine delay compensation and bandpass correction"; phase
  *                      angles in double precision, rotate each sample               -> oracle_rotate
+ *   P:L368            phase angles from the residual delay at block start and end,
+ *                      interpolated linearly (reading A21) -> oracle_rotate_interp
  *   P:L360            "computes the correlations of all pairs of antenna fields
  *                      and averages in time"                                        -> oracle_correlate
  * The paper prints no formulas; every formula below is the reading fixed in
@@ -25,7 +27,8 @@
  * Pins (tests/test_oracle_pins.py): P2 firwin, P3 DC, P4 tone closed form, P5
  * impulse, P6 numpy.fft special case, P7 Hermitian, P8 identical streams, P9
  * delay slope, P10 history carry, P11 brute force (oracle_channel_direct below
- * + a numpy brute force), P12 linearity, P13 statistics.  No function here is
+ * + a numpy brute force), P12 linearity, P13 statistics, P16 time-varying delay
+ * (equal ends = static rotation; closed-form geometric series).  No function here is
  * "parity unpinned".
  *
  * Layouts (all row-major, last index fastest):
