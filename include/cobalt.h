@@ -148,8 +148,10 @@ int cobalt_set_mode(cobalt_plan_t *plan, int mode);
  *                     rounded to fp16, so channel isolation is that of the fp32 filter bank;
  *   COBALT_DFT_TENSOR two 16-point DFT passes as fp16 GEMMs on the tensor cores (C = 256 only; other C and
  *                     EXACT mode silently keep COBALT_DFT_FP32).  1-4 % faster on config 3, but the FIR output
- *                     is rounded to fp16 BEFORE the DFT: a channel holding 2^-11 or less of the amplitude of
- *                     the strongest channel of the same spectrum is no longer within the 2e-3 tolerance.
+ *                     is rounded to fp16 BEFORE the DFT: the rounding noise of a spectrum (2^-12 of each FIR output)
+ *                     spreads over its channels, about 1e-5 of the strongest channel's amplitude in every channel
+ *                     (-100 dB), so a channel more than ~40 dB weaker than the strongest channel of the same
+ *                     spectrum is no longer within the 2e-3 relative tolerance.
  * Takes effect at the next cobalt_process. */
 #define COBALT_DFT_FP32 0
 #define COBALT_DFT_TENSOR 1
