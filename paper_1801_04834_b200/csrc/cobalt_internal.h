@@ -82,8 +82,8 @@ struct cobalt_plan_s {
     std::vector<float> h_weights;
     void *d_hist[2] = {nullptr, nullptr};   // raw integer samples [B][S][2][15 C][2]; ping-pong
     int hist_cur = 0;
-    float2 *d_phase = nullptr;         // [chunk][S][C]  s b[j] exp(-2 pi i frac(f tau))
-    float *d_dstep = nullptr;          // [chunk][S][C] phase step per spectrum in cycles (cobalt_process_interp)
+    float2 *d_phase = nullptr;         // [B][S][C]  s b[j] exp(-2 pi i frac(f tau)), built once per call
+    float *d_dstep = nullptr;          // [B][S][C] phase step per spectrum in cycles (cobalt_process_interp)
     const double *cur_delays_end = nullptr;   // device [S], set for the duration of cobalt_process_interp
     float *d_scale = nullptr;          // {s, 1/s, 1/s^2}: power-of-two scale of the fp16 intermediate (1 in EXACT mode)
     float amp_max = 0.f;               // worst-case |F| for full-scale input: sum|g| * sqrt(2) * 2^(bits-1)

@@ -645,9 +645,10 @@ __global__ void phase_table_kernel(const double *__restrict__ delays, const floa
         double sn, cs;
         sincospi(-2.0 * frac, &sn, &cs);
         const double b = (double)bandpass[j] * sc;
-        out[idx] = make_float2((float)(b * cs), (float)(b * sn));
+        const long long o = (long long)b0 * S * C + idx;      // tables are indexed by the subband of the plan
+        out[o] = make_float2((float)(b * cs), (float)(b * sn));
         // time-varying delay (reading A21): phase step per spectrum, in cycles, from the fp64 delays
-        if (delays_end) step_out[idx] = (float)(f * (delays_end[s] - delays[s]) * inv_n_t);
+        if (delays_end) step_out[o] = (float)(f * (delays_end[s] - delays[s]) * inv_n_t);
     }
 }
 
@@ -753,8 +754,8 @@ cudaError_t launch_fstage(const cobalt_plan_s *p, cudaStream_t st, const void *s
     a.samples = static_cast<const unsigned char *>(samples_b0);
     a.hist = static_cast<const unsigned char *>(p->d_hist[p->hist_cur]);
     a.weights = p->d_weights;
-    a.phase = p->d_phase;
-    a.dstep = p->cur_delays_end ? p->d_dstep : nullptr;
+    a.phase = p->d_phase + (size_t)b0 * p->S * p->C;
+    a.dstep = p->cur_delays_end ? p->d_dstep + (size_t)b0 * p->S * p->C : nullptr;
     a.z = static_cast<unsigned char *>(p->d_z);
     a.N = p->N;
     a.n_t = p->n_t;

@@ -513,7 +513,7 @@ cudaError_t launch_fstage_tc(const cobalt_plan_s *p, cudaStream_t st, const void
     a.samples = static_cast<const unsigned char *>(samples_b0);
     a.hist = static_cast<const unsigned char *>(p->d_hist[p->hist_cur]);
     a.weights = p->d_weights;
-    a.phase = p->d_phase;
+    a.phase = p->d_phase + (size_t)b0 * p->S * p->C;
     a.N = p->N;
     a.n_t = p->n_t;
     a.S = p->S;

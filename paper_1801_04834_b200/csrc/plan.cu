@@ -107,15 +107,15 @@ int alloc_scratch(cobalt_plan_s *p, int chunk_request) {
     p->chunk = chunk;
     CK(p, cudaMalloc(&p->d_z, (size_t)chunk * p->z_subband_bytes));
     CK(p, cudaMemset(p->d_z, 0, (size_t)chunk * p->z_subband_bytes));   // zero rows 2S..Mpad stay zero forever
-    CK(p, cudaMalloc(&p->d_phase, (size_t)chunk * p->S * p->C * sizeof(float2)));
-    CK(p, cudaMalloc(&p->d_dstep, (size_t)chunk * p->S * p->C * sizeof(float)));
+    CK(p, cudaMalloc(&p->d_phase, (size_t)p->B * p->S * p->C * sizeof(float2)));
+    CK(p, cudaMalloc(&p->d_dstep, (size_t)p->B * p->S * p->C * sizeof(float)));
     CK(p, cudaDeviceSynchronize());
     {
         const int rc = build_zmap(p);
         if (rc != COBALT_OK) return rc;
     }
     const size_t hist = (size_t)p->B * p->M * (kTaps - 1) * p->C * sample_bytes(p->bits);
-    p->scratch_bytes = (size_t)chunk * p->z_subband_bytes + (size_t)chunk * p->S * p->C * sizeof(float2) + 2 * hist +
+    p->scratch_bytes = (size_t)chunk * p->z_subband_bytes + (size_t)p->B * p->S * p->C * (sizeof(float2) + sizeof(float)) + 2 * hist +
                        (size_t)kTaps * p->C * sizeof(float) + (size_t)p->B * sizeof(double);
     return COBALT_OK;
 }
@@ -124,7 +124,7 @@ int alloc_scratch(cobalt_plan_s *p, int chunk_request) {
 int enqueue_chunk(cobalt_plan_s *p, cudaStream_t st, const void *samples_b0, const double *d_delays,
                   const float *d_bandpass, float2 *vis_b0, int b0, int nb, StageEvents *ev) {
     if (ev) CK(p, cudaEventRecord(ev->e[0], st));
-    CK(p, launch_phase_table(p, st, d_delays, d_bandpass, b0, nb));
+    if (b0 == 0) CK(p, launch_phase_table(p, st, d_delays, d_bandpass, 0, p->B));   // every subband's table in one launch
     if (ev) CK(p, cudaEventRecord(ev->e[1], st));
     CK(p, launch_fstage(p, st, samples_b0, b0, nb));
     if (ev) CK(p, cudaEventRecord(ev->e[2], st));
@@ -133,7 +133,7 @@ int enqueue_chunk(cobalt_plan_s *p, cudaStream_t st, const void *samples_b0, con
     if (p->mode == COBALT_MODE_TENSOR_FP16) CK(p, launch_xstage_tc(p, st, p->d_z, nb, vis_b0));
     else CK(p, launch_xstage_simt(p, st, p->d_z, nb, vis_b0));
     if (ev) CK(p, cudaEventRecord(ev->e[4], st));
-    p->launches += 4;
+    p->launches += b0 == 0 ? 4 : 3;
     return COBALT_OK;
 }
 
