@@ -526,7 +526,7 @@ cudaError_t launch_xstage_tc(const cobalt_plan_s *p, cudaStream_t st, const void
     for (const XJob &j : p->jobs) max_rows = (j.ld_nrows[0] + j.ld_nrows[1]) > max_rows ? (j.ld_nrows[0] + j.ld_nrows[1]) : max_rows;
     a.stage_bytes = max_rows * 256;
     a.out_off = (uint32_t)p->x_out_off;
-    auto kern = p->x_staged ? xstage_tc_kernel<true> : xstage_tc_kernel<false>;
+    auto kern = p->x_staged ? xstage_tc_kernel<true> : xstage_tc_kernel<false>;   // d_vis is 16-byte aligned (cobalt_process)
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->x_smem_bytes);
     if (e != cudaSuccess) return e;
     const int grid = a.total_jobs < p->sm_count ? a.total_jobs : p->sm_count;

@@ -386,6 +386,30 @@ def test_time_varying_delay_with_equal_ends_is_the_static_call(cobalt, dev):
     assert np.max(np.abs(out[0] - out[1])) <= 2e-6 * scale
 
 
+def test_output_pointer_not_16_byte_aligned_is_rejected_in_tensor_mode(cobalt, dev):
+    """The tensor-mode X-stage writes 16-byte pieces (and whole channel blocks with one bulk store): an 8-byte
+    aligned visibility buffer is a COBALT_ERR_BAD_ARG, not a fault; EXACT mode (8-byte stores) accepts it."""
+    synth = _synth()
+    cfg = synth.scaled(synth.CONFIGS[2], S=5, B=2, C=64, N=64 * 70)
+    data = synth.generate(cfg, device="cpu")
+    args = (data["samples"].to(dev), data["delays"].to(dev), data["bandpass"].to(dev))
+    for mode in (cobalt.COBALT_MODE_TENSOR_FP16, cobalt.COBALT_MODE_EXACT_FP32):
+        with cobalt.Correlator(cfg.S, cfg.B, cfg.C, cfg.N, cfg.bits, mode=mode) as cor:
+            ref = cor.process(*args)
+            cor.reset()
+            shape = cor.vis_shape()
+            flat = torch.zeros(int(np.prod(shape)) + 1, dtype=torch.complex64, device=dev)
+            out = flat[1:].view(shape)
+            assert out.data_ptr() % 16 == 8
+            if mode == cobalt.COBALT_MODE_TENSOR_FP16:
+                with pytest.raises(Exception, match="16-byte"):
+                    cor.process(*args, out=out)
+            else:
+                cor.process(*args, out=out)
+                torch.cuda.synchronize()
+                assert torch.equal(ref, out) and flat[0] == 0
+
+
 def test_golden_tiny_case_on_gpu(cobalt, dev):
     """The frozen oracle values of tests/golden/ (written by the oracle alone) against both GPU modes."""
     import os
