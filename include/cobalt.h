@@ -99,8 +99,8 @@ int cobalt_plan(cobalt_plan_t **out, int stations, int subbands, int channels, i
  *   d_visibilities device, [B][C][n_bl][2][2] complex64 (float re, float im); fully
  *                  overwritten.  Baseline (i <= k) at index k(k+1)/2 + i, then
  *                  [pol of i][pol of k] (A9).  Must be 16-byte aligned in COBALT_MODE_TENSOR_FP16
- *                  (COBALT_ERR_BAD_ARG otherwise); d_samples may have any alignment (16-byte
- *                  aligned streams take the bulk-copy path).
+ *                  (COBALT_ERR_BAD_ARG otherwise); d_samples needs the alignment of one complex
+ *                  sample (4 / 2 bytes); 16-byte aligned streams take the bulk-copy path.
  *
  * Per subband s and stream (station a, pol p), with x = the integer samples as floats
  * (bit-exact two's complement value, A12) preceded by the carried history:

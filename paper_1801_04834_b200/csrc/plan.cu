@@ -273,6 +273,8 @@ int cobalt_process(cobalt_plan_t *p, void *cuda_stream, const void *d_samples, c
                    const float *d_bandpass, void *d_visibilities) {
     if (!p) return fail(nullptr, COBALT_ERR_BAD_ARG, "plan is NULL");
     if (!d_samples || !d_delays || !d_bandpass || !d_visibilities) return fail(p, COBALT_ERR_BAD_ARG, "NULL buffer");
+    if ((reinterpret_cast<uintptr_t>(d_samples) & (sample_bytes(p->bits) - 1)) != 0)
+        return fail(p, COBALT_ERR_BAD_ARG, "d_samples must be aligned to one complex sample");
     if (p->mode == COBALT_MODE_TENSOR_FP16 && (reinterpret_cast<uintptr_t>(d_visibilities) & 15u) != 0)
         return fail(p, COBALT_ERR_BAD_ARG, "d_visibilities must be 16-byte aligned in COBALT_MODE_TENSOR_FP16");
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
