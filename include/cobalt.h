@@ -158,7 +158,9 @@ int cobalt_set_mode(cobalt_plan_t *plan, int mode);
 #define COBALT_DFT_FP32 0
 #define COBALT_DFT_TENSOR 1
 int cobalt_set_dft_engine(cobalt_plan_t *plan, int engine);
-/* Subbands per internal launch group (>= 1, clipped to B).  Reallocates scratch. */
+/* Subbands per internal launch group (>= 1, clipped to B).  Reallocates scratch.  Default: as many as fit in 8 GiB of
+ * intermediate (at most a quarter of the free device memory), split evenly over the call; cobalt_process_host moves
+ * and computes in groups of about 1 GiB. */
 int cobalt_set_chunk_subbands(cobalt_plan_t *plan, int chunk);
 /* Zero the FIR history (as after cobalt_plan).  Enqueued on the legacy default stream and
  * synchronised before returning. */

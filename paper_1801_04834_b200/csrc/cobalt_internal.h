@@ -74,6 +74,7 @@ struct cobalt_plan_s {
     long long N = 0, n_t = 0, N_u = 0, n_bl = 0;
     int M = 0, Mpad = 0, n_kt = 0;
     int chunk = 1;
+    int host_chunk = 1;                // subbands per group of cobalt_process_host (<= chunk)
     int device = 0, sm_count = 0;
     double f_s = 195312.5;
     std::vector<double> f_sb;

@@ -99,12 +99,24 @@ int alloc_scratch(cobalt_plan_s *p, int chunk_request) {
     if (p->mode == COBALT_MODE_TENSOR_FP16) p->z_subband_bytes = (size_t)p->C * p->n_kt * 2 * p->Mpad * 128;
     else p->z_subband_bytes = (size_t)p->C * p->M * (size_t)p->n_t * sizeof(float2);
     int chunk = chunk_request;
-    if (chunk <= 0) {   // default: about 1 GiB of intermediate per launch group
-        chunk = (int)(((size_t)1 << 30) / p->z_subband_bytes);
+    if (chunk <= 0) {
+        // Default: up to 8 GiB of intermediate per launch group, at most a quarter of the free device memory.  Long
+        // launches keep the tail of the F-stage (CTAs of equal length on 148 SMs: 8 subbands of config 3 are 8.3 waves)
+        // and the kernel switches small: config 3 runs 5 % faster with 61 subbands per group than with 8.
+        size_t free_b = 0, total_b = 0;
+        size_t budget = (size_t)8 << 30;
+        if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess && free_b / 4 < budget) budget = free_b / 4;
+        chunk = (int)(budget / p->z_subband_bytes);
         if (chunk < 1) chunk = 1;
+        // equal groups: B = 244 with room for 64 becomes 4 x 61, not 3 x 64 + 52
+        if (chunk < p->B) chunk = (p->B + (p->B + chunk - 1) / chunk - 1) / ((p->B + chunk - 1) / chunk);
     }
     if (chunk > p->B) chunk = p->B;
     p->chunk = chunk;
+    // the host-buffer path pipelines H2D / compute / D2H group by group: keep its groups at about 1 GiB of intermediate
+    p->host_chunk = (int)(((size_t)1 << 30) / p->z_subband_bytes);
+    if (p->host_chunk < 1) p->host_chunk = 1;
+    if (p->host_chunk > chunk) p->host_chunk = chunk;
     CK(p, cudaMalloc(&p->d_z, (size_t)chunk * p->z_subband_bytes));
     CK(p, cudaMemset(p->d_z, 0, (size_t)chunk * p->z_subband_bytes));   // zero rows 2S..Mpad stay zero forever
     CK(p, cudaMalloc(&p->d_phase, (size_t)p->B * p->S * p->C * sizeof(float2)));
@@ -325,20 +337,20 @@ int cobalt_process_host(cobalt_plan_t *p, const void *h_samples, const double *h
     }
     if (!p->d_in[0]) {
         for (int i = 0; i < 2; ++i) {
-            CK(p, cudaMalloc(&p->d_in[i], (size_t)p->chunk * in_b));
-            CK(p, cudaMalloc(&p->d_out[i], (size_t)p->chunk * out_b));
+            CK(p, cudaMalloc(&p->d_in[i], (size_t)p->host_chunk * in_b));
+            CK(p, cudaMalloc(&p->d_out[i], (size_t)p->host_chunk * out_b));
         }
     }
     cudaStream_t s_in = p->hs[0], s_cmp = p->hs[1], s_out = p->hs[2];
     CK(p, cudaMemcpyAsync(p->d_delays_h, h_delays, (size_t)p->S * sizeof(double), cudaMemcpyHostToDevice, s_cmp));
     CK(p, cudaMemcpyAsync(p->d_bandpass_h, h_bandpass, (size_t)p->C * sizeof(float), cudaMemcpyHostToDevice, s_cmp));
-    const int n_chunks = (p->B + p->chunk - 1) / p->chunk;
+    const int n_chunks = (p->B + p->host_chunk - 1) / p->host_chunk;
     p->launches = 0;
     p->n_chunks_timed = 0;
     for (int ci = 0; ci < n_chunks; ++ci) {
         const int buf = ci & 1;
-        const int b0 = ci * p->chunk;
-        const int nb = (p->B - b0) < p->chunk ? (p->B - b0) : p->chunk;
+        const int b0 = ci * p->host_chunk;
+        const int nb = (p->B - b0) < p->host_chunk ? (p->B - b0) : p->host_chunk;
         if (ci >= 2) CK(p, cudaStreamWaitEvent(s_in, p->ev_cmp[buf], 0));     // d_in[buf] consumed
         CK(p, cudaMemcpyAsync(p->d_in[buf], static_cast<const unsigned char *>(h_samples) + (size_t)b0 * in_b,
                               (size_t)nb * in_b, cudaMemcpyHostToDevice, s_in));
