@@ -9,7 +9,7 @@
 //
 // fstage_kernel<C, BITS, TENSOR> is warp specialised (17 warps, one CTA per SM):
 //   CTA      = 256 / C consecutive streams (subband, station, pol) x a run of 64-spectrum k-tiles,
-//              walked in sub-tiles of 16 spectra.
+//              walked in sub-tiles of 16 spectra; for C = 256 the two polarisations of a station one after the other.
 //   warp 16  = producer: the raw integer rows of the next sub-tiles (time-contiguous, so one bulk
 //              copy -- cp.async.bulk, SASS UBLKCP -- per stream and sub-tile) land in a 4-deep
 //              shared-memory ring signalled on mbarriers; the first sub-tile of a CTA is the 16-row
@@ -152,6 +152,9 @@ struct FShape {
     static constexpr int SB = BITS == 16 ? 4 : 2;          // bytes per complex sample
     static constexpr int SPC = 256 / C;                    // streams per CTA
     static constexpr int R = C / 16;                       // threads per spectrum in the FFT
+    // C = 256: a CTA works through the two polarisations of one station back to back (same rotation table and FIR
+    // weights), so that the pipeline fills and drains once per two streams
+    static constexpr int IPC = C == 256 ? 2 : 1;           // items (groups of SPC streams) per CTA
     // FIR-output tile [16 spectra][SPC streams][YS] float2.
     //   C = 256: branch ph = r + 16 q sits at 18 r + q, so that the FFT thread r reads its 16 inputs, and rewrites
     //            them in the in-place exchange, as 16-byte pairs, conflict free; the FIR lanes are permuted to match.
@@ -240,8 +243,9 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, con
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int grp = blockIdx.x;                          // stream group within the chunk
     const int bl = grp / a.groups_per_subband;
-    const int m0 = (grp - bl * a.groups_per_subband) * SPC;
-    const int n_valid = min(SPC, a.M - m0);              // streams of this CTA that exist
+    constexpr int IPC = Sh::IPC;
+    const int m0 = (grp - bl * a.groups_per_subband) * SPC * IPC;   // first stream of the CTA
+    const int n_items = min(IPC, (a.M - m0 + SPC - 1) / SPC);       // items of this CTA that exist
     const int kt0 = blockIdx.y * a.tiles_per_seg;
     const int kt1 = min(kt0 + a.tiles_per_seg, a.n_kt);
     const int n_sub = (kt1 - kt0) * (kKTile / kSubTile);
@@ -291,15 +295,18 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, con
 
     if (warp == kProducerWarp) {
         // ------------------------------------------------------------------ producer
+        for (int item = 0; item < n_items; ++item)
         for (int j = 0; j <= n_sub; ++j) {
-            const int s = j % kRawStages;
-            const uint32_t ph = (uint32_t)(j / kRawStages) & 1u;
+            const int mi = m0 + item * SPC, n_valid = min(SPC, a.M - mi);
+            const int jg = item * (n_sub + 1) + j;               // position in the ring, over all items
+            const int s = jg % kRawStages;
+            const uint32_t ph = (uint32_t)(jg / kRawStages) & 1u;
             mbar_wait(bar_raw_empty + 8 * s, ph ^ 1u);
             const long long tb = t0 - kSubTile + (long long)j * kSubTile;     // first row of the sub-tile
             const uint32_t full = bar_raw_full + 8 * s;
             uint32_t tx = 0;
             for (int sl = 0; sl < n_valid; ++sl) {
-                const size_t stream = (size_t)bl * a.M + (m0 + sl);
+                const size_t stream = (size_t)bl * a.M + (mi + sl);
                 const uint32_t dst0 = sbase + Sh::OFF_RAW + s * Sh::RAW_STAGE + sl * (kSubTile * C * SB);
 #pragma unroll
                 for (int part = 0; part < 2; ++part) {
@@ -309,7 +316,7 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, con
                     if (part == 0) {
                         lo = max(tb, -(long long)(kTaps - 1));
                         hi = min(tb + kSubTile, 0ll);
-                        src = a.hist + (((size_t)(a.b0 + bl) * a.M + (m0 + sl)) * (kTaps - 1) + (size_t)(lo + kTaps - 1)) * C * SB;
+                        src = a.hist + (((size_t)(a.b0 + bl) * a.M + (mi + sl)) * (kTaps - 1) + (size_t)(lo + kTaps - 1)) * C * SB;
                     } else {
                         lo = max(tb, 0ll);
                         hi = min(tb + kSubTile, a.n_t);
@@ -345,13 +352,15 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, con
         // the 32 spectra of a tile are therefore the 64-byte half (tile & 1) ^ ((m >> 2) & 1) of the row, permuted
         // inside by m & 3 (done by the FFT threads); m >> 2 is the same for the <= 4 streams of a box.
         if (TENSOR && elect_one()) {
+            for (int item = 0; item < n_items; ++item)
             for (int tile = 0; tile < n_sub / 2; ++tile) {
+                const int tg = item * (n_sub / 2) + tile;        // n_sub / 2 is even: the buffer parity carries over
                 const int sbuf = tile & 1;
-                mbar_wait(bar_stg_full + 8 * sbuf, (uint32_t)(tile >> 1) & 1u);
+                mbar_wait(bar_stg_full + 8 * sbuf, (uint32_t)(tg >> 1) & 1u);
                 const int kt = kt0 + (tile >> 1);
 #pragma unroll
                 for (int b = 0; b < Sh::BOXES; ++b) {
-                    const int mb = m0 + b * Sh::SPB;
+                    const int mb = m0 + item * SPC + b * Sh::SPB;
                     if (mb >= a.Mpad) break;
                     const int c0 = 32 * ((tile & 1) ^ ((mb >> 2) & 1));
                     asm volatile(
@@ -387,15 +396,18 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, con
         const uint32_t raw_thread = sbase + Sh::OFF_RAW + sl * (kSubTile * C * SB) + ph * SB;
         float2 *ybuf = reinterpret_cast<float2 *>(smem + Sh::OFF_Y) + sl * YS + (R == 16 ? 18 * (ph & 15) + (ph >> 4) : ph + (ph >> 4));
 
+        for (int item = 0; item < n_items; ++item)
         for (int j = 0; j <= n_sub; ++j) {
-            const int s = j % kRawStages;
-            mbar_wait(bar_raw_full + 8 * s, (uint32_t)(j / kRawStages) & 1u);
+            const int jg = item * (n_sub + 1) + j;
+            const int s = jg % kRawStages;
+            mbar_wait(bar_raw_full + 8 * s, (uint32_t)(jg / kRawStages) & 1u);
             const int jj = j - 1;                         // real sub-tile index (j = 0 is the warm-up)
-            const int yb = jj % kYBufs;
+            const int jjg = item * n_sub + jj;
+            const int yb = jjg % kYBufs;
             const uint32_t raw = raw_thread + s * Sh::RAW_STAGE;
-            // The warm-up sub-tile (jj < 0) also stores: into buffer 0, which nobody reads before the first real
-            // sub-tile has overwritten it and signalled y_full.
-            if (jj >= 0) mbar_wait(bar_y_empty + 8 * yb, ((uint32_t)(jj / kYBufs) & 1u) ^ 1u);
+            // The warm-up sub-tile (jj < 0) stores nothing: its 16 samples only re-initialise the pending outputs (every
+            // slot gets its first tap from one of them), also when the accumulators still hold the previous item's sums.
+            if (jj >= 0) mbar_wait(bar_y_empty + 8 * yb, ((uint32_t)(jjg / kYBufs) & 1u) ^ 1u);
             float2 *yrow = ybuf + (size_t)(jj >= 0 ? yb : 0) * (Sh::Y_BUF / 8);
 #pragma unroll
             for (int half = 0; half < 2; ++half) {
@@ -418,7 +430,7 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, con
 #pragma unroll
                     for (int k = 0; k < kTaps - 1; ++k)
                         acc[(i + k) & 15] = __ffma2_rn(make_float2(wk[k], wk[k]), x, acc[(i + k) & 15]);
-                    yrow[i * Sh::TS] = acc[i];
+                    if (jj >= 0) yrow[i * Sh::TS] = acc[i];
                     acc[(i + 15) & 15] = __fmul2_rn(make_float2(wk[15], wk[15]), x);   // first tap of output u + 15
                 }
             }
@@ -449,19 +461,21 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, con
         const float4 *zero4 = reinterpret_cast<const float4 *>(smem + Sh::OFF_ZERO);
         const float *steps = reinterpret_cast<const float *>(smem + Sh::OFF_STEP + (sl * R + r) * Sh::STEP_ROW);
         const float4 *tw4 = reinterpret_cast<const float4 *>(smem + Sh::OFF_TW + r * Sh::TAB_ROW);
-        const int m = m0 + sl;
         // staging word of (channel c, plane, pair p of the tile): box b = sl / SPB, then [stream][plane][channel][64 B],
         // the 16-byte chunk (p >> 2) stored at (p >> 2) ^ (m & 3), 64-byte swizzled like the tensor store reads it
         const uint32_t stg_thread = (uint32_t)((sl / Sh::SPB) * Sh::BOX_BYTES + (sl % Sh::SPB) * (2 * C * 64));
         unsigned char *zsub = a.z + (size_t)bl * a.z_subband_bytes;
 
+        for (int item = 0; item < n_items; ++item)
         for (int jj = tm; jj < n_sub; jj += kFftTeams) {
-            const int yb = jj % kYBufs;
+            const int m = m0 + item * SPC + sl;
+            const int jjg = item * n_sub + jj;                   // n_sub is a multiple of 4: team and staging parities carry over
+            const int yb = jjg % kYBufs;
             const int kt = kt0 + (jj >> 2), sub = jj & 3;
             const long long t_spec = (long long)kt * kKTile + sub * kSubTile + 2 * tp;   // first of the two spectra
             float2 *y0 = ybase + (size_t)yb * (Sh::Y_BUF / 8);
             float2 *y1 = y0 + Sh::TS;
-            mbar_wait(bar_y_full + 8 * yb, (uint32_t)(jj / kYBufs) & 1u);
+            mbar_wait(bar_y_full + 8 * yb, (uint32_t)(jjg / kYBufs) & 1u);
             float2 o0[16], o1[16];
             if (R == 16) {
 #pragma unroll
@@ -539,7 +553,7 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, con
             const bool live0 = t_spec < a.n_t, live1 = t_spec + 1 < a.n_t;
             const float4 *wt = live0 ? wtab4 : zero4;
             if (TENSOR) {
-                const int tile = jj >> 1, sbuf = tile & 1;
+                const int tile = jjg >> 1, sbuf = tile & 1;
                 const int p = 8 * (jj & 1) + tp;          // pair of spectra within the 32-spectrum tile
                 const uint32_t msk = live1 || !live0 ? 0xffffffffu : 0x0000ffffu;   // n_t odd: last pair is half live
                 mbar_wait(bar_stg_empty + 8 * sbuf, ((uint32_t)(tile >> 1) & 1u) ^ 1u);
@@ -702,7 +716,7 @@ cudaError_t launch_f(const cobalt_plan_s *p, cudaStream_t st, const FArgs &a, in
     FArgs args = a;
     // One CTA per SM: enough CTAs for >= 8 waves when the chunk allows, as few time segments as
     // possible (each segment re-reads its 16 warm-up rows).
-    args.groups_per_subband = (p->M + Sh::SPC - 1) / Sh::SPC;
+    args.groups_per_subband = (p->M + Sh::SPC * Sh::IPC - 1) / (Sh::SPC * Sh::IPC);
     const long long groups = (long long)nb * args.groups_per_subband;
     const long long want = (long long)p->sm_count * 8;
     int n_seg = (int)((want + groups - 1) / groups);
