@@ -110,6 +110,8 @@ int cobalt_plan(cobalt_plan_t **out, int stations, int subbands, int channels, i
  *   z[t][j]  = F[t][j] b[j] exp(-2 pi i frac(f[s][j] tau_a))   (frac in fp64)
  *   V[s][j][bl(i,k)][p][q] = sum_t z_{i,p}[t][j] conj(z_{k,q}[t][j])              (A9, A10)
  * and the last 15 C consumed samples of every stream become the new history (stateful!).
+ * The call only enqueues kernels on `cuda_stream` (no synchronisation, no allocation): it can be captured in a CUDA
+ * graph; the history alternates between two buffers from call to call, so capture calls in pairs.
  * Only the first N_u = floor(N/C) C samples of each stream are consumed (A11). */
 int cobalt_process(cobalt_plan_t *plan, void *cuda_stream, const void *d_samples,
                    const double *d_delays, const float *d_bandpass, void *d_visibilities);
