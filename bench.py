@@ -46,8 +46,6 @@ def parse_args(argv=None):
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json config index (1-5)")
     ap.add_argument("--subbands", type=int, default=0, help="override the number of subbands (debugging)")
     ap.add_argument("--mode", default="tensor", choices=["tensor", "exact"])
-    ap.add_argument("--dft", default="fp32", choices=["fp32", "tensor"],
-                    help="F-stage DFT engine (cobalt_set_dft_engine); tensor: C = 256 only")
     ap.add_argument("--interp", action="store_true",
                     help="time cobalt_process_interp (delay running linearly over the block, SURVEY.md sec 8(f) row 1)")
     ap.add_argument("--chunk", type=int, default=0, help="subbands per launch group (0 = library default)")
@@ -101,7 +99,7 @@ class ClockSampler(threading.Thread):
     def __init__(self, index: int, period: float = 0.05):
         super().__init__(daemon=True)
         self.index, self.period = index, period
-        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self.samples, self.reasons, self.max_mhz, self.power = [], set(), None, []
         self._halt = threading.Event()
         self.ok = False
         try:
@@ -130,6 +128,7 @@ class ClockSampler(threading.Thread):
         while not self._halt.is_set():
             try:
                 self.samples.append(float(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                self.power.append(nv.nvmlDeviceGetPowerUsage(self.h) / 1e3)
                 r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
                 for bit, name in names.items():
                     if r & bit:
@@ -141,9 +140,9 @@ class ClockSampler(threading.Thread):
     def stop(self):
         self._halt.set()
         self.join(timeout=2)
-        s = sorted(self.samples)
+        s, w = sorted(self.samples), sorted(self.power)
         return {"sm_mhz": s[len(s) // 2] if s else None, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
-                "samples": len(s)}
+                "samples": len(s), "power_w": w[len(w) // 2] if w else None, "power_w_max": w[-1] if w else None}
 
 
 def physical_gpu_index(local_rank: int) -> int:
@@ -194,34 +193,38 @@ def units_per_step(cfg) -> float:
 
 # ----------------------------------------------------------------------------- the oracle leg (CPU)
 def oracle_sample(cfg, steps: int, warmup: int):
-    """Times oracle.process_subband on ONE subband of the workload (first subband, zero history, the
-    first n_t_sample spectra) per step; returns (units/s, seconds per step, description, threads)."""
+    """Times oracle.process_subband on the first, middle and last subband of the workload (one
+    subband when the workload has fewer than three), zero history, the first n_t_sample spectra of each, per step;
+    the throughput is the sample's and stands, extrapolated linearly, for the whole config.
+    Returns (units/s, seconds per step, description, threads)."""
     import numpy as np
 
     import oracle
     from paper_1801_04834_b200 import synth
 
     oracle.build()
+    sbs = sorted({0, cfg.B // 2, cfg.B - 1})
     # bound the sample to roughly 10-30 s of CPU work: ~1.2e11 naive flop (DFT 8 C^2 + X 32 n_bl per spectrum-channel)
     flop_per_spectrum = 2 * cfg.S * 8.0 * cfg.C * cfg.C + 32.0 * cfg.n_bl * cfg.C
-    n_t_s = int(max(16, min(cfg.n_t, 1.2e11 // flop_per_spectrum)))
+    n_t_s = int(max(16, min(cfg.n_t, 1.2e11 // (flop_per_spectrum * len(sbs)))))
     sub = synth.scaled(cfg, B=1, N=n_t_s * cfg.C)
     geo = synth.geometry(cfg, "cpu")
-    full = synth.generate_subband(cfg, 0, "cpu", geo)
-    samples = full[:, :, : sub.N, :].contiguous().numpy()
+    samples = [synth.generate_subband(cfg, sb, "cpu", geo)[:, :, : sub.N, :].contiguous().numpy() for sb in sbs]
     delays = geo["delays"].numpy()
     bandpass = geo["bandpass"].numpy().astype(np.float64)
     times = []
     for it in range(warmup + steps):
         t0 = time.perf_counter()
-        oracle.process_subband(samples, cfg.C, delays, bandpass, oracle.default_subband_frequency(0))
+        for sb, x in zip(sbs, samples):
+            oracle.process_subband(x, cfg.C, delays, bandpass, oracle.default_subband_frequency(sb))
         dt = time.perf_counter() - t0
         if it >= warmup:
             times.append(dt)
     sec = sum(times) / len(times)
-    units = float(cfg.n_bl) * n_t_s * cfg.C
-    desc = (f"oracle.process_subband on 1 of {cfg.B} subbands, first {n_t_s} of {cfg.n_t} spectra "
-            f"({cfg.S} stations, {cfg.C} channels); float64, direct FIR, naive O(C^2) DFT, per-baseline loops")
+    units = float(cfg.n_bl) * n_t_s * cfg.C * len(sbs)
+    desc = (f"oracle.process_subband on subbands {sbs} of {cfg.B}, first {n_t_s} of {cfg.n_t} spectra of each "
+            f"({cfg.S} stations, {cfg.C} channels); float64, direct FIR, naive O(C^2) DFT, per-baseline loops; "
+            f"throughput of the sample, extrapolated linearly to the whole config")
     return units / sec, sec, desc, oracle.num_threads()
 
 
@@ -279,8 +282,6 @@ def run_ours(args, rank, world, local):
     cor = pkg.Correlator(cfg.S, cfg.B, cfg.C, cfg.N, cfg.bits, mode=mode)
     if args.chunk > 0:
         cor.set_chunk_subbands(args.chunk)
-    if args.dft == "tensor":
-        cor.set_dft_engine(pkg.COBALT_DFT_TENSOR)
     info = cor.info
     vis = torch.empty(cor.vis_shape(), dtype=torch.complex64, device=dev)
     stream = torch.cuda.current_stream()
@@ -320,8 +321,7 @@ def run_ours(args, rank, world, local):
     n_samples = float(cfg.B) * 2 * cfg.S * (cfg.n_t * cfg.C)               # complex samples per pol-stream
     f_bytes = n_samples * F_BYTES_PER_SAMPLE[cfg.bits] if args.mode == "tensor" else n_samples * (cfg.bits // 4 + 8)
     x_flop = units * X_FLOP_PER_BASELINE_SAMPLE
-    # --dft tensor: C = 256 in tensor mode runs the DFT on the tensor cores (csrc/fstage_tc.cu)
-    f_kernel = "fstage_tc_kernel" if (cfg.C == 256 and args.mode == "tensor" and args.dft == "tensor") else "fstage_kernel"
+    f_kernel = "fstage_kernel"
     roof_f = {"kernel": f_kernel, "bound": "hbm", "achieved": f_bytes / t_f / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
               "frac": f_bytes / t_f / 1e9 / peaks["hbm_gbs"], "traffic": stored_traffic(f_kernel) if cfg.name == "full-array-16bit" else None,
               "peak_source": peaks["source"], "ms_per_launch": t_f * 1e3 / n_chunks, "launches_per_step": n_chunks,
@@ -332,7 +332,7 @@ def run_ours(args, rank, world, local):
     alu_peak = 148 * 128 * 2 * 1.965e9 / 1e12
     roof_alu = {"kernel": f_kernel, "bound": "alu", "achieved": f_flop / t_f / 1e12, "peak": alu_peak, "unit": "TFLOP/s",
                 "frac": f_flop / t_f / 1e12 / alu_peak, "traffic": None,
-                "peak_source": "148 SMs x 128 FP32 lanes x 2 flop x 1.965 GHz (DESIGN.md)",
+                "peak_source": "nominal, not measured: 148 SMs x 128 FP32 lanes x 2 flop x 1.965 GHz (DESIGN.md); the run's clock is in `clocks`",
                 "algorithmic_flop_per_sample": 64 + 5 * math.log2(cfg.C) + 8}
     roof_x = {"kernel": "xstage_tc_kernel" if args.mode == "tensor" else "xstage_simt_kernel", "bound": "tensor",
               "achieved": x_flop / t_x / 1e12, "peak": peaks["tensor_tflops_sustained"], "unit": "TFLOP/s",
@@ -362,7 +362,7 @@ def run_ours(args, rank, world, local):
             "dtype": "f32 (fp16 tensor-core operands, fp32 accumulate; fp64 phase angles)" if args.mode == "tensor" else "f32",
             "data": "synthetic",
             "config": {"workload": cfg.name, "stations": cfg.S, "subbands": cfg.B, "channels": cfg.C, "taps": 16,
-                       "samples_per_integration": cfg.N, "input_bits": cfg.bits, "baselines": cfg.n_bl, "mode": args.mode, "dft": args.dft,
+                       "samples_per_integration": cfg.N, "input_bits": cfg.bits, "baselines": cfg.n_bl, "mode": args.mode,
                        "call": "cobalt_process_interp" if args.interp else "cobalt_process",
                        "chunk_subbands": info.chunk_subbands, "parallelism": "replicas" if world > 1 else "single-gpu",
                        "l2": f"inputs ({cfg.input_bytes / 1e9:.2f} GB per step) exceed the 126 MB L2; no flush needed"},

@@ -132,7 +132,7 @@ int cobalt_process_host(cobalt_plan_t *plan, const void *h_samples, const double
  * f (tau_e - tau_b) / n_t are computed in fp64; the per-spectrum factor in fp32, accurate while
  * |f (tau_e - tau_b)| stays below about 100 cycles per block.  d_delays_end: device [S] doubles; everything else as
  * cobalt_process (same buffers, asynchrony, history carry, errors).  delays_end == delays_begin gives
- * cobalt_process to rounding.  The F-stage always uses COBALT_DFT_FP32 in this call. */
+ * cobalt_process to rounding. */
 int cobalt_process_interp(cobalt_plan_t *plan, void *cuda_stream, const void *d_samples,
                           const double *d_delays_begin, const double *d_delays_end, const float *d_bandpass,
                           void *d_visibilities);
@@ -144,22 +144,12 @@ int cobalt_destroy(cobalt_plan_t *plan);
 /* --------------------------------------------------------------------------- settings */
 /* Subband centre (sky) frequencies in Hz, host array [B] (A6).  Takes effect next call. */
 int cobalt_set_subband_frequencies(cobalt_plan_t *plan, const double *h_hz);
+/* Subband sample rate f_s in Hz (A6: the channel spacing is f_s / C).  While cobalt_set_subband_frequencies has not
+ * been called the default ladder f_sb[s] = 100 MHz + (12 + s) f_s is rebuilt with the new rate; a ladder the caller
+ * has set is kept as it is.  Takes effect next call. */
 int cobalt_set_sample_rate(cobalt_plan_t *plan, double hz);
 /* Switch COBALT_MODE_*; reallocates the intermediate scratch, keeps the history. */
 int cobalt_set_mode(cobalt_plan_t *plan, int mode);
-/* Where the F-stage computes the C-point DFT (step a3) in COBALT_MODE_TENSOR_FP16:
- *   COBALT_DFT_FP32   (default) radix-16 FFT in fp32 on the FP32 pipe; only the final channelised value is
- *                     rounded to fp16, so channel isolation is that of the fp32 filter bank;
- *   COBALT_DFT_TENSOR two 16-point DFT passes as fp16 GEMMs on the tensor cores (C = 256 only; other C and
- *                     EXACT mode silently keep COBALT_DFT_FP32).  1-4 % faster on config 3, but the FIR output
- *                     is rounded to fp16 BEFORE the DFT: the rounding noise of a spectrum (2^-12 of each FIR output)
- *                     spreads over its channels, about 1e-5 of the strongest channel's amplitude in every channel
- *                     (-100 dB), so a channel more than ~40 dB weaker than the strongest channel of the same
- *                     spectrum is no longer within the 2e-3 relative tolerance.
- * Takes effect at the next cobalt_process. */
-#define COBALT_DFT_FP32 0
-#define COBALT_DFT_TENSOR 1
-int cobalt_set_dft_engine(cobalt_plan_t *plan, int engine);
 /* Subbands per internal launch group (>= 1, clipped to B).  Reallocates scratch.  Default: as many as fit in 8 GiB of
  * intermediate (at most a quarter of the free device memory), split evenly over the call; cobalt_process_host moves
  * and computes in groups of about 1 GiB. */

@@ -23,8 +23,6 @@ COBALT_ERR_CUDA = -3
 COBALT_ERR_UNSUPPORTED_DEVICE = -4
 COBALT_MODE_TENSOR_FP16 = 0
 COBALT_MODE_EXACT_FP32 = 1
-COBALT_DFT_FP32 = 0
-COBALT_DFT_TENSOR = 1
 
 F_S = 195312.5
 
@@ -32,7 +30,7 @@ F_S = 195312.5
 ABI_SYMBOLS = (
     "cobalt_plan", "cobalt_process", "cobalt_process_interp", "cobalt_process_host", "cobalt_destroy",
     "cobalt_set_subband_frequencies", "cobalt_set_sample_rate", "cobalt_set_mode",
-    "cobalt_set_dft_engine", "cobalt_set_chunk_subbands", "cobalt_reset", "cobalt_info", "cobalt_strerror", "cobalt_last_error",
+    "cobalt_set_chunk_subbands", "cobalt_reset", "cobalt_info", "cobalt_strerror", "cobalt_last_error",
     "cobalt_set_timing", "cobalt_get_timing", "cobalt_get_kernel_timing",
     "cobalt_debug_fir_weights", "cobalt_debug_unpack", "cobalt_debug_channelised", "cobalt_debug_correlate",
 )
@@ -78,7 +76,6 @@ def load(path: str | None = None):
     lib.cobalt_set_subband_frequencies.argtypes = [_vp, _vp]
     lib.cobalt_set_sample_rate.argtypes = [_vp, ctypes.c_double]
     lib.cobalt_set_mode.argtypes = [_vp, ctypes.c_int]
-    lib.cobalt_set_dft_engine.argtypes = [_vp, ctypes.c_int]
     lib.cobalt_set_chunk_subbands.argtypes = [_vp, ctypes.c_int]
     lib.cobalt_reset.argtypes = [_vp]
     lib.cobalt_info.argtypes = [_vp, ctypes.POINTER(cobalt_info_t)]
@@ -203,9 +200,6 @@ class Correlator:
     def set_mode(self, mode):
         _check(load().cobalt_set_mode(self._h, mode), self._h)
         self.info = cobalt_info(self._h)
-
-    def set_dft_engine(self, engine):
-        _check(load().cobalt_set_dft_engine(self._h, engine), self._h)
 
     def set_chunk_subbands(self, chunk):
         _check(load().cobalt_set_chunk_subbands(self._h, chunk), self._h)

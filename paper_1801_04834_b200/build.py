@@ -9,8 +9,8 @@ PKG_DIR = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(PKG_DIR)
 CSRC = os.path.join(PKG_DIR, "csrc")
 LIB = os.path.join(PKG_DIR, "libcobalt_b200.so")
-SOURCES = ["plan.cu", "fstage.cu", "fstage_tc.cu", "layout.cu", "xstage_simt.cu", "xstage_tc.cu"]
-HEADERS = [os.path.join(CSRC, "cobalt_internal.h"), os.path.join(ROOT, "include", "cobalt.h")]
+SOURCES = ["plan.cu", "fstage.cu", "layout.cu", "xstage_simt.cu", "xstage_tc.cu"]
+HEADERS = [os.path.join(CSRC, "cobalt_internal.h"), os.path.join(CSRC, "ptx.cuh"), os.path.join(ROOT, "include", "cobalt.h")]
 
 
 def nvcc_path() -> str:

@@ -70,7 +70,6 @@ struct StageEvents {
 
 struct cobalt_plan_s {
     int S = 0, B = 0, C = 0, T = 0, bits = 0, mode = COBALT_MODE_TENSOR_FP16;
-    int dft_engine = COBALT_DFT_FP32;  // cobalt_set_dft_engine
     long long N = 0, n_t = 0, N_u = 0, n_bl = 0;
     int M = 0, Mpad = 0, n_kt = 0;
     int chunk = 1;
@@ -78,6 +77,8 @@ struct cobalt_plan_s {
     int device = 0, sm_count = 0;
     double f_s = 195312.5;
     std::vector<double> f_sb;
+    bool f_sb_user = false;            // cobalt_set_subband_frequencies was called: cobalt_set_sample_rate keeps the ladder
+    bool scratch_ok = false;           // alloc_scratch completed; cobalt_process* refuse to run otherwise
     double *d_f_sb = nullptr;          // [B]
     float *d_weights = nullptr;        // [16][C], tap k (0 = newest block), branch ph
     std::vector<float> h_weights;
@@ -122,8 +123,6 @@ cudaError_t launch_phase_table(const cobalt_plan_s *p, cudaStream_t st, const do
                                const float *d_bandpass, int b0, int nb);
 // samples_b0 points at the first subband of the chunk [b0, b0 + nb)
 cudaError_t launch_fstage(const cobalt_plan_s *p, cudaStream_t st, const void *samples_b0, int b0, int nb);
-// fstage_tc.cu (C = 256, TENSOR_FP16: DFT on the tensor cores) ------------------------------
-cudaError_t launch_fstage_tc(const cobalt_plan_s *p, cudaStream_t st, const void *samples_b0, int b0, int nb);
 cudaError_t launch_history_update(const cobalt_plan_s *p, cudaStream_t st, const void *samples_b0, int b0, int nb);
 cudaError_t launch_unpack(cudaStream_t st, int bits, const void *d_in, long long n, float *d_out);
 // layout.cu ---------------------------------------------------------------------------------

@@ -25,6 +25,7 @@
 //              128-byte runs (EXACT).  The (-1)^ph needed for the ascending-frequency channel order
 //              (D[(j + C/2) mod C]) is folded into the FIR weights, so the reorder is free.
 #include "cobalt_internal.h"
+#include "ptx.cuh"
 
 namespace cobalt {
 
@@ -99,43 +100,6 @@ __device__ __forceinline__ void dft16(float2 (&a)[16]) {
     for (int k1 = 0; k1 < 4; ++k1) dft4(a[4 * k1], a[4 * k1 + 1], a[4 * k1 + 2], a[4 * k1 + 3]);   // -> a[4 k1 + k2]
 }
 
-// ------------------------------------------------------------------ mbarrier / bulk-copy helpers
-__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
-}
-__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-}
-// The waiting warp is suspended in hardware for up to the hint instead of re-issuing the test every few cycles
-// (the spin otherwise takes issue slots from the arithmetic warps of the same SM sub-partition).
-constexpr uint32_t kSuspendHintNs = 20000;
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-    uint32_t done;
-    do {
-        asm volatile(
-            "{\n\t"
-            ".reg .pred p;\n\t"
-            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\t"
-            "selp.u32 %0, 1, 0, p;\n\t"
-            "}"
-            : "=r"(done)
-            : "r"(bar), "r"(parity), "r"(kSuspendHintNs)
-            : "memory");
-    } while (!done);
-}
-__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t bytes, uint32_t bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
-                 "l"(src), "r"(bytes), "r"(bar)
-                 : "memory");
-}
-__device__ __forceinline__ void bar_sync_named(int id, int threads) {
-    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(threads) : "memory");
-}
-
 // Thread roles: warps 0-7 FIR, warps 8-15 FFT (two teams of four warps taking alternate sub-tiles), warp 16 the
 // bulk-copy producer, warp 17 the tensor-store issuer.
 constexpr int kFirThreads = 256, kFftThreads = 256, kFftTeam = 128, kFftTeams = 2;
@@ -188,25 +152,6 @@ struct FShape {
     static constexpr int TOTAL = OFF_STEP + (INTERP ? 16 * STEP_ROW : 0);
     static_assert(TOTAL <= 227 * 1024, "shared memory budget");
 };
-
-template <int BITS>
-__device__ __forceinline__ float2 unpack_sample(uint32_t raw) {
-    // Step a1: the two's-complement integer value as a float, exact.
-    if (BITS == 16) return make_float2((float)(short)(raw & 0xffffu), (float)(short)(raw >> 16));
-    return make_float2((float)(signed char)(raw & 0xffu), (float)(signed char)((raw >> 8) & 0xffu));
-}
-
-__device__ __forceinline__ bool elect_one() {
-    uint32_t pred;
-    asm volatile(
-        "{\n\t"
-        ".reg .pred p;\n\t"
-        "elect.sync _|p, 0xffffffff;\n\t"
-        "selp.u32 %0, 1, 0, p;\n\t"
-        "}"
-        : "=r"(pred));
-    return pred != 0;
-}
 
 __device__ __forceinline__ uint32_t pack_half2(float lo, float hi) {
     const __half2 t = __floats2half2_rn(lo, hi);
@@ -264,7 +209,7 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, con
             mbar_init(bar_stg_full + 8 * b, kFftThreads / 32);
             mbar_init(bar_stg_empty + 8 * b, 1);
         }
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        mbar_fence_init();
     }
     {   // rotation * bandpass of the CTA's streams (station = m >> 1) in the FFT threads' register order, zeros for
         // streams that do not exist (their staged rows are then exact zeros), and the inter-pass twiddles
@@ -698,11 +643,22 @@ __global__ void history_vec_kernel(const uint4 *__restrict__ samples, uint4 *__r
     }
 }
 
-template <typename I>
-__global__ void unpack_kernel(const I *__restrict__ in, long long n, float *__restrict__ out) {
-    for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < n;
-         idx += (long long)gridDim.x * blockDim.x)
-        out[idx] = (float)in[idx];
+// cobalt_debug_unpack (pin P1): step a1 alone, through the SAME unpack_sample<BITS> the fused kernel applies to the
+// packed complex samples it reads from shared memory (ptx.cuh).  n components = n / 2 complex samples (+ one odd
+// component, taken as the low half of a word whose high half is zero).
+template <int BITS>
+__global__ void unpack_kernel(const unsigned char *__restrict__ in, long long n, float *__restrict__ out) {
+    constexpr int SB = BITS == 16 ? 4 : 2;             // bytes per complex sample
+    const long long pairs = n / 2;
+    for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < pairs + (n & 1);
+         idx += (long long)gridDim.x * blockDim.x) {
+        uint32_t raw;
+        if (idx < pairs) raw = SB == 4 ? *reinterpret_cast<const uint32_t *>(in + idx * 4) : *reinterpret_cast<const unsigned short *>(in + idx * 2);
+        else raw = SB == 4 ? *reinterpret_cast<const unsigned short *>(in + idx * 4) : in[idx * 2];
+        const float2 v = unpack_sample<BITS>(raw);
+        out[2 * idx] = v.x;
+        if (idx < pairs) out[2 * idx + 1] = v.y;
+    }
 }
 
 template <int C, int BITS, bool TENSOR, bool INTERP>
@@ -762,8 +718,6 @@ cudaError_t launch_set_unit_scale(const cobalt_plan_s *p, cudaStream_t st) {
 }
 
 cudaError_t launch_fstage(const cobalt_plan_s *p, cudaStream_t st, const void *samples_b0, int b0, int nb) {
-    if (p->C == 256 && p->mode == COBALT_MODE_TENSOR_FP16 && p->dft_engine == COBALT_DFT_TENSOR && !p->cur_delays_end)
-        return launch_fstage_tc(p, st, samples_b0, b0, nb);      // DFT on the tensor cores (fstage_tc.cu)
     FArgs a;
     a.samples = static_cast<const unsigned char *>(samples_b0);
     a.hist = static_cast<const unsigned char *>(p->d_hist[p->hist_cur]);
@@ -821,10 +775,11 @@ cudaError_t launch_history_update(const cobalt_plan_s *p, cudaStream_t st, const
 cudaError_t launch_unpack(cudaStream_t st, int bits, const void *d_in, long long n, float *d_out) {
     if (n <= 0) return cudaSuccess;
     const int threads = 256;
-    long long blocks = (n + threads - 1) / threads;
+    long long blocks = ((n + 1) / 2 + threads - 1) / threads;
     if (blocks > 65535) blocks = 65535;
-    if (bits == 16) unpack_kernel<short><<<(unsigned)blocks, threads, 0, st>>>(static_cast<const short *>(d_in), n, d_out);
-    else unpack_kernel<signed char><<<(unsigned)blocks, threads, 0, st>>>(static_cast<const signed char *>(d_in), n, d_out);
+    const unsigned char *in = static_cast<const unsigned char *>(d_in);
+    if (bits == 16) unpack_kernel<16><<<(unsigned)blocks, threads, 0, st>>>(in, n, d_out);
+    else unpack_kernel<8><<<(unsigned)blocks, threads, 0, st>>>(in, n, d_out);
     return cudaGetLastError();
 }
 

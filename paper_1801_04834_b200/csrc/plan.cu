@@ -95,6 +95,7 @@ int build_zmap(cobalt_plan_s *p) {
 
 // (Re)allocate the per-chunk scratch for the current mode / chunk size.
 int alloc_scratch(cobalt_plan_s *p, int chunk_request) {
+    p->scratch_ok = false;      // until everything below has succeeded the plan refuses to process
     free_scratch(p);
     if (p->mode == COBALT_MODE_TENSOR_FP16) p->z_subband_bytes = (size_t)p->C * p->n_kt * 2 * p->Mpad * 128;
     else p->z_subband_bytes = (size_t)p->C * p->M * (size_t)p->n_t * sizeof(float2);
@@ -129,6 +130,7 @@ int alloc_scratch(cobalt_plan_s *p, int chunk_request) {
     const size_t hist = (size_t)p->B * p->M * (kTaps - 1) * p->C * sample_bytes(p->bits);
     p->scratch_bytes = (size_t)chunk * p->z_subband_bytes + (size_t)p->B * p->S * p->C * (sizeof(float2) + sizeof(float)) + 2 * hist +
                        (size_t)kTaps * p->C * sizeof(float) + (size_t)p->B * sizeof(double);
+    p->scratch_ok = true;
     return COBALT_OK;
 }
 
@@ -285,6 +287,7 @@ int cobalt_process(cobalt_plan_t *p, void *cuda_stream, const void *d_samples, c
                    const float *d_bandpass, void *d_visibilities) {
     if (!p) return fail(nullptr, COBALT_ERR_BAD_ARG, "plan is NULL");
     if (!d_samples || !d_delays || !d_bandpass || !d_visibilities) return fail(p, COBALT_ERR_BAD_ARG, "NULL buffer");
+    if (!p->scratch_ok) return fail(p, COBALT_ERR_NO_MEMORY, "the plan has no scratch (an earlier cobalt_set_mode / cobalt_set_chunk_subbands failed)");
     if ((reinterpret_cast<uintptr_t>(d_samples) & (sample_bytes(p->bits) - 1)) != 0)
         return fail(p, COBALT_ERR_BAD_ARG, "d_samples must be aligned to one complex sample");
     if (p->mode == COBALT_MODE_TENSOR_FP16 && (reinterpret_cast<uintptr_t>(d_visibilities) & 15u) != 0)
@@ -324,6 +327,7 @@ int cobalt_process_host(cobalt_plan_t *p, const void *h_samples, const double *h
                         void *h_visibilities) {
     if (!p) return fail(nullptr, COBALT_ERR_BAD_ARG, "plan is NULL");
     if (!h_samples || !h_delays || !h_bandpass || !h_visibilities) return fail(p, COBALT_ERR_BAD_ARG, "NULL buffer");
+    if (!p->scratch_ok) return fail(p, COBALT_ERR_NO_MEMORY, "the plan has no scratch (an earlier cobalt_set_mode / cobalt_set_chunk_subbands failed)");
     const size_t in_b = subband_input_bytes(p), out_b = subband_output_bytes(p);
     if (!p->hs[0]) {
         for (int i = 0; i < 3; ++i) CK(p, cudaStreamCreateWithFlags(&p->hs[i], cudaStreamNonBlocking));
@@ -342,8 +346,22 @@ int cobalt_process_host(cobalt_plan_t *p, const void *h_samples, const double *h
         }
     }
     cudaStream_t s_in = p->hs[0], s_cmp = p->hs[1], s_out = p->hs[2];
-    CK(p, cudaMemcpyAsync(p->d_delays_h, h_delays, (size_t)p->S * sizeof(double), cudaMemcpyHostToDevice, s_cmp));
-    CK(p, cudaMemcpyAsync(p->d_bandpass_h, h_bandpass, (size_t)p->C * sizeof(float), cudaMemcpyHostToDevice, s_cmp));
+    // On any failure below the copies already enqueued still touch the caller's host buffers: drain the three
+    // streams before returning the error.
+    auto drain = [&](int rc) {
+        cudaStreamSynchronize(s_in);
+        cudaStreamSynchronize(s_cmp);
+        cudaStreamSynchronize(s_out);
+        return rc;
+    };
+#define CKH(call)                                                                                             \
+    do {                                                                                                      \
+        cudaError_t e__ = (call);                                                                             \
+        if (e__ != cudaSuccess)                                                                               \
+            return drain(fail(p, COBALT_ERR_CUDA, std::string(#call) + ": " + cudaGetErrorString(e__)));      \
+    } while (0)
+    CKH(cudaMemcpyAsync(p->d_delays_h, h_delays, (size_t)p->S * sizeof(double), cudaMemcpyHostToDevice, s_cmp));
+    CKH(cudaMemcpyAsync(p->d_bandpass_h, h_bandpass, (size_t)p->C * sizeof(float), cudaMemcpyHostToDevice, s_cmp));
     const int n_chunks = (p->B + p->host_chunk - 1) / p->host_chunk;
     p->launches = 0;
     p->n_chunks_timed = 0;
@@ -351,25 +369,26 @@ int cobalt_process_host(cobalt_plan_t *p, const void *h_samples, const double *h
         const int buf = ci & 1;
         const int b0 = ci * p->host_chunk;
         const int nb = (p->B - b0) < p->host_chunk ? (p->B - b0) : p->host_chunk;
-        if (ci >= 2) CK(p, cudaStreamWaitEvent(s_in, p->ev_cmp[buf], 0));     // d_in[buf] consumed
-        CK(p, cudaMemcpyAsync(p->d_in[buf], static_cast<const unsigned char *>(h_samples) + (size_t)b0 * in_b,
-                              (size_t)nb * in_b, cudaMemcpyHostToDevice, s_in));
-        CK(p, cudaEventRecord(p->ev_in[buf], s_in));
-        CK(p, cudaStreamWaitEvent(s_cmp, p->ev_in[buf], 0));
-        if (ci >= 2) CK(p, cudaStreamWaitEvent(s_cmp, p->ev_out[buf], 0));    // d_out[buf] drained
+        if (ci >= 2) CKH(cudaStreamWaitEvent(s_in, p->ev_cmp[buf], 0));     // d_in[buf] consumed
+        CKH(cudaMemcpyAsync(p->d_in[buf], static_cast<const unsigned char *>(h_samples) + (size_t)b0 * in_b,
+                            (size_t)nb * in_b, cudaMemcpyHostToDevice, s_in));
+        CKH(cudaEventRecord(p->ev_in[buf], s_in));
+        CKH(cudaStreamWaitEvent(s_cmp, p->ev_in[buf], 0));
+        if (ci >= 2) CKH(cudaStreamWaitEvent(s_cmp, p->ev_out[buf], 0));    // d_out[buf] drained
         int rc = enqueue_chunk(p, s_cmp, p->d_in[buf], p->d_delays_h, p->d_bandpass_h,
                                static_cast<float2 *>(p->d_out[buf]), b0, nb, nullptr);
-        if (rc != COBALT_OK) return rc;
-        CK(p, cudaEventRecord(p->ev_cmp[buf], s_cmp));
-        CK(p, cudaStreamWaitEvent(s_out, p->ev_cmp[buf], 0));
-        CK(p, cudaMemcpyAsync(static_cast<unsigned char *>(h_visibilities) + (size_t)b0 * out_b, p->d_out[buf],
-                              (size_t)nb * out_b, cudaMemcpyDeviceToHost, s_out));
-        CK(p, cudaEventRecord(p->ev_out[buf], s_out));
+        if (rc != COBALT_OK) return drain(rc);
+        CKH(cudaEventRecord(p->ev_cmp[buf], s_cmp));
+        CKH(cudaStreamWaitEvent(s_out, p->ev_cmp[buf], 0));
+        CKH(cudaMemcpyAsync(static_cast<unsigned char *>(h_visibilities) + (size_t)b0 * out_b, p->d_out[buf],
+                            (size_t)nb * out_b, cudaMemcpyDeviceToHost, s_out));
+        CKH(cudaEventRecord(p->ev_out[buf], s_out));
     }
     p->hist_cur ^= 1;
-    CK(p, cudaStreamSynchronize(s_in));
-    CK(p, cudaStreamSynchronize(s_cmp));
-    CK(p, cudaStreamSynchronize(s_out));
+    CKH(cudaStreamSynchronize(s_in));
+    CKH(cudaStreamSynchronize(s_cmp));
+    CKH(cudaStreamSynchronize(s_out));
+#undef CKH
     return COBALT_OK;
 }
 
@@ -379,6 +398,7 @@ int cobalt_set_subband_frequencies(cobalt_plan_t *p, const double *h_hz) {
         if (!(h_hz[s] == h_hz[s]) || std::fabs(h_hz[s]) > 1e12) return fail(p, COBALT_ERR_BAD_ARG, "frequency not finite");
     CK(p, cudaDeviceSynchronize());
     p->f_sb.assign(h_hz, h_hz + p->B);
+    p->f_sb_user = true;
     CK(p, cudaMemcpy(p->d_f_sb, p->f_sb.data(), (size_t)p->B * sizeof(double), cudaMemcpyHostToDevice));
     return COBALT_OK;
 }
@@ -386,6 +406,11 @@ int cobalt_set_subband_frequencies(cobalt_plan_t *p, const double *h_hz) {
 int cobalt_set_sample_rate(cobalt_plan_t *p, double hz) {
     if (!p || !(hz > 0.0) || hz > 1e12) return fail(p, COBALT_ERR_BAD_ARG, "sample rate must be positive and finite");
     p->f_s = hz;
+    if (!p->f_sb_user) {   // the default ladder is defined in terms of f_s (reading A6): it follows the new rate
+        CK(p, cudaDeviceSynchronize());
+        for (int s = 0; s < p->B; ++s) p->f_sb[s] = 100.0e6 + (12 + s) * p->f_s;
+        CK(p, cudaMemcpy(p->d_f_sb, p->f_sb.data(), (size_t)p->B * sizeof(double), cudaMemcpyHostToDevice));
+    }
     return COBALT_OK;
 }
 
@@ -395,12 +420,6 @@ int cobalt_set_mode(cobalt_plan_t *p, int mode) {
     CK(p, cudaDeviceSynchronize());
     p->mode = mode;
     return alloc_scratch(p, 0);
-}
-
-int cobalt_set_dft_engine(cobalt_plan_t *p, int engine) {
-    if (!p || (engine != COBALT_DFT_FP32 && engine != COBALT_DFT_TENSOR)) return fail(p, COBALT_ERR_BAD_ARG, "unknown DFT engine");
-    p->dft_engine = engine;
-    return COBALT_OK;
 }
 
 int cobalt_set_chunk_subbands(cobalt_plan_t *p, int chunk) {

@@ -399,3 +399,36 @@ def test_p16_linear_delay_drift_is_a_geometric_series(oracle, drift_cycles):
     assert abs(got - want) <= 1e-9 * abs(A) ** 2 * n_t
     # autocorrelation of the drifting station is unaffected (a pure phase)
     assert abs(v[C // 2, oracle.baseline_index(1, 1), 0, 0] - abs(A) ** 2 * n_t) <= 1e-9 * abs(A) ** 2 * n_t
+
+
+@pytest.mark.parametrize("m", [-5, 3])
+def test_p16_drift_at_an_off_centre_channel_uses_that_channels_frequency(oracle, m):
+    """Same closed form as above at channel j = C/2 + m: a warmed-up tone at the exact centre of channel j
+    (x[n] = A exp(2 pi i m n / C), periodic in C) gives F[t][j] = A in every spectrum, and the drift of station 1 turns
+    with THAT channel's sky frequency f_j = f_sb + m f_s / C (reading A6), not with f_sb: the per-channel term of the
+    interpolated phase ("channel-dependent phase angles")."""
+    C, n_t = 16, 160
+    A = 1.25 + 0.5j
+    f_sb, f_s = 1.0e8, oracle.F_S
+    j = C // 2 + m
+    f_j = f_sb + m * f_s / C
+    tau_b = 1.0e-6
+    tau_e = tau_b + (12 * n_t + 0.1) / f_sb                     # 12 cycles per spectrum at f_sb (+ 0.1 over the block);
+                                                                # f_j adds or removes about a cycle over the block
+    n = np.arange(-(T - 1) * C, n_t * C)
+    tone = A * np.exp(2j * np.pi * m * (n % C) / C)
+    hist = np.broadcast_to(tone[:(T - 1) * C], (2, 2, (T - 1) * C)).copy()
+    x = np.broadcast_to(tone[(T - 1) * C:], (2, 2, n_t * C)).copy()
+    z = oracle.fstage(x, C, hist=hist, delays=np.array([0.0, tau_b]), bandpass=np.ones(C), f_sb=f_sb,
+                      delays_end=np.array([0.0, tau_e]))
+    np.testing.assert_allclose(z[0, 0, :, j], A, rtol=0, atol=1e-11)
+    v = oracle.correlate(z)
+    step = f_j * (tau_e - tau_b) / n_t                          # cycles per spectrum
+    r = np.exp(2j * np.pi * step)
+    want = abs(A) ** 2 * np.exp(2j * np.pi * f_j * tau_b) * (1 - r ** n_t) / (1 - r)
+    got = v[j, oracle.baseline_index(0, 1), 0, 0]
+    assert abs(got - want) <= 1e-7 * abs(A) ** 2 * n_t
+    # and it is NOT the series of the subband centre frequency
+    r0 = np.exp(2j * np.pi * f_sb * (tau_e - tau_b) / n_t)
+    wrong = abs(A) ** 2 * np.exp(2j * np.pi * f_sb * tau_b) * (1 - r0 ** n_t) / (1 - r0)
+    assert abs(got - wrong) > 1e-2 * abs(A) ** 2 * n_t

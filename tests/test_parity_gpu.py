@@ -68,6 +68,9 @@ def _assert_parity(vg, vo, mode_tensor, what):
 # ------------------------------------------------------------------ P1: unpack bit-exact
 @pytest.mark.parametrize("bits", [16, 8])
 def test_p1_unpack_every_value_bit_exact(cobalt, oracle, dev, bits):
+    """cobalt_debug_unpack runs unpack_sample<BITS> of csrc/ptx.cuh on packed complex samples: the very routine (not
+    a look-alike) the fused F-stage kernels apply to the words they read from shared memory.  Every value appears
+    both as the re (low) and as the im (high) half of a sample; the odd length exercises the single-component tail."""
     if bits == 16:
         x = np.arange(-32768, 32768, dtype=np.int64).astype(np.int16)
     else:
@@ -138,6 +141,25 @@ def test_p14_correlate_small_integers_bit_exact(cobalt, oracle, dev, S, n_t, mod
         torch.cuda.synchronize()
         vis = vis.cpu().numpy()                                    # [C][n_bl][2][2]
     zo = z.astype(np.complex128).reshape(C, S, 2, n_t).transpose(1, 2, 3, 0)   # -> [S][2][n_t][C]
+    want = oracle.correlate(np.ascontiguousarray(zo))
+    assert np.array_equal(vis.astype(np.complex128), want)
+
+
+@pytest.mark.parametrize("S,C,n_t", [(77, 256, 768), (77, 64, 1500), (288, 64, 768), (130, 64, 700), (48, 64, 3072)])
+def test_p14_bit_exact_through_the_full_size_control_paths(cobalt, oracle, dev, S, C, n_t):
+    """P14 at sizes where a CTA runs several jobs one after the other (C * jobs-per-channel > 148 SMs: second and
+    later jobs flip the tmem_full / tmem_empty phases and reuse the staged output block), the load ring wraps many
+    times (n_t / 64 k-tiles > ring depth) and, for S = 48 with few jobs, the k-range of a channel is split over
+    several CTAs.  Integers |v| <= 8: every product and every partial sum is exact in fp32 (< 2^24), so the result
+    must equal integer arithmetic bit for bit, element by element."""
+    rng = np.random.default_rng(1400 + S + C)
+    z = torch.from_numpy(rng.integers(-8, 9, size=(C, 2 * S, n_t, 2)).astype(np.float32))
+    zc = torch.view_as_complex(z).contiguous()
+    with cobalt.Correlator(S, 1, C, n_t * C, 16, mode=cobalt.COBALT_MODE_TENSOR_FP16) as cor:
+        vis = cor.correlate(zc.to(dev))
+        torch.cuda.synchronize()
+        vis = vis.cpu().numpy()
+    zo = zc.numpy().astype(np.complex128).reshape(C, S, 2, n_t).transpose(1, 2, 3, 0)   # -> [S][2][n_t][C]
     want = oracle.correlate(np.ascontiguousarray(zo))
     assert np.array_equal(vis.astype(np.complex128), want)
 
@@ -225,8 +247,7 @@ def test_reset_zeroes_history(cobalt, dev, mode_tensor):
 @pytest.mark.parametrize("C,n_t", [(64, 80), (256, 48)])
 @pytest.mark.parametrize("bits", [16, 8])
 def test_extreme_sample_values(cobalt, oracle, dev, bits, C, n_t):
-    """Full-scale input incl. -32768 / -128: no overflow of the fp16 intermediate (C = 256: nor of the fp16
-    operands of the tensor-core DFT passes), parity holds."""
+    """Full-scale input incl. -32768 / -128: no overflow of the fp16 intermediate, parity holds."""
     synth = _synth()
     S = 2
     rng = np.random.default_rng(5)
@@ -280,8 +301,9 @@ def test_process_host_matches_device_path(cobalt, dev):
 @pytest.mark.parametrize("C,n_t,t0", [(64, 64, 40), (256, 32, 20)])
 def test_fp16_scale_worst_case_amplitude(cobalt, oracle, dev, C, n_t, t0):
     """Sign-matched full-scale input rotated by 45 degrees drives one component of z to
-    sum|g| * sqrt(2) * 32767 ~ 7.8e4 > 65504: without the power-of-two operand scales fp16 overflows
-    (C = 256 also exercises the operands of the tensor-core DFT: FIR output at its maximum in every branch)."""
+    sum|g| * sqrt(2) * 32767 ~ 7.8e4 > 65504: without the power-of-two operand scale fp16 overflows.  Every channel
+    but the centre one is empty here (leakage only), so the per-channel 2e-3 also checks that the F-stage keeps the
+    dynamic range of an fp32 filter bank."""
     S = 2
     g = oracle.fir_prototype(C)
     samples = np.zeros((1, S, 2, n_t * C, 2), dtype=np.int16)
@@ -312,33 +334,6 @@ def test_fp16_scale_follows_bandpass_gain(cobalt, oracle, dev, gain):
     _assert_parity(vg[0], vo[0], True, f"bandpass gain {gain}")
 
 
-@pytest.mark.parametrize("bits,S,n_t", [(16, 3, 70), (8, 2, 129), (16, 1, 16)])
-def test_tensor_dft_engine_matches_oracle_and_differs_from_fp32(cobalt, oracle, dev, bits, S, n_t):
-    """cobalt_set_dft_engine(COBALT_DFT_TENSOR) (C = 256: two fp16 GEMM passes on tcgen05, csrc/fstage_tc.cu):
-    within the 2e-3 tolerance on noise-like input incl. a ragged last k-tile, and really a different code path."""
-    synth = _synth()
-    cfg = synth.scaled(synth.CONFIGS[3 if bits == 16 else 4], S=S, B=2, C=256, N=256 * n_t + 7)
-    data = synth.generate(cfg, device="cpu")
-    vo = _run_oracle(oracle, cfg, data)[0]                          # [B][C][n_bl][2][2]
-    out = {}
-    for engine in (cobalt.COBALT_DFT_FP32, cobalt.COBALT_DFT_TENSOR):
-        with cobalt.Correlator(cfg.S, cfg.B, cfg.C, cfg.N, cfg.bits) as cor:
-            cor.set_dft_engine(engine)
-            vg = cor.process(data["samples"].to(dev), data["delays"].to(dev), data["bandpass"].to(dev))
-            torch.cuda.synchronize()
-            out[engine] = vg.cpu().numpy()
-        for b in range(cfg.B):
-            _assert_parity(out[engine][b], vo[b], True, f"dft engine {engine}, subband {b}")
-    assert not np.array_equal(out[cobalt.COBALT_DFT_FP32], out[cobalt.COBALT_DFT_TENSOR])
-
-
-def test_dft_engine_rejects_unknown_value(cobalt, dev):
-    with cobalt.Correlator(2, 1, 64, 64 * 20, 16) as cor:
-        with pytest.raises(Exception):
-            cor.set_dft_engine(7)
-        cor.set_dft_engine(cobalt.COBALT_DFT_TENSOR)      # accepted for any C; C != 256 keeps the fp32 FFT
-
-
 # ------------------------------------------------------------------ time-varying delay (SURVEY.md sec 8(f) row 1, reading A21)
 @pytest.mark.parametrize("C,bits,S,n_t,drift", [(16, 16, 3, 150, 0.15), (64, 16, 2, 203, -2.5), (256, 16, 2, 70, 0.15),
                                                 (64, 8, 3, 130, 30.0), (256, 8, 1, 65, -0.4)])
@@ -356,7 +351,6 @@ def test_time_varying_delay_matches_oracle(cobalt, oracle, dev, C, bits, S, n_t,
     samples = data["samples"].numpy()
     mode = cobalt.COBALT_MODE_TENSOR_FP16 if mode_tensor else cobalt.COBALT_MODE_EXACT_FP32
     with cobalt.Correlator(cfg.S, cfg.B, cfg.C, cfg.N, cfg.bits, mode=mode) as cor:
-        cor.set_dft_engine(cobalt.COBALT_DFT_TENSOR)            # ignored by this call: it always uses the fp32 FFT
         vg = cor.process(data["samples"].to(dev), data["delays"].to(dev), data["bandpass"].to(dev),
                          delays_end=torch.from_numpy(tau_e).to(dev))
         vs = cor.process(data["samples"].to(dev), data["delays"].to(dev), data["bandpass"].to(dev))   # second call: history carried
@@ -464,3 +458,84 @@ def test_golden_tiny_case_on_gpu(cobalt, dev):
                               torch.from_numpy(mg.BANDPASS.astype(np.float32)).to(dev))
             torch.cuda.synchronize()
         _assert_parity(vis.cpu().numpy(), exp, tensor, f"golden tiny case, tensor={tensor}")
+
+
+# ------------------------------------------------------------------ frequency settings (reading A6)
+def _delayed(s, d):
+    k = np.fft.fftfreq(s.size)
+    return np.fft.ifft(np.fft.fft(s) * np.exp(-2j * np.pi * k * d))
+
+
+@pytest.mark.parametrize("mode_tensor", [False, True])
+def test_p9_baseband_delay_slope_and_compensation_on_gpu(cobalt, oracle, dev, mode_tensor):
+    """GPU counterpart of pin P9 through cobalt_set_subband_frequencies: with f_sb = 0 (pure baseband) a station
+    delayed by d samples shows arg V01[j] = 2 pi d (j - C/2) / C, and tau_1 = -d / f_s flattens it; the same with a
+    non-default sample rate through cobalt_set_sample_rate.  Checked against the closed form AND the oracle."""
+    rng = np.random.default_rng(909)
+    C, n_t, d, S = 64, 1200, 9.77, 2
+    N = n_t * C
+    s0 = (rng.standard_normal(N) + 1j * rng.standard_normal(N)) * 2000.0
+    x = np.zeros((1, S, 2, N, 2), dtype=np.int16)
+    for a, sig in enumerate((s0, _delayed(s0, d))):
+        x[0, a, :, :, 0] = np.rint(sig.real)
+        x[0, a, :, :, 1] = np.rint(sig.imag)
+    bandpass = np.ones(C, dtype=np.float32)
+    mode = cobalt.COBALT_MODE_TENSOR_FP16 if mode_tensor else cobalt.COBALT_MODE_EXACT_FP32
+    bl01 = oracle.baseline_index(0, 1)
+    for f_s in (oracle.F_S, 200.0e3):
+        with cobalt.Correlator(S, 1, C, N, 16, mode=mode) as cor:
+            cor.set_subband_frequencies(np.array([0.0]))
+            if f_s != oracle.F_S:
+                cor.set_sample_rate(f_s)
+            args = (torch.from_numpy(x).to(dev), torch.from_numpy(bandpass).to(dev))
+            v_raw = cor.process(args[0], torch.zeros(S, dtype=torch.float64, device=dev), args[1]).cpu().numpy()[0]
+            cor.reset()
+            tau = np.array([0.0, -d / f_s])
+            v_cmp = cor.process(args[0], torch.from_numpy(tau).to(dev), args[1]).cpu().numpy()[0]
+        ph = np.unwrap(np.angle(v_raw[:, bl01, 0, 0]))
+        slope = np.polyfit(np.arange(C)[4:-4], ph[4:-4], 1)[0]
+        assert abs(slope - 2 * np.pi * d / C) < 2e-3, slope
+        assert np.max(np.abs(np.angle(v_cmp[2:-2, bl01, 0, 0]))) < 0.03
+        vo = oracle.process_subband(x[0], C, tau, bandpass.astype(np.float64), 0.0, f_s=f_s)
+        _assert_parity(v_cmp, vo, mode_tensor, f"baseband P9, f_s = {f_s}")
+
+
+@pytest.mark.parametrize("mode_tensor", [False, True])
+def test_shuffled_frequency_ladder_and_sample_rate_match_oracle(cobalt, oracle, dev, mode_tensor):
+    """cobalt_set_subband_frequencies with a non-monotonic ladder (incl. a negative and a zero frequency) and
+    cobalt_set_sample_rate, several launch groups: every subband is rotated with ITS frequency."""
+    synth = _synth()
+    cfg = synth.scaled(synth.CONFIGS[3], S=4, B=5, C=64, N=64 * 90 + 5)
+    data = synth.generate(cfg, device="cpu")
+    f_sb = np.array([151.3e6, 0.0, 37.25e6, -12.5e6, 240.0e6])
+    f_s = 180.0e3
+    delays = np.random.default_rng(3).uniform(-40e-6, 40e-6, cfg.S)
+    mode = cobalt.COBALT_MODE_TENSOR_FP16 if mode_tensor else cobalt.COBALT_MODE_EXACT_FP32
+    with cobalt.Correlator(cfg.S, cfg.B, cfg.C, cfg.N, cfg.bits, mode=mode) as cor:
+        cor.set_chunk_subbands(2)
+        cor.set_subband_frequencies(f_sb)
+        cor.set_sample_rate(f_s)                     # a ladder the caller has set is kept
+        vg = cor.process(data["samples"].to(dev), torch.from_numpy(delays).to(dev), data["bandpass"].to(dev)).cpu().numpy()
+    bp = data["bandpass"].numpy().astype(np.float64)
+    for b in range(cfg.B):
+        vo = oracle.process_subband(data["samples"].numpy()[b], cfg.C, delays, bp, float(f_sb[b]), f_s=f_s)
+        _assert_parity(vg[b], vo, mode_tensor, f"custom ladder, subband {b}")
+    # the ladder matters: subband 0 with the default frequency is a different answer
+    wrong = oracle.process_subband(data["samples"].numpy()[0], cfg.C, delays, bp, oracle.default_subband_frequency(0), f_s=f_s)
+    assert err_frobenius(vg[0], wrong) > 10 * TOL_TENSOR
+
+
+def test_set_sample_rate_rebuilds_the_default_ladder(cobalt, oracle, dev):
+    """include/cobalt.h: while the caller has not set the ladder, f_sb[s] = 100 MHz + (12 + s) f_s follows f_s."""
+    synth = _synth()
+    cfg = synth.scaled(synth.CONFIGS[3], S=3, B=3, C=16, N=16 * 130)
+    data = synth.generate(cfg, device="cpu")
+    f_s = 150.0e3
+    delays = np.array([0.0, 31.7e-6, -18.2e-6])
+    with cobalt.Correlator(cfg.S, cfg.B, cfg.C, cfg.N, cfg.bits, mode=cobalt.COBALT_MODE_EXACT_FP32) as cor:
+        cor.set_sample_rate(f_s)
+        vg = cor.process(data["samples"].to(dev), torch.from_numpy(delays).to(dev), data["bandpass"].to(dev)).cpu().numpy()
+    bp = data["bandpass"].numpy().astype(np.float64)
+    for b in range(cfg.B):
+        vo = oracle.process_subband(data["samples"].numpy()[b], cfg.C, delays, bp, 100.0e6 + (12 + b) * f_s, f_s=f_s)
+        _assert_parity(vg[b], vo, False, f"default ladder at f_s = {f_s}, subband {b}")
