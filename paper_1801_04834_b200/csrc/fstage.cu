@@ -100,64 +100,12 @@ __device__ __forceinline__ void dft16(float2 (&a)[16]) {
     for (int k1 = 0; k1 < 4; ++k1) dft4(a[4 * k1], a[4 * k1 + 1], a[4 * k1 + 2], a[4 * k1 + 3]);   // -> a[4 k1 + k2]
 }
 
-
-// ------------------------------------------------------------------ FIR on the tensor cores (C = 64)
-// For one polyphase branch the 16-tap FIR over a block of 16 spectra is  Y = L X_cur + U X_prev  with the lower /
-// strictly upper triangular Toeplitz matrices L[i][j] = w[i - j], U[i][j] = w[16 + i - j] of the branch's taps
-// (w[k] multiplies x[t - k], reading A2).  The CTA's 4 streams x (re, im) are 8 series that share the branch: with the
-// data as the A operand (rows 0-7 the 8 series, rows 8-15 the same series 8 spectra later) and the taps as the B operand
-// the 16 outputs of the 8 series are one mma.sync.m16n8k16 + one m16n8k8 (24 of the 31 input rows; fp32 accumulate).  The integer samples are
-// EXACT in fp16 (int8 directly; int16 = 256 H + L split into the signed high byte and the unsigned low byte), the
-// fp32 weights are split w = w_hi + w_lo (both fp16, residual 2^-22 |w|), every product is exact in fp32 and the
-// accumulation is fp32: the result is the fp32 FIR to rounding, at 1/4 (int8) to 1/2 (int16) of its issue slots.
-__device__ __forceinline__ void mma_16816(float (&d)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3, uint32_t b0, uint32_t b1) {
-    asm("mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
-                 : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
-                 : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
-}
-__device__ __forceinline__ void mma_1688(float (&d)[4], uint32_t a0, uint32_t a1, uint32_t b0) {
-    asm("mma.sync.aligned.m16n8k8.row.col.f32.f16.f16.f32 {%0,%1,%2,%3}, {%4,%5}, {%6}, {%0,%1,%2,%3};"
-                 : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
-                 : "r"(a0), "r"(a1), "r"(b0));
-}
-__device__ __forceinline__ uint32_t h2_bits(__half2 h) { return *reinterpret_cast<uint32_t *>(&h); }
-__device__ __forceinline__ __half2 bits_h2(uint32_t u) { return *reinterpret_cast<__half2 *>(&u); }
-// (a, b) as fp16 pair (a low): high parts and the fp16-rounded residuals
-__device__ __forceinline__ void split_pair(float wa, float wb, uint32_t &hi, uint32_t &lo) {
-    const __half ha = __float2half_rn(wa), hb = __float2half_rn(wb);
-    hi = h2_bits(__halves2half2(ha, hb));
-    lo = h2_bits(__halves2half2(__float2half_rn(wa - __half2float(ha)), __float2half_rn(wb - __half2float(hb))));
-}
-// Byte `sel`-selected from each of two words -> the two integers as an exact fp16 pair (step a1 for the tensor-core FIR;
-// bit-exact by construction: 0x6400 | u is the fp16 number 1024 + u for 0 <= u < 1024).
-//   SIGNED: the bytes are two's complement (int8 sample, or high byte of an int16): u = byte ^ 0x80 = value + 128.
-//   else  : unsigned low byte of an int16, returned divided by 256 (the int16 operand is x / 256 = H + L / 256).
-template <bool SIGNED>
-__device__ __forceinline__ uint32_t bytes_to_h2(uint32_t w0, uint32_t w1, uint32_t sel, uint32_t mask, uint32_t magic) {
-    const uint32_t x = __byte_perm(w0, w1, sel);                   // (byte of w0, -, byte of w1, -)
-    uint32_t y;                                                    // (x & 0x00ff00ff) ^ magic in one LOP3 (constants in registers)
-    asm("lop3.b32 %0, %1, %2, %3, 0x6A;" : "=r"(y) : "r"(x), "r"(mask), "r"(magic));
-    if (SIGNED) return h2_bits(__hadd2(bits_h2(y), __float2half2_rn(-1152.f)));        // magic = 0x64806480
-    return h2_bits(__hfma2(bits_h2(y), __float2half2_rn(0.00390625f), __float2half2_rn(-4.f)));   // magic = 0x64006400
-}
-// y = D * fir_output_gain: the int16 data operand is x / 256, the weight operand w * fir_mma_weight_scale (both exact)
-__host__ __device__ constexpr float fir_mma_weight_scale(int C);
-__host__ __device__ constexpr float fir_output_gain(int C, int bits) {
-    return C == 64 ? (bits == 16 ? 256.f : 1.f) / (64.f * (float)C) : 1.f;
-}
-// power-of-two scale of the fp16 weights (max |w| C ~ 1: the largest weight becomes ~64, the split residuals stay normal)
-__host__ __device__ constexpr float fir_mma_weight_scale(int C) { return 64.f * (float)C; }
-
 // Thread roles: warps 0-7 FIR, warps 8-15 FFT (two teams of four warps taking alternate sub-tiles), warp 16 the
 // bulk-copy producer, warp 17 the tensor-store issuer.
 constexpr int kFirThreads = 256, kFftThreads = 256, kFftTeam = 128, kFftTeams = 2;
 constexpr int kProducerWarp = (kFirThreads + kFftThreads) / 32;
 constexpr int kStoreWarp = kProducerWarp + 1;
 constexpr int kFThreads = kFirThreads + kFftThreads + 64;
-// The tensor-core FIR variant (C = 64) runs with a complete fifth warp group (two idle warps) so that the group can
-// hand its registers to the FIR warps (setmaxnreg works per group of four warps and only moves registers that a
-// group of the same CTA has released).
-constexpr int fthreads(int C) { return C == 64 ? kFThreads + 64 : kFThreads; }
 constexpr int kRawStages = 3;      // ring of raw sub-tiles (bulk copies in flight)
 constexpr int kYBufs = 3;          // ring of FIR-output sub-tiles
 constexpr int kStgTile = 32;       // spectra per staged output tile (= one tensor store per box)
@@ -175,19 +123,12 @@ struct FShape {
     //   C = 256: branch ph = r + 16 q sits at 18 r + q, so that the FFT thread r reads its 16 inputs, and rewrites
     //            them in the in-place exchange, as 16-byte pairs, conflict free; the FIR lanes are permuted to match.
     //   C < 256: branch ph sits at ph + (ph >> 4).
-    // C = 64 (tensor-core FIR): one more pad element per stream makes the FIR's 4-byte stores (lane = (spectrum pair q,
-    // stream, component), bank = 8 q + 10 stream + component) conflict free.
-    static constexpr int YS = R == 16 ? 16 * 18 : C + R + (C == 64 ? 1 : 0);
-    // C = 64: the FIR runs on the tensor cores (mma.sync, see the FIR role).  Its operand loads read four rows of one
-    // stream per 128-bit instruction, so the raw rows are kept at a pitch of one row + 16 bytes (conflict free) and
-    // arrive with one bulk copy per row.
-    static constexpr bool FIRMMA = C == 64;
-    static constexpr int RAW_PITCH = C * SB + (FIRMMA ? 16 : 0);   // bytes per raw row of one stream
-    static constexpr int RAW_STAGE = kSubTile * SPC * RAW_PITCH;   // bytes: [SPC][16 rows][RAW_PITCH]
+    static constexpr int YS = R == 16 ? 16 * 18 : C + R;
+    static constexpr int RAW_STAGE = kSubTile * 256 * SB;  // bytes: [SPC][16 rows][C] samples
     // One spectrum of the tile = SPC * YS float2; for C = 64 two pad elements make the stride of a spectrum PAIR
     // 4 (mod 16) eight-byte words, so that the four pairs of an FFT half-warp (lane = (pair, residue r)) hit
     // distinct banks in every load and store of the exchange (without them: 4-way conflicts, LSU pipe 91 % busy).
-    static constexpr int TS = SPC * YS + (R == 4 ? 6 : 0);   // = 2 (mod 8)
+    static constexpr int TS = SPC * YS + (R == 4 ? 2 : 0);
     static constexpr int Y_BUF = kSubTile * TS * 8;        // bytes
     // TENSOR: staged output tile = kStgTile spectra of every (stream, channel) of the CTA as fp16 planes, laid out
     // as the shared-memory side of the tensor store: boxes of [SPB streams][2 planes][C channels][32 spectra]
@@ -232,7 +173,7 @@ __device__ __forceinline__ constexpr int out_reg(int i) {
 // cycles (computed in fp64), and the per-spectrum factor exp(-2 pi i frac(t step)) is formed in fp32 ("sin/cos and
 // complex multiply in single precision").
 template <int C, int BITS, bool TENSOR, bool INTERP>
-__global__ void __launch_bounds__(fthreads(C), 1) fstage_kernel(const FArgs a, const __grid_constant__ CUtensorMap zmap) {
+__global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, const __grid_constant__ CUtensorMap zmap) {
     using Sh = FShape<C, BITS, TENSOR, INTERP>;
     constexpr int SB = Sh::SB, SPC = Sh::SPC, R = Sh::R, YS = Sh::YS;
     extern __shared__ __align__(1024) unsigned char smem[];
@@ -257,7 +198,7 @@ __global__ void __launch_bounds__(fthreads(C), 1) fstage_kernel(const FArgs a, c
 
     if (tid == 0) {
         for (int s = 0; s < kRawStages; ++s) {
-            mbar_init(bar_raw_full + 8 * s, Sh::FIRMMA ? 32 : 1);
+            mbar_init(bar_raw_full + 8 * s, 1);
             mbar_init(bar_raw_empty + 8 * s, kFirThreads / 32);
         }
         for (int b = 0; b < kYBufs; ++b) {
@@ -272,14 +213,14 @@ __global__ void __launch_bounds__(fthreads(C), 1) fstage_kernel(const FArgs a, c
     }
     {   // rotation * bandpass of the CTA's streams (station = m >> 1) in the FFT threads' register order, zeros for
         // streams that do not exist (their staged rows are then exact zeros), and the inter-pass twiddles
-        for (int idx = tid; idx < 256; idx += (int)blockDim.x) {
+        for (int idx = tid; idx < 256; idx += kFThreads) {
             const int sl = idx / C, rr = (idx % C) / 16, i = idx % 16;
             const int m = m0 + sl;
             reinterpret_cast<float2 *>(smem + Sh::OFF_WTAB + (idx >> 4) * Sh::TAB_ROW)[i] =
                 m < a.M ? a.phase[((size_t)bl * a.S + (m >> 1)) * C + out_channel<R>(rr, i)] : make_float2(0.f, 0.f);
         }
         if (INTERP) {
-            for (int idx = tid; idx < 256; idx += (int)blockDim.x) {
+            for (int idx = tid; idx < 256; idx += kFThreads) {
                 const int sl = idx / C, rr = (idx % C) / 16, i = idx % 16;
                 const int m = m0 + sl;
                 reinterpret_cast<float *>(smem + Sh::OFF_STEP + (idx >> 4) * Sh::STEP_ROW)[i] =
@@ -288,7 +229,7 @@ __global__ void __launch_bounds__(fthreads(C), 1) fstage_kernel(const FArgs a, c
         }
         if (tid < 16) reinterpret_cast<float2 *>(smem + Sh::OFF_ZERO)[tid] = make_float2(0.f, 0.f);
         if (R > 1) {
-            for (int idx = tid; idx < R * 16; idx += (int)blockDim.x) {
+            for (int idx = tid; idx < R * 16; idx += kFThreads) {
                 float sn, cs;
                 sincospif(-2.0f * (float)((idx / 16) * (idx % 16)) / (float)C, &sn, &cs);   // entry [r][k1]
                 reinterpret_cast<float2 *>(smem + Sh::OFF_TW + (idx >> 4) * Sh::TAB_ROW)[idx & 15] = make_float2(cs, sn);
@@ -297,15 +238,8 @@ __global__ void __launch_bounds__(fthreads(C), 1) fstage_kernel(const FArgs a, c
     }
     __syncthreads();
 
-    // Register budget (FIRMMA: 640 threads at 96 registers): the fifth warp group (producer, store issuer, two idle warps)
-    // drops to 32 registers = 8192 released, and the two FIR warp groups, which keep their weight fragments and the
-    // previous data fragments in registers, rise to 128 = 8192 taken (setmaxnreg at the head of each role's branch).
-    if (warp > kStoreWarp) {
-        if (Sh::FIRMMA) asm volatile("setmaxnreg.dec.sync.aligned.u32 32;");
-    } else if (warp == kProducerWarp) {
+    if (warp == kProducerWarp) {
         // ------------------------------------------------------------------ producer
-        if (Sh::FIRMMA) asm volatile("setmaxnreg.dec.sync.aligned.u32 32;");
-        const bool aligned16 = ((reinterpret_cast<uintptr_t>(a.samples) | reinterpret_cast<uintptr_t>(a.hist) | (uintptr_t)(a.N * SB)) & 15u) == 0;
         for (int item = 0; item < n_items; ++item)
         for (int j = 0; j <= n_sub; ++j) {
             const int mi = m0 + item * SPC, n_valid = min(SPC, a.M - mi);
@@ -315,63 +249,10 @@ __global__ void __launch_bounds__(fthreads(C), 1) fstage_kernel(const FArgs a, c
             mbar_wait(bar_raw_empty + 8 * s, ph ^ 1u);
             const long long tb = t0 - kSubTile + (long long)j * kSubTile;     // first row of the sub-tile
             const uint32_t full = bar_raw_full + 8 * s;
-            if constexpr (Sh::FIRMMA) {
-                // Padded rows (FShape): every lane copies 16-byte pieces (cp.async -> SASS LDGSTS) to their padded places and
-                // the mbarrier counts one arrival per lane, triggered when that lane's copies have landed.  A lane owns the
-                // pieces (row = lane / CPR + k RPI, column piece lane % CPR), k = 0 .. 16 / RPI - 1, of every stream.
-                constexpr int CPR = C * SB / 16;                 // 16-byte pieces per row
-                constexpr int RPI = 32 / CPR;                    // rows covered by one instruction of the warp
-                const int prow = lane / CPR;
-                const uint32_t lane_dst = sbase + Sh::OFF_RAW + s * Sh::RAW_STAGE + prow * Sh::RAW_PITCH + (lane % CPR) * 16;
-                const size_t lane_src = (size_t)prow * C * SB + (lane % CPR) * 16;
-                const unsigned char *smp0 = a.samples + ((size_t)bl * a.M + mi) * (size_t)a.N * SB + lane_src;
-                if (aligned16 && tb >= 0 && tb + kSubTile <= a.n_t) {
-                    // interior sub-tile (all but the first and the last few of a segment): straight copies
-                    const unsigned char *src = smp0 + (size_t)tb * C * SB;
-                    for (int sl = 0; sl < n_valid; ++sl) {
-#pragma unroll
-                        for (int k = 0; k < kSubTile / RPI; ++k)
-                            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(lane_dst + (sl * kSubTile + k * RPI) * Sh::RAW_PITCH),
-                                         "l"(src + (size_t)k * RPI * C * SB)
-                                         : "memory");
-                        src += (size_t)a.N * SB;
-                    }
-                    asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(full) : "memory");
-                } else {
-                    // boundary sub-tiles: rows before the block come from the carried history, rows t < -15 or t >= n_t are
-                    // never used by a live output and are left as they are; unaligned streams (odd N) go element by element
-                    const unsigned char *hst0 = a.hist + ((size_t)(a.b0 + bl) * a.M + mi) * (size_t)(kTaps - 1) * C * SB + lane_src;
-                    for (int sl = 0; sl < n_valid; ++sl) {
-                        for (int k = 0; k < kSubTile / RPI; ++k) {
-                            const long long t = tb + prow + k * RPI;
-                            if (t < -(long long)(kTaps - 1) || t >= a.n_t) continue;
-                            const unsigned char *src = t < 0 ? hst0 + ((size_t)sl * (kTaps - 1) + (size_t)(t + kTaps - 1)) * C * SB - (size_t)prow * C * SB
-                                                             : smp0 + (size_t)sl * a.N * SB + (size_t)(t - prow) * C * SB;
-                            const uint32_t dst = lane_dst + (sl * kSubTile + k * RPI) * Sh::RAW_PITCH;
-                            if (aligned16) {
-                                asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
-                            } else {
-                                for (int e = 0; e < 16; e += SB) {
-                                    if (SB == 4) {
-                                        const uint32_t v = __ldg(reinterpret_cast<const uint32_t *>(src + e));
-                                        asm volatile("st.shared.b32 [%0], %1;" ::"r"(dst + e), "r"(v) : "memory");
-                                    } else {
-                                        const unsigned short v = __ldg(reinterpret_cast<const unsigned short *>(src + e));
-                                        asm volatile("st.shared.b16 [%0], %1;" ::"r"(dst + e), "h"(v) : "memory");
-                                    }
-                                }
-                            }
-                        }
-                    }
-                    if (aligned16) asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(full) : "memory");
-                    else mbar_arrive(full);
-                }
-                continue;
-            }
             uint32_t tx = 0;
             for (int sl = 0; sl < n_valid; ++sl) {
                 const size_t stream = (size_t)bl * a.M + (mi + sl);
-                const uint32_t dst0 = sbase + Sh::OFF_RAW + s * Sh::RAW_STAGE + sl * (kSubTile * Sh::RAW_PITCH);
+                const uint32_t dst0 = sbase + Sh::OFF_RAW + s * Sh::RAW_STAGE + sl * (kSubTile * C * SB);
 #pragma unroll
                 for (int part = 0; part < 2; ++part) {
                     // part 0: rows from the carried history (t < 0); part 1: rows of this call's block
@@ -388,19 +269,18 @@ __global__ void __launch_bounds__(fthreads(C), 1) fstage_kernel(const FArgs a, c
                     }
                     if (hi <= lo) continue;
                     const uint32_t bytes = (uint32_t)(hi - lo) * C * SB;
-                    const uint32_t dst = dst0 + (uint32_t)(lo - tb) * Sh::RAW_PITCH;
+                    const uint32_t dst = dst0 + (uint32_t)(lo - tb) * C * SB;
                     if ((reinterpret_cast<uintptr_t>(src) & 15u) == 0) {
                         if (lane == 0) bulk_g2s(dst, src, bytes, full);
                         tx += bytes;
                     } else {   // stream not 16-byte aligned (odd N): element-wise copy by the warp
                         for (uint32_t e = lane * SB; e < bytes; e += 32 * SB) {
-                            const uint32_t d = dst + (e / (C * SB)) * Sh::RAW_PITCH + e % (C * SB);
                             if (SB == 4) {
                                 const uint32_t v = __ldg(reinterpret_cast<const uint32_t *>(src + e));
-                                asm volatile("st.shared.b32 [%0], %1;" ::"r"(d), "r"(v) : "memory");
+                                asm volatile("st.shared.b32 [%0], %1;" ::"r"(dst + e), "r"(v) : "memory");
                             } else {
                                 const unsigned short v = __ldg(reinterpret_cast<const unsigned short *>(src + e));
-                                asm volatile("st.shared.b16 [%0], %1;" ::"r"(d), "h"(v) : "memory");
+                                asm volatile("st.shared.b16 [%0], %1;" ::"r"(dst + e), "h"(v) : "memory");
                             }
                         }
                     }
@@ -410,7 +290,6 @@ __global__ void __launch_bounds__(fthreads(C), 1) fstage_kernel(const FArgs a, c
             if (lane == 0) mbar_arrive_expect_tx(full, tx);
         }
     } else if (warp == kStoreWarp) {
-        if (Sh::FIRMMA) asm volatile("setmaxnreg.dec.sync.aligned.u32 32;");
         // ------------------------------------------------------------------ tensor-store issuer (step a7)
         // One staged tile = 32 spectra of every (stream, channel) of the CTA.  Row (channel c, k-tile kt, row group
         // m / 8, plane, m % 8) of z is 128 bytes = 64 spectra whose 16-byte chunk q sits at q ^ (m & 7) (cobalt_internal.h;
@@ -442,122 +321,6 @@ __global__ void __launch_bounds__(fthreads(C), 1) fstage_kernel(const FArgs a, c
         }
     } else if (warp < kFirThreads / 32) {
         // ------------------------------------------------------------------ FIR (steps a1, a2)
-        if constexpr (Sh::FIRMMA) {
-            asm volatile("setmaxnreg.inc.sync.aligned.u32 128;");
-            // Tensor-core FIR (see the comment at mma_16816).  Warp w owns the 8 branches 8 w .. 8 w + 7 for the whole kernel:
-            // their weight fragments (B operands) live in registers.  The A operand is the data: row g = lane >> 2 is
-            // the series (stream g >> 1, component g & 1), rows 8-15 the same series 8 spectra later, so that one
-            //   k16 product over the rows t' in [T0 - 16, T0)   A = {h0, h1, h1, h2},  B = {R, Q}
-            //   k8  product over the rows t' in [T0, T0 + 8)    A = {h2, h3},          B = {P}
-            // gives the 16 outputs T0 .. T0 + 15 of 8 series; h0..h3 are the series' half-blocks of 8 rows (h0, h1 from the
-            // previous sub-tile, h2, h3 this one), each one register: the fp16 pair of rows q and q + 4 of the half-block,
-            // q = lane & 3 (the k index of the instruction is this permutation of t', in the weight fragments too).
-            constexpr int NP = BITS == 16 ? 2 : 1;           // data parts (int16: high byte, low byte / 256)
-            constexpr int WPB = 16 / SB;                     // branches per 16-byte load: 8 (int8) or 4 (int16)
-            const int g = lane >> 2, q = lane & 3, sl = g >> 1, comp = g & 1;
-            // weight fragments for output n = g: R = (T(d + 16), T(d + 12)), Q = (T(d + 8), T(d + 4)), P = (T(d), T(d - 4)),
-            // d = g - q, T(k) = w[k] for 0 <= k <= 15, else 0 (w[k] multiplies x[t - k]); [.][0] = fp16 high part, [1] = residual
-            uint32_t wRQ[8][2][2], wP[8][2];
-#pragma unroll
-            for (int i = 0; i < 8; ++i) {
-                const int ph = 8 * warp + i;
-                const float sc = ((ph & 1) ? -1.f : 1.f) * fir_mma_weight_scale(C);   // (-1)^ph: channel j <- bin (j + C/2) mod C
-                auto T = [&](int k) { return (k >= 0 && k < kTaps) ? a.weights[k * C + ph] * sc : 0.f; };
-                const int d = g - q;
-                split_pair(T(d + 16), T(d + 12), wRQ[i][0][0], wRQ[i][1][0]);
-                split_pair(T(d + 8), T(d + 4), wRQ[i][0][1], wRQ[i][1][1]);
-                split_pair(T(d), T(d - 4), wP[i][0], wP[i][1]);
-            }
-            // byte selectors of __byte_perm: the thread's component of sample e (of the WPB in a 16-byte chunk)
-            //   int8 : word = two samples (re0, im0, re1, im1): byte 2 (e & 1) + comp
-            //   int16: word = one sample (re lo, re hi, im lo, im hi): low byte 2 comp, high byte 2 comp + 1
-            uint32_t selA[2], selB;
-            if (BITS == 8) {
-                selA[0] = (uint32_t)comp | ((uint32_t)(4 + comp) << 8);
-                selA[1] = (uint32_t)(2 + comp) | ((uint32_t)(6 + comp) << 8);
-                selB = 0;
-            } else {
-                selA[0] = selA[1] = (uint32_t)(2 * comp + 1) | ((uint32_t)(5 + 2 * comp) << 8);   // high bytes
-                selB = (uint32_t)(2 * comp) | ((uint32_t)(4 + 2 * comp) << 8);                    // low bytes
-            }
-            uint32_t kmask, kmagic_s, kmagic_u;              // opaque to the compiler so that they stay in registers (one LOP3)
-            asm volatile("mov.b32 %0, 0x00ff00ff;" : "=r"(kmask));
-            asm volatile("mov.b32 %0, 0x64806480;" : "=r"(kmagic_s));
-            asm volatile("mov.b32 %0, 0x64006400;" : "=r"(kmagic_u));
-            uint32_t hprev[8][NP][2];                        // h0, h1: the half-blocks of the previous sub-tile
-#pragma unroll
-            for (int i = 0; i < 8; ++i)
-#pragma unroll
-                for (int pp = 0; pp < NP; ++pp) hprev[i][pp][0] = hprev[i][pp][1] = 0u;
-            // row q + 4 j of stream sl, the warp's 16-byte chunk(s)
-            const uint32_t raw_thread = sbase + Sh::OFF_RAW + (sl * kSubTile + q) * Sh::RAW_PITCH + warp * 8 * SB;
-            // y[t][stream][branch] as floats: component comp of spectrum 2 q (+1, +8, +9) of the sub-tile
-            float *ybuf = reinterpret_cast<float *>(smem + Sh::OFF_Y) + 2 * (2 * q * Sh::TS + sl * YS + 8 * warp + ((8 * warp) >> 4)) + comp;
-
-            for (int item = 0; item < n_items; ++item)
-            for (int j = 0; j <= n_sub; ++j) {
-                const int jg = item * (n_sub + 1) + j;
-                const int s = jg % kRawStages;
-                mbar_wait(bar_raw_full + 8 * s, (uint32_t)(jg / kRawStages) & 1u);
-                const int jj = j - 1;                         // real sub-tile index (j = 0 is the warm-up: fragments only)
-                const int jjg = item * n_sub + jj;
-                const int yb = jjg % kYBufs;
-                const uint32_t raw = raw_thread + s * Sh::RAW_STAGE;
-                if (jj >= 0) mbar_wait(bar_y_empty + 8 * yb, ((uint32_t)(jjg / kYBufs) & 1u) ^ 1u);
-                float *yrow = ybuf + (size_t)(jj >= 0 ? yb : 0) * (Sh::Y_BUF / 4);
-#pragma unroll
-                for (int c = 0; c < 8 / WPB; ++c) {
-                uint4 rw[4];                                  // rows q, q + 4, q + 8, q + 12: WPB branches each
-#pragma unroll
-                for (int r4 = 0; r4 < 4; ++r4)
-                    asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];"
-                                 : "=r"(rw[r4].x), "=r"(rw[r4].y), "=r"(rw[r4].z), "=r"(rw[r4].w)
-                                 : "r"(raw + r4 * 4 * Sh::RAW_PITCH + c * 16));
-#pragma unroll
-                for (int ii = 0; ii < WPB; ++ii) {
-                    const int i = c * WPB + ii;
-                    // the 32-bit word of row q + 4 r4 holding sample i of the warp's branches
-                    auto word = [&](int r4) {
-                        const int wi = BITS == 8 ? ii >> 1 : ii;
-                        const uint4 &v = rw[r4];
-                        return wi == 0 ? v.x : wi == 1 ? v.y : wi == 2 ? v.z : v.w;
-                    };
-                    uint32_t hc[NP][2];                       // h2, h3 (step a1: exact integer -> fp16)
-                    hc[0][0] = bytes_to_h2<true>(word(0), word(1), selA[i & 1], kmask, kmagic_s);
-                    hc[0][1] = bytes_to_h2<true>(word(2), word(3), selA[i & 1], kmask, kmagic_s);
-                    if (NP == 2) {
-                        hc[NP - 1][0] = bytes_to_h2<false>(word(0), word(1), selB, kmask, kmagic_u);
-                        hc[NP - 1][1] = bytes_to_h2<false>(word(2), word(3), selB, kmask, kmagic_u);
-                    }
-                    if (jj >= 0) {
-                        float d[4] = {0.f, 0.f, 0.f, 0.f};
-#pragma unroll
-                        for (int pp = 0; pp < NP; ++pp)
-#pragma unroll
-                            for (int hl = 0; hl < 2; ++hl) {
-                                mma_16816(d, hprev[i][pp][0], hprev[i][pp][1], hprev[i][pp][1], hc[pp][0], wRQ[i][hl][0], wRQ[i][hl][1]);
-                                mma_1688(d, hc[pp][0], hc[pp][1], wP[i][hl]);
-                            }
-                        // d[0], d[1] = y[2 q], y[2 q + 1]; d[2], d[3] = y[2 q + 8], y[2 q + 9] of series g, branch 8 w + i
-                        yrow[2 * i] = d[0];
-                        yrow[2 * (Sh::TS + i)] = d[1];
-                        yrow[2 * (8 * Sh::TS + i)] = d[2];
-                        yrow[2 * (9 * Sh::TS + i)] = d[3];
-                    }
-#pragma unroll
-                    for (int pp = 0; pp < NP; ++pp) {
-                        hprev[i][pp][0] = hc[pp][0];
-                        hprev[i][pp][1] = hc[pp][1];
-                    }
-                }
-                }
-                __syncwarp();
-                if (lane == 0) {
-                    mbar_arrive(bar_raw_empty + 8 * s);
-                    if (jj >= 0) mbar_arrive(bar_y_full + 8 * yb);
-                }
-            }
-        } else {
         int sl, ph;
         if (R == 16) {   // lane permutation matching the 18 r + q tile (see FShape)
             sl = 0;
@@ -622,7 +385,6 @@ __global__ void __launch_bounds__(fthreads(C), 1) fstage_kernel(const FArgs a, c
                 if (jj >= 0) mbar_arrive(bar_y_full + 8 * yb);
             }
         }
-        }   // !FIRMMA
     } else {
         // ------------------------------------------------------------------ FFT, rotate, transpose (steps a3-a7)
         // Team tm takes the sub-tiles jj = tm, tm + 2, ...; a thread owns TWO consecutive spectra (so that the fp16
@@ -804,7 +566,7 @@ __global__ void phase_table_kernel(const double *__restrict__ delays, const floa
                                    const double *__restrict__ f_sb, int b0, int nb, int S, int C, double f_s,
                                    float amp_max, int tensor, float *__restrict__ scale_out,
                                    float2 *__restrict__ out, const double *__restrict__ delays_end, double inv_n_t,
-                                   float *__restrict__ step_out, float fir_gain) {
+                                   float *__restrict__ step_out) {
     __shared__ float s_max[32];
     __shared__ float s_scale;
     float bm = 0.f;
@@ -829,8 +591,7 @@ __global__ void phase_table_kernel(const double *__restrict__ delays, const floa
         }
     }
     __syncthreads();
-    // fir_gain: the tensor-core FIR (C = 64) works on power-of-two scaled operands; the exact factor is undone here
-    const double sc = (double)s_scale * (double)fir_gain;
+    const double sc = (double)s_scale;
     const long long total = (long long)nb * S * C;
     for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < total;
          idx += (long long)gridDim.x * blockDim.x) {
@@ -921,7 +682,7 @@ cudaError_t launch_f(const cobalt_plan_s *p, cudaStream_t st, const FArgs &a, in
     args.tiles_per_seg = (p->n_kt + n_seg - 1) / n_seg;
     n_seg = (p->n_kt + args.tiles_per_seg - 1) / args.tiles_per_seg;
     dim3 grid((unsigned)groups, (unsigned)n_seg);
-    kern<<<grid, fthreads(C), smem, st>>>(args, p->zmap);
+    kern<<<grid, kFThreads, smem, st>>>(args, p->zmap);
     return cudaGetLastError();
 }
 
@@ -947,7 +708,7 @@ cudaError_t launch_phase_table(const cobalt_plan_s *p, cudaStream_t st, const do
     phase_table_kernel<<<(unsigned)blocks, threads, 0, st>>>(d_delays, d_bandpass, p->d_f_sb, b0, nb, p->S, p->C,
                                                              p->f_s, p->amp_max, p->mode == COBALT_MODE_TENSOR_FP16 ? 1 : 0,
                                                              p->d_scale, p->d_phase, p->cur_delays_end, 1.0 / (double)p->n_t,
-                                                             p->d_dstep, fir_output_gain(p->C, p->bits));
+                                                             p->d_dstep);
     return cudaGetLastError();
 }
 
