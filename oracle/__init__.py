@@ -71,6 +71,12 @@ def _load():
         lib.oracle_channel_direct.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_longlong, _D, _D,
                                               _D, _D, _D, ctypes.c_double, ctypes.c_double, ctypes.c_int, _D, _D]
         lib.oracle_channel_direct.restype = ctypes.c_int
+        lib.oracle_unpack_i4.argtypes = [ctypes.c_void_p, ctypes.c_longlong, _D]
+        lib.oracle_phase_offsets.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_longlong, _D, _D]
+        lib.oracle_flag_tiles.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_longlong, ctypes.c_int, ctypes.c_void_p, _D]
+        lib.oracle_valid_counts.argtypes = [ctypes.c_int, ctypes.c_longlong, ctypes.c_int, ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p]
+        lib.oracle_correlate_dumps.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_longlong, ctypes.c_int, ctypes.c_int, _D, _D]
+        lib.oracle_correlate_dumps.restype = ctypes.c_int
         _lib = lib
     return _lib
 
@@ -253,3 +259,87 @@ def channel_direct(x: np.ndarray, C: int, j: int, hist: np.ndarray | None = None
     if rc:
         raise MemoryError("oracle_channel_direct")
     return _r2c(zc), _r2c(vc)
+
+
+# ------------------------------------------------------------------ SURVEY.md sec 8(f) rows 1-3
+TILE = 64  # spectra per valid-sample tile and per dump granule (the correlator's time tile, readings A23 / A24)
+
+
+def unpack4(packed: np.ndarray) -> np.ndarray:
+    """uint8 [...] (re low nibble, im high nibble, 4-bit two's complement) -> float64 [..., 2] (reading A27)."""
+    s = np.ascontiguousarray(packed, dtype=np.uint8)
+    out = np.empty(s.shape + (2,), dtype=np.float64)
+    _load().oracle_unpack_i4(s.ctypes.data, s.size, _p(out))
+    return out
+
+
+def coarse_shift(samples: np.ndarray, offsets, N: int) -> np.ndarray:
+    """Reading A25 ("coarse delay compensation ... by shifting"): station a's block of N samples starts at sample
+    offsets[a] of its (longer) input stream.  samples [S][2][N_in][2] -> [S][2][N][2]; pure indexing."""
+    S = samples.shape[0]
+    out = np.empty((S, 2, N, 2), dtype=samples.dtype)
+    for a in range(S):
+        o = int(offsets[a])
+        assert 0 <= o and o + N <= samples.shape[2]
+        out[a] = samples[a, :, o:o + N, :]
+    return out
+
+
+def pol_minor_to_planar(x: np.ndarray) -> np.ndarray:
+    """Reading A26: LOFAR wire order [S][N][2 pol][2] (time-major, polarisation-minor) -> [S][2][N][2]; pure indexing."""
+    return np.ascontiguousarray(np.swapaxes(x, 1, 2))
+
+
+def phase_offsets(z: np.ndarray, phase0) -> np.ndarray:
+    """z complex [S][2][n_t][C] -> z exp(-i phase0[a][p]) (reading A22)."""
+    zr = _c2r(z).copy()
+    S, _, n_t, C = zr.shape[:4]
+    _load().oracle_phase_offsets(S, C, n_t, _p(_f64(phase0, (S, 2))), _p(zr))
+    return _r2c(zr)
+
+
+def flag_tiles(z: np.ndarray, valid) -> np.ndarray:
+    """z complex [S][2][n_t][C], valid uint8 [S][ceil(n_t / 64)] -> z with the lost tiles zeroed (reading A24)."""
+    zr = _c2r(z).copy()
+    S, _, n_t, C = zr.shape[:4]
+    v = np.ascontiguousarray(valid, dtype=np.uint8)
+    assert v.shape == (S, (n_t + TILE - 1) // TILE)
+    _load().oracle_flag_tiles(S, C, n_t, TILE, v.ctypes.data, _p(zr))
+    return _r2c(zr)
+
+
+def valid_counts(S: int, n_t: int, valid, dumps: int = 1) -> np.ndarray:
+    """-> int64 [dumps][n_bl]: spectra of each dump in which both stations of the baseline are valid."""
+    v = np.ascontiguousarray(valid, dtype=np.uint8)
+    out = np.empty((dumps, n_baselines(S)), dtype=np.int64)
+    _load().oracle_valid_counts(S, n_t, dumps, TILE, v.ctypes.data, out.ctypes.data)
+    return out
+
+
+def correlate_dumps(z: np.ndarray, dumps: int) -> np.ndarray:
+    """z complex [S][2][n_t][C] -> vis complex [dumps][C][n_bl][2][2] (reading A23)."""
+    zr = _c2r(z)
+    S, two, n_t, C = zr.shape[:4]
+    vis = np.empty((dumps, C, n_baselines(S), 2, 2, 2), dtype=np.float64)
+    if _load().oracle_correlate_dumps(S, C, n_t, dumps, TILE, _p(zr), _p(vis)):
+        raise ValueError("dumps must divide ceil(n_t / 64)")
+    return _r2c(vis)
+
+
+def process_subband_ext(samples: np.ndarray, C: int, delays, bandpass, f_sb: float, hist: np.ndarray | None = None,
+                        f_s: float = F_S, T: int = TAPS, delays_end=None, phase0=None, valid=None, dumps: int = 1):
+    """process_subband with the rows of SURVEY.md sec 8(f): per-(station, pol) phase offsets (A22), valid-sample
+    flags (A24) and several dumps per block (A23).  samples int16/int8 [S][2][N][2] (or uint8 [S][2][N] 4-bit packed,
+    A27) -> vis complex [dumps][C][n_bl][2][2]."""
+    s = np.ascontiguousarray(samples)
+    if s.dtype == np.uint8:
+        x = _r2c(unpack4(s))
+    else:
+        x = _r2c(unpack(s))
+    S = x.shape[0]
+    z = fstage(x, C, hist=hist, delays=delays, bandpass=bandpass, f_sb=f_sb, f_s=f_s, T=T, delays_end=delays_end)
+    if phase0 is not None:
+        z = phase_offsets(z, phase0)
+    if valid is not None:
+        z = flag_tiles(z, valid)
+    return correlate_dumps(z, dumps)

@@ -28,7 +28,8 @@
  * impulse, P6 numpy.fft special case, P7 Hermitian, P8 identical streams, P9
  * delay slope, P10 history carry, P11 brute force (oracle_channel_direct below
  * + a numpy brute force), P12 linearity, P13 statistics, P16 time-varying delay
- * (equal ends = static rotation; closed-form geometric series).  No function here is
+ * (equal ends = static rotation; closed-form geometric series), P17-P21 (coarse shift,
+ * phase offsets, dumps, valid-sample flags and counts, 4-bit unpack).  No function here is
  * "parity unpinned".
  *
  * Layouts (all row-major, last index fastest):
@@ -299,6 +300,102 @@ int oracle_process_subband_interp(int S, int C, int T, long long N, int bits, co
     free(g);
     if (!z_out) free(z);
     return rc;
+}
+
+
+/* =====================================================================================================
+ * SURVEY.md sec 8(f) rows 1-3 (the rows marked "next"): clock / phase offsets, sub-second dumps, valid-sample
+ * weights, 4-bit samples.  Each is the plain definition of the reading named beside it.
+ * ===================================================================================================== */
+
+/* Reading A27 ("4-bit ... mode"): one byte per complex sample, re in the low nibble, im in the high
+ * nibble, both 4-bit two's complement (-8 .. 7), no scaling. */
+void oracle_unpack_i4(const uint8_t *in, long long n_samples, double *out /*[n_samples][2]*/) {
+    for (long long i = 0; i < n_samples; ++i) {
+        int lo = in[i] & 15, hi = (in[i] >> 4) & 15;
+        out[2 * i] = (double)(lo >= 8 ? lo - 16 : lo);
+        out[2 * i + 1] = (double)(hi >= 8 ? hi - 16 : hi);
+    }
+}
+
+/* Reading A22 ("bandpass and clock corrections"): a constant phase per (station, polarisation),
+ * phase0 in radians, with the sign sense of the delay term:  z <- z exp(-i phase0[a][p]). */
+void oracle_phase_offsets(int S, int C, long long n_t, const double *phase0 /*[S][2]*/, double *z /*[S][2][n_t][C][2]*/) {
+    for (int sp = 0; sp < 2 * S; ++sp) {
+        const double wr = cos(phase0[sp]), wi = -sin(phase0[sp]);
+        double *zz = z + 2 * (long long)sp * n_t * C;
+        for (long long i = 0; i < n_t * C; ++i) {
+            double a = zz[2 * i], b = zz[2 * i + 1];
+            zz[2 * i] = a * wr - b * wi;
+            zz[2 * i + 1] = a * wi + b * wr;
+        }
+    }
+}
+
+/* Reading A24 (P:L298 lost data is "encoded in the metadata"; P:L282-288 block granularity): valid[a][v] = 0 marks
+ * the spectra [v tile, (v+1) tile) of station a (both polarisations) as lost.  Their channelised samples count as
+ * zero in the correlation (the FIR still runs over whatever the input buffer holds: masking happens after it). */
+void oracle_flag_tiles(int S, int C, long long n_t, int tile, const unsigned char *valid /*[S][ceil(n_t/tile)]*/,
+                       double *z /*[S][2][n_t][C][2]*/) {
+    const long long n_vt = (n_t + tile - 1) / tile;
+    for (int a = 0; a < S; ++a)
+        for (int p = 0; p < 2; ++p)
+            for (long long t = 0; t < n_t; ++t)
+                if (!valid[a * n_vt + t / tile]) {
+                    double *zz = z + 2 * ((((long long)a * 2 + p) * n_t + t) * C);
+                    for (int j = 0; j < 2 * C; ++j) zz[j] = 0.0;
+                }
+}
+
+/* ... and the weight that goes with a visibility: the number of spectra of dump d in which BOTH stations of the
+ * baseline are valid.  counts [D][n_bl].  Dumps as in oracle_correlate_dumps. */
+void oracle_valid_counts(int S, long long n_t, int D, int tile, const unsigned char *valid, long long *counts) {
+    const long long n_vt = (n_t + tile - 1) / tile;
+    const long long n_bl = (long long)S * (S + 1) / 2;
+    const long long dump_len = ((n_vt / D) * tile);
+    for (int d = 0; d < D; ++d)
+        for (int k = 0; k < S; ++k)
+            for (int i = 0; i <= k; ++i) {
+                long long c = 0;
+                for (long long t = d * dump_len; t < n_t && t < (d + 1) * dump_len; ++t)
+                    if (valid[i * n_vt + t / tile] && valid[k * n_vt + t / tile]) ++c;
+                counts[d * n_bl + (long long)k * (k + 1) / 2 + i] = c;
+            }
+}
+
+/* Reading A23 (P:L103 integration time down to a fraction of a second): D dumps per block.  Dump
+ * boundaries fall on multiples of `tile` spectra (the correlator's time tile, 64): with n_vt = ceil(n_t / tile)
+ * tiles, D must divide n_vt and dump d integrates the spectra [d L, min((d+1) L, n_t)), L = (n_vt / D) tile; the
+ * last dump is shorter when n_t is not a multiple of the tile.  vis [D][C][n_bl][2][2][2]; D = 1 is oracle_correlate.
+ * Returns 1 when D does not divide n_vt. */
+int oracle_correlate_dumps(int S, int C, long long n_t, int D, int tile, const double *z /*[S][2][n_t][C][2]*/,
+                           double *vis /*[D][C][n_bl][2][2][2]*/) {
+    const long long n_vt = (n_t + tile - 1) / tile;
+    const long long n_bl = (long long)S * (S + 1) / 2;
+    if (D < 1 || n_vt % D) return 1;
+    const long long L = (n_vt / D) * tile;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int j = 0; j < C; ++j)
+        for (int d = 0; d < D; ++d)
+            for (int k = 0; k < S; ++k)
+                for (int i = 0; i <= k; ++i)
+                    for (int p = 0; p < 2; ++p)
+                        for (int q = 0; q < 2; ++q) {
+                            const double *zi = z + 2 * ((((long long)i * 2 + p) * n_t) * C);
+                            const double *zk = z + 2 * ((((long long)k * 2 + q) * n_t) * C);
+                            double re = 0.0, im = 0.0;
+                            for (long long t = d * L; t < n_t && t < (d + 1) * L; ++t) {
+                                double ar = zi[2 * (t * C + j)], ai = zi[2 * (t * C + j) + 1];
+                                double br = zk[2 * (t * C + j)], bi = zk[2 * (t * C + j) + 1];
+                                re += ar * br + ai * bi;
+                                im += ai * br - ar * bi;
+                            }
+                            long long bl = (long long)k * (k + 1) / 2 + i;
+                            double *o = vis + 2 * (((((long long)d * C + j) * n_bl + bl) * 2 + p) * 2 + q);
+                            o[0] = re;
+                            o[1] = im;
+                        }
+    return 0;
 }
 
 /* ------------------------------------------------- pin P11: single-sum form */
