@@ -65,11 +65,14 @@ typedef struct {
     long long n_consumed;                /* N_u = n_t * C                                   */
     long long n_baselines;               /* n_bl = S (S+1) / 2, autocorrelations included  */
     long long input_bytes;               /* B*S*2*N*2*(bits/8): extent read from `samples` */
-    long long output_bytes;              /* B*C*n_bl*4*8: extent written to `visibilities` */
+    long long output_bytes;              /* D*B*C*n_bl*4*8: extent written to `visibilities` */
     long long scratch_bytes;             /* device memory owned by the plan                */
     int chunk_subbands;                  /* subbands processed per internal launch group   */
     int sm_count;
     double sample_rate_hz;
+    int dumps;                           /* D, cobalt_set_dumps                               */
+    int n_tiles;                         /* ceil(n_t / 64): extent of `valid` per station   */
+    long long samples_allocated;         /* stream stride of `samples` (cobalt_set_coarse_delays) */
 } cobalt_info_t;
 
 /* ---------------------------------------------------------------------------------------
@@ -78,7 +81,9 @@ typedef struct {
  * an observation"; the paper's run-time compilation becomes template specialisation on
  * (channels, input_bits).)
  *   stations  >= 1 (dual polarisation each), subbands >= 1,
- *   channels  in {16, 64, 256}, taps == 16, input_bits in {16, 8},
+ *   channels  in {16, 64, 256}, taps == 16, input_bits in {16, 8, 4}
+ *             (4: one byte per complex sample, re in the low nibble, im in the high nibble, two's complement
+ *              -8 .. 7, reading A27 / P:L121; expanded to int8 by a pre-pass, see cobalt_set_input_layout),
  *   samples_per_integration >= channels.
  * The prototype filter is the Hann-windowed sinc of reading A1 (== scipy.signal.firwin(16 C,
  * 1/C, window="hann")), evaluated in double and rounded once to fp32.  History starts as zeros
@@ -137,6 +142,32 @@ int cobalt_process_interp(cobalt_plan_t *plan, void *cuda_stream, const void *d_
                           const double *d_delays_begin, const double *d_delays_end, const float *d_bandpass,
                           void *d_visibilities);
 
+
+/* ---------------------------------------------------------------------------------------
+ * cobalt_process_ex: cobalt_process with every optional input and output of SURVEY.md sec 8(f) rows 1-2 in one
+ * argument block (cobalt_process / cobalt_process_interp are this call with the optional members NULL).
+ * All pointers are DEVICE pointers; same asynchrony, history carry and errors as cobalt_process.
+ *   samples, delays, bandpass, visibilities   as cobalt_process (delays = the delay at the first spectrum);
+ *   delays_end     NULL, or [S] double: the delay runs linearly to this value over the block (cobalt_process_interp, A21);
+ *   valid          NULL (nothing lost), or [B][S][n_tiles] bytes, n_tiles = ceil(n_t / 64): 0 marks the 64 spectra
+ *                  [64 v, 64 v + 64) of a station (both polarisations) as lost ("lost data ... encoded in the
+ *                  metadata", reading A24): their channelised samples count as zero in the correlation; the FIR still
+ *                  runs over whatever the input holds;
+ *   valid_counts   NULL, or [B][D][n_bl] unsigned: the number of spectra of dump d in which both stations of the
+ *                  baseline are valid -- the weight that goes with the visibility (n_t per dump when valid == NULL);
+ *   visibilities   [D][B][C][n_bl][2][2] complex64 with D = cobalt_set_dumps (default 1: the layout of cobalt_process).
+ */
+typedef struct {
+    const void *samples;
+    const double *delays;
+    const double *delays_end;
+    const float *bandpass;
+    const unsigned char *valid;
+    void *visibilities;
+    unsigned int *valid_counts;
+} cobalt_io_t;
+int cobalt_process_ex(cobalt_plan_t *plan, void *cuda_stream, const cobalt_io_t *io);
+
 /* Frees all plan state.  cobalt_destroy(NULL) is a no-op returning COBALT_OK.  The caller must
  * have synchronised every stream that still runs work of this plan. */
 int cobalt_destroy(cobalt_plan_t *plan);
@@ -148,6 +179,26 @@ int cobalt_set_subband_frequencies(cobalt_plan_t *plan, const double *h_hz);
  * been called the default ladder f_sb[s] = 100 MHz + (12 + s) f_s is rebuilt with the new rate; a ladder the caller
  * has set is kept as it is.  Takes effect next call. */
 int cobalt_set_sample_rate(cobalt_plan_t *plan, double hz);
+/* Reading A22 ("bandpass and clock corrections"): a constant phase per (station, polarisation) with the
+ * sign sense of the delay term, z <- z exp(-i phase0[a][p]).  h_phase0: host [S][2] doubles, radians, or NULL = none.
+ * Folded (in fp32) into the rotation table of the F-stage.  Takes effect next call. */
+int cobalt_set_phase_offsets(cobalt_plan_t *plan, const double *h_phase0);
+/* Reading A25 ("coarse delay compensation ... by shifting"): station a's block of N samples starts at sample
+ * h_offsets[a] of its input stream, which is samples_allocated >= N + max offset samples long (the stream stride of
+ * d_samples becomes samples_allocated).  Applied by the F-stage's loads (free when the offset is a multiple of 16 bytes;
+ * other offsets take a slower element-wise load path).  The FIR history is the last 15 C samples the previous call
+ * consumed of the shifted stream.  h_offsets: host [S] ints >= 0, or NULL = none (and samples_allocated = N). */
+int cobalt_set_coarse_delays(cobalt_plan_t *plan, const int *h_offsets, long long samples_allocated);
+/* Reading A23: D dumps per block.  Dump boundaries fall on multiples of 64 spectra: D must divide
+ * n_tiles = ceil(n_t / 64); dump d integrates the spectra [d L, min((d + 1) L, n_t)), L = 64 n_tiles / D.  The
+ * visibility buffer becomes [D][B][C][n_bl][2][2]. */
+int cobalt_set_dumps(cobalt_plan_t *plan, int dumps_per_block);
+/* Reading A26: order of d_samples.  COBALT_LAYOUT_PLANAR (default) = [B][S][2 pol][N][2]; COBALT_LAYOUT_POL_MINOR =
+ * LOFAR's wire order [B][S][N][2 pol][2] (time-major, polarisation-minor).  Pol-minor input (and 4-bit input in either
+ * order) goes through a re-ordering pre-pass into plan-owned scratch (one extra read and write of the input). */
+#define COBALT_LAYOUT_PLANAR 0
+#define COBALT_LAYOUT_POL_MINOR 1
+int cobalt_set_input_layout(cobalt_plan_t *plan, int layout);
 /* Switch COBALT_MODE_*; reallocates the intermediate scratch, keeps the history. */
 int cobalt_set_mode(cobalt_plan_t *plan, int mode);
 /* Subbands per internal launch group (>= 1, clipped to B).  Reallocates scratch.  Default: as many as fit in 8 GiB of
@@ -180,7 +231,8 @@ int cobalt_get_kernel_timing(cobalt_plan_t *plan, double *ms4, int *kernel_launc
 /* FIR weights exactly as the kernels use them, host [16][C] float, weight of tap k (k = 0 is
  * the newest block) and branch ph at [k*C + ph] == fp32(g[(15-k) C + ph]). */
 int cobalt_debug_fir_weights(const cobalt_plan_t *plan, float *h_weights);
-/* Step a1 alone: n integer components (int16 or int8 per input_bits) -> n floats, device. */
+/* Step a1 alone: n integer components (int16 or int8 per input_bits) -> n floats, device; input_bits 4: n BYTES ->
+ * 2 n floats. */
 int cobalt_debug_unpack(void *cuda_stream, int input_bits, const void *d_in, long long n, float *d_out);
 /* Steps a1-a7 for ONE subband `sb` of d_samples (full [B][..] array as in cobalt_process):
  * d_z receives z as [C][2S][n_t] complex64 (input index = 2*station + pol).  Reads the history

@@ -23,13 +23,16 @@ COBALT_ERR_CUDA = -3
 COBALT_ERR_UNSUPPORTED_DEVICE = -4
 COBALT_MODE_TENSOR_FP16 = 0
 COBALT_MODE_EXACT_FP32 = 1
+COBALT_LAYOUT_PLANAR = 0
+COBALT_LAYOUT_POL_MINOR = 1
 
 F_S = 195312.5
 
 # every symbol include/cobalt.h declares (tests check the library exports exactly these)
 ABI_SYMBOLS = (
-    "cobalt_plan", "cobalt_process", "cobalt_process_interp", "cobalt_process_host", "cobalt_destroy",
+    "cobalt_plan", "cobalt_process", "cobalt_process_interp", "cobalt_process_ex", "cobalt_process_host", "cobalt_destroy",
     "cobalt_set_subband_frequencies", "cobalt_set_sample_rate", "cobalt_set_mode",
+    "cobalt_set_phase_offsets", "cobalt_set_coarse_delays", "cobalt_set_dumps", "cobalt_set_input_layout",
     "cobalt_set_chunk_subbands", "cobalt_reset", "cobalt_info", "cobalt_strerror", "cobalt_last_error",
     "cobalt_set_timing", "cobalt_get_timing", "cobalt_get_kernel_timing",
     "cobalt_debug_fir_weights", "cobalt_debug_unpack", "cobalt_debug_channelised", "cobalt_debug_correlate",
@@ -50,6 +53,15 @@ class cobalt_info_t(ctypes.Structure):
         ("n_consumed", ctypes.c_longlong), ("n_baselines", ctypes.c_longlong),
         ("input_bytes", ctypes.c_longlong), ("output_bytes", ctypes.c_longlong), ("scratch_bytes", ctypes.c_longlong),
         ("chunk_subbands", ctypes.c_int), ("sm_count", ctypes.c_int), ("sample_rate_hz", ctypes.c_double),
+        ("dumps", ctypes.c_int), ("n_tiles", ctypes.c_int), ("samples_allocated", ctypes.c_longlong),
+    ]
+
+
+class cobalt_io_t(ctypes.Structure):
+    _fields_ = [
+        ("samples", ctypes.c_void_p), ("delays", ctypes.c_void_p), ("delays_end", ctypes.c_void_p),
+        ("bandpass", ctypes.c_void_p), ("valid", ctypes.c_void_p), ("visibilities", ctypes.c_void_p),
+        ("valid_counts", ctypes.c_void_p),
     ]
 
 
@@ -71,7 +83,12 @@ def load(path: str | None = None):
                                 ctypes.c_longlong, ctypes.c_int]
     lib.cobalt_process.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp]
     lib.cobalt_process_interp.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp, _vp]
+    lib.cobalt_process_ex.argtypes = [_vp, _vp, ctypes.POINTER(cobalt_io_t)]
     lib.cobalt_process_host.argtypes = [_vp, _vp, _vp, _vp, _vp]
+    lib.cobalt_set_phase_offsets.argtypes = [_vp, _vp]
+    lib.cobalt_set_coarse_delays.argtypes = [_vp, _vp, ctypes.c_longlong]
+    lib.cobalt_set_dumps.argtypes = [_vp, ctypes.c_int]
+    lib.cobalt_set_input_layout.argtypes = [_vp, ctypes.c_int]
     lib.cobalt_destroy.argtypes = [_vp]
     lib.cobalt_set_subband_frequencies.argtypes = [_vp, _vp]
     lib.cobalt_set_sample_rate.argtypes = [_vp, ctypes.c_double]
@@ -152,6 +169,13 @@ def cobalt_process_interp(plan, stream, d_samples, d_delays_begin, d_delays_end,
                                         _ptr(d_bandpass), _ptr(d_visibilities)), plan)
 
 
+def cobalt_process_ex(plan, stream, d_samples, d_delays, d_bandpass, d_visibilities, d_delays_end=None, d_valid=None,
+                      d_valid_counts=None):
+    io = cobalt_io_t(_ptr(d_samples), _ptr(d_delays), _ptr(d_delays_end), _ptr(d_bandpass), _ptr(d_valid), _ptr(d_visibilities),
+                     _ptr(d_valid_counts))
+    _check(load().cobalt_process_ex(plan, _stream_ptr(stream), ctypes.byref(io)), plan)
+
+
 def cobalt_process_host(plan, h_samples, h_delays, h_bandpass, h_visibilities):
     _check(load().cobalt_process_host(plan, _ptr(h_samples), _ptr(h_delays), _ptr(h_bandpass), _ptr(h_visibilities)), plan)
 
@@ -215,6 +239,37 @@ class Correlator:
     def set_sample_rate(self, hz):
         _check(load().cobalt_set_sample_rate(self._h, float(hz)), self._h)
 
+    def set_phase_offsets(self, phase0):
+        """phase0: [S][2] radians (host), or None to clear (reading A22)."""
+        import numpy as np
+
+        if phase0 is None:
+            _check(load().cobalt_set_phase_offsets(self._h, None), self._h)
+            return
+        a = np.ascontiguousarray(phase0, dtype=np.float64)
+        assert a.shape == (self.info.stations, 2)
+        _check(load().cobalt_set_phase_offsets(self._h, a.ctypes.data), self._h)
+
+    def set_coarse_delays(self, offsets, samples_allocated=0):
+        """offsets: [S] first sample of each station's block (host ints), or None to clear (reading A25)."""
+        import numpy as np
+
+        if offsets is None:
+            _check(load().cobalt_set_coarse_delays(self._h, None, 0), self._h)
+        else:
+            a = np.ascontiguousarray(offsets, dtype=np.int32)
+            assert a.shape == (self.info.stations,)
+            _check(load().cobalt_set_coarse_delays(self._h, a.ctypes.data, int(samples_allocated)), self._h)
+        self.info = cobalt_info(self._h)
+
+    def set_dumps(self, dumps):
+        _check(load().cobalt_set_dumps(self._h, int(dumps)), self._h)
+        self.info = cobalt_info(self._h)
+
+    def set_input_layout(self, layout):
+        _check(load().cobalt_set_input_layout(self._h, int(layout)), self._h)
+        self.info = cobalt_info(self._h)
+
     def reset(self):
         _check(load().cobalt_reset(self._h), self._h)
 
@@ -235,9 +290,18 @@ class Correlator:
     # -- the hot path
     def vis_shape(self):
         i = self.info
-        return (i.subbands, i.channels, i.n_baselines, 2, 2)
+        one = (i.subbands, i.channels, i.n_baselines, 2, 2)
+        return one if i.dumps == 1 else (i.dumps,) + one
 
-    def process(self, samples, delays, bandpass, out=None, stream=None, delays_end=None):
+    def samples_shape(self, layout=COBALT_LAYOUT_PLANAR):
+        """Shape of the sample tensor the plan expects (4-bit: uint8, one byte per complex sample, no trailing axis)."""
+        i = self.info
+        n = i.samples_allocated
+        s = (i.subbands, i.stations, 2, n) if layout == COBALT_LAYOUT_PLANAR else (i.subbands, i.stations, n, 2)
+        return s if i.input_bits == 4 else s + (2,)
+
+    def process(self, samples, delays, bandpass, out=None, stream=None, delays_end=None, valid=None, valid_counts=None,
+                layout=COBALT_LAYOUT_PLANAR):
         """samples int16/int8 [B][S][2][N][2], delays float64 [S], bandpass float32 [C] (CUDA tensors)
         -> complex64 [B][C][n_bl][2][2].  Enqueues on ``stream`` (default: torch's current stream).
         ``delays_end`` (float64 [S]) selects cobalt_process_interp: the delay runs linearly from ``delays`` at the first
@@ -245,19 +309,29 @@ class Correlator:
         import torch
 
         i = self.info
-        want = torch.int16 if i.input_bits == 16 else torch.int8
+        want = {16: torch.int16, 8: torch.int8, 4: torch.uint8}[i.input_bits]
         assert samples.is_cuda and samples.is_contiguous() and samples.dtype == want
-        assert tuple(samples.shape) == (i.subbands, i.stations, 2, i.samples_per_integration, 2), tuple(samples.shape)
+        assert tuple(samples.shape) == self.samples_shape(layout), (tuple(samples.shape), self.samples_shape(layout))
         assert delays.is_cuda and delays.dtype == torch.float64 and delays.is_contiguous() and delays.numel() == i.stations
         assert bandpass.is_cuda and bandpass.dtype == torch.float32 and bandpass.is_contiguous() and bandpass.numel() == i.channels
         if out is None:
             out = torch.empty(self.vis_shape(), dtype=torch.complex64, device=samples.device)
         assert out.is_cuda and out.is_contiguous() and out.dtype == torch.complex64 and tuple(out.shape) == self.vis_shape()
-        if delays_end is None:
-            cobalt_process(self._h, stream, samples, delays, bandpass, out)
-        else:
+        if valid is not None:
+            assert valid.is_cuda and valid.dtype == torch.uint8 and valid.is_contiguous()
+            assert tuple(valid.shape) == (i.subbands, i.stations, i.n_tiles)
+        if valid_counts is not None:
+            assert valid_counts.is_cuda and valid_counts.dtype == torch.int32 and valid_counts.is_contiguous()
+            assert tuple(valid_counts.shape) == (i.subbands, i.dumps, i.n_baselines)
+        if delays_end is not None:
             assert delays_end.is_cuda and delays_end.dtype == torch.float64 and delays_end.is_contiguous() and delays_end.numel() == i.stations
-            cobalt_process_interp(self._h, stream, samples, delays, delays_end, bandpass, out)
+        if valid is None and valid_counts is None and i.dumps == 1:
+            if delays_end is None:
+                cobalt_process(self._h, stream, samples, delays, bandpass, out)
+            else:
+                cobalt_process_interp(self._h, stream, samples, delays, delays_end, bandpass, out)
+        else:
+            cobalt_process_ex(self._h, stream, samples, delays, bandpass, out, delays_end, valid, valid_counts)
         return out
 
     def process_host(self, samples, delays, bandpass, out):
@@ -293,17 +367,19 @@ class Correlator:
         i = self.info
         assert z.is_cuda and z.is_contiguous() and z.dtype == torch.complex64
         assert tuple(z.shape) == (i.channels, 2 * i.stations, i.n_spectra)
-        vis = torch.empty((i.channels, i.n_baselines, 2, 2), dtype=torch.complex64, device=z.device)
+        shape = (i.channels, i.n_baselines, 2, 2)
+        vis = torch.empty(shape if i.dumps == 1 else (i.dumps,) + shape, dtype=torch.complex64, device=z.device)
         _check(load().cobalt_debug_correlate(self._h, _stream_ptr(stream), z.data_ptr(), vis.data_ptr()), self._h)
         return vis
 
 
 def unpack(x, stream=None):
-    """Step a1 alone: int16/int8 CUDA tensor -> float32 CUDA tensor of the same shape."""
+    """Step a1 alone: int16/int8 CUDA tensor -> float32 CUDA tensor of the same shape; uint8 (4-bit packed complex
+    samples, reading A27) -> float32 [..., 2]."""
     import torch
 
-    assert x.is_cuda and x.is_contiguous() and x.dtype in (torch.int16, torch.int8)
-    out = torch.empty(x.shape, dtype=torch.float32, device=x.device)
-    bits = 16 if x.dtype == torch.int16 else 8
+    assert x.is_cuda and x.is_contiguous() and x.dtype in (torch.int16, torch.int8, torch.uint8)
+    out = torch.empty(x.shape + (2,) if x.dtype == torch.uint8 else x.shape, dtype=torch.float32, device=x.device)
+    bits = 16 if x.dtype == torch.int16 else 8 if x.dtype == torch.int8 else 4
     _check(load().cobalt_debug_unpack(_stream_ptr(stream), bits, x.data_ptr(), x.numel(), out.data_ptr()))
     return out

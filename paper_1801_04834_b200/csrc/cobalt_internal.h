@@ -69,7 +69,16 @@ struct StageEvents {
 }  // namespace cobalt
 
 struct cobalt_plan_s {
-    int S = 0, B = 0, C = 0, T = 0, bits = 0, mode = COBALT_MODE_TENSOR_FP16;
+    int S = 0, B = 0, C = 0, T = 0, bits = 0, mode = COBALT_MODE_TENSOR_FP16;   // bits: what the fused kernel reads (16 or 8)
+    int bits_in = 0;                   // what the caller passes (16, 8 or 4); 4 is expanded to 8 by the ingest pre-pass
+    int layout = COBALT_LAYOUT_PLANAR; // order of the caller's samples (cobalt_set_input_layout)
+    int dumps = 1;                     // D, cobalt_set_dumps
+    long long N_in = 0;                // stream stride of the caller's samples (cobalt_set_coarse_delays), >= N
+    int *d_coarse = nullptr;           // [S] first sample of each station's block, or nullptr (all zero)
+    float2 *d_poff = nullptr;          // [2S] exp(-i phase0) per stream, or nullptr (cobalt_set_phase_offsets)
+    void *d_ingest = nullptr;          // planar copy of one chunk for pol-minor / 4-bit input
+    int x_splits = 1;                  // X-stage: k-range of a (dump, subband, channel) split over this many jobs
+    float2 *d_xpart = nullptr;         // partial visibilities of the split jobs of one chunk
     long long N = 0, n_t = 0, N_u = 0, n_bl = 0;
     int M = 0, Mpad = 0, n_kt = 0;
     int chunk = 1;
@@ -86,7 +95,6 @@ struct cobalt_plan_s {
     int hist_cur = 0;
     float2 *d_phase = nullptr;         // [B][S][C]  s b[j] exp(-2 pi i frac(f tau)), built once per call
     float *d_dstep = nullptr;          // [B][S][C] phase step per spectrum in cycles (cobalt_process_interp)
-    const double *cur_delays_end = nullptr;   // device [S], set for the duration of cobalt_process_interp
     float *d_scale = nullptr;          // {s, 1/s, 1/s^2}: power-of-two scale of the fp16 intermediate (1 in EXACT mode)
     float amp_max = 0.f;               // worst-case |F| for full-scale input: sum|g| * sqrt(2) * 2^(bits-1)
     void *d_z = nullptr;               // intermediate of one chunk (layout per mode)
@@ -118,21 +126,33 @@ namespace cobalt {
 
 inline size_t sample_bytes(int bits) { return bits == 16 ? 4 : 2; }   // one complex sample
 
+// The per-call inputs beyond the plan (cobalt_io_t) as the launch helpers see them for one chunk.
+struct FCall {
+    const double *delays_end = nullptr;    // device [S] or nullptr (static delay)
+    const unsigned char *valid = nullptr;  // device [B][S][n_kt] or nullptr
+    const int *coarse = nullptr;           // device [S] or nullptr: first sample of each station's block
+    long long n_in = 0;                    // stream stride of the samples the fused kernel reads
+};
+
 // fstage.cu ---------------------------------------------------------------------------------
 cudaError_t launch_phase_table(const cobalt_plan_s *p, cudaStream_t st, const double *d_delays,
-                               const float *d_bandpass, int b0, int nb);
+                               const float *d_bandpass, int b0, int nb, const double *d_delays_end);
 // samples_b0 points at the first subband of the chunk [b0, b0 + nb)
-cudaError_t launch_fstage(const cobalt_plan_s *p, cudaStream_t st, const void *samples_b0, int b0, int nb);
-cudaError_t launch_history_update(const cobalt_plan_s *p, cudaStream_t st, const void *samples_b0, int b0, int nb);
+cudaError_t launch_fstage(const cobalt_plan_s *p, cudaStream_t st, const void *samples_b0, int b0, int nb, const FCall &call);
+cudaError_t launch_history_update(const cobalt_plan_s *p, cudaStream_t st, const void *samples_b0, int b0, int nb, const FCall &call);
 cudaError_t launch_unpack(cudaStream_t st, int bits, const void *d_in, long long n, float *d_out);
+// caller's order / width -> planar int16 / int8 [nb][2S][N] in d_out, coarse offsets applied (layout.cu)
+cudaError_t launch_ingest(const cobalt_plan_s *p, cudaStream_t st, const void *samples_b0, int nb, void *d_out);
+cudaError_t launch_valid_counts(const cobalt_plan_s *p, cudaStream_t st, const unsigned char *d_valid, int b0, int nb, unsigned int *d_counts);
 // layout.cu ---------------------------------------------------------------------------------
 cudaError_t launch_set_unit_scale(const cobalt_plan_s *p, cudaStream_t st);
 cudaError_t launch_z_to_float(const cobalt_plan_s *p, cudaStream_t st, const void *d_zsub, float2 *d_out);
 cudaError_t launch_float_to_z(const cobalt_plan_s *p, cudaStream_t st, const float2 *d_in, void *d_zsub);
 // xstage_simt.cu ----------------------------------------------------------------------------
-cudaError_t launch_xstage_simt(const cobalt_plan_s *p, cudaStream_t st, const void *d_z, int nb, float2 *d_vis);
+// d_vis points at subband b0 of dump 0; dump d is dump_stride float2 further
+cudaError_t launch_xstage_simt(const cobalt_plan_s *p, cudaStream_t st, const void *d_z, int nb, float2 *d_vis, size_t dump_stride);
 // xstage_tc.cu ------------------------------------------------------------------------------
 void build_xjobs(cobalt_plan_s *p);
-cudaError_t launch_xstage_tc(const cobalt_plan_s *p, cudaStream_t st, const void *d_z, int nb, float2 *d_vis);
+cudaError_t launch_xstage_tc(const cobalt_plan_s *p, cudaStream_t st, const void *d_z, int nb, float2 *d_vis, size_t dump_stride);
 
 }  // namespace cobalt

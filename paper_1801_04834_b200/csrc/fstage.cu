@@ -37,10 +37,15 @@ struct FArgs {
     const float *weights;           // [16][C]
     const float2 *phase;            // [nb][S][C]
     const float *dstep;             // [nb][S][C] phase step per spectrum in cycles (time-varying delay), or nullptr
+    const float2 *poff;             // [2S] exp(-i phase0) per stream (reading A22), or nullptr
+    const unsigned char *valid;     // [B][S][n_kt] valid-sample flags per 64-spectrum tile (reading A24), or nullptr
+    const int *coarse;              // [S] first sample of each station's block (reading A25), or nullptr
     unsigned char *z;               // chunk intermediate
-    long long N, n_t;
+    long long N, n_t;               // N = stream stride of `samples`
     size_t z_subband_bytes;
     int S, M, Mpad, n_kt, b0, tiles_per_seg, groups_per_subband;
+    int ipc;                        // items (groups of SPC streams) per CTA: 2 for C = 256 (both polarisations of a station
+                                    // share one rotation table), 1 otherwise and whenever the polarisations differ (poff)
 };
 
 // Packed fp32 pairs (fma.rn.f32x2 family, SASS FFMA2/FADD2/FMUL2): a complex value is one 64-bit
@@ -188,9 +193,8 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, con
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int grp = blockIdx.x;                          // stream group within the chunk
     const int bl = grp / a.groups_per_subband;
-    constexpr int IPC = Sh::IPC;
-    const int m0 = (grp - bl * a.groups_per_subband) * SPC * IPC;   // first stream of the CTA
-    const int n_items = min(IPC, (a.M - m0 + SPC - 1) / SPC);       // items of this CTA that exist
+    const int m0 = (grp - bl * a.groups_per_subband) * SPC * a.ipc;   // first stream of the CTA
+    const int n_items = min(a.ipc, (a.M - m0 + SPC - 1) / SPC);       // items of this CTA that exist
     const int kt0 = blockIdx.y * a.tiles_per_seg;
     const int kt1 = min(kt0 + a.tiles_per_seg, a.n_kt);
     const int n_sub = (kt1 - kt0) * (kKTile / kSubTile);
@@ -216,8 +220,9 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, con
         for (int idx = tid; idx < 256; idx += kFThreads) {
             const int sl = idx / C, rr = (idx % C) / 16, i = idx % 16;
             const int m = m0 + sl;
-            reinterpret_cast<float2 *>(smem + Sh::OFF_WTAB + (idx >> 4) * Sh::TAB_ROW)[i] =
-                m < a.M ? a.phase[((size_t)bl * a.S + (m >> 1)) * C + out_channel<R>(rr, i)] : make_float2(0.f, 0.f);
+            float2 w = m < a.M ? a.phase[((size_t)bl * a.S + (m >> 1)) * C + out_channel<R>(rr, i)] : make_float2(0.f, 0.f);
+            if (a.poff && m < a.M) w = cmul_tab2(w, a.poff[m]);      // clock / phase offset of this (station, polarisation)
+            reinterpret_cast<float2 *>(smem + Sh::OFF_WTAB + (idx >> 4) * Sh::TAB_ROW)[i] = w;
         }
         if (INTERP) {
             for (int idx = tid; idx < 256; idx += kFThreads) {
@@ -265,7 +270,7 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, con
                     } else {
                         lo = max(tb, 0ll);
                         hi = min(tb + kSubTile, a.n_t);
-                        src = a.samples + (stream * (size_t)a.N + (size_t)lo * C) * SB;
+                        src = a.samples + (stream * (size_t)a.N + (size_t)(a.coarse ? a.coarse[(mi + sl) >> 1] : 0) + (size_t)lo * C) * SB;
                     }
                     if (hi <= lo) continue;
                     const uint32_t bytes = (uint32_t)(hi - lo) * C * SB;
@@ -496,7 +501,9 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, con
             // steps a5-a7: rotate * bandpass, convert, stage transposed.  Spectra t >= n_t (padding of the last
             // k-tile) leave as exact zeros: the rotation table is replaced by zeros.
             const bool live0 = t_spec < a.n_t, live1 = t_spec + 1 < a.n_t;
-            const float4 *wt = live0 ? wtab4 : zero4;
+            // a lost tile (valid-sample flags, reading A24) leaves as exact zeros, like the padding
+            const bool lost = a.valid && m < a.M && a.valid[((size_t)(a.b0 + bl) * a.S + (m >> 1)) * a.n_kt + kt] == 0;
+            const float4 *wt = live0 && !lost ? wtab4 : zero4;
             if (TENSOR) {
                 const int tile = jjg >> 1, sbuf = tile & 1;
                 const int p = 8 * (jj & 1) + tp;          // pair of spectra within the 32-spectrum tile
@@ -619,7 +626,8 @@ __global__ void unit_scale_kernel(float *scale_out) {
 // 15 C consumed samples of (old history ++ block); raw integers, so the carry is bit-exact.
 template <typename W>
 __global__ void history_kernel(const W *__restrict__ samples, const W *__restrict__ hist_old, W *__restrict__ hist_new,
-                               long long streams, long long stream0, long long N, long long N_u, int HC) {
+                               long long streams, long long stream0, long long N, long long N_u, int HC,
+                               const int *__restrict__ coarse, int S) {
     const long long total = streams * HC;
     for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < total;
          idx += (long long)gridDim.x * blockDim.x) {
@@ -627,7 +635,8 @@ __global__ void history_kernel(const W *__restrict__ samples, const W *__restric
         const int i = (int)(idx - st * HC);
         const long long src = N_u - HC + i;
         const long long h = (stream0 + st) * HC;
-        hist_new[h + i] = src >= 0 ? samples[st * N + src] : hist_old[h + (HC + src)];
+        const long long off = coarse ? coarse[(st % (2 * S)) >> 1] : 0;   // reading A25: the block starts at this sample
+        hist_new[h + i] = src >= 0 ? samples[st * N + off + src] : hist_old[h + (HC + src)];
     }
 }
 
@@ -648,6 +657,14 @@ __global__ void history_vec_kernel(const uint4 *__restrict__ samples, uint4 *__r
 // component, taken as the low half of a word whose high half is zero).
 template <int BITS>
 __global__ void unpack_kernel(const unsigned char *__restrict__ in, long long n, float *__restrict__ out) {
+    if (BITS == 4) {                                   // n bytes = n complex samples -> 2 n floats (reading A27)
+        for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < n; idx += (long long)gridDim.x * blockDim.x) {
+            const float2 v = unpack_sample<4>(in[idx]);
+            out[2 * idx] = v.x;
+            out[2 * idx + 1] = v.y;
+        }
+        return;
+    }
     constexpr int SB = BITS == 16 ? 4 : 2;             // bytes per complex sample
     const long long pairs = n / 2;
     for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < pairs + (n & 1);
@@ -672,7 +689,8 @@ cudaError_t launch_f(const cobalt_plan_s *p, cudaStream_t st, const FArgs &a, in
     FArgs args = a;
     // One CTA per SM: enough CTAs for >= 8 waves when the chunk allows, as few time segments as
     // possible (each segment re-reads its 16 warm-up rows).
-    args.groups_per_subband = (p->M + Sh::SPC * Sh::IPC - 1) / (Sh::SPC * Sh::IPC);
+    args.ipc = a.poff ? 1 : Sh::IPC;     // per-polarisation phase offsets: one rotation table per stream
+    args.groups_per_subband = (p->M + Sh::SPC * args.ipc - 1) / (Sh::SPC * args.ipc);
     const long long groups = (long long)nb * args.groups_per_subband;
     const long long want = (long long)p->sm_count * 8;
     int n_seg = (int)((want + groups - 1) / groups);
@@ -700,14 +718,14 @@ cudaError_t launch_f_c(const cobalt_plan_s *p, cudaStream_t st, const FArgs &a, 
 }  // namespace
 
 cudaError_t launch_phase_table(const cobalt_plan_s *p, cudaStream_t st, const double *d_delays,
-                               const float *d_bandpass, int b0, int nb) {
+                               const float *d_bandpass, int b0, int nb, const double *d_delays_end) {
     const long long total = (long long)nb * p->S * p->C;
     const int threads = 256;
     long long blocks = (total + threads - 1) / threads;
     if (blocks > 4096) blocks = 4096;
     phase_table_kernel<<<(unsigned)blocks, threads, 0, st>>>(d_delays, d_bandpass, p->d_f_sb, b0, nb, p->S, p->C,
                                                              p->f_s, p->amp_max, p->mode == COBALT_MODE_TENSOR_FP16 ? 1 : 0,
-                                                             p->d_scale, p->d_phase, p->cur_delays_end, 1.0 / (double)p->n_t,
+                                                             p->d_scale, p->d_phase, d_delays_end, 1.0 / (double)p->n_t,
                                                              p->d_dstep);
     return cudaGetLastError();
 }
@@ -717,15 +735,18 @@ cudaError_t launch_set_unit_scale(const cobalt_plan_s *p, cudaStream_t st) {
     return cudaGetLastError();
 }
 
-cudaError_t launch_fstage(const cobalt_plan_s *p, cudaStream_t st, const void *samples_b0, int b0, int nb) {
+cudaError_t launch_fstage(const cobalt_plan_s *p, cudaStream_t st, const void *samples_b0, int b0, int nb, const FCall &call) {
     FArgs a;
     a.samples = static_cast<const unsigned char *>(samples_b0);
     a.hist = static_cast<const unsigned char *>(p->d_hist[p->hist_cur]);
     a.weights = p->d_weights;
     a.phase = p->d_phase + (size_t)b0 * p->S * p->C;
-    a.dstep = p->cur_delays_end ? p->d_dstep + (size_t)b0 * p->S * p->C : nullptr;
+    a.dstep = call.delays_end ? p->d_dstep + (size_t)b0 * p->S * p->C : nullptr;
+    a.poff = p->d_poff;
+    a.valid = call.valid;
+    a.coarse = call.coarse;
     a.z = static_cast<unsigned char *>(p->d_z);
-    a.N = p->N;
+    a.N = call.n_in;
     a.n_t = p->n_t;
     a.z_subband_bytes = p->z_subband_bytes;
     a.S = p->S;
@@ -742,7 +763,7 @@ cudaError_t launch_fstage(const cobalt_plan_s *p, cudaStream_t st, const void *s
     return cudaErrorInvalidValue;
 }
 
-cudaError_t launch_history_update(const cobalt_plan_s *p, cudaStream_t st, const void *samples_b0, int b0, int nb) {
+cudaError_t launch_history_update(const cobalt_plan_s *p, cudaStream_t st, const void *samples_b0, int b0, int nb, const FCall &call) {
     const long long streams = (long long)nb * p->M, stream0 = (long long)b0 * p->M;
     const int HC = (kTaps - 1) * p->C;
     const long long total = streams * HC;
@@ -752,23 +773,24 @@ cudaError_t launch_history_update(const cobalt_plan_s *p, cudaStream_t st, const
     const void *ho = p->d_hist[p->hist_cur];
     void *hn = p->d_hist[p->hist_cur ^ 1];
     const size_t sb = sample_bytes(p->bits);
-    if (p->N_u >= HC && (p->N * sb) % 16 == 0 && ((p->N_u - HC) * sb) % 16 == 0 && (HC * sb) % 16 == 0 &&
+    const long long N = call.n_in;
+    if (!call.coarse && p->N_u >= HC && (N * sb) % 16 == 0 && ((p->N_u - HC) * sb) % 16 == 0 && (HC * sb) % 16 == 0 &&
         (reinterpret_cast<uintptr_t>(samples_b0) & 15u) == 0) {
         const int hist_vecs = (int)(HC * sb / 16);
         long long vb = (streams * hist_vecs + threads - 1) / threads;
         if (vb > 65535) vb = 65535;
         history_vec_kernel<<<(unsigned)vb, threads, 0, st>>>(static_cast<const uint4 *>(samples_b0), static_cast<uint4 *>(hn), streams,
-                                                          stream0, (long long)(p->N * sb / 16), (long long)((p->N_u - HC) * sb / 16), hist_vecs);
+                                                          stream0, (long long)(N * sb / 16), (long long)((p->N_u - HC) * sb / 16), hist_vecs);
         return cudaGetLastError();
     }
     if (p->bits == 16)
         history_kernel<unsigned int><<<(unsigned)blocks, threads, 0, st>>>(
             static_cast<const unsigned int *>(samples_b0), static_cast<const unsigned int *>(ho),
-            static_cast<unsigned int *>(hn), streams, stream0, p->N, p->N_u, HC);
+            static_cast<unsigned int *>(hn), streams, stream0, N, p->N_u, HC, call.coarse, p->S);
     else
         history_kernel<unsigned short><<<(unsigned)blocks, threads, 0, st>>>(
             static_cast<const unsigned short *>(samples_b0), static_cast<const unsigned short *>(ho),
-            static_cast<unsigned short *>(hn), streams, stream0, p->N, p->N_u, HC);
+            static_cast<unsigned short *>(hn), streams, stream0, N, p->N_u, HC, call.coarse, p->S);
     return cudaGetLastError();
 }
 
@@ -779,7 +801,8 @@ cudaError_t launch_unpack(cudaStream_t st, int bits, const void *d_in, long long
     if (blocks > 65535) blocks = 65535;
     const unsigned char *in = static_cast<const unsigned char *>(d_in);
     if (bits == 16) unpack_kernel<16><<<(unsigned)blocks, threads, 0, st>>>(in, n, d_out);
-    else unpack_kernel<8><<<(unsigned)blocks, threads, 0, st>>>(in, n, d_out);
+    else if (bits == 8) unpack_kernel<8><<<(unsigned)blocks, threads, 0, st>>>(in, n, d_out);
+    else unpack_kernel<4><<<(unsigned)blocks, threads, 0, st>>>(in, n, d_out);
     return cudaGetLastError();
 }
 

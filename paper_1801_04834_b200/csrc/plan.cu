@@ -50,10 +50,19 @@ void build_weights(int C, std::vector<float> &w, double &sum_abs) {
     for (float v : w) sum_abs += std::fabs((double)v);
 }
 
-size_t subband_input_bytes(const cobalt_plan_s *p) { return (size_t)p->M * (size_t)p->N * sample_bytes(p->bits); }
+// bytes of one complex sample as the CALLER passes it (4-bit: one byte)
+size_t caller_sample_bytes(const cobalt_plan_s *p) { return p->bits_in == 16 ? 4 : p->bits_in == 8 ? 2 : 1; }
+// one subband of the caller's samples (stream stride N_in) / of one dump of the visibilities
+size_t subband_input_bytes(const cobalt_plan_s *p) { return (size_t)p->M * (size_t)p->N_in * caller_sample_bytes(p); }
 size_t subband_output_bytes(const cobalt_plan_s *p) { return (size_t)p->C * (size_t)p->n_bl * 4 * sizeof(float2); }
+// the fused kernel cannot read the caller's samples directly: pol-minor order or 4-bit samples go through launch_ingest
+bool needs_ingest(const cobalt_plan_s *p) { return p->layout != COBALT_LAYOUT_PLANAR || p->bits_in == 4; }
 
 void free_scratch(cobalt_plan_s *p) {
+    cudaFree(p->d_ingest);
+    cudaFree(p->d_xpart);
+    p->d_ingest = nullptr;
+    p->d_xpart = nullptr;
     cudaFree(p->d_z);
     cudaFree(p->d_dstep);
     p->d_dstep = nullptr;
@@ -122,6 +131,28 @@ int alloc_scratch(cobalt_plan_s *p, int chunk_request) {
     CK(p, cudaMemset(p->d_z, 0, (size_t)chunk * p->z_subband_bytes));   // zero rows 2S..Mpad stay zero forever
     CK(p, cudaMalloc(&p->d_phase, (size_t)p->B * p->S * p->C * sizeof(float2)));
     CK(p, cudaMalloc(&p->d_dstep, (size_t)p->B * p->S * p->C * sizeof(float)));
+    size_t extra = 0;
+    if (needs_ingest(p)) {
+        extra += (size_t)chunk * p->M * p->N * sample_bytes(p->bits);
+        CK(p, cudaMalloc(&p->d_ingest, (size_t)chunk * p->M * p->N * sample_bytes(p->bits)));
+    }
+    // X-stage in tensor mode: with fewer (dump, subband, channel) problems than two per SM each one's time range is split
+    // over up to 8 jobs whose partial blocks are added up afterwards (xstage_tc.cu)
+    p->x_splits = 1;
+    if (p->mode == COBALT_MODE_TENSOR_FP16) {
+        const long long probs = (long long)chunk * p->C * p->dumps * (long long)p->jobs.size();
+        if (probs < 2LL * p->sm_count) {
+            long long sp = (2LL * p->sm_count + probs - 1) / probs;
+            if (sp > 8) sp = 8;
+            if (sp > p->n_kt / p->dumps) sp = p->n_kt / p->dumps;
+            p->x_splits = sp < 1 ? 1 : (int)sp;
+        }
+        if (p->x_splits > 1) {
+            const size_t bytes = (size_t)chunk * p->C * p->dumps * p->x_splits * p->n_bl * 4 * sizeof(float2);
+            extra += bytes;
+            CK(p, cudaMalloc(&p->d_xpart, bytes));
+        }
+    }
     CK(p, cudaDeviceSynchronize());
     {
         const int rc = build_zmap(p);
@@ -129,25 +160,49 @@ int alloc_scratch(cobalt_plan_s *p, int chunk_request) {
     }
     const size_t hist = (size_t)p->B * p->M * (kTaps - 1) * p->C * sample_bytes(p->bits);
     p->scratch_bytes = (size_t)chunk * p->z_subband_bytes + (size_t)p->B * p->S * p->C * (sizeof(float2) + sizeof(float)) + 2 * hist +
-                       (size_t)kTaps * p->C * sizeof(float) + (size_t)p->B * sizeof(double);
+                       (size_t)kTaps * p->C * sizeof(float) + (size_t)p->B * sizeof(double) + extra;
     p->scratch_ok = true;
     return COBALT_OK;
 }
 
-// One chunk of subbands [b0, b0 + nb): samples_b0 / vis_b0 point at subband b0.
-int enqueue_chunk(cobalt_plan_s *p, cudaStream_t st, const void *samples_b0, const double *d_delays,
-                  const float *d_bandpass, float2 *vis_b0, int b0, int nb, StageEvents *ev) {
+// One chunk of subbands [b0, b0 + nb): samples_b0 / vis_b0 point at subband b0 (of dump 0); io holds the per-call pointers.
+int enqueue_chunk(cobalt_plan_s *p, cudaStream_t st, const void *samples_b0, const cobalt_io_t &io, float2 *vis_b0, int b0, int nb,
+                  StageEvents *ev) {
     if (ev) CK(p, cudaEventRecord(ev->e[0], st));
-    if (b0 == 0) CK(p, launch_phase_table(p, st, d_delays, d_bandpass, 0, p->B));   // every subband's table in one launch
+    if (b0 == 0) CK(p, launch_phase_table(p, st, io.delays, io.bandpass, 0, p->B, io.delays_end));   // every subband's table in one launch
     if (ev) CK(p, cudaEventRecord(ev->e[1], st));
-    CK(p, launch_fstage(p, st, samples_b0, b0, nb));
+    FCall call;
+    call.delays_end = io.delays_end;
+    call.valid = io.valid;
+    const void *fsamples = samples_b0;
+    int extra = 0;
+    if (needs_ingest(p)) {     // pol-minor order / 4-bit samples: re-ordered, widened, coarse offsets applied
+        CK(p, launch_ingest(p, st, samples_b0, nb, p->d_ingest));
+        fsamples = p->d_ingest;
+        call.coarse = nullptr;
+        call.n_in = p->N;
+        extra = 1;
+    } else {
+        call.coarse = p->d_coarse;
+        call.n_in = p->N_in;
+    }
+    CK(p, launch_fstage(p, st, fsamples, b0, nb, call));
     if (ev) CK(p, cudaEventRecord(ev->e[2], st));
-    CK(p, launch_history_update(p, st, samples_b0, b0, nb));
+    CK(p, launch_history_update(p, st, fsamples, b0, nb, call));
     if (ev) CK(p, cudaEventRecord(ev->e[3], st));
-    if (p->mode == COBALT_MODE_TENSOR_FP16) CK(p, launch_xstage_tc(p, st, p->d_z, nb, vis_b0));
-    else CK(p, launch_xstage_simt(p, st, p->d_z, nb, vis_b0));
+    const size_t dump_stride = (size_t)p->B * p->C * p->n_bl * 4;      // float2 between dumps
+    if (p->mode == COBALT_MODE_TENSOR_FP16) {
+        CK(p, launch_xstage_tc(p, st, p->d_z, nb, vis_b0, dump_stride));
+        if (p->x_splits > 1) extra += 1;
+    } else {
+        CK(p, launch_xstage_simt(p, st, p->d_z, nb, vis_b0, dump_stride));
+    }
+    if (io.valid_counts) {
+        CK(p, launch_valid_counts(p, st, io.valid, b0, nb, io.valid_counts));
+        extra += 1;
+    }
     if (ev) CK(p, cudaEventRecord(ev->e[4], st));
-    p->launches += b0 == 0 ? 4 : 3;
+    p->launches += (b0 == 0 ? 4 : 3) + extra;
     return COBALT_OK;
 }
 
@@ -186,7 +241,7 @@ int cobalt_plan(cobalt_plan_t **out, int stations, int subbands, int channels, i
     if (channels != 16 && channels != 64 && channels != 256)
         return fail(nullptr, COBALT_ERR_BAD_ARG, "channels must be 16, 64 or 256");
     if (taps != kTaps) return fail(nullptr, COBALT_ERR_BAD_ARG, "taps must be 16");
-    if (input_bits != 16 && input_bits != 8) return fail(nullptr, COBALT_ERR_BAD_ARG, "input_bits must be 16 or 8");
+    if (input_bits != 16 && input_bits != 8 && input_bits != 4) return fail(nullptr, COBALT_ERR_BAD_ARG, "input_bits must be 16, 8 or 4");
     if (samples_per_integration < channels)
         return fail(nullptr, COBALT_ERR_BAD_ARG, "samples_per_integration must be >= channels");
     if (samples_per_integration / channels > (1ll << 30))
@@ -211,8 +266,10 @@ int cobalt_plan(cobalt_plan_t **out, int stations, int subbands, int channels, i
     p->B = subbands;
     p->C = channels;
     p->T = taps;
-    p->bits = input_bits;
+    p->bits_in = input_bits;
+    p->bits = input_bits == 16 ? 16 : 8;      // 4-bit samples are expanded to int8 by the ingest pre-pass
     p->N = samples_per_integration;
+    p->N_in = p->N;
     p->n_t = p->N / p->C;
     p->N_u = p->n_t * p->C;
     p->n_bl = (long long)stations * (stations + 1) / 2;
@@ -226,7 +283,7 @@ int cobalt_plan(cobalt_plan_t **out, int stations, int subbands, int channels, i
     double sum_abs_g = 0.0;
     build_weights(p->C, p->h_weights, sum_abs_g);
     // worst-case modulus of a channelised sample for full-scale input: sum|g| sqrt(2) 2^(bits-1)
-    p->amp_max = (float)(sum_abs_g * 1.4142135623730951 * (input_bits == 16 ? 32768.0 : 128.0));
+    p->amp_max = (float)(sum_abs_g * 1.4142135623730951 * (input_bits == 16 ? 32768.0 : input_bits == 8 ? 128.0 : 8.0));
     build_xjobs(p);
 
     int rc = COBALT_OK;
@@ -268,6 +325,8 @@ int cobalt_destroy(cobalt_plan_t *p) {
     cudaFree(p->d_hist[1]);
     cudaFree(p->d_jobs);
     cudaFree(p->d_scale);
+    cudaFree(p->d_coarse);
+    cudaFree(p->d_poff);
     cudaFree(p->d_delays_h);
     cudaFree(p->d_bandpass_h);
     for (auto &e : p->events)
@@ -283,14 +342,13 @@ int cobalt_destroy(cobalt_plan_t *p) {
     return COBALT_OK;
 }
 
-int cobalt_process(cobalt_plan_t *p, void *cuda_stream, const void *d_samples, const double *d_delays,
-                   const float *d_bandpass, void *d_visibilities) {
+int cobalt_process_ex(cobalt_plan_t *p, void *cuda_stream, const cobalt_io_t *io) {
     if (!p) return fail(nullptr, COBALT_ERR_BAD_ARG, "plan is NULL");
-    if (!d_samples || !d_delays || !d_bandpass || !d_visibilities) return fail(p, COBALT_ERR_BAD_ARG, "NULL buffer");
+    if (!io || !io->samples || !io->delays || !io->bandpass || !io->visibilities) return fail(p, COBALT_ERR_BAD_ARG, "NULL buffer");
     if (!p->scratch_ok) return fail(p, COBALT_ERR_NO_MEMORY, "the plan has no scratch (an earlier cobalt_set_mode / cobalt_set_chunk_subbands failed)");
-    if ((reinterpret_cast<uintptr_t>(d_samples) & (sample_bytes(p->bits) - 1)) != 0)
+    if ((reinterpret_cast<uintptr_t>(io->samples) & (caller_sample_bytes(p) - 1)) != 0)
         return fail(p, COBALT_ERR_BAD_ARG, "d_samples must be aligned to one complex sample");
-    if (p->mode == COBALT_MODE_TENSOR_FP16 && (reinterpret_cast<uintptr_t>(d_visibilities) & 15u) != 0)
+    if (p->mode == COBALT_MODE_TENSOR_FP16 && (reinterpret_cast<uintptr_t>(io->visibilities) & 15u) != 0)
         return fail(p, COBALT_ERR_BAD_ARG, "d_visibilities must be 16-byte aligned in COBALT_MODE_TENSOR_FP16");
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     const int n_chunks = (p->B + p->chunk - 1) / p->chunk;
@@ -303,9 +361,9 @@ int cobalt_process(cobalt_plan_t *p, void *cuda_stream, const void *d_samples, c
     for (int ci = 0; ci < n_chunks; ++ci) {
         const int b0 = ci * p->chunk;
         const int nb = (p->B - b0) < p->chunk ? (p->B - b0) : p->chunk;
-        const unsigned char *sm = static_cast<const unsigned char *>(d_samples) + (size_t)b0 * subband_input_bytes(p);
-        float2 *vis = reinterpret_cast<float2 *>(static_cast<unsigned char *>(d_visibilities) + (size_t)b0 * subband_output_bytes(p));
-        int rc = enqueue_chunk(p, st, sm, d_delays, d_bandpass, vis, b0, nb, p->timing ? &p->events[ci] : nullptr);
+        const unsigned char *sm = static_cast<const unsigned char *>(io->samples) + (size_t)b0 * subband_input_bytes(p);
+        float2 *vis = reinterpret_cast<float2 *>(static_cast<unsigned char *>(io->visibilities) + (size_t)b0 * subband_output_bytes(p));
+        int rc = enqueue_chunk(p, st, sm, *io, vis, b0, nb, p->timing ? &p->events[ci] : nullptr);
         if (rc != COBALT_OK) return rc;
     }
     if (p->timing) p->n_chunks_timed = n_chunks;
@@ -313,14 +371,26 @@ int cobalt_process(cobalt_plan_t *p, void *cuda_stream, const void *d_samples, c
     return COBALT_OK;
 }
 
+int cobalt_process(cobalt_plan_t *p, void *cuda_stream, const void *d_samples, const double *d_delays,
+                   const float *d_bandpass, void *d_visibilities) {
+    cobalt_io_t io{};
+    io.samples = d_samples;
+    io.delays = d_delays;
+    io.bandpass = d_bandpass;
+    io.visibilities = d_visibilities;
+    return cobalt_process_ex(p, cuda_stream, &io);
+}
+
 int cobalt_process_interp(cobalt_plan_t *p, void *cuda_stream, const void *d_samples, const double *d_delays_begin,
                           const double *d_delays_end, const float *d_bandpass, void *d_visibilities) {
-    if (!p) return fail(nullptr, COBALT_ERR_BAD_ARG, "plan is NULL");
-    if (!d_delays_end) return fail(p, COBALT_ERR_BAD_ARG, "NULL buffer");
-    p->cur_delays_end = d_delays_end;      // read by the launch helpers of this call only
-    const int rc = cobalt_process(p, cuda_stream, d_samples, d_delays_begin, d_bandpass, d_visibilities);
-    p->cur_delays_end = nullptr;
-    return rc;
+    if (p && !d_delays_end) return fail(p, COBALT_ERR_BAD_ARG, "NULL buffer");
+    cobalt_io_t io{};
+    io.samples = d_samples;
+    io.delays = d_delays_begin;
+    io.delays_end = d_delays_end;
+    io.bandpass = d_bandpass;
+    io.visibilities = d_visibilities;
+    return cobalt_process_ex(p, cuda_stream, &io);
 }
 
 int cobalt_process_host(cobalt_plan_t *p, const void *h_samples, const double *h_delays, const float *h_bandpass,
@@ -328,6 +398,7 @@ int cobalt_process_host(cobalt_plan_t *p, const void *h_samples, const double *h
     if (!p) return fail(nullptr, COBALT_ERR_BAD_ARG, "plan is NULL");
     if (!h_samples || !h_delays || !h_bandpass || !h_visibilities) return fail(p, COBALT_ERR_BAD_ARG, "NULL buffer");
     if (!p->scratch_ok) return fail(p, COBALT_ERR_NO_MEMORY, "the plan has no scratch (an earlier cobalt_set_mode / cobalt_set_chunk_subbands failed)");
+    if (p->dumps != 1) return fail(p, COBALT_ERR_BAD_ARG, "cobalt_process_host writes one dump per block (cobalt_set_dumps(plan, 1))");
     const size_t in_b = subband_input_bytes(p), out_b = subband_output_bytes(p);
     if (!p->hs[0]) {
         for (int i = 0; i < 3; ++i) CK(p, cudaStreamCreateWithFlags(&p->hs[i], cudaStreamNonBlocking));
@@ -375,8 +446,10 @@ int cobalt_process_host(cobalt_plan_t *p, const void *h_samples, const double *h
         CKH(cudaEventRecord(p->ev_in[buf], s_in));
         CKH(cudaStreamWaitEvent(s_cmp, p->ev_in[buf], 0));
         if (ci >= 2) CKH(cudaStreamWaitEvent(s_cmp, p->ev_out[buf], 0));    // d_out[buf] drained
-        int rc = enqueue_chunk(p, s_cmp, p->d_in[buf], p->d_delays_h, p->d_bandpass_h,
-                               static_cast<float2 *>(p->d_out[buf]), b0, nb, nullptr);
+        cobalt_io_t io{};
+        io.delays = p->d_delays_h;
+        io.bandpass = p->d_bandpass_h;
+        int rc = enqueue_chunk(p, s_cmp, p->d_in[buf], io, static_cast<float2 *>(p->d_out[buf]), b0, nb, nullptr);
         if (rc != COBALT_OK) return drain(rc);
         CKH(cudaEventRecord(p->ev_cmp[buf], s_cmp));
         CKH(cudaStreamWaitEvent(s_out, p->ev_cmp[buf], 0));
@@ -414,6 +487,63 @@ int cobalt_set_sample_rate(cobalt_plan_t *p, double hz) {
     return COBALT_OK;
 }
 
+int cobalt_set_phase_offsets(cobalt_plan_t *p, const double *h_phase0) {
+    if (!p) return fail(nullptr, COBALT_ERR_BAD_ARG, "plan is NULL");
+    CK(p, cudaDeviceSynchronize());
+    if (!h_phase0) {
+        cudaFree(p->d_poff);
+        p->d_poff = nullptr;
+        return COBALT_OK;
+    }
+    std::vector<float2> w((size_t)p->M);
+    for (int m = 0; m < p->M; ++m) {
+        if (!(h_phase0[m] == h_phase0[m]) || std::fabs(h_phase0[m]) > 1e9) return fail(p, COBALT_ERR_BAD_ARG, "phase offset not finite");
+        w[m] = make_float2((float)std::cos(h_phase0[m]), (float)-std::sin(h_phase0[m]));   // exp(-i phase0), reading A22
+    }
+    if (!p->d_poff) CK(p, cudaMalloc(&p->d_poff, (size_t)p->M * sizeof(float2)));
+    CK(p, cudaMemcpy(p->d_poff, w.data(), (size_t)p->M * sizeof(float2), cudaMemcpyHostToDevice));
+    return COBALT_OK;
+}
+
+int cobalt_set_coarse_delays(cobalt_plan_t *p, const int *h_offsets, long long samples_allocated) {
+    if (!p) return fail(nullptr, COBALT_ERR_BAD_ARG, "plan is NULL");
+    CK(p, cudaDeviceSynchronize());
+    if (!h_offsets) {
+        cudaFree(p->d_coarse);
+        p->d_coarse = nullptr;
+        p->N_in = p->N;
+        return COBALT_OK;
+    }
+    if (samples_allocated < p->N) return fail(p, COBALT_ERR_BAD_ARG, "samples_allocated must be >= samples_per_integration");
+    for (int a = 0; a < p->S; ++a)
+        if (h_offsets[a] < 0 || (long long)h_offsets[a] + p->N > samples_allocated)
+            return fail(p, COBALT_ERR_BAD_ARG, "coarse delay outside [0, samples_allocated - samples_per_integration]");
+    if (!p->d_coarse) CK(p, cudaMalloc(&p->d_coarse, (size_t)p->S * sizeof(int)));
+    CK(p, cudaMemcpy(p->d_coarse, h_offsets, (size_t)p->S * sizeof(int), cudaMemcpyHostToDevice));
+    p->N_in = samples_allocated;
+    cudaFree(p->d_in[0]);     // the host-path staging buffers are sized by the stream stride
+    cudaFree(p->d_in[1]);
+    p->d_in[0] = p->d_in[1] = nullptr;
+    return COBALT_OK;
+}
+
+int cobalt_set_dumps(cobalt_plan_t *p, int dumps) {
+    if (!p) return fail(nullptr, COBALT_ERR_BAD_ARG, "plan is NULL");
+    if (dumps < 1 || p->n_kt % dumps != 0) return fail(p, COBALT_ERR_BAD_ARG, "dumps_per_block must divide ceil(n_t / 64)");
+    if (dumps == p->dumps) return COBALT_OK;
+    CK(p, cudaDeviceSynchronize());
+    p->dumps = dumps;
+    return alloc_scratch(p, p->chunk);
+}
+
+int cobalt_set_input_layout(cobalt_plan_t *p, int layout) {
+    if (!p || (layout != COBALT_LAYOUT_PLANAR && layout != COBALT_LAYOUT_POL_MINOR)) return fail(p, COBALT_ERR_BAD_ARG, "unknown layout");
+    if (layout == p->layout) return COBALT_OK;
+    CK(p, cudaDeviceSynchronize());
+    p->layout = layout;
+    return alloc_scratch(p, p->chunk);
+}
+
 int cobalt_set_mode(cobalt_plan_t *p, int mode) {
     if (!p || (mode != COBALT_MODE_TENSOR_FP16 && mode != COBALT_MODE_EXACT_FP32)) return fail(p, COBALT_ERR_BAD_ARG, "unknown mode");
     if (mode == p->mode) return COBALT_OK;
@@ -444,18 +574,21 @@ int cobalt_info(const cobalt_plan_t *p, cobalt_info_t *info) {
     info->subbands = p->B;
     info->channels = p->C;
     info->taps = p->T;
-    info->input_bits = p->bits;
+    info->input_bits = p->bits_in;
     info->mode = p->mode;
     info->samples_per_integration = p->N;
     info->n_spectra = p->n_t;
     info->n_consumed = p->N_u;
     info->n_baselines = p->n_bl;
     info->input_bytes = (long long)((size_t)p->B * subband_input_bytes(p));
-    info->output_bytes = (long long)((size_t)p->B * subband_output_bytes(p));
+    info->output_bytes = (long long)((size_t)p->dumps * p->B * subband_output_bytes(p));
     info->scratch_bytes = (long long)p->scratch_bytes;
     info->chunk_subbands = p->chunk;
     info->sm_count = p->sm_count;
     info->sample_rate_hz = p->f_s;
+    info->dumps = p->dumps;
+    info->n_tiles = p->n_kt;
+    info->samples_allocated = p->N_in;
     return COBALT_OK;
 }
 
@@ -499,7 +632,7 @@ int cobalt_debug_fir_weights(const cobalt_plan_t *p, float *h_weights) {
 }
 
 int cobalt_debug_unpack(void *cuda_stream, int input_bits, const void *d_in, long long n, float *d_out) {
-    if ((input_bits != 16 && input_bits != 8) || n < 0 || (n > 0 && (!d_in || !d_out)))
+    if ((input_bits != 16 && input_bits != 8 && input_bits != 4) || n < 0 || (n > 0 && (!d_in || !d_out)))
         return fail(nullptr, COBALT_ERR_BAD_ARG, "bad unpack arguments");
     CK(nullptr, launch_unpack(static_cast<cudaStream_t>(cuda_stream), input_bits, d_in, n, d_out));
     return COBALT_OK;
@@ -511,8 +644,18 @@ int cobalt_debug_channelised(cobalt_plan_t *p, void *cuda_stream, const void *d_
     if (sb < 0 || sb >= p->B) return fail(p, COBALT_ERR_BAD_ARG, "subband out of range");
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     const unsigned char *sm = static_cast<const unsigned char *>(d_samples) + (size_t)sb * subband_input_bytes(p);
-    CK(p, launch_phase_table(p, st, d_delays, d_bandpass, sb, 1));
-    CK(p, launch_fstage(p, st, sm, sb, 1));
+    CK(p, launch_phase_table(p, st, d_delays, d_bandpass, sb, 1, nullptr));
+    FCall call;
+    const void *fsamples = sm;
+    if (needs_ingest(p)) {
+        CK(p, launch_ingest(p, st, sm, 1, p->d_ingest));
+        fsamples = p->d_ingest;
+        call.n_in = p->N;
+    } else {
+        call.coarse = p->d_coarse;
+        call.n_in = p->N_in;
+    }
+    CK(p, launch_fstage(p, st, fsamples, sb, 1, call));
     CK(p, launch_z_to_float(p, st, p->d_z, static_cast<float2 *>(d_z)));
     return COBALT_OK;
 }
@@ -522,8 +665,9 @@ int cobalt_debug_correlate(cobalt_plan_t *p, void *cuda_stream, const void *d_z,
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     CK(p, launch_set_unit_scale(p, st));   // caller-supplied operands are taken as they are
     CK(p, launch_float_to_z(p, st, static_cast<const float2 *>(d_z), p->d_z));
-    if (p->mode == COBALT_MODE_TENSOR_FP16) CK(p, launch_xstage_tc(p, st, p->d_z, 1, static_cast<float2 *>(d_vis)));
-    else CK(p, launch_xstage_simt(p, st, p->d_z, 1, static_cast<float2 *>(d_vis)));
+    const size_t dump_stride = (size_t)p->C * p->n_bl * 4;     // one subband: [D][C][n_bl][2][2]
+    if (p->mode == COBALT_MODE_TENSOR_FP16) CK(p, launch_xstage_tc(p, st, p->d_z, 1, static_cast<float2 *>(d_vis), dump_stride));
+    else CK(p, launch_xstage_simt(p, st, p->d_z, 1, static_cast<float2 *>(d_vis), dump_stride));
     return COBALT_OK;
 }
 

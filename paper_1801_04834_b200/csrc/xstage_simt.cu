@@ -15,7 +15,8 @@ namespace {
 constexpr int kTile = 32, kTk = 16;
 
 __global__ void __launch_bounds__(256) xstage_simt_kernel(const float2 *__restrict__ z, float2 *__restrict__ vis, int C,
-                                                         int M, long long n_t, long long n_bl, size_t z_sub_elems) {
+                                                         int M, long long n_t, long long n_bl, size_t z_sub_elems, int nb,
+                                                         long long dump_len, size_t dump_stride) {
     __shared__ float2 As[kTk][kTile + 1];
     __shared__ float2 Bs[kTk][kTile + 1];
     const int pair = blockIdx.x;
@@ -23,7 +24,9 @@ __global__ void __launch_bounds__(256) xstage_simt_kernel(const float2 *__restri
     while (tj * (tj + 1) / 2 > pair) --tj;
     while ((tj + 1) * (tj + 2) / 2 <= pair) ++tj;
     const int ti = pair - tj * (tj + 1) / 2;
-    const int c = blockIdx.y, bl = blockIdx.z;
+    // blockIdx.z = dump * nb + subband of the chunk; dump d integrates the spectra [d dump_len, min((d + 1) dump_len, n_t))
+    const int c = blockIdx.y, d = blockIdx.z / nb, bl = blockIdx.z - d * nb;
+    const long long t_begin = (long long)d * dump_len, t_end = min(n_t, t_begin + dump_len);
     const float2 *zc = z + (size_t)bl * z_sub_elems + (size_t)c * M * n_t;
     const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
 
@@ -33,14 +36,14 @@ __global__ void __launch_bounds__(256) xstage_simt_kernel(const float2 *__restri
 #pragma unroll
         for (int v = 0; v < 2; ++v) acc[u][v] = make_float2(0.f, 0.f);
 
-    for (long long t0 = 0; t0 < n_t; t0 += kTk) {
+    for (long long t0 = t_begin; t0 < t_end; t0 += kTk) {
 #pragma unroll
         for (int e = tid; e < kTile * kTk; e += 256) {
             const int tt = e & (kTk - 1), row = e >> 4;
             const long long t = t0 + tt;
             const int ra = ti * kTile + row, rb = tj * kTile + row;
-            As[tt][row] = (ra < M && t < n_t) ? zc[(size_t)ra * n_t + t] : make_float2(0.f, 0.f);
-            Bs[tt][row] = (rb < M && t < n_t) ? zc[(size_t)rb * n_t + t] : make_float2(0.f, 0.f);
+            As[tt][row] = (ra < M && t < t_end) ? zc[(size_t)ra * n_t + t] : make_float2(0.f, 0.f);
+            Bs[tt][row] = (rb < M && t < t_end) ? zc[(size_t)rb * n_t + t] : make_float2(0.f, 0.f);
         }
         __syncthreads();
 #pragma unroll
@@ -60,7 +63,7 @@ __global__ void __launch_bounds__(256) xstage_simt_kernel(const float2 *__restri
         }
         __syncthreads();
     }
-    float2 *vc = vis + ((size_t)bl * C + c) * n_bl * 4;
+    float2 *vc = vis + (size_t)d * dump_stride + ((size_t)bl * C + c) * n_bl * 4;
 #pragma unroll
     for (int u = 0; u < 2; ++u)
 #pragma unroll
@@ -73,11 +76,11 @@ __global__ void __launch_bounds__(256) xstage_simt_kernel(const float2 *__restri
 
 }  // namespace
 
-cudaError_t launch_xstage_simt(const cobalt_plan_s *p, cudaStream_t st, const void *d_z, int nb, float2 *d_vis) {
+cudaError_t launch_xstage_simt(const cobalt_plan_s *p, cudaStream_t st, const void *d_z, int nb, float2 *d_vis, size_t dump_stride) {
     const int ntile = (p->M + kTile - 1) / kTile;
-    dim3 grid((unsigned)(ntile * (ntile + 1) / 2), (unsigned)p->C, (unsigned)nb);
+    dim3 grid((unsigned)(ntile * (ntile + 1) / 2), (unsigned)p->C, (unsigned)(nb * p->dumps));
     xstage_simt_kernel<<<grid, 256, 0, st>>>(static_cast<const float2 *>(d_z), d_vis, p->C, p->M, p->n_t, p->n_bl,
-                                             p->z_subband_bytes / sizeof(float2));
+                                             p->z_subband_bytes / sizeof(float2), nb, (long long)(p->n_kt / p->dumps) * kKTile, dump_stride);
     return cudaGetLastError();
 }
 

@@ -45,7 +45,30 @@ struct XArgs {
     long long n_bl;
     int C, M, Mpad, n_kt, jobs_per_channel, total_jobs, stages, stage_bytes;
     uint32_t out_off;       // STAGED: byte offset of the visibility staging block from the 1024-aligned smem base
+    // dumps (reading A23) and split time ranges: job id = ((dump * nbC + subband-of-chunk * C + channel) * splits + split) *
+    // jobs_per_channel + job-of-channel; it integrates the k-tiles [dump * K + K split / splits, dump * K + K (split + 1) / splits)
+    float2 *part;           // splits > 1: partial visibilities, one channel block per (dump, subband, channel, split)
+    size_t dump_stride;     // float2 between the dumps of `vis`
+    int D, K, splits, nbC;
 };
+
+struct XWork {
+    int jl, prob, kt0, nkt;
+    float2 *out;
+};
+__device__ __forceinline__ XWork decode_job(const XArgs &a, int jid) {
+    XWork w;
+    w.jl = jid % a.jobs_per_channel;
+    const int slot = jid / a.jobs_per_channel;
+    const int sp = slot % a.splits, j = slot / a.splits;
+    const int d = j / a.nbC;
+    w.prob = j - d * a.nbC;
+    const int k0 = (a.K * sp) / a.splits, k1 = (a.K * (sp + 1)) / a.splits;
+    w.kt0 = d * a.K + k0;
+    w.nkt = k1 - k0;
+    w.out = a.splits > 1 ? a.part + (size_t)slot * a.n_bl * 4 : a.vis + (size_t)d * a.dump_stride + (size_t)w.prob * a.n_bl * 4;
+    return w;
+}
 
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
@@ -137,13 +160,13 @@ __global__ void __launch_bounds__(kThreads, 1) xstage_tc_kernel(const XArgs a) {
             uint32_t ph = 0;
             const size_t kt_bytes = (size_t)a.Mpad * 256;     // [Mpad / 8][2 planes][8 rows][128 B]
             for (int jid = blockIdx.x; jid < a.total_jobs; jid += gridDim.x) {
-                const int jl = jid % a.jobs_per_channel;
-                const int prob = jid / a.jobs_per_channel;           // subband-of-chunk * C + channel
-                const int bl = prob / a.C, c = prob - bl * a.C;
+                const XWork w = decode_job(a, jid);
+                const int jl = w.jl;
+                const int bl = w.prob / a.C, c = w.prob - bl * a.C;   // prob = subband-of-chunk * C + channel
                 const int r0 = jobs[jl].ld_row[0], r1 = jobs[jl].ld_row[1];
                 const uint32_t b0 = (uint32_t)jobs[jl].ld_nrows[0] * 256, b1 = (uint32_t)jobs[jl].ld_nrows[1] * 256;
-                const unsigned char *src = a.z + (size_t)bl * a.z_subband_bytes + (size_t)c * a.n_kt * kt_bytes;
-                for (int kt = 0; kt < a.n_kt; ++kt, src += kt_bytes) {
+                const unsigned char *src = a.z + (size_t)bl * a.z_subband_bytes + ((size_t)c * a.n_kt + w.kt0) * kt_bytes;
+                for (int kt = 0; kt < w.nkt; ++kt, src += kt_bytes) {
                     mbar_wait(bar_base + 8 * (16 + s), ph ^ 1);
                     const uint32_t full = bar_base + 8 * s;
                     const uint32_t dst = stage_base + (uint32_t)s * a.stage_bytes;
@@ -168,7 +191,8 @@ __global__ void __launch_bounds__(kThreads, 1) xstage_tc_kernel(const XArgs a) {
             const uint64_t desc_both = make_smem_desc(stage_base, 1024);    // [Zr; Zi] stacked 8 rows at a time
             const uint32_t stage_units = (uint32_t)a.stage_bytes >> 4;
             for (int jid = blockIdx.x; jid < a.total_jobs; jid += gridDim.x, ++it) {
-                const XJob *job = jobs + jid % a.jobs_per_channel;
+                const XWork w = decode_job(a, jid);
+                const XJob *job = jobs + w.jl;
                 const int n_groups = job->n_groups;
                 uint32_t g_a[kMaxMmaGroups], g_b[kMaxMmaGroups], g_d[kMaxMmaGroups], g_n[kMaxMmaGroups];
                 uint32_t g_pos[kMaxMmaGroups], g_neg[kMaxMmaGroups], g_kind[kMaxMmaGroups];
@@ -185,7 +209,7 @@ __global__ void __launch_bounds__(kThreads, 1) xstage_tc_kernel(const XArgs a) {
                 }
                 mbar_wait_spin(tmem_empty, (it & 1) ^ 1);  // epilogue has drained the accumulators
                 tc_fence_after();
-                for (int kt = 0; kt < a.n_kt; ++kt) {
+                for (int kt = 0; kt < w.nkt; ++kt) {
                     mbar_wait(bar_base + 8 * s, ph);
                     tc_fence_after();
                     const uint64_t so = (uint64_t)((uint32_t)s * stage_units);
@@ -230,11 +254,10 @@ __global__ void __launch_bounds__(kThreads, 1) xstage_tc_kernel(const XArgs a) {
         const float inv_s2 = __ldg(a.scale + 2);           // undo the power-of-two operand scale (exact)
         uint32_t it = 0;
         for (int jid = blockIdx.x; jid < a.total_jobs; jid += gridDim.x, ++it) {
-            const int jl = jid % a.jobs_per_channel;
-            const int prob = jid / a.jobs_per_channel;
-            const XJob *job = jobs + jl;
+            const XWork w = decode_job(a, jid);
+            const XJob *job = jobs + w.jl;
             const int n_groups = job->n_groups;
-            float4 *vg = reinterpret_cast<float4 *>(a.vis + (size_t)prob * a.n_bl * 4);
+            float4 *vg = reinterpret_cast<float4 *>(w.out);
             float4 *vc = STAGED ? reinterpret_cast<float4 *>(smem_raw + (smem_base - smem_u32(smem_raw)) + a.out_off) : vg;
             if (STAGED && it > 0) {
                 // the previous job's bulk store must have read the staging block before it is overwritten
@@ -446,7 +469,9 @@ void build_xjobs(cobalt_plan_s *p) {
     p->x_smem_bytes = fixed + (size_t)stages * stage_bytes + out_bytes;
 }
 
-cudaError_t launch_xstage_tc(const cobalt_plan_s *p, cudaStream_t st, const void *d_z, int nb, float2 *d_vis) {
+cudaError_t launch_xsum_n(const cobalt_plan_s *p, cudaStream_t st, int nb, float2 *d_vis, size_t dump_stride, int splits);   // ingest.cu
+
+cudaError_t launch_xstage_tc(const cobalt_plan_s *p, cudaStream_t st, const void *d_z, int nb, float2 *d_vis, size_t dump_stride) {
     if (p->x_stages < 2) return cudaErrorInvalidConfiguration;
     XArgs a;
     a.z = static_cast<const unsigned char *>(d_z);
@@ -460,7 +485,21 @@ cudaError_t launch_xstage_tc(const cobalt_plan_s *p, cudaStream_t st, const void
     a.Mpad = p->Mpad;
     a.n_kt = p->n_kt;
     a.jobs_per_channel = (int)p->jobs.size();
-    a.total_jobs = nb * p->C * a.jobs_per_channel;
+    a.D = p->dumps;
+    a.K = p->n_kt / p->dumps;
+    a.nbC = nb * p->C;
+    // too few (dump, subband, channel) problems to fill the SMs (config 2: 64 channels on 148 SMs): split each one's time
+    // range over several jobs, into partial blocks that xsum_kernel adds up
+    a.splits = 1;
+    if (p->d_xpart && (long long)a.nbC * a.D * a.jobs_per_channel < 2 * p->sm_count) {
+        a.splits = (int)((2LL * p->sm_count + (long long)a.nbC * a.D * a.jobs_per_channel - 1) / ((long long)a.nbC * a.D * a.jobs_per_channel));
+        if (a.splits > p->x_splits) a.splits = p->x_splits;
+        if (a.splits > a.K) a.splits = a.K;
+        if (a.splits < 1) a.splits = 1;
+    }
+    a.part = p->d_xpart;
+    a.dump_stride = dump_stride;
+    a.total_jobs = a.nbC * a.D * a.splits * a.jobs_per_channel;
     a.stages = p->x_stages;
     int max_rows = 0;
     for (const XJob &j : p->jobs) max_rows = (j.ld_nrows[0] + j.ld_nrows[1]) > max_rows ? (j.ld_nrows[0] + j.ld_nrows[1]) : max_rows;
@@ -471,7 +510,9 @@ cudaError_t launch_xstage_tc(const cobalt_plan_s *p, cudaStream_t st, const void
     if (e != cudaSuccess) return e;
     const int grid = a.total_jobs < p->sm_count ? a.total_jobs : p->sm_count;
     kern<<<grid, kThreads, p->x_smem_bytes, st>>>(a);
-    return cudaGetLastError();
+    e = cudaGetLastError();
+    if (e != cudaSuccess || a.splits == 1) return e;
+    return launch_xsum_n(p, st, nb, d_vis, dump_stride, a.splits);
 }
 
 }  // namespace cobalt

@@ -38,7 +38,7 @@ def test_strerror_and_null_destroy(cobalt):
     (4, 1, 32, 16, 6400, 16),      # channels not in {16, 64, 256}
     (4, 1, 64, 8, 6400, 16),       # taps != 16
     (4, 1, 64, 16, 63, 16),        # N < C
-    (4, 1, 64, 16, 6400, 4),       # input_bits not in {8, 16}
+    (4, 1, 64, 16, 6400, 12),      # input_bits not in {4, 8, 16}
 ])
 def test_plan_rejects_bad_arguments(cobalt, args):
     h = ctypes.c_void_p(1234)
@@ -67,6 +67,11 @@ def test_null_plan_calls(cobalt):
     lib = cobalt.load()
     assert lib.cobalt_process(None, None, None, None, None, None) == cobalt.COBALT_ERR_BAD_ARG
     assert lib.cobalt_process_host(None, None, None, None, None) == cobalt.COBALT_ERR_BAD_ARG
+    assert lib.cobalt_process_ex(None, None, None) == cobalt.COBALT_ERR_BAD_ARG
+    assert lib.cobalt_set_dumps(None, 2) == cobalt.COBALT_ERR_BAD_ARG
+    assert lib.cobalt_set_phase_offsets(None, None) == cobalt.COBALT_ERR_BAD_ARG
+    assert lib.cobalt_set_coarse_delays(None, None, 0) == cobalt.COBALT_ERR_BAD_ARG
+    assert lib.cobalt_set_input_layout(None, 1) == cobalt.COBALT_ERR_BAD_ARG
     assert lib.cobalt_reset(None) == cobalt.COBALT_ERR_BAD_ARG
     assert lib.cobalt_info(None, None) == cobalt.COBALT_ERR_BAD_ARG
     assert lib.cobalt_debug_unpack(None, 12, None, 0, None) == cobalt.COBALT_ERR_BAD_ARG
