@@ -169,12 +169,23 @@ def measured_peaks():
 
 
 def stored_traffic(key: str):
-    """DRAM bytes per launch of a kernel from the committed ncu --set full capture (profiles/traffic.json)."""
+    """DRAM bytes per launch of a kernel from the committed `ncu --set full` capture named in profiles/traffic.json.
+    bench.py cannot run ncu on itself, so the figure is a stored one: it is only reported while the kernel's source
+    file still has the sha256 recorded with the capture; otherwise None (and `traffic_source` says why)."""
+    import hashlib
+
     try:
         with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
-            return json.load(f).get(key)
-    except Exception:  # noqa: BLE001
-        return None
+            ent = json.load(f).get(key)
+        if not isinstance(ent, dict):
+            return None, "no capture recorded"
+        with open(os.path.join(ROOT, ent["file"]), "rb") as f:
+            sha = hashlib.sha256(f.read()).hexdigest()
+        if sha != ent["sha256"]:
+            return None, f"stale: {ent['file']} changed since {ent['source']}"
+        return ent["bytes"], ent["source"]
+    except Exception as e:  # noqa: BLE001
+        return None, f"unavailable: {e!r}"
 
 
 def workload(args):
@@ -322,8 +333,10 @@ def run_ours(args, rank, world, local):
     f_bytes = n_samples * F_BYTES_PER_SAMPLE[cfg.bits] if args.mode == "tensor" else n_samples * (cfg.bits // 4 + 8)
     x_flop = units * X_FLOP_PER_BASELINE_SAMPLE
     f_kernel = "fstage_kernel"
+    tr_f, tr_f_src = stored_traffic(f_kernel) if (cfg.name == "full-array-16bit" and args.mode == "tensor") else (None, "captured for config 3 only")
+    tr_x, tr_x_src = stored_traffic("xstage_tc_kernel") if (cfg.name == "full-array-16bit" and args.mode == "tensor") else (None, "captured for config 3 only")
     roof_f = {"kernel": f_kernel, "bound": "hbm", "achieved": f_bytes / t_f / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-              "frac": f_bytes / t_f / 1e9 / peaks["hbm_gbs"], "traffic": stored_traffic(f_kernel) if cfg.name == "full-array-16bit" else None,
+              "frac": f_bytes / t_f / 1e9 / peaks["hbm_gbs"], "traffic": tr_f, "traffic_source": tr_f_src,
               "peak_source": peaks["source"], "ms_per_launch": t_f * 1e3 / n_chunks, "launches_per_step": n_chunks,
               "algorithmic_bytes_per_launch": f_bytes / n_chunks}
     # the F-stage is bound by FP32 dispatch, not by HBM: the same launches against the FP32 peak
@@ -337,7 +350,7 @@ def run_ours(args, rank, world, local):
     roof_x = {"kernel": "xstage_tc_kernel" if args.mode == "tensor" else "xstage_simt_kernel", "bound": "tensor",
               "achieved": x_flop / t_x / 1e12, "peak": peaks["tensor_tflops_sustained"], "unit": "TFLOP/s",
               "frac": x_flop / t_x / 1e12 / peaks["tensor_tflops_sustained"],
-              "traffic": stored_traffic("xstage_tc_kernel") if cfg.name == "full-array-16bit" else None,
+              "traffic": tr_x, "traffic_source": tr_x_src,
               "peak_source": peaks["source"] + " (sustained bf16; fp16 runs at the same rate)",
               "ms_per_launch": t_x * 1e3 / n_chunks, "launches_per_step": n_chunks,
               "algorithmic_flop_per_launch": x_flop / n_chunks,

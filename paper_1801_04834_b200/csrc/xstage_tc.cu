@@ -491,11 +491,18 @@ cudaError_t launch_xstage_tc(const cobalt_plan_s *p, cudaStream_t st, const void
     // too few (dump, subband, channel) problems to fill the SMs (config 2: 64 channels on 148 SMs): split each one's time
     // range over several jobs, into partial blocks that xsum_kernel adds up
     a.splits = 1;
-    if (p->d_xpart && (long long)a.nbC * a.D * a.jobs_per_channel < 2 * p->sm_count) {
-        a.splits = (int)((2LL * p->sm_count + (long long)a.nbC * a.D * a.jobs_per_channel - 1) / ((long long)a.nbC * a.D * a.jobs_per_channel));
-        if (a.splits > p->x_splits) a.splits = p->x_splits;
-        if (a.splits > a.K) a.splits = a.K;
-        if (a.splits < 1) a.splits = 1;
+    if (p->d_xpart) {
+        // cost of s splits in k-tile times: waves x (k-tiles per job + ~3.5 for the prologue and the exposed epilogue)
+        const long long probs = (long long)a.nbC * a.D * a.jobs_per_channel;
+        double best = 1e30;
+        for (int sp = 1; sp <= p->x_splits && sp <= a.K; ++sp) {
+            const long long waves = (probs * sp + p->sm_count - 1) / p->sm_count;
+            const double cost = (double)waves * ((double)((a.K + sp - 1) / sp) + 3.5);
+            if (cost < best - 1e-9) {
+                best = cost;
+                a.splits = sp;
+            }
+        }
     }
     a.part = p->d_xpart;
     a.dump_stride = dump_stride;
