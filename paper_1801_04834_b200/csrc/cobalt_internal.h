@@ -93,9 +93,10 @@ struct cobalt_plan_s {
     std::vector<float> h_weights;
     void *d_hist[2] = {nullptr, nullptr};   // raw integer samples [B][S][2][15 C][2]; ping-pong
     int hist_cur = 0;
-    float2 *d_phase = nullptr;         // [B][S][C]  s b[j] exp(-2 pi i frac(f tau)), built once per call
+    float2 *d_phase = nullptr;         // [B][S][C]  b[j] exp(-2 pi i frac(f tau)), built once per call; applied by the X-stage
     float *d_dstep = nullptr;          // [B][S][C] phase step per spectrum in cycles (cobalt_process_interp)
-    float *d_scale = nullptr;          // {s, 1/s, 1/s^2}: power-of-two scale of the fp16 intermediate (1 in EXACT mode)
+    float zscale = 1.f;                // power-of-two scale s of the fp16 intermediate (reading R1): 2^-e,
+                                       // e = ceil(log2(amp_max / 32768)) in TENSOR mode, 1 in EXACT mode
     float amp_max = 0.f;               // worst-case |F| for full-scale input: sum|g| * sqrt(2) * 2^(bits-1)
     void *d_z = nullptr;               // intermediate of one chunk (layout per mode)
     CUtensorMap zmap;                  // TENSOR mode: d_z as (spectrum-in-k-tile, chunk subband * C + channel, plane, row m, k-tile)
@@ -106,6 +107,7 @@ struct cobalt_plan_s {
     int x_stages = 0;
     bool x_staged = false;             // X-stage epilogue through a shared-memory image of the channel's output block
     size_t x_out_off = 0;
+    size_t x_rot_bytes = 0;            // one of the two per-job rotation tables of the X-stage epilogue
     size_t scratch_bytes = 0;
     // host-buffer path
     cudaStream_t hs[3] = {nullptr, nullptr, nullptr};
@@ -134,6 +136,16 @@ struct FCall {
     long long n_in = 0;                    // stream stride of the samples the fused kernel reads
 };
 
+// What the X-stage applies to the raw correlations of one chunk: V_ik <- V_ik w_i conj(w_k) / s^2 with
+// w_m = phase[(b0 + subband) S + m / 2][channel] * poff[m] (steps a5, a6 and reading A22 moved behind the integration: the
+// same product, one multiplication per visibility instead of one per sample), s = the fp16 operand scale.
+struct XCall {
+    const float2 *phase = nullptr;     // plan's d_phase [B][S][C], or nullptr: no rotation (cobalt_debug_correlate)
+    const float2 *poff = nullptr;      // [2S] or nullptr
+    int b0 = 0;                        // first subband of the chunk
+    float inv_s2 = 1.f;
+};
+
 // fstage.cu ---------------------------------------------------------------------------------
 cudaError_t launch_phase_table(const cobalt_plan_s *p, cudaStream_t st, const double *d_delays,
                                const float *d_bandpass, int b0, int nb, const double *d_delays_end);
@@ -145,14 +157,14 @@ cudaError_t launch_unpack(cudaStream_t st, int bits, const void *d_in, long long
 cudaError_t launch_ingest(const cobalt_plan_s *p, cudaStream_t st, const void *samples_b0, int nb, void *d_out);
 cudaError_t launch_valid_counts(const cobalt_plan_s *p, cudaStream_t st, const unsigned char *d_valid, int b0, int nb, unsigned int *d_counts);
 // layout.cu ---------------------------------------------------------------------------------
-cudaError_t launch_set_unit_scale(const cobalt_plan_s *p, cudaStream_t st);
-cudaError_t launch_z_to_float(const cobalt_plan_s *p, cudaStream_t st, const void *d_zsub, float2 *d_out);
+// z of one subband -> [C][2S][n_t] complex64, rotated like the X-stage would (xc) so that the tap shows steps a1-a7
+cudaError_t launch_z_to_float(const cobalt_plan_s *p, cudaStream_t st, const void *d_zsub, float2 *d_out, const XCall &xc);
 cudaError_t launch_float_to_z(const cobalt_plan_s *p, cudaStream_t st, const float2 *d_in, void *d_zsub);
 // xstage_simt.cu ----------------------------------------------------------------------------
 // d_vis points at subband b0 of dump 0; dump d is dump_stride float2 further
-cudaError_t launch_xstage_simt(const cobalt_plan_s *p, cudaStream_t st, const void *d_z, int nb, float2 *d_vis, size_t dump_stride);
+cudaError_t launch_xstage_simt(const cobalt_plan_s *p, cudaStream_t st, const void *d_z, int nb, float2 *d_vis, size_t dump_stride, const XCall &xc);
 // xstage_tc.cu ------------------------------------------------------------------------------
 void build_xjobs(cobalt_plan_s *p);
-cudaError_t launch_xstage_tc(const cobalt_plan_s *p, cudaStream_t st, const void *d_z, int nb, float2 *d_vis, size_t dump_stride);
+cudaError_t launch_xstage_tc(const cobalt_plan_s *p, cudaStream_t st, const void *d_z, int nb, float2 *d_vis, size_t dump_stride, const XCall &xc);
 
 }  // namespace cobalt

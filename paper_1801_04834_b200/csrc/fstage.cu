@@ -35,17 +35,14 @@ struct FArgs {
     const unsigned char *samples;   // [nb][S][2][N] complex integers, first subband of the chunk
     const unsigned char *hist;      // [B][S][2][15 C] complex integers
     const float *weights;           // [16][C]
-    const float2 *phase;            // [nb][S][C]
     const float *dstep;             // [nb][S][C] phase step per spectrum in cycles (time-varying delay), or nullptr
-    const float2 *poff;             // [2S] exp(-i phase0) per stream (reading A22), or nullptr
+    float zscale;                   // power-of-two scale s of the fp16 intermediate (1 in EXACT mode), folded into the FIR weights
     const unsigned char *valid;     // [B][S][n_kt] valid-sample flags per 64-spectrum tile (reading A24), or nullptr
     const int *coarse;              // [S] first sample of each station's block (reading A25), or nullptr
     unsigned char *z;               // chunk intermediate
     long long N, n_t;               // N = stream stride of `samples`
     size_t z_subband_bytes;
     int S, M, Mpad, n_kt, b0, tiles_per_seg, groups_per_subband;
-    int ipc;                        // items (groups of SPC streams) per CTA: 2 for C = 256 (both polarisations of a station
-                                    // share one rotation table), 1 otherwise and whenever the polarisations differ (poff)
 };
 
 // Packed fp32 pairs (fma.rn.f32x2 family, SASS FFMA2/FADD2/FMUL2): a complex value is one 64-bit
@@ -59,9 +56,10 @@ __device__ __forceinline__ float2 cmul_tab2(float2 v, float2 t) {
     return __ffma2_rn(make_float2(-t.y, t.x), make_float2(v.y, v.y), p);
 }
 
-// Time-varying delay: rotation w (for the delay at the start of the block) times exp(-2 pi i frac(t step)) for the
-// spectra t and t + 1; step in cycles per spectrum.  fp32 throughout.
-__device__ __forceinline__ void interp_factors(float step, long long t, float2 w, float2 &w0, float2 &w1) {
+// Time-varying delay (reading A21): exp(-2 pi i frac(t step)) for the spectra t and t + 1, step in cycles per spectrum
+// (from the fp64 phase_table_kernel); the factor itself in fp32.  The static part of the rotation (the delay at the
+// first spectrum, bandpass, phase offsets) is applied to the visibilities by the X-stage.
+__device__ __forceinline__ void interp_factors(float step, long long t, float2 &w0, float2 &w1) {
     float p0 = step * (float)t;
     p0 -= rintf(p0);
     float p1 = p0 + step;
@@ -69,8 +67,8 @@ __device__ __forceinline__ void interp_factors(float step, long long t, float2 w
     float s0, c0, s1, c1;
     __sincosf(-6.283185307179586f * p0, &s0, &c0);
     __sincosf(-6.283185307179586f * p1, &s1, &c1);
-    w0 = cmul_tab2(w, make_float2(c0, s0));
-    w1 = cmul_tab2(w, make_float2(c1, s1));
+    w0 = make_float2(c0, s0);
+    w1 = make_float2(c1, s1);
 }
 
 // Forward 4-point DFT in place: X[k] = sum_n a[n] (-i)^{nk}.
@@ -193,8 +191,9 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, con
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int grp = blockIdx.x;                          // stream group within the chunk
     const int bl = grp / a.groups_per_subband;
-    const int m0 = (grp - bl * a.groups_per_subband) * SPC * a.ipc;   // first stream of the CTA
-    const int n_items = min(a.ipc, (a.M - m0 + SPC - 1) / SPC);       // items of this CTA that exist
+    constexpr int IPC = Sh::IPC;
+    const int m0 = (grp - bl * a.groups_per_subband) * SPC * IPC;   // first stream of the CTA
+    const int n_items = min(IPC, (a.M - m0 + SPC - 1) / SPC);       // items of this CTA that exist
     const int kt0 = blockIdx.y * a.tiles_per_seg;
     const int kt1 = min(kt0 + a.tiles_per_seg, a.n_kt);
     const int n_sub = (kt1 - kt0) * (kKTile / kSubTile);
@@ -215,15 +214,8 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, con
         }
         mbar_fence_init();
     }
-    {   // rotation * bandpass of the CTA's streams (station = m >> 1) in the FFT threads' register order, zeros for
-        // streams that do not exist (their staged rows are then exact zeros), and the inter-pass twiddles
-        for (int idx = tid; idx < 256; idx += kFThreads) {
-            const int sl = idx / C, rr = (idx % C) / 16, i = idx % 16;
-            const int m = m0 + sl;
-            float2 w = m < a.M ? a.phase[((size_t)bl * a.S + (m >> 1)) * C + out_channel<R>(rr, i)] : make_float2(0.f, 0.f);
-            if (a.poff && m < a.M) w = cmul_tab2(w, a.poff[m]);      // clock / phase offset of this (station, polarisation)
-            reinterpret_cast<float2 *>(smem + Sh::OFF_WTAB + (idx >> 4) * Sh::TAB_ROW)[i] = w;
-        }
+    {   // per-CTA tables: the phase step per spectrum of the CTA's streams (INTERP) in the FFT threads' register order, and
+        // the inter-pass twiddles
         if (INTERP) {
             for (int idx = tid; idx < 256; idx += kFThreads) {
                 const int sl = idx / C, rr = (idx % C) / 16, i = idx % 16;
@@ -232,7 +224,6 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, con
                     m < a.M ? a.dstep[((size_t)bl * a.S + (m >> 1)) * C + out_channel<R>(rr, i)] : 0.f;
             }
         }
-        if (tid < 16) reinterpret_cast<float2 *>(smem + Sh::OFF_ZERO)[tid] = make_float2(0.f, 0.f);
         if (R > 1) {
             for (int idx = tid; idx < R * 16; idx += kFThreads) {
                 float sn, cs;
@@ -336,7 +327,8 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, con
         }
         float wk[kTaps];
         {
-            const float sgn = (ph & 1) ? -1.f : 1.f;      // (-1)^ph: channel j <- DFT bin (j + C/2) mod C
+            // (-1)^ph: channel j <- DFT bin (j + C/2) mod C; zscale: the power-of-two scale of the fp16 intermediate (exact)
+            const float sgn = ((ph & 1) ? -1.f : 1.f) * a.zscale;
 #pragma unroll
             for (int k = 0; k < kTaps; ++k) wk[k] = a.weights[k * C + ph] * sgn;
         }
@@ -407,8 +399,6 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, con
             r = (ft & 15) % R;
         }
         float2 *ybase = reinterpret_cast<float2 *>(smem + Sh::OFF_Y) + 2 * tp * Sh::TS + sl * YS;
-        const float4 *wtab4 = reinterpret_cast<const float4 *>(smem + Sh::OFF_WTAB + (sl * R + r) * Sh::TAB_ROW);
-        const float4 *zero4 = reinterpret_cast<const float4 *>(smem + Sh::OFF_ZERO);
         const float *steps = reinterpret_cast<const float *>(smem + Sh::OFF_STEP + (sl * R + r) * Sh::STEP_ROW);
         const float4 *tw4 = reinterpret_cast<const float4 *>(smem + Sh::OFF_TW + r * Sh::TAB_ROW);
         // staging word of (channel c, plane, pair p of the tile): box b = sl / SPB, then [stream][plane][channel][64 B],
@@ -498,16 +488,16 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, con
                 __syncwarp();
                 if (lane == 0) mbar_arrive(bar_y_empty + 8 * yb);
             }
-            // steps a5-a7: rotate * bandpass, convert, stage transposed.  Spectra t >= n_t (padding of the last
-            // k-tile) leave as exact zeros: the rotation table is replaced by zeros.
+            // steps a5-a7.  The static rotation * bandpass (a5, a6) is a per-(input, channel) constant and is applied to the
+            // visibilities by the X-stage (V_ik <- w_i conj(w_k) V_ik, the same product); here only the time-varying part of
+            // cobalt_process_interp, then the conversion and the transposed staging (a7).  Spectra t >= n_t (padding of the last
+            // k-tile), rows m >= 2S and lost tiles (valid-sample flags, reading A24) leave as exact zeros.
             const bool live0 = t_spec < a.n_t, live1 = t_spec + 1 < a.n_t;
-            // a lost tile (valid-sample flags, reading A24) leaves as exact zeros, like the padding
-            const bool lost = a.valid && m < a.M && a.valid[((size_t)(a.b0 + bl) * a.S + (m >> 1)) * a.n_kt + kt] == 0;
-            const float4 *wt = live0 && !lost ? wtab4 : zero4;
+            const bool lost = m >= a.M || (a.valid && a.valid[((size_t)(a.b0 + bl) * a.S + (m >> 1)) * a.n_kt + kt] == 0);
             if (TENSOR) {
                 const int tile = jjg >> 1, sbuf = tile & 1;
                 const int p = 8 * (jj & 1) + tp;          // pair of spectra within the 32-spectrum tile
-                const uint32_t msk = live1 || !live0 ? 0xffffffffu : 0x0000ffffu;   // n_t odd: last pair is half live
+                const uint32_t msk = !live0 || lost ? 0u : live1 ? 0xffffffffu : 0x0000ffffu;   // n_t odd: last pair is half live
                 mbar_wait(bar_stg_empty + 8 * sbuf, ((uint32_t)(tile >> 1) & 1u) ^ 1u);
                 unsigned char *stg = smem + Sh::OFF_STG + sbuf * Sh::STG + stg_thread;
                 // byte offset of (channel j, plane re, this pair) in the box: 64 j + 16 ((p >> 2) ^ (m & 3)) + 4 (p & 3), then
@@ -520,20 +510,19 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, con
 #pragma unroll
                 for (int v = 0; v < 4; ++v) stg_v[v] = stg + (base ^ (uint32_t)(v << 4));
 #pragma unroll
-                for (int i = 0; i < 16; i += 2) {
-                    const float4 w = wt[i >> 1];
-#pragma unroll
-                    for (int e = 0; e < 2; ++e) {
-                        const int oi = out_reg<R>(i + e);
-                        const int dj = out_channel<R>(0, i + e);                 // compile-time part of the channel index
-                        const int ibits = R == 16 ? 0 : R == 4 ? ((i + e) >> 3) & 1 : ((i + e) >> 1) & 3;
-                        const float2 ww = e ? make_float2(w.z, w.w) : make_float2(w.x, w.y);
-                        float2 ww0 = ww, ww1 = ww;
-                        if (INTERP) interp_factors(steps[i + e], t_spec, ww, ww0, ww1);
-                        const float2 z0 = cmul_tab2(o0[oi], ww0), z1 = cmul_tab2(o1[oi], ww1);
-                        *reinterpret_cast<uint32_t *>(stg_v[ibits] + dj * 64) = pack_half2(z0.x, z1.x) & msk;
-                        *reinterpret_cast<uint32_t *>(stg_v[ibits] + dj * 64 + C * 64) = pack_half2(z0.y, z1.y) & msk;
+                for (int i = 0; i < 16; ++i) {
+                    const int oi = out_reg<R>(i);
+                    const int dj = out_channel<R>(0, i);                     // compile-time part of the channel index
+                    const int ibits = R == 16 ? 0 : R == 4 ? (i >> 3) & 1 : (i >> 1) & 3;
+                    float2 z0 = o0[oi], z1 = o1[oi];
+                    if (INTERP) {
+                        float2 w0, w1;
+                        interp_factors(steps[i], t_spec, w0, w1);
+                        z0 = cmul_tab2(z0, w0);
+                        z1 = cmul_tab2(z1, w1);
                     }
+                    *reinterpret_cast<uint32_t *>(stg_v[ibits] + dj * 64) = pack_half2(z0.x, z1.x) & msk;
+                    *reinterpret_cast<uint32_t *>(stg_v[ibits] + dj * 64 + C * 64) = pack_half2(z0.y, z1.y) & msk;
                 }
                 asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy writes -> visible to the store
                 __syncwarp();
@@ -542,18 +531,19 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, con
                 // EXACT mode (parity instrument): fp32 values straight to z [C][M][n_t]
                 if (m < a.M) {
 #pragma unroll
-                    for (int i = 0; i < 16; i += 2) {
-                        const float4 w = wt[i >> 1];
-#pragma unroll
-                        for (int e = 0; e < 2; ++e) {
-                            const int j = out_channel<R>(r, i + e), oi = out_reg<R>(i + e);
-                            const float2 ww = e ? make_float2(w.z, w.w) : make_float2(w.x, w.y);
-                            float2 ww0 = ww, ww1 = ww;
-                            if (INTERP) interp_factors(steps[i + e], t_spec, ww, ww0, ww1);
-                            float2 *dst = reinterpret_cast<float2 *>(zsub) + ((size_t)j * a.M + m) * a.n_t + t_spec;
-                            if (live0) dst[0] = cmul_tab2(o0[oi], ww0);
-                            if (live1) dst[1] = cmul_tab2(o1[oi], ww1);
+                    for (int i = 0; i < 16; ++i) {
+                        const int j = out_channel<R>(r, i), oi = out_reg<R>(i);
+                        float2 z0 = o0[oi], z1 = o1[oi];
+                        if (INTERP) {
+                            float2 w0, w1;
+                            interp_factors(steps[i], t_spec, w0, w1);
+                            z0 = cmul_tab2(z0, w0);
+                            z1 = cmul_tab2(z1, w1);
                         }
+                        if (lost) z0 = z1 = make_float2(0.f, 0.f);
+                        float2 *dst = reinterpret_cast<float2 *>(zsub) + ((size_t)j * a.M + m) * a.n_t + t_spec;
+                        if (live0) dst[0] = z0;
+                        if (live1) dst[1] = z1;
                     }
                 }
             }
@@ -561,44 +551,15 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, con
     }
 }
 
-// "we compute the channel-dependent phase angles in double precision".  One entry per
-// (subband of the chunk, station, channel): s b[j] exp(-2 pi i frac(f[s][j] tau_a)), f per reading A6.
-//
-// s is the power-of-two scale of the fp16 intermediate (TENSOR mode; 1 otherwise): with
-// e = ceil(log2(max_j |b_j| * amp_max / 32768)) and s = 2^-e, full-scale input cannot overflow fp16
-// (|z s| <= 32768) and tiny bandpass weights cannot push z into the fp16 subnormals.  The X-stage
-// epilogue multiplies the visibilities by 1/s^2; both factors are exact.  Every block derives the
-// same s from the same C weights; block 0 publishes {s, 1/s, 1/s^2} for the X-stage.
+// "we compute the channel-dependent phase angles in double precision".  One entry per (subband, station,
+// channel): w = b[j] exp(-2 pi i frac(f[s][j] tau_a)), f per reading A6; fp64 up to the final rounding.  The X-stage
+// applies w_i conj(w_k) to the visibility of baseline (i, k) -- the same product as rotating every sample (a5, a6).
+// delays_end != nullptr (reading A21): also the phase step per spectrum f (tau_e - tau_b) / n_t in cycles, for the
+// time-varying part the F-stage applies.
 __global__ void phase_table_kernel(const double *__restrict__ delays, const float *__restrict__ bandpass,
                                    const double *__restrict__ f_sb, int b0, int nb, int S, int C, double f_s,
-                                   float amp_max, int tensor, float *__restrict__ scale_out,
                                    float2 *__restrict__ out, const double *__restrict__ delays_end, double inv_n_t,
                                    float *__restrict__ step_out) {
-    __shared__ float s_max[32];
-    __shared__ float s_scale;
-    float bm = 0.f;
-    for (int j = threadIdx.x; j < C; j += blockDim.x) bm = fmaxf(bm, fabsf(bandpass[j]));
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) bm = fmaxf(bm, __shfl_xor_sync(0xffffffffu, bm, o));
-    if ((threadIdx.x & 31) == 0) s_max[threadIdx.x >> 5] = bm;
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        float m = 0.f;
-        for (int w = 0; w < (int)((blockDim.x + 31) >> 5); ++w) m = fmaxf(m, s_max[w]);
-        int e = 0;
-        if (tensor && m > 0.f && m < 3.0e38f) {
-            e = (int)ceilf(log2f(m * amp_max / 32768.f));
-            e = max(-40, min(40, e));
-        }
-        s_scale = scalbnf(1.f, -e);
-        if (blockIdx.x == 0) {
-            scale_out[0] = scalbnf(1.f, -e);
-            scale_out[1] = scalbnf(1.f, e);
-            scale_out[2] = scalbnf(1.f, 2 * e);
-        }
-    }
-    __syncthreads();
-    const double sc = (double)s_scale;
     const long long total = (long long)nb * S * C;
     for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < total;
          idx += (long long)gridDim.x * blockDim.x) {
@@ -610,16 +571,11 @@ __global__ void phase_table_kernel(const double *__restrict__ delays, const floa
         const double frac = cyc - floor(cyc);
         double sn, cs;
         sincospi(-2.0 * frac, &sn, &cs);
-        const double b = (double)bandpass[j] * sc;
+        const double b = (double)bandpass[j];
         const long long o = (long long)b0 * S * C + idx;      // tables are indexed by the subband of the plan
         out[o] = make_float2((float)(b * cs), (float)(b * sn));
-        // time-varying delay (reading A21): phase step per spectrum, in cycles, from the fp64 delays
         if (delays_end) step_out[o] = (float)(f * (delays_end[s] - delays[s]) * inv_n_t);
     }
-}
-
-__global__ void unit_scale_kernel(float *scale_out) {
-    if (threadIdx.x < 3) scale_out[threadIdx.x] = 1.f;
 }
 
 // P:L360 "We carry FIR filter history samples across to the next block": new history = the last
@@ -689,8 +645,7 @@ cudaError_t launch_f(const cobalt_plan_s *p, cudaStream_t st, const FArgs &a, in
     FArgs args = a;
     // One CTA per SM: enough CTAs for >= 8 waves when the chunk allows, as few time segments as
     // possible (each segment re-reads its 16 warm-up rows).
-    args.ipc = a.poff ? 1 : Sh::IPC;     // per-polarisation phase offsets: one rotation table per stream
-    args.groups_per_subband = (p->M + Sh::SPC * args.ipc - 1) / (Sh::SPC * args.ipc);
+    args.groups_per_subband = (p->M + Sh::SPC * Sh::IPC - 1) / (Sh::SPC * Sh::IPC);
     const long long groups = (long long)nb * args.groups_per_subband;
     const long long want = (long long)p->sm_count * 8;
     int n_seg = (int)((want + groups - 1) / groups);
@@ -723,15 +678,8 @@ cudaError_t launch_phase_table(const cobalt_plan_s *p, cudaStream_t st, const do
     const int threads = 256;
     long long blocks = (total + threads - 1) / threads;
     if (blocks > 4096) blocks = 4096;
-    phase_table_kernel<<<(unsigned)blocks, threads, 0, st>>>(d_delays, d_bandpass, p->d_f_sb, b0, nb, p->S, p->C,
-                                                             p->f_s, p->amp_max, p->mode == COBALT_MODE_TENSOR_FP16 ? 1 : 0,
-                                                             p->d_scale, p->d_phase, d_delays_end, 1.0 / (double)p->n_t,
-                                                             p->d_dstep);
-    return cudaGetLastError();
-}
-
-cudaError_t launch_set_unit_scale(const cobalt_plan_s *p, cudaStream_t st) {
-    unit_scale_kernel<<<1, 32, 0, st>>>(p->d_scale);
+    phase_table_kernel<<<(unsigned)blocks, threads, 0, st>>>(d_delays, d_bandpass, p->d_f_sb, b0, nb, p->S, p->C, p->f_s, p->d_phase,
+                                                             d_delays_end, 1.0 / (double)p->n_t, p->d_dstep);
     return cudaGetLastError();
 }
 
@@ -740,9 +688,8 @@ cudaError_t launch_fstage(const cobalt_plan_s *p, cudaStream_t st, const void *s
     a.samples = static_cast<const unsigned char *>(samples_b0);
     a.hist = static_cast<const unsigned char *>(p->d_hist[p->hist_cur]);
     a.weights = p->d_weights;
-    a.phase = p->d_phase + (size_t)b0 * p->S * p->C;
     a.dstep = call.delays_end ? p->d_dstep + (size_t)b0 * p->S * p->C : nullptr;
-    a.poff = p->d_poff;
+    a.zscale = p->zscale;
     a.valid = call.valid;
     a.coarse = call.coarse;
     a.z = static_cast<unsigned char *>(p->d_z);

@@ -131,6 +131,13 @@ int alloc_scratch(cobalt_plan_s *p, int chunk_request) {
     CK(p, cudaMemset(p->d_z, 0, (size_t)chunk * p->z_subband_bytes));   // zero rows 2S..Mpad stay zero forever
     CK(p, cudaMalloc(&p->d_phase, (size_t)p->B * p->S * p->C * sizeof(float2)));
     CK(p, cudaMalloc(&p->d_dstep, (size_t)p->B * p->S * p->C * sizeof(float)));
+    {   // Reading R1: power-of-two scale of the fp16 intermediate so that full-scale input cannot overflow it
+        // (|F s| <= amp_max s <= 32768); undone exactly (1/s^2) by the X-stage.  The bandpass no longer enters: it is
+        // applied to the visibilities in fp32.
+        int e = 0;
+        if (p->mode == COBALT_MODE_TENSOR_FP16) e = (int)std::ceil(std::log2((double)p->amp_max / 32768.0));
+        p->zscale = std::ldexp(1.f, -e);
+    }
     size_t extra = 0;
     if (needs_ingest(p)) {
         extra += (size_t)chunk * p->M * p->N * sample_bytes(p->bits);
@@ -191,11 +198,16 @@ int enqueue_chunk(cobalt_plan_s *p, cudaStream_t st, const void *samples_b0, con
     CK(p, launch_history_update(p, st, fsamples, b0, nb, call));
     if (ev) CK(p, cudaEventRecord(ev->e[3], st));
     const size_t dump_stride = (size_t)p->B * p->C * p->n_bl * 4;      // float2 between dumps
+    XCall xc;
+    xc.phase = p->d_phase;
+    xc.poff = p->d_poff;
+    xc.b0 = b0;
+    xc.inv_s2 = 1.f / (p->zscale * p->zscale);
     if (p->mode == COBALT_MODE_TENSOR_FP16) {
-        CK(p, launch_xstage_tc(p, st, p->d_z, nb, vis_b0, dump_stride));
+        CK(p, launch_xstage_tc(p, st, p->d_z, nb, vis_b0, dump_stride, xc));
         if (p->x_splits > 1) extra += 1;
     } else {
-        CK(p, launch_xstage_simt(p, st, p->d_z, nb, vis_b0, dump_stride));
+        CK(p, launch_xstage_simt(p, st, p->d_z, nb, vis_b0, dump_stride, xc));
     }
     if (io.valid_counts) {
         CK(p, launch_valid_counts(p, st, io.valid, b0, nb, io.valid_counts));
@@ -298,7 +310,6 @@ int cobalt_plan(cobalt_plan_t **out, int stations, int subbands, int channels, i
     guard(cudaMalloc(&p->d_hist[0], hist), "cudaMalloc history");
     guard(cudaMalloc(&p->d_hist[1], hist), "cudaMalloc history");
     guard(cudaMalloc(&p->d_jobs, p->jobs.size() * sizeof(XJob)), "cudaMalloc jobs");
-    guard(cudaMalloc(&p->d_scale, 4 * sizeof(float)), "cudaMalloc scale");
     if (rc == COBALT_OK) {
         guard(cudaMemcpy(p->d_weights, p->h_weights.data(), p->h_weights.size() * sizeof(float), cudaMemcpyHostToDevice), "weights H2D");
         guard(cudaMemcpy(p->d_f_sb, p->f_sb.data(), (size_t)p->B * sizeof(double), cudaMemcpyHostToDevice), "f_sb H2D");
@@ -324,7 +335,6 @@ int cobalt_destroy(cobalt_plan_t *p) {
     cudaFree(p->d_hist[0]);
     cudaFree(p->d_hist[1]);
     cudaFree(p->d_jobs);
-    cudaFree(p->d_scale);
     cudaFree(p->d_coarse);
     cudaFree(p->d_poff);
     cudaFree(p->d_delays_h);
@@ -656,18 +666,23 @@ int cobalt_debug_channelised(cobalt_plan_t *p, void *cuda_stream, const void *d_
         call.n_in = p->N_in;
     }
     CK(p, launch_fstage(p, st, fsamples, sb, 1, call));
-    CK(p, launch_z_to_float(p, st, p->d_z, static_cast<float2 *>(d_z)));
+    XCall xc;
+    xc.phase = p->d_phase;
+    xc.poff = p->d_poff;
+    xc.b0 = sb;
+    xc.inv_s2 = 1.f / (p->zscale * p->zscale);
+    CK(p, launch_z_to_float(p, st, p->d_z, static_cast<float2 *>(d_z), xc));
     return COBALT_OK;
 }
 
 int cobalt_debug_correlate(cobalt_plan_t *p, void *cuda_stream, const void *d_z, void *d_vis) {
     if (!p || !d_z || !d_vis) return fail(p, COBALT_ERR_BAD_ARG, "NULL argument");
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    CK(p, launch_set_unit_scale(p, st));   // caller-supplied operands are taken as they are
     CK(p, launch_float_to_z(p, st, static_cast<const float2 *>(d_z), p->d_z));
     const size_t dump_stride = (size_t)p->C * p->n_bl * 4;     // one subband: [D][C][n_bl][2][2]
-    if (p->mode == COBALT_MODE_TENSOR_FP16) CK(p, launch_xstage_tc(p, st, p->d_z, 1, static_cast<float2 *>(d_vis), dump_stride));
-    else CK(p, launch_xstage_simt(p, st, p->d_z, 1, static_cast<float2 *>(d_vis), dump_stride));
+    const XCall xc;                                            // caller-supplied operands are taken as they are: no rotation, unit scale
+    if (p->mode == COBALT_MODE_TENSOR_FP16) CK(p, launch_xstage_tc(p, st, p->d_z, 1, static_cast<float2 *>(d_vis), dump_stride, xc));
+    else CK(p, launch_xstage_simt(p, st, p->d_z, 1, static_cast<float2 *>(d_vis), dump_stride, xc));
     return COBALT_OK;
 }
 

@@ -16,7 +16,8 @@ constexpr int kTile = 32, kTk = 16;
 
 __global__ void __launch_bounds__(256) xstage_simt_kernel(const float2 *__restrict__ z, float2 *__restrict__ vis, int C,
                                                          int M, long long n_t, long long n_bl, size_t z_sub_elems, int nb,
-                                                         long long dump_len, size_t dump_stride) {
+                                                         long long dump_len, size_t dump_stride, const float2 *__restrict__ phase,
+                                                         const float2 *__restrict__ poff, int b0, float inv_s2) {
     __shared__ float2 As[kTk][kTile + 1];
     __shared__ float2 Bs[kTk][kTile + 1];
     const int pair = blockIdx.x;
@@ -70,17 +71,34 @@ __global__ void __launch_bounds__(256) xstage_simt_kernel(const float2 *__restri
         for (int v = 0; v < 2; ++v) {
             const int a = ti * kTile + ty * 2 + u, b = tj * kTile + tx * 2 + v;
             const int i = a >> 1, k = b >> 1;
-            if (a < M && b < M && i <= k) vc[((size_t)k * (k + 1) / 2 + i) * 4 + (a & 1) * 2 + (b & 1)] = acc[u][v];
+            if (a < M && b < M && i <= k) {
+                // steps a5, a6 (and reading A22) behind the integration: V_ik <- V_ik w_a conj(w_b), w = rotation * bandpass
+                float2 r = make_float2(acc[u][v].x * inv_s2, acc[u][v].y * inv_s2);
+                if (phase) {
+                    const int S = M >> 1;
+                    float2 wa = phase[((size_t)(b0 + bl) * S + i) * C + c], wb = phase[((size_t)(b0 + bl) * S + k) * C + c];
+                    if (poff) {
+                        const float2 qa = poff[a], qb = poff[b];
+                        wa = make_float2(wa.x * qa.x - wa.y * qa.y, wa.x * qa.y + wa.y * qa.x);
+                        wb = make_float2(wb.x * qb.x - wb.y * qb.y, wb.x * qb.y + wb.y * qb.x);
+                    }
+                    const float2 t = make_float2(wa.x * wb.x + wa.y * wb.y, wa.y * wb.x - wa.x * wb.y);   // wa conj(wb)
+                    r = make_float2(r.x * t.x - r.y * t.y, r.x * t.y + r.y * t.x);
+                }
+                vc[((size_t)k * (k + 1) / 2 + i) * 4 + (a & 1) * 2 + (b & 1)] = r;
+            }
         }
 }
 
 }  // namespace
 
-cudaError_t launch_xstage_simt(const cobalt_plan_s *p, cudaStream_t st, const void *d_z, int nb, float2 *d_vis, size_t dump_stride) {
+cudaError_t launch_xstage_simt(const cobalt_plan_s *p, cudaStream_t st, const void *d_z, int nb, float2 *d_vis, size_t dump_stride,
+                               const XCall &xc) {
     const int ntile = (p->M + kTile - 1) / kTile;
     dim3 grid((unsigned)(ntile * (ntile + 1) / 2), (unsigned)p->C, (unsigned)(nb * p->dumps));
     xstage_simt_kernel<<<grid, 256, 0, st>>>(static_cast<const float2 *>(d_z), d_vis, p->C, p->M, p->n_t, p->n_bl,
-                                             p->z_subband_bytes / sizeof(float2), nb, (long long)(p->n_kt / p->dumps) * kKTile, dump_stride);
+                                             p->z_subband_bytes / sizeof(float2), nb, (long long)(p->n_kt / p->dumps) * kKTile, dump_stride,
+                                             xc.phase, xc.poff, xc.b0, xc.inv_s2);
     return cudaGetLastError();
 }
 

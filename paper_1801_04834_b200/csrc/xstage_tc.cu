@@ -32,7 +32,10 @@ namespace {
 
 constexpr int kEpiWarps = 16;           // four per TMEM lane quarter, taking every fourth 16-column chunk
 constexpr int kEpiSub = kEpiWarps / 4;
-constexpr int kThreads = 64 + 32 * kEpiWarps;
+// Warp group 0 = producer, MMA issuer and two idle warps: it drops to 32 registers so that the four epilogue warp groups can
+// rise to 112 (setmaxnreg moves registers between complete groups of four warps of one CTA).
+constexpr int kFirstEpiWarp = 4;
+constexpr int kThreads = 32 * (kFirstEpiWarp + kEpiWarps);
 constexpr int kBarrierBytes = 4096;       // mbarriers (first 512 bytes) + a copy of the job table
 constexpr int kMaxSmemJobs = (kBarrierBytes - 512) / (int)sizeof(XJob);
 
@@ -40,7 +43,11 @@ struct XArgs {
     const unsigned char *z;
     float2 *vis;
     const XJob *jobs;
-    const float *scale;     // {s, 1/s, 1/s^2} of the fp16 intermediate (fstage.cu)
+    // V_ik <- V_ik w_i conj(w_k) / s^2 (XCall, cobalt_internal.h): w_m = phase[((b0 + subband) S + m / 2) C + channel] poff[m]
+    const float2 *phase, *poff;
+    int b0, S;
+    float inv_s2;           // 1 / s^2, s = power-of-two scale of the fp16 intermediate (exact)
+    uint32_t rot_off, rot_bytes;   // two per-job tables of w_m (one per job parity) in shared memory, before the stages
     size_t z_subband_bytes;
     long long n_bl;
     int C, M, Mpad, n_kt, jobs_per_channel, total_jobs, stages, stage_bytes;
@@ -104,6 +111,13 @@ __device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&v)[16]) {
 }
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 
+// Two visibilities (same row input, column inputs b and b + 1) times u conj(w_b), u conj(w_{b+1}): u = w_row / s^2, wb = (w_b, w_{b+1}).
+__device__ __forceinline__ float4 rotate2(float re0, float im0, float re1, float im1, float2 u, float4 wb) {
+    const float t0r = u.x * wb.x + u.y * wb.y, t0i = u.y * wb.x - u.x * wb.y;
+    const float t1r = u.x * wb.z + u.y * wb.w, t1i = u.y * wb.z - u.x * wb.w;
+    return make_float4(re0 * t0r - im0 * t0i, re0 * t0i + im0 * t0r, re1 * t1r - im1 * t1i, re1 * t1i + im1 * t1r);
+}
+
 // STAGED (one job per channel and the channel's [n_bl][2][2] block fits in shared memory): the epilogue writes
 // the visibilities into a shared-memory image of the channel's output block and one thread sends it to global
 // memory with a single bulk copy (cp.async.bulk, SASS UBLKCP) that drains while the next job's MMAs run; the
@@ -116,7 +130,7 @@ __global__ void __launch_bounds__(kThreads, 1) xstage_tc_kernel(const XArgs a) {
     const uint32_t bar_base = smem_base;                       // full[s] at +8 s, empty[s] at +8 (16 + s)
     const uint32_t tmem_full = bar_base + 8 * 32, tmem_empty = bar_base + 8 * 33;
     const uint32_t tmem_slot = bar_base + 8 * 34;              // 4 bytes: TMEM base address
-    const uint32_t stage_base = smem_base + kBarrierBytes;
+    const uint32_t stage_base = smem_base + kBarrierBytes + 2 * a.rot_bytes;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int stages = a.stages;
 
@@ -155,6 +169,7 @@ __global__ void __launch_bounds__(kThreads, 1) xstage_tc_kernel(const XArgs a) {
 
     if (warp == 0) {
         // ------------------------------------------------------------------ producer
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 32;");
         if (elect_one()) {
             int s = 0;
             uint32_t ph = 0;
@@ -182,6 +197,7 @@ __global__ void __launch_bounds__(kThreads, 1) xstage_tc_kernel(const XArgs a) {
         }
     } else if (warp == 1) {
         // ------------------------------------------------------------------ MMA issuer
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 32;");
         if (elect_one()) {
             int s = 0;
             uint32_t ph = 0, it = 0;
@@ -244,24 +260,46 @@ __global__ void __launch_bounds__(kThreads, 1) xstage_tc_kernel(const XArgs a) {
                 tc_commit(tmem_full);                      // accumulators complete
             }
         }
+    } else if (warp < kFirstEpiWarp) {
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 32;");      // the two idle warps of warp group 0
     } else {
         // ------------------------------------------------------------------ epilogue
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 112;");
         // Warps 2..9: warp w reads TMEM lane quarter w % 4 (the only one it may access); the two warps of a quarter
         // take alternate 16-column chunks.  The TMEM load of a warp's next chunk is in flight while it stores the
         // current one.
         const int wq = warp & 3;
-        const int sub = (warp - 2) >> 2;
-        const float inv_s2 = __ldg(a.scale + 2);           // undo the power-of-two operand scale (exact)
+        const int sub = (warp - kFirstEpiWarp) >> 2;
+        const float inv_s2 = a.inv_s2;                     // undo the power-of-two operand scale (exact)
+        unsigned char *smem_al = smem_raw + (smem_base - smem_u32(smem_raw));
         uint32_t it = 0;
         for (int jid = blockIdx.x; jid < a.total_jobs; jid += gridDim.x, ++it) {
             const XWork w = decode_job(a, jid);
             const XJob *job = jobs + w.jl;
             const int n_groups = job->n_groups;
             float4 *vg = reinterpret_cast<float4 *>(w.out);
-            float4 *vc = STAGED ? reinterpret_cast<float4 *>(smem_raw + (smem_base - smem_u32(smem_raw)) + a.out_off) : vg;
+            float4 *vc = STAGED ? reinterpret_cast<float4 *>(smem_al + a.out_off) : vg;
+            // this job's rotation table w_m (steps a5, a6, reading A22 applied behind the integration), loaded while the MMAs run;
+            // two tables alternate: a warp is never more than one job ahead of the slowest one (tmem_empty needs all of them)
+            float2 *rot = reinterpret_cast<float2 *>(smem_al + a.rot_off + (it & 1) * a.rot_bytes);
+            {
+                const int bl = w.prob / a.C, c = w.prob - bl * a.C;
+                for (int m = threadIdx.x - 32 * kFirstEpiWarp; m < a.Mpad; m += 32 * kEpiWarps) {
+                    float2 wv = make_float2(1.f, 0.f);
+                    if (a.phase && m < a.M) {
+                        wv = a.phase[((size_t)(a.b0 + bl) * a.S + (m >> 1)) * a.C + c];
+                        if (a.poff) {
+                            const float2 q = a.poff[m];
+                            wv = make_float2(wv.x * q.x - wv.y * q.y, wv.x * q.y + wv.y * q.x);
+                        }
+                    }
+                    rot[m] = wv;
+                }
+                asm volatile("bar.sync 3, %0;" ::"n"(32 * kEpiWarps) : "memory");
+            }
             if (STAGED && it > 0) {
                 // the previous job's bulk store must have read the staging block before it is overwritten
-                if (threadIdx.x == 64) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+                if (threadIdx.x == 32 * kFirstEpiWarp) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
                 asm volatile("bar.sync 1, %0;" ::"n"(32 * kEpiWarps) : "memory");
             }
             mbar_wait(tmem_full, it & 1);
@@ -302,12 +340,14 @@ __global__ void __launch_bounds__(kThreads, 1) xstage_tc_kernel(const XArgs a) {
                                 im[q] = pl ? val[4 + q] : got;
                             }
                             const int b0 = job->g[g].out_col + 8 * c + 4 * pl;      // input index of column q = 0
+                            const float2 ur = rot[min(mrow, a.Mpad - 1)];
+                            const float2 u = make_float2(ur.x * inv_s2, ur.y * inv_s2);
 #pragma unroll
                             for (int e = 0; e < 2; ++e) {
                                 const int b = b0 + 2 * e, k = b >> 1;
                                 if (row_ok && b < a.M && i <= k)
-                                    vc[((size_t)k * (k + 1) / 2 + i) * 2 + p] =
-                                        make_float4(re[2 * e] * inv_s2, im[2 * e] * inv_s2, re[2 * e + 1] * inv_s2, im[2 * e + 1] * inv_s2);
+                                    vc[((size_t)k * (k + 1) / 2 + i) * 2 + p] = rotate2(re[2 * e], im[2 * e], re[2 * e + 1], im[2 * e + 1], u,
+                                                                                    *reinterpret_cast<const float4 *>(rot + b));
                             }
                         }
                     }
@@ -328,13 +368,18 @@ __global__ void __launch_bounds__(kThreads, 1) xstage_tc_kernel(const XArgs a) {
                     tmem_ld16(t0 + c_first * 16, re);
                     tmem_ld16(t0 + gn + c_first * 16, im);
                 }
+                const float2 ur = rot[min(arow, a.Mpad - 1)];
+                const float2 u = make_float2(ur.x * inv_s2, ur.y * inv_s2);
                 for (int c = c_first; c < c_end; c += kEpiSub) {
+                    float4 wb[8];                           // column factors of this chunk: w_b, w_{b+1} per pair (no TMEM dependence)
+#pragma unroll
+                    for (int e = 0; e < 8; ++e) wb[e] = *reinterpret_cast<const float4 *>(rot + out_col + c * 16 + 2 * e);
                     tmem_ld_wait();
                     float4 v[8];
 #pragma unroll
                     for (int e = 0; e < 8; ++e)
-                        v[e] = make_float4(__uint_as_float(re[2 * e]) * inv_s2, __uint_as_float(im[2 * e]) * inv_s2,
-                                           __uint_as_float(re[2 * e + 1]) * inv_s2, __uint_as_float(im[2 * e + 1]) * inv_s2);
+                        v[e] = rotate2(__uint_as_float(re[2 * e]), __uint_as_float(im[2 * e]), __uint_as_float(re[2 * e + 1]),
+                                       __uint_as_float(im[2 * e + 1]), u, wb[e]);
                     if (c + kEpiSub < c_end) {
                         tmem_ld16(t0 + (c + kEpiSub) * 16, re);
                         tmem_ld16(t0 + gn + (c + kEpiSub) * 16, im);
@@ -366,13 +411,13 @@ __global__ void __launch_bounds__(kThreads, 1) xstage_tc_kernel(const XArgs a) {
             if (STAGED) {
                 asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy writes -> visible to the bulk copy
                 asm volatile("bar.sync 2, %0;" ::"n"(32 * kEpiWarps) : "memory");
-                if (threadIdx.x == 64) {
+                if (threadIdx.x == 32 * kFirstEpiWarp) {
                     bulk_s2g(vg, smem_base + a.out_off, (uint32_t)(a.n_bl * 32));
                     asm volatile("cp.async.bulk.commit_group;" ::: "memory");
                 }
             }
         }
-        if (STAGED && threadIdx.x == 64) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+        if (STAGED && threadIdx.x == 32 * kFirstEpiWarp) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
     }
 
     tc_fence_before();
@@ -458,26 +503,35 @@ void build_xjobs(cobalt_plan_s *p) {
     const size_t slack = (size_t)slack_rows * 256;
     // staged epilogue: the whole [n_bl][2][2] block of a channel, if that still leaves three load stages
     size_t out_bytes = ((size_t)p->n_bl * 32 + 127) / 128 * 128;
-    const size_t fixed = 1024 /*alignment*/ + kBarrierBytes + slack;
+    const size_t rot_bytes = ((size_t)p->Mpad * sizeof(float2) + 511) / 512 * 512;    // two tables: a multiple of 1024 together
+    p->x_rot_bytes = rot_bytes;
+    const size_t fixed = 1024 /*alignment*/ + kBarrierBytes + 2 * rot_bytes + slack;
     p->x_staged = p->jobs.size() == 1 && fixed + out_bytes + 3 * stage_bytes <= (size_t)227 * 1024;
     if (!p->x_staged) out_bytes = 0;
     const size_t budget = 227 * 1024 - fixed - out_bytes;
     int stages = (int)(budget / stage_bytes);
     if (stages > 8) stages = 8;
     p->x_stages = stages;
-    p->x_out_off = kBarrierBytes + (size_t)stages * stage_bytes + slack;
+    p->x_out_off = kBarrierBytes + 2 * rot_bytes + (size_t)stages * stage_bytes + slack;
     p->x_smem_bytes = fixed + (size_t)stages * stage_bytes + out_bytes;
 }
 
 cudaError_t launch_xsum_n(const cobalt_plan_s *p, cudaStream_t st, int nb, float2 *d_vis, size_t dump_stride, int splits);   // ingest.cu
 
-cudaError_t launch_xstage_tc(const cobalt_plan_s *p, cudaStream_t st, const void *d_z, int nb, float2 *d_vis, size_t dump_stride) {
+cudaError_t launch_xstage_tc(const cobalt_plan_s *p, cudaStream_t st, const void *d_z, int nb, float2 *d_vis, size_t dump_stride,
+                             const XCall &xc) {
     if (p->x_stages < 2) return cudaErrorInvalidConfiguration;
     XArgs a;
     a.z = static_cast<const unsigned char *>(d_z);
     a.vis = d_vis;
     a.jobs = p->d_jobs;
-    a.scale = p->d_scale;
+    a.phase = xc.phase;
+    a.poff = xc.poff;
+    a.b0 = xc.b0;
+    a.S = p->S;
+    a.inv_s2 = xc.inv_s2;
+    a.rot_off = kBarrierBytes;
+    a.rot_bytes = (uint32_t)p->x_rot_bytes;
     a.z_subband_bytes = p->z_subband_bytes;
     a.n_bl = p->n_bl;
     a.C = p->C;
