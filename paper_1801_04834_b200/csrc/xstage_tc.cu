@@ -109,6 +109,11 @@ __device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&v)[16]) {
           "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
         : "r"(taddr));
 }
+__device__ __forceinline__ void tmem_ld8(uint32_t taddr, uint32_t (&v)[8]) {
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7])
+                 : "r"(taddr));
+}
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 
 // Two visibilities (same row input, column inputs b and b + 1) times u conj(w_b), u conj(w_{b+1}): u = w_row / s^2, wb = (w_b, w_{b+1}).
@@ -363,46 +368,56 @@ __global__ void __launch_bounds__(kThreads, 1) xstage_tc_kernel(const XArgs a) {
                 const int c_first = (max(0, (max(row0, row_min) & ~1) - out_col) >> 4) + sub;   // first chunk touching k >= i
                 const int c_end = (min(gn, a.M - out_col) + 15) >> 4;
                 const int i_max = (min(row0 + rows_w, a.M) - 1) >> 1;           // last station of this warp's rows
-                uint32_t re[16], im[16];
-                if (c_first < c_end) {
-                    tmem_ld16(t0 + c_first * 16, re);
-                    tmem_ld16(t0 + gn + c_first * 16, im);
-                }
+                // The warp's chunks as pieces of 8 columns (4 station-pol pairs), double buffered: the TMEM load of the next
+                // piece is issued before the current one is rotated and stored, so that the load latency (TMEM reads are the
+                // floor of this exposed epilogue) overlaps the arithmetic.  tcgen05.wait::ld waits for every outstanding load,
+                // hence exactly one load pair is in flight at each wait.
                 const float2 ur = rot[min(arow, a.Mpad - 1)];
                 const float2 u = make_float2(ur.x * inv_s2, ur.y * inv_s2);
-                for (int c = c_first; c < c_end; c += kEpiSub) {
-                    float4 wb[8];                           // column factors of this chunk: w_b, w_{b+1} per pair (no TMEM dependence)
+                const int n_pieces = c_first < c_end ? 2 * ((c_end - c_first + kEpiSub - 1) / kEpiSub) : 0;
+                auto piece_col = [&](int pc) { return (c_first + (pc >> 1) * kEpiSub) * 16 + 8 * (pc & 1); };   // column within the group
+                auto process = [&](const uint32_t (&re)[8], const uint32_t (&im)[8], int pc) {
+                    const int col0 = out_col + piece_col(pc);
+                    float4 v[4];
 #pragma unroll
-                    for (int e = 0; e < 8; ++e) wb[e] = *reinterpret_cast<const float4 *>(rot + out_col + c * 16 + 2 * e);
-                    tmem_ld_wait();
-                    float4 v[8];
-#pragma unroll
-                    for (int e = 0; e < 8; ++e)
+                    for (int e = 0; e < 4; ++e)
                         v[e] = rotate2(__uint_as_float(re[2 * e]), __uint_as_float(im[2 * e]), __uint_as_float(re[2 * e + 1]),
-                                       __uint_as_float(im[2 * e + 1]), u, wb[e]);
-                    if (c + kEpiSub < c_end) {
-                        tmem_ld16(t0 + (c + kEpiSub) * 16, re);
-                        tmem_ld16(t0 + gn + (c + kEpiSub) * 16, im);
-                    }
-                    const int col0 = out_col + c * 16;
+                                       __uint_as_float(im[2 * e + 1]), u, *reinterpret_cast<const float4 *>(rot + col0 + 2 * e));
                     const int k0 = col0 >> 1;
-                    if (k0 >= i_max && col0 + 16 <= a.M) {
-                        // whole chunk above the diagonal for every row of the warp: baseline index of (i, k0 + e) steps by k
+                    if (k0 >= i_max && col0 + 8 <= a.M) {
+                        // whole piece above the diagonal for every row of the warp: baseline index of (i, k0 + e) steps by k
                         if (lane_ok) {
                             int idx = (k0 * (k0 + 1) / 2 + i) * 2 + p;
 #pragma unroll
-                            for (int e = 0; e < 8; ++e) {
+                            for (int e = 0; e < 4; ++e) {
                                 vc[idx] = v[e];
                                 idx += 2 * (k0 + e + 1);
                             }
                         }
                     } else {
 #pragma unroll
-                        for (int e = 0; e < 8; ++e) {
+                        for (int e = 0; e < 4; ++e) {
                             const int b = col0 + 2 * e, k = b >> 1;
                             if (lane_ok && b < a.M && i <= k) vc[((size_t)k * (k + 1) / 2 + i) * 2 + p] = v[e];
                         }
                     }
+                };
+                uint32_t reA[8], imA[8], reB[8], imB[8];
+                if (n_pieces > 0) {
+                    tmem_ld8(t0 + piece_col(0), reA);
+                    tmem_ld8(t0 + gn + piece_col(0), imA);
+                }
+                for (int pc = 0; pc < n_pieces; pc += 2) {
+                    tmem_ld_wait();
+                    tmem_ld8(t0 + piece_col(pc + 1), reB);            // n_pieces is even
+                    tmem_ld8(t0 + gn + piece_col(pc + 1), imB);
+                    process(reA, imA, pc);
+                    tmem_ld_wait();
+                    if (pc + 2 < n_pieces) {
+                        tmem_ld8(t0 + piece_col(pc + 2), reA);
+                        tmem_ld8(t0 + gn + piece_col(pc + 2), imA);
+                    }
+                    process(reB, imB, pc + 1);
                 }
             }
             tc_fence_before();
