@@ -51,8 +51,8 @@ typedef enum {
 typedef enum {
     /* X-stage on tcgen05 tensor cores, fp16 operands, fp32 accumulation in TMEM.
      * Tolerance vs the float64 oracle: ||dV||_F / ||V||_F <= 2e-3 per (subband, channel).
-     * The fp16 operands carry a power-of-two scale chosen per call from max|bandpass| so that
-     * full-scale input cannot overflow (undone exactly in the X-stage epilogue). */
+     * The fp16 operands carry a power-of-two scale fixed by input_bits and the FIR gain so that full-scale
+     * input cannot overflow (undone exactly in the X-stage epilogue). */
     COBALT_MODE_TENSOR_FP16 = 0,
     /* Everything in fp32 (SIMT FMA correlator).  Tolerance: max |dV| / sqrt(V_ii V_kk) <= 1e-4. */
     COBALT_MODE_EXACT_FP32 = 1
@@ -115,6 +115,8 @@ int cobalt_plan(cobalt_plan_t **out, int stations, int subbands, int channels, i
  *   z[t][j]  = F[t][j] b[j] exp(-2 pi i frac(f[s][j] tau_a))   (frac in fp64)
  *   V[s][j][bl(i,k)][p][q] = sum_t z_{i,p}[t][j] conj(z_{k,q}[t][j])              (A9, A10)
  * and the last 15 C consumed samples of every stream become the new history (stateful!).
+ * The factor w_a[j] = b[j] exp(-2 pi i frac(f[s][j] tau_a)) is constant over the call, so the library correlates F and
+ * multiplies each visibility by w_i conj(w_k) (the same product; w from the fp64 phase table, the multiplication in fp32).
  * The call only enqueues kernels on `cuda_stream` (no synchronisation, no allocation): it can be captured in a CUDA
  * graph; the history alternates between two buffers from call to call, so capture calls in pairs.
  * Only the first N_u = floor(N/C) C samples of each stream are consumed (A11). */
@@ -237,7 +239,7 @@ int cobalt_debug_unpack(void *cuda_stream, int input_bits, const void *d_in, lon
 /* Steps a1-a7 for ONE subband `sb` of d_samples (full [B][..] array as in cobalt_process):
  * d_z receives z as [C][2S][n_t] complex64 (input index = 2*station + pol).  Reads the history
  * of that subband but does NOT advance it.  In TENSOR_FP16 mode the values are the fp16
- * operands (converted back to fp32) that the X-stage would consume. */
+ * operands that the X-stage consumes, converted back to fp32 and multiplied by the rotation w_a[j] the X-stage applies. */
 int cobalt_debug_channelised(cobalt_plan_t *plan, void *cuda_stream, const void *d_samples,
                              const double *d_delays, const float *d_bandpass, int sb, void *d_z);
 /* Step a8-a9 alone for one subband: d_z [C][2S][n_t] complex64 (caller supplied) ->

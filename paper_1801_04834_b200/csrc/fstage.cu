@@ -1,29 +1,31 @@
 // F-stage of the Cobalt correlator pipeline, hand-written for sm_100a.
 //
-// One fused kernel per chunk of subbands does steps a1-a7 of SURVEY.md sec 8(a) (P:L360, P:L89,
-// P:L368): int16/int8 -> fp32 unpack, 16-tap polyphase FIR with history, C-point forward DFT,
-// ascending-frequency channel order, delay-phase rotation * bandpass, and the transposed write of
-// the channelised data in the layout the X-stage consumes (cobalt_internal.h).  A tiny fp64 kernel
-// builds the per-(station, channel) rotation table first (phase angles in double precision),
-// and a copy kernel carries the FIR history to the next call.
+// One fused kernel per chunk of subbands does steps a1-a4 and a7 of SURVEY.md sec 8(a): int16/int8 -> fp32
+// unpack, 16-tap polyphase FIR with history, C-point forward DFT, ascending-frequency channel order, and the transposed write
+// of the channelised data in the layout the X-stage consumes (cobalt_internal.h).  The delay-phase rotation and the bandpass
+// (a5, a6) are constants per (input, channel) within a call: the fp64 phase_table_kernel below builds them and the
+// X-stage multiplies every visibility by w_i conj(w_k) -- the same product as rotating every sample, once per visibility
+// instead of once per sample.  Only the time-varying part of cobalt_process_interp (reading A21) is applied here, per sample.
+// A copy kernel carries the FIR history to the next call.
 //
-// fstage_kernel<C, BITS, TENSOR> is warp specialised (17 warps, one CTA per SM):
+// fstage_kernel<C, BITS, TENSOR, INTERP> is warp specialised (18 warps, one CTA per SM):
 //   CTA      = 256 / C consecutive streams (subband, station, pol) x a run of 64-spectrum k-tiles,
 //              walked in sub-tiles of 16 spectra; for C = 256 the two polarisations of a station one after the other.
 //   warp 16  = producer: the raw integer rows of the next sub-tiles (time-contiguous, so one bulk
-//              copy -- cp.async.bulk, SASS UBLKCP -- per stream and sub-tile) land in a 4-deep
-//              shared-memory ring signalled on mbarriers; the first sub-tile of a CTA is the 16-row
-//              warm-up taken from the carried history (or from the preceding samples).
+//              copy -- cp.async.bulk, SASS UBLKCP -- per stream and sub-tile, starting at the station's coarse sample
+//              offset, reading A25) land in a 3-deep shared-memory ring signalled on mbarriers; the first sub-tile of a CTA
+//              is the 16-row warm-up taken from the carried history (or from the preceding samples).
 //   warps 0-7  = FIR: thread = polyphase branch.  Transposed-form filter: every new sample is
 //              converted once and added, scaled by its 16 weights, to the 16 pending outputs held
 //              in registers as (re, im) pairs (packed fma.rn.f32x2: one issue slot per two FMAs);
-//              the completed output goes to a double-buffered shared-memory tile.
-//   warps 8-15 = FFT + rotate + transpose: thread = (spectrum, 1/16 of its channels): radix-16 pass
-//              in registers, twiddle, warp-local shared-memory exchange, radix-R pass (C = 16 R),
-//              rotation * bandpass from a per-CTA table, fp16 (or fp32) conversion, staged
-//              transposed in shared memory and flushed as whole 32-byte sectors (TENSOR) /
-//              128-byte runs (EXACT).  The (-1)^ph needed for the ascending-frequency channel order
-//              (D[(j + C/2) mod C]) is folded into the FIR weights, so the reorder is free.
+//              the completed output goes to a 3-deep ring of shared-memory tiles.  The weights carry (-1)^ph (the
+//              ascending-frequency channel order D[(j + C/2) mod C] for free) and the power-of-two scale of the fp16
+//              intermediate (exact).
+//   warps 8-15 = FFT + transpose, two teams of four warps on alternate sub-tiles: thread = (two spectra, 1/16 of their
+//              channels): radix-16 pass in registers, twiddle, warp-local shared-memory exchange, radix-R pass (C = 16 R),
+//              [INTERP: exp(-2 pi i t step)], fp16 (or fp32) conversion, staged transposed in shared memory.  Spectra beyond
+//              n_t, rows beyond 2S and lost tiles (valid-sample flags, reading A24) leave as exact zeros.
+//   warp 17  = issues the 5-D tensor stores (cp.async.bulk.tensor, SASS UTMASTG) of the staged tiles.
 #include "cobalt_internal.h"
 #include "ptx.cuh"
 

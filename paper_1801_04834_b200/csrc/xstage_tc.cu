@@ -19,8 +19,9 @@
 //   real products at once; the epilogue adds / subtracts its quadrants)            (2S <= 192)
 // or, for large arrays, one (128-row block) x (<= 256-column chunk) tile per job.
 //
-// Warp roles (576 threads, persistent CTAs, one per SM): warp 0 = bulk-copy producer, warp 1 = TMEM
-// allocator + single-thread MMA issuer, warps 2-17 = epilogue (tcgen05.ld -> triangular baseline
+// Warp roles (640 threads, persistent CTAs, one per SM): warp 0 = bulk-copy producer, warp 1 = TMEM
+// allocator + single-thread MMA issuer, warps 2-3 idle (they complete the warp group that hands its registers
+// to the epilogue), warps 4-19 = epilogue (tcgen05.ld -> rotation w_i conj(w_k) / s^2 -> triangular baseline
 // index -> 16-byte stores of (re, im) pairs into a shared-memory image of the channel's output block,
 // which leaves with one bulk store; direct global stores when the block does not fit).
 #include "cobalt_internal.h"
@@ -270,7 +271,7 @@ __global__ void __launch_bounds__(kThreads, 1) xstage_tc_kernel(const XArgs a) {
     } else {
         // ------------------------------------------------------------------ epilogue
         asm volatile("setmaxnreg.inc.sync.aligned.u32 112;");
-        // Warps 2..9: warp w reads TMEM lane quarter w % 4 (the only one it may access); the two warps of a quarter
+        // Warps 4..19: warp w reads TMEM lane quarter w % 4 (the only one it may access); the two warps of a quarter
         // take alternate 16-column chunks.  The TMEM load of a warp's next chunk is in flight while it stores the
         // current one.
         const int wq = warp & 3;
