@@ -77,6 +77,15 @@ def _load():
         lib.oracle_valid_counts.argtypes = [ctypes.c_int, ctypes.c_longlong, ctypes.c_int, ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p]
         lib.oracle_correlate_dumps.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_longlong, ctypes.c_int, ctypes.c_int, _D, _D]
         lib.oracle_correlate_dumps.restype = ctypes.c_int
+        lib.oracle_beamform_coherent.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_longlong, ctypes.c_int, _D,
+                                                 ctypes.c_double, ctypes.c_double, _D, _D]
+        lib.oracle_stokes.argtypes = [ctypes.c_longlong, _D, _D, ctypes.c_int, _D]
+        lib.oracle_integrate.argtypes = [ctypes.c_longlong, ctypes.c_longlong, ctypes.c_int, _D, _D]
+        lib.oracle_coherent_stokes.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_longlong, ctypes.c_int, _D, ctypes.c_double,
+                                               ctypes.c_double, _D, ctypes.c_int, ctypes.c_int, _D]
+        lib.oracle_coherent_stokes.restype = ctypes.c_int
+        lib.oracle_incoherent_stokes.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_longlong, _D, ctypes.c_int, ctypes.c_int, _D]
+        lib.oracle_incoherent_stokes.restype = ctypes.c_int
         _lib = lib
     return _lib
 
@@ -343,3 +352,68 @@ def process_subband_ext(samples: np.ndarray, C: int, delays, bandpass, f_sb: flo
     if valid is not None:
         z = flag_tiles(z, valid)
     return correlate_dumps(z, dumps)
+
+
+# ------------------------------------------------------------------ beamformer
+def beamform_coherent(z: np.ndarray, beam_delays, f_sb: float, f_s: float = F_S) -> np.ndarray:
+    """z complex [S][2][n_t][C], beam_delays [n_beams][S] seconds -> Y complex [n_beams][2][C][n_t] (reading A28)."""
+    zr = _c2r(z)
+    S, _, n_t, C = zr.shape[:4]
+    bd = _f64(beam_delays)
+    assert bd.ndim == 2 and bd.shape[1] == S
+    y = np.empty((bd.shape[0], 2, C, n_t, 2), dtype=np.float64)
+    _load().oracle_beamform_coherent(S, C, n_t, bd.shape[0], _p(bd), f_sb, f_s, _p(zr), _p(y))
+    return _r2c(y)
+
+
+def stokes(x: np.ndarray, y: np.ndarray, n_stokes: int = 4) -> np.ndarray:
+    """x, y complex [...] -> float64 [n_stokes][...]: I, Q, U, V of the dual-polarisation sample (reading A29)."""
+    assert n_stokes in (1, 4) and x.shape == y.shape
+    xr, yr = _c2r(x), _c2r(y)
+    out = np.empty((n_stokes,) + x.shape, dtype=np.float64)
+    _load().oracle_stokes(x.size, _p(xr), _p(yr), n_stokes, _p(out))
+    return out
+
+
+def integrate(a: np.ndarray, t_int: int) -> np.ndarray:
+    """float64 [..., n_t] -> [..., n_t // t_int]: sums of t_int consecutive samples, tail dropped (reading A30)."""
+    a = _f64(a)
+    n_t = a.shape[-1]
+    out = np.empty(a.shape[:-1] + (n_t // t_int,), dtype=np.float64)
+    _load().oracle_integrate(a.size // n_t if n_t else 0, n_t, t_int, _p(a), _p(out))
+    return out
+
+
+def coherent_stokes(z: np.ndarray, beam_delays, f_sb: float, n_stokes: int, t_int: int, f_s: float = F_S) -> np.ndarray:
+    """z complex [S][2][n_t][C] -> float64 [n_beams][n_stokes][C][n_t // t_int] (A28 -> A29 -> A30)."""
+    zr = _c2r(z)
+    S, _, n_t, C = zr.shape[:4]
+    bd = _f64(beam_delays)
+    out = np.empty((bd.shape[0], n_stokes, C, n_t // t_int), dtype=np.float64)
+    if _load().oracle_coherent_stokes(S, C, n_t, bd.shape[0], _p(bd), f_sb, f_s, _p(zr), n_stokes, t_int, _p(out)):
+        raise MemoryError("oracle_coherent_stokes")
+    return out
+
+
+def incoherent_stokes(z: np.ndarray, n_stokes: int, t_int: int) -> np.ndarray:
+    """z complex [S][2][n_t][C] -> float64 [n_stokes][C][n_t // t_int] (reading A31)."""
+    zr = _c2r(z)
+    S, _, n_t, C = zr.shape[:4]
+    out = np.empty((n_stokes, C, n_t // t_int), dtype=np.float64)
+    if _load().oracle_incoherent_stokes(S, C, n_t, _p(zr), n_stokes, t_int, _p(out)):
+        raise MemoryError("oracle_incoherent_stokes")
+    return out
+
+
+def channelise_subband(samples: np.ndarray, C: int, delays, bandpass, f_sb: float, hist: np.ndarray | None = None,
+                       f_s: float = F_S, T: int = TAPS, delays_end=None, phase0=None, valid=None) -> np.ndarray:
+    """Steps 1-7 (+ A22 offsets, A24 flags) of one subband: integer samples [S][2][N][2] -> z complex [S][2][n_t][C]:
+    the input of the beamformer functions above ("the first four kernels in common")."""
+    s = np.ascontiguousarray(samples)
+    x = _r2c(unpack4(s)) if s.dtype == np.uint8 else _r2c(unpack(s))
+    z = fstage(x, C, hist=hist, delays=delays, bandpass=bandpass, f_sb=f_sb, f_s=f_s, T=T, delays_end=delays_end)
+    if phase0 is not None:
+        z = phase_offsets(z, phase0)
+    if valid is not None:
+        z = flag_tiles(z, valid)
+    return z

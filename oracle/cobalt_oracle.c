@@ -29,7 +29,8 @@
  * delay slope, P10 history carry, P11 brute force (oracle_channel_direct below
  * + a numpy brute force), P12 linearity, P13 statistics, P16 time-varying delay
  * (equal ends = static rotation; closed-form geometric series), P17-P21 (coarse shift,
- * phase offsets, dumps, valid-sample flags and counts, 4-bit unpack).  No function here is
+ * phase offsets, dumps, valid-sample flags and counts, 4-bit unpack), P22-P25 (beamformer: coherent sum,
+ * Stokes parameters, time integration, incoherent sum; tests/test_oracle_pins_bf.py).  No function here is
  * "parity unpinned".
  *
  * Layouts (all row-major, last index fastest):
@@ -395,6 +396,136 @@ int oracle_correlate_dumps(int S, int C, long long n_t, int D, int tile, const d
                             o[0] = re;
                             o[1] = im;
                         }
+    return 0;
+}
+
+/* =====================================================================================================
+ * the beamformer pipeline, at the channel resolution of the
+ * plan ("Cobalt performs delay compensation, bandpass correction and beamforming at 256 channels per subband").
+ * Input of every function below is z, the delay-compensated, bandpass-corrected channelised data of steps 1-7
+ * ("Both beam types have the first four kernels in common").  Readings A28-A31 of DESIGN.md.  The final
+ * transformation "to the requested output resolution" (inverse FFT / second FFT) is not part of this row.
+ * ===================================================================================================== */
+
+/* Reading A28 ("Coherent beamforming first adjusts the beam direction with a phase shift and sums over
+ * antenna fields"; "The beamforming kernel operates in a similar way [to delay compensation] to form beams
+ * with an offset from the center": the phase angle of (beam, station, channel) in double precision):
+ *   Y[b][p][j][t] = sum_a exp(-2 pi i frac(f[j] taub[b][a])) z[a][p][t][j]
+ * taub[b][a] = the delay of station a for beam b relative to the phase centre, seconds, with the sign sense of the
+ * station delay of step 7 (a positive value delays station a's signal); f[j] = the channel's sky frequency (A6).
+ * No normalisation by the number of stations (like A10: a scalar the caller can apply). */
+void oracle_beamform_coherent(int S, int C, long long n_t, int n_beams, const double *beam_delays /*[n_beams][S]*/,
+                              double f_sb, double f_s, const double *z /*[S][2][n_t][C][2]*/,
+                              double *y /*[n_beams][2][C][n_t][2]*/) {
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int b = 0; b < n_beams; ++b)
+        for (int p = 0; p < 2; ++p)
+            for (int j = 0; j < C; ++j) {
+                const double f = oracle_channel_frequency(C, f_sb, f_s, j);
+                for (long long t = 0; t < n_t; ++t) {
+                    double re = 0.0, im = 0.0;
+                    for (int a = 0; a < S; ++a) {
+                        double cyc = f * beam_delays[(long long)b * S + a];
+                        double frac = cyc - floor(cyc);
+                        double wr = cos(-2.0 * ORACLE_PI * frac), wi = sin(-2.0 * ORACLE_PI * frac);
+                        const double *zz = z + 2 * ((((long long)a * 2 + p) * n_t + t) * C + j);
+                        re += wr * zz[0] - wi * zz[1];
+                        im += wr * zz[1] + wi * zz[0];
+                    }
+                    double *o = y + 2 * ((((long long)b * 2 + p) * C + j) * n_t + t);
+                    o[0] = re;
+                    o[1] = im;
+                }
+            }
+}
+
+/* Reading A29 ("Stokes I only or Stokes IQUV"): the Stokes parameters of one dual-polarisation complex
+ * sample (X, Y), linear feeds:
+ *   I = |X|^2 + |Y|^2,  Q = |X|^2 - |Y|^2,  U = 2 Re(X conj(Y)),  V = 2 Im(X conj(Y)).
+ * n_stokes = 1 (I only) or 4.  out [n_stokes][n]. */
+void oracle_stokes(long long n, const double *x /*[n][2]*/, const double *y /*[n][2]*/, int n_stokes, double *out) {
+    for (long long i = 0; i < n; ++i) {
+        double xr = x[2 * i], xi = x[2 * i + 1], yr = y[2 * i], yi = y[2 * i + 1];
+        double px = xr * xr + xi * xi, py = yr * yr + yi * yi;
+        out[i] = px + py;
+        if (n_stokes == 4) {
+            out[n + i] = px - py;
+            out[2 * n + i] = 2.0 * (xr * yr + xi * yi);
+            out[3 * n + i] = 2.0 * (xi * yr - xr * yi);
+        }
+    }
+}
+
+/* Reading A30 ("Time resolution can be traded against frequency resolution"; "complex voltages cannot
+ * be time averaged", so Stokes only): output sample u of a row is the plain sum of the t_int input samples
+ * [u t_int, (u+1) t_int); n_out = floor(n_t / t_int), trailing samples are not consumed (as in A11).
+ * in [rows][n_t] -> out [rows][n_out]. */
+void oracle_integrate(long long rows, long long n_t, int t_int, const double *in, double *out) {
+    const long long n_out = n_t / t_int;
+    for (long long r = 0; r < rows; ++r)
+        for (long long u = 0; u < n_out; ++u) {
+            double s = 0.0;
+            for (int k = 0; k < t_int; ++k) s += in[r * n_t + u * t_int + k];
+            out[r * n_out + u] = s;
+        }
+}
+
+/* P:L362 "coherent beamforming ... sums over antenna fields, then optionally computes Stokes parameters":
+ * A28 -> A29 per (beam, channel, spectrum) -> A30.  out [n_beams][n_stokes][C][n_out].  Returns 1 on allocation failure. */
+int oracle_coherent_stokes(int S, int C, long long n_t, int n_beams, const double *beam_delays, double f_sb, double f_s,
+                           const double *z, int n_stokes, int t_int, double *out) {
+    const long long n_out = n_t / t_int, n = (long long)C * n_t;
+    double *y = (double *)malloc(sizeof(double) * 2 * (size_t)n_beams * 2 * (size_t)n);
+    double *st = (double *)malloc(sizeof(double) * (size_t)n_stokes * (size_t)n);
+    if (!y || !st) {
+        free(y);
+        free(st);
+        return 1;
+    }
+    oracle_beamform_coherent(S, C, n_t, n_beams, beam_delays, f_sb, f_s, z, y);
+    for (int b = 0; b < n_beams; ++b) {
+        oracle_stokes(n, y + 2 * ((long long)b * 2) * n, y + 2 * ((long long)b * 2 + 1) * n, n_stokes, st);   /* [k][C][n_t] */
+        oracle_integrate((long long)n_stokes * C, n_t, t_int, st, out + (long long)b * n_stokes * C * n_out);
+    }
+    free(y);
+    free(st);
+    return 0;
+}
+
+/* Reading A31 ("incoherent beamforming first computes Stokes parameters and then sums over antenna fields"):
+ *   S_k[j][t] = sum_a stokes_k(z[a][X][t][j], z[a][Y][t][j]),  then A30.  out [n_stokes][C][n_out]. */
+int oracle_incoherent_stokes(int S, int C, long long n_t, const double *z /*[S][2][n_t][C][2]*/, int n_stokes, int t_int,
+                             double *out) {
+    const long long n_out = n_t / t_int, n = (long long)C * n_t;
+    double *xs = (double *)malloc(sizeof(double) * 2 * (size_t)n);     /* one station, [C][n_t] per polarisation */
+    double *ys = (double *)malloc(sizeof(double) * 2 * (size_t)n);
+    double *st = (double *)malloc(sizeof(double) * (size_t)n_stokes * (size_t)n);
+    double *acc = (double *)calloc((size_t)n_stokes * (size_t)n, sizeof(double));
+    if (!xs || !ys || !st || !acc) {
+        free(xs);
+        free(ys);
+        free(st);
+        free(acc);
+        return 1;
+    }
+    for (int a = 0; a < S; ++a) {
+        for (int j = 0; j < C; ++j)
+            for (long long t = 0; t < n_t; ++t) {
+                const double *zx = z + 2 * ((((long long)a * 2 + 0) * n_t + t) * C + j);
+                const double *zy = z + 2 * ((((long long)a * 2 + 1) * n_t + t) * C + j);
+                xs[2 * (j * n_t + t)] = zx[0];
+                xs[2 * (j * n_t + t) + 1] = zx[1];
+                ys[2 * (j * n_t + t)] = zy[0];
+                ys[2 * (j * n_t + t) + 1] = zy[1];
+            }
+        oracle_stokes(n, xs, ys, n_stokes, st);
+        for (long long i = 0; i < (long long)n_stokes * n; ++i) acc[i] += st[i];
+    }
+    oracle_integrate((long long)n_stokes * C, n_t, t_int, acc, out);
+    free(xs);
+    free(ys);
+    free(st);
+    free(acc);
     return 0;
 }
 
