@@ -170,6 +170,56 @@ typedef struct {
 } cobalt_io_t;
 int cobalt_process_ex(cobalt_plan_t *plan, void *cuda_stream, const cobalt_io_t *io);
 
+/* ---------------------------------------------------------------------------------------
+ * cobalt_beamform: the beamformer pipeline of SURVEY.md sec 8(f) row 4 for one block, at the
+ * plan's channel count ("Cobalt performs delay compensation, bandpass correction and beamforming at 256 channels per
+ * subband"); enqueued on `cuda_stream` like cobalt_process, with the same channelisation (steps a1-a4), delay
+ * compensation, bandpass, phase offsets, coarse delays, input layouts and valid-sample flags, and the same history
+ * carry (stateful; a plan serves either the correlator or the beamformer stream of an observation).
+ * With z[a][p][t][j] the delay-compensated, bandpass-corrected channelised sample of station a, polarisation p
+ * (cobalt_process, line "z[t][j] = ..."):
+ *   coherent beam b (reading A28; "adjusts the beam direction with a phase shift and sums over antenna fields",
+ *   P:L368 "The beamforming kernel operates in a similar way": the phase angle in fp64):
+ *       Y[b][p][j][t] = sum_a exp(-2 pi i frac(f[s][j] tau_{b,a})) z[a][p][t][j]
+ *   Stokes parameters of a dual-polarisation sample (X, Y) (reading A29):
+ *       I = |X|^2 + |Y|^2,  Q = |X|^2 - |Y|^2,  U = 2 Re(X conj(Y)),  V = 2 Im(X conj(Y))
+ *   time integration (reading A30; Stokes only, "complex voltages cannot be time averaged"): output sample u is the sum
+ *       of the t_int spectra [u t_int, (u+1) t_int); n_out = floor(n_t / t_int), the tail is not consumed
+ *   incoherent beam (reading A31; "first computes Stokes parameters and then sums over antenna fields"):
+ *       S_k[j][t] = sum_a stokes_k(z[a][X][t][j], z[a][Y][t][j]).
+ * No division by the number of stations or samples.  The paper's final step, "transforms to the requested output
+ * resolution" (an inverse and a second FFT), is not part of this call.
+ *   samples, delays, delays_end, bandpass, valid   device, as in cobalt_io_t (delays_end and valid may be NULL)
+ *   beam_delays  device [n_beams][S] double, seconds: tau_{b,a}, the delay of station a for beam b relative to the phase
+ *                centre, with the sign sense of `delays`; ignored for COBALT_BF_INCOHERENT_STOKES
+ *   n_beams      >= 1 (coherent products)
+ *   product      COBALT_BF_COHERENT_VOLTAGES   out = [B][n_beams][2 pol][C][n_t] complex64
+ *                COBALT_BF_COHERENT_STOKES     out = [B][n_beams][n_stokes][C][n_out] float
+ *                COBALT_BF_INCOHERENT_STOKES   out = [B][n_stokes][C][n_out] float
+ *   n_stokes     1 (I) or 4 (I, Q, U, V); t_int a power of two in [1, 128] (both ignored for voltages)
+ *   out          device, 8-byte aligned, fully overwritten.
+ * COBALT_MODE_TENSOR_FP16: the coherent sum runs on tcgen05 from the fp16 intermediate (fp16 weights, fp32 accumulation);
+ * tolerance vs the float64 oracle ||dY||_F / ||Y||_F <= 2e-3 per (subband, channel) (same for the Stokes outputs);
+ * needs 2 S <= 208 (COBALT_ERR_BAD_ARG otherwise).  COBALT_MODE_EXACT_FP32: fp32 FMAs, 1e-4 of the same norm.
+ * For t_int > 32 the tensor path adds two or four partial sums per output sample with atomics (t_int = 128: the order of
+ * four fp32 additions is not fixed). */
+#define COBALT_BF_COHERENT_VOLTAGES 0
+#define COBALT_BF_COHERENT_STOKES 1
+#define COBALT_BF_INCOHERENT_STOKES 2
+typedef struct {
+    const void *samples;
+    const double *delays;
+    const double *delays_end;
+    const float *bandpass;
+    const unsigned char *valid;
+    const double *beam_delays;
+    int n_beams, product, n_stokes, t_int;
+    void *out;
+} cobalt_bf_io_t;
+int cobalt_beamform(cobalt_plan_t *plan, void *cuda_stream, const cobalt_bf_io_t *io);
+/* Extent in bytes that cobalt_beamform writes to `out` for these settings (0 on bad arguments). */
+long long cobalt_beamform_output_bytes(const cobalt_plan_t *plan, int n_beams, int product, int n_stokes, int t_int);
+
 /* Frees all plan state.  cobalt_destroy(NULL) is a no-op returning COBALT_OK.  The caller must
  * have synchronised every stream that still runs work of this plan. */
 int cobalt_destroy(cobalt_plan_t *plan);

@@ -25,6 +25,9 @@ COBALT_MODE_TENSOR_FP16 = 0
 COBALT_MODE_EXACT_FP32 = 1
 COBALT_LAYOUT_PLANAR = 0
 COBALT_LAYOUT_POL_MINOR = 1
+COBALT_BF_COHERENT_VOLTAGES = 0
+COBALT_BF_COHERENT_STOKES = 1
+COBALT_BF_INCOHERENT_STOKES = 2
 
 F_S = 195312.5
 
@@ -36,6 +39,7 @@ ABI_SYMBOLS = (
     "cobalt_set_chunk_subbands", "cobalt_reset", "cobalt_info", "cobalt_strerror", "cobalt_last_error",
     "cobalt_set_timing", "cobalt_get_timing", "cobalt_get_kernel_timing",
     "cobalt_debug_fir_weights", "cobalt_debug_unpack", "cobalt_debug_channelised", "cobalt_debug_correlate",
+    "cobalt_beamform", "cobalt_beamform_output_bytes",
 )
 
 
@@ -62,6 +66,15 @@ class cobalt_io_t(ctypes.Structure):
         ("samples", ctypes.c_void_p), ("delays", ctypes.c_void_p), ("delays_end", ctypes.c_void_p),
         ("bandpass", ctypes.c_void_p), ("valid", ctypes.c_void_p), ("visibilities", ctypes.c_void_p),
         ("valid_counts", ctypes.c_void_p),
+    ]
+
+
+class cobalt_bf_io_t(ctypes.Structure):
+    _fields_ = [
+        ("samples", ctypes.c_void_p), ("delays", ctypes.c_void_p), ("delays_end", ctypes.c_void_p),
+        ("bandpass", ctypes.c_void_p), ("valid", ctypes.c_void_p), ("beam_delays", ctypes.c_void_p),
+        ("n_beams", ctypes.c_int), ("product", ctypes.c_int), ("n_stokes", ctypes.c_int), ("t_int", ctypes.c_int),
+        ("out", ctypes.c_void_p),
     ]
 
 
@@ -108,9 +121,12 @@ def load(path: str | None = None):
     lib.cobalt_debug_unpack.argtypes = [_vp, ctypes.c_int, _vp, ctypes.c_longlong, _vp]
     lib.cobalt_debug_channelised.argtypes = [_vp, _vp, _vp, _vp, _vp, ctypes.c_int, _vp]
     lib.cobalt_debug_correlate.argtypes = [_vp, _vp, _vp, _vp]
+    lib.cobalt_beamform.argtypes = [_vp, _vp, ctypes.POINTER(cobalt_bf_io_t)]
+    lib.cobalt_beamform_output_bytes.argtypes = [_vp, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int]
+    lib.cobalt_beamform_output_bytes.restype = ctypes.c_longlong
     for name in ABI_SYMBOLS:
         fn = getattr(lib, name)
-        if name not in ("cobalt_strerror", "cobalt_last_error"):
+        if name not in ("cobalt_strerror", "cobalt_last_error", "cobalt_beamform_output_bytes"):
             fn.restype = ctypes.c_int
     _lib = lib
     return lib
@@ -178,6 +194,13 @@ def cobalt_process_ex(plan, stream, d_samples, d_delays, d_bandpass, d_visibilit
 
 def cobalt_process_host(plan, h_samples, h_delays, h_bandpass, h_visibilities):
     _check(load().cobalt_process_host(plan, _ptr(h_samples), _ptr(h_delays), _ptr(h_bandpass), _ptr(h_visibilities)), plan)
+
+
+def cobalt_beamform(plan, stream, d_samples, d_delays, d_bandpass, d_beam_delays, n_beams, product, n_stokes, t_int, d_out,
+                    d_delays_end=None, d_valid=None):
+    io = cobalt_bf_io_t(_ptr(d_samples), _ptr(d_delays), _ptr(d_delays_end), _ptr(d_bandpass), _ptr(d_valid), _ptr(d_beam_delays),
+                        int(n_beams), int(product), int(n_stokes), int(t_int), _ptr(d_out))
+    _check(load().cobalt_beamform(plan, _stream_ptr(stream), ctypes.byref(io)), plan)
 
 
 def cobalt_destroy(plan):
@@ -332,6 +355,43 @@ class Correlator:
                 cobalt_process_interp(self._h, stream, samples, delays, delays_end, bandpass, out)
         else:
             cobalt_process_ex(self._h, stream, samples, delays, bandpass, out, delays_end, valid, valid_counts)
+        return out
+
+    def beamform_shape(self, product, n_beams=1, n_stokes=1, t_int=1):
+        """Shape and dtype name of the output of ``beamform`` (reading A32)."""
+        i = self.info
+        if product == COBALT_BF_COHERENT_VOLTAGES:
+            return (i.subbands, n_beams, 2, i.channels, i.n_spectra), "complex64"
+        n_out = i.n_spectra // t_int
+        if product == COBALT_BF_COHERENT_STOKES:
+            return (i.subbands, n_beams, n_stokes, i.channels, n_out), "float32"
+        return (i.subbands, n_stokes, i.channels, n_out), "float32"
+
+    def beamform(self, samples, delays, bandpass, product, beam_delays=None, n_stokes=1, t_int=1, out=None, stream=None,
+                 delays_end=None, valid=None, layout=COBALT_LAYOUT_PLANAR):
+        """cobalt_beamform: samples, delays, bandpass as in ``process``; beam_delays float64
+        [n_beams][S] (CUDA) for the coherent products.  Returns the output tensor (see ``beamform_shape``)."""
+        import torch
+
+        i = self.info
+        want = {16: torch.int16, 8: torch.int8, 4: torch.uint8}[i.input_bits]
+        assert samples.is_cuda and samples.is_contiguous() and samples.dtype == want
+        assert tuple(samples.shape) == self.samples_shape(layout), (tuple(samples.shape), self.samples_shape(layout))
+        assert delays.is_cuda and delays.dtype == torch.float64 and delays.is_contiguous() and delays.numel() == i.stations
+        assert bandpass.is_cuda and bandpass.dtype == torch.float32 and bandpass.is_contiguous() and bandpass.numel() == i.channels
+        n_beams = 1
+        if product != COBALT_BF_INCOHERENT_STOKES:
+            assert beam_delays.is_cuda and beam_delays.dtype == torch.float64 and beam_delays.is_contiguous()
+            assert beam_delays.dim() == 2 and beam_delays.shape[1] == i.stations
+            n_beams = beam_delays.shape[0]
+        shape, dt = self.beamform_shape(product, n_beams, n_stokes, t_int)
+        if out is None:
+            out = torch.empty(shape, dtype=getattr(torch, dt), device=samples.device)
+        assert out.is_cuda and out.is_contiguous() and tuple(out.shape) == shape and out.dtype == getattr(torch, dt)
+        nbytes = load().cobalt_beamform_output_bytes(self._h, n_beams, product, n_stokes, t_int)
+        assert nbytes == out.numel() * out.element_size(), (nbytes, out.numel() * out.element_size())
+        cobalt_beamform(self._h, stream, samples, delays, bandpass, beam_delays, n_beams, product, n_stokes, t_int, out,
+                        delays_end, valid)
         return out
 
     def process_host(self, samples, delays, bandpass, out):

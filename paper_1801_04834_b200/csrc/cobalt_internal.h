@@ -146,6 +146,14 @@ struct XCall {
     float inv_s2 = 1.f;
 };
 
+// One chunk of a cobalt_beamform call as the launch helper sees it (beamform.cu).
+struct BfCall {
+    const double *beam_delays = nullptr;   // device [n_beams][S] seconds (coherent products)
+    const float *bandpass = nullptr;       // device [C]
+    void *out = nullptr;                   // first subband of the chunk in the caller's output
+    int n_beams = 0, product = 0, n_stokes = 1, t_int = 1;
+};
+
 // fstage.cu ---------------------------------------------------------------------------------
 cudaError_t launch_phase_table(const cobalt_plan_s *p, cudaStream_t st, const double *d_delays,
                                const float *d_bandpass, int b0, int nb, const double *d_delays_end);
@@ -166,5 +174,10 @@ cudaError_t launch_xstage_simt(const cobalt_plan_s *p, cudaStream_t st, const vo
 // xstage_tc.cu ------------------------------------------------------------------------------
 void build_xjobs(cobalt_plan_s *p);
 cudaError_t launch_xstage_tc(const cobalt_plan_s *p, cudaStream_t st, const void *d_z, int nb, float2 *d_vis, size_t dump_stride, const XCall &xc);
+
+// beamform.cu -------------------------------------------------------------------------------
+// p->d_phase must hold the pure station phases of the call (launch_phase_table with d_bandpass == nullptr)
+cudaError_t launch_beamform(const cobalt_plan_s *p, cudaStream_t st, const void *d_z, int b0, int nb, const BfCall &bc);
+bool bf_tc_shape(const cobalt_plan_s *p, int n_beams, int &bpb, int &stages, size_t &w_bytes, size_t &stage_bytes, size_t &smem);
 
 }  // namespace cobalt

@@ -573,7 +573,7 @@ __global__ void phase_table_kernel(const double *__restrict__ delays, const floa
         const double frac = cyc - floor(cyc);
         double sn, cs;
         sincospi(-2.0 * frac, &sn, &cs);
-        const double b = (double)bandpass[j];
+        const double b = bandpass ? (double)bandpass[j] : 1.0;      // nullptr: pure phase (the beamformer applies b[j] itself)
         const long long o = (long long)b0 * S * C + idx;      // tables are indexed by the subband of the plan
         out[o] = make_float2((float)(b * cs), (float)(b * sn));
         if (delays_end) step_out[o] = (float)(f * (delays_end[s] - delays[s]) * inv_n_t);

@@ -403,6 +403,91 @@ int cobalt_process_interp(cobalt_plan_t *p, void *cuda_stream, const void *d_sam
     return cobalt_process_ex(p, cuda_stream, &io);
 }
 
+long long cobalt_beamform_output_bytes(const cobalt_plan_t *p, int n_beams, int product, int n_stokes, int t_int) {
+    if (!p) return 0;
+    const bool stokes = product != COBALT_BF_COHERENT_VOLTAGES;
+    if (product < COBALT_BF_COHERENT_VOLTAGES || product > COBALT_BF_INCOHERENT_STOKES) return 0;
+    if (product != COBALT_BF_INCOHERENT_STOKES && (n_beams < 1 || n_beams > 4096)) return 0;
+    if (stokes && ((n_stokes != 1 && n_stokes != 4) || t_int < 1 || t_int > 128 || (t_int & (t_int - 1)) != 0)) return 0;
+    const long long beams = product == COBALT_BF_INCOHERENT_STOKES ? 1 : n_beams;
+    if (!stokes) return (long long)p->B * beams * 2 * p->C * p->n_t * (long long)sizeof(float2);
+    return (long long)p->B * beams * n_stokes * p->C * (p->n_t / t_int) * (long long)sizeof(float);
+}
+
+int cobalt_beamform(cobalt_plan_t *p, void *cuda_stream, const cobalt_bf_io_t *io) {
+    if (!p) return fail(nullptr, COBALT_ERR_BAD_ARG, "plan is NULL");
+    if (!io || !io->samples || !io->delays || !io->bandpass || !io->out) return fail(p, COBALT_ERR_BAD_ARG, "NULL buffer");
+    if (!p->scratch_ok) return fail(p, COBALT_ERR_NO_MEMORY, "the plan has no scratch (an earlier cobalt_set_mode / cobalt_set_chunk_subbands failed)");
+    const int t_int = io->product == COBALT_BF_COHERENT_VOLTAGES ? 1 : io->t_int;
+    const int n_stokes = io->product == COBALT_BF_COHERENT_VOLTAGES ? 1 : io->n_stokes;
+    const long long total = cobalt_beamform_output_bytes(p, io->n_beams, io->product, n_stokes, t_int);
+    if (total <= 0) return fail(p, COBALT_ERR_BAD_ARG, "bad beamformer settings (product, n_beams, n_stokes in {1, 4}, t_int a power of two <= 128 with floor(n_t / t_int) >= 1)");
+    if (io->product != COBALT_BF_INCOHERENT_STOKES && !io->beam_delays) return fail(p, COBALT_ERR_BAD_ARG, "NULL buffer");
+    if ((reinterpret_cast<uintptr_t>(io->out) & 7u) != 0) return fail(p, COBALT_ERR_BAD_ARG, "out must be 8-byte aligned");
+    if ((reinterpret_cast<uintptr_t>(io->samples) & (caller_sample_bytes(p) - 1)) != 0)
+        return fail(p, COBALT_ERR_BAD_ARG, "d_samples must be aligned to one complex sample");
+    const bool tensor = p->mode == COBALT_MODE_TENSOR_FP16;
+    if (tensor && io->product != COBALT_BF_INCOHERENT_STOKES) {
+        int bpb, stages;
+        size_t wb, sb, sm;
+        if (!bf_tc_shape(p, io->n_beams, bpb, stages, wb, sb, sm))
+            return fail(p, COBALT_ERR_BAD_ARG, "too many stations for the tensor-core beamformer (2 S <= 208); use COBALT_MODE_EXACT_FP32");
+    }
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const size_t out_sb = (size_t)(total / p->B);
+    // the tensor path adds the partial sums of windows longer than a warp with atomics: start from zero
+    if (tensor && io->product == COBALT_BF_COHERENT_STOKES && t_int > 32) CK(p, cudaMemsetAsync(io->out, 0, (size_t)total, st));
+    const int n_chunks = (p->B + p->chunk - 1) / p->chunk;
+    if (p->timing) {
+        int rc = ensure_events(p, n_chunks);
+        if (rc != COBALT_OK) return rc;
+    }
+    p->launches = 0;
+    p->n_chunks_timed = 0;
+    for (int ci = 0; ci < n_chunks; ++ci) {
+        const int b0 = ci * p->chunk;
+        const int nb = (p->B - b0) < p->chunk ? (p->B - b0) : p->chunk;
+        const unsigned char *sm = static_cast<const unsigned char *>(io->samples) + (size_t)b0 * subband_input_bytes(p);
+        StageEvents *ev = p->timing ? &p->events[ci] : nullptr;
+        if (ev) CK(p, cudaEventRecord(ev->e[0], st));
+        // pure station phases (no bandpass: the beamformer scales its outputs by b[j] in fp32), every subband in one launch
+        if (b0 == 0) CK(p, launch_phase_table(p, st, io->delays, nullptr, 0, p->B, io->delays_end));
+        if (ev) CK(p, cudaEventRecord(ev->e[1], st));
+        FCall call;
+        call.delays_end = io->delays_end;
+        call.valid = io->valid;
+        const void *fsamples = sm;
+        int extra = 0;
+        if (needs_ingest(p)) {
+            CK(p, launch_ingest(p, st, sm, nb, p->d_ingest));
+            fsamples = p->d_ingest;
+            call.n_in = p->N;
+            extra = 1;
+        } else {
+            call.coarse = p->d_coarse;
+            call.n_in = p->N_in;
+        }
+        CK(p, launch_fstage(p, st, fsamples, b0, nb, call));
+        if (ev) CK(p, cudaEventRecord(ev->e[2], st));
+        CK(p, launch_history_update(p, st, fsamples, b0, nb, call));
+        if (ev) CK(p, cudaEventRecord(ev->e[3], st));
+        BfCall bc;
+        bc.beam_delays = io->beam_delays;
+        bc.bandpass = io->bandpass;
+        bc.out = static_cast<unsigned char *>(io->out) + (size_t)b0 * out_sb;
+        bc.n_beams = io->n_beams;
+        bc.product = io->product;
+        bc.n_stokes = n_stokes;
+        bc.t_int = t_int;
+        CK(p, launch_beamform(p, st, p->d_z, b0, nb, bc));
+        if (ev) CK(p, cudaEventRecord(ev->e[4], st));
+        p->launches += (b0 == 0 ? 4 : 3) + extra;
+    }
+    if (p->timing) p->n_chunks_timed = n_chunks;
+    p->hist_cur ^= 1;
+    return COBALT_OK;
+}
+
 int cobalt_process_host(cobalt_plan_t *p, const void *h_samples, const double *h_delays, const float *h_bandpass,
                         void *h_visibilities) {
     if (!p) return fail(nullptr, COBALT_ERR_BAD_ARG, "plan is NULL");

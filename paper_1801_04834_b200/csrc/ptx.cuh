@@ -1,5 +1,5 @@
 // Inline-PTX wrappers shared by the kernels of libcobalt_b200.so (sm_100a): mbarriers, bulk copies
-// (cp.async.bulk -> SASS UBLKCP), warp election, and the one integer -> float conversion of the hot path.
+// (cp.async.bulk -> SASS UBLKCP), warp election, the tcgen05 / TMEM wrappers, and the one integer -> float conversion of the hot path.
 // Device code only; nothing here is part of the ABI and nothing is shared with oracle/.
 #pragma once
 
@@ -83,6 +83,51 @@ __device__ __forceinline__ bool elect_one() {
         : "=r"(pred));
     return pred != 0;
 }
+
+// ------------------------------------------------------------------ tcgen05 (5th-generation tensor cores, TMEM)
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_commit(uint32_t bar) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+// D[tmem] (+)= A[smem] * B[smem]^T, 128 x N x 16, fp16 in, fp32 accumulate.
+__device__ __forceinline__ void tc_mma(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t acc) {
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t"
+        "}" ::"r"(d_tmem),
+        "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(acc)
+        : "memory");
+}
+// Shared-memory operand descriptor, 128-byte swizzle, descriptor version 1 (sm_100).
+//   K-major operand (rows = M or N index, 64 K-elements per 128-byte row): 8-row groups sbo bytes apart; lbo unused (1).
+//   MN-major operand (rows = K index, 64 M/N-elements per 128-byte row): 8-row K-groups sbo bytes apart, blocks of 64
+//   M/N-elements lbo bytes apart.
+__device__ __forceinline__ uint64_t make_smem_desc_lbo(uint32_t addr, uint32_t lbo, uint32_t sbo) {
+    return (uint64_t)((addr >> 4) & 0x3FFFu) | ((uint64_t)((lbo >> 4) & 0x3FFFu) << 16) | ((uint64_t)((sbo >> 4) & 0x3FFFu) << 32) |
+           (1ull << 46) | (2ull << 61);
+}
+__device__ __forceinline__ uint64_t make_smem_desc(uint32_t addr, uint32_t sbo) { return make_smem_desc_lbo(addr, 16, sbo); }
+// kind::f16 instruction descriptor: D = f32, A = B = f16; A K-major (a_mn = 0) or MN-major (1), B K-major.
+__device__ __forceinline__ uint32_t make_idesc(int m, int n, int neg_a, int a_mn = 0) {
+    return (1u << 4) | ((uint32_t)neg_a << 13) | ((uint32_t)a_mn << 15) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(m >> 4) << 24);
+}
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&v)[16]) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, "
+        "[%16];"
+        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]),
+          "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+        : "r"(taddr));
+}
+__device__ __forceinline__ void tmem_ld8(uint32_t taddr, uint32_t (&v)[8]) {
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7])
+                 : "r"(taddr));
+}
+__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 
 // ------------------------------------------------------------------ step a1
 // One complex sample as it sits in memory (int16: re in bits 0-15, im in bits 16-31; int8: re in bits 0-7, im in
