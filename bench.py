@@ -49,6 +49,10 @@ def parse_args(argv=None):
     ap.add_argument("--interp", action="store_true",
                     help="time cobalt_process_interp (delay running linearly over the block, SURVEY.md sec 8(f) row 1)")
     ap.add_argument("--chunk", type=int, default=0, help="subbands per launch group (0 = library default)")
+    ap.add_argument("--beamform", default="", choices=["", "stokes-i", "iquv", "voltages", "incoherent"],
+                    help="time cobalt_beamform (SURVEY.md sec 8(f) row 4) on the beamformer workload (synth config 6) instead")
+    ap.add_argument("--beams", type=int, default=127)
+    ap.add_argument("--t-int", type=int, default=16)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args(argv)
@@ -191,7 +195,7 @@ def stored_traffic(key: str):
 def workload(args):
     from paper_1801_04834_b200 import synth
 
-    cfg = synth.CONFIGS[args.config]
+    cfg = synth.CONFIGS[6 if (args.beamform and args.config == 3) else args.config]
     if args.subbands > 0:
         cfg = synth.scaled(cfg, B=args.subbands)
     return cfg
@@ -390,6 +394,100 @@ def run_ours(args, rank, world, local):
     return 0
 
 
+def run_beamform(args, rank, world, local):
+    """`--beamform`: one step = one cobalt_beamform over the whole beamformer workload (F-stage + beamformer kernel)."""
+    import torch
+
+    import paper_1801_04834_b200 as pkg
+    from paper_1801_04834_b200 import synth
+
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py --impl ours needs a CUDA device: there is no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    pkg.load()
+    cfg = workload(args)
+    peaks = measured_peaks()
+    product = {"stokes-i": pkg.COBALT_BF_COHERENT_STOKES, "iquv": pkg.COBALT_BF_COHERENT_STOKES,
+               "voltages": pkg.COBALT_BF_COHERENT_VOLTAGES, "incoherent": pkg.COBALT_BF_INCOHERENT_STOKES}[args.beamform]
+    n_stokes = 4 if args.beamform == "iquv" else 1
+    t_int = 1 if args.beamform == "voltages" else args.t_int
+    n_beams = 1 if args.beamform == "incoherent" else args.beams
+    if args.beamform == "voltages" and args.subbands <= 0:      # complex voltages of 127 beams: 0.4 GB per subband
+        cfg = synth.scaled(cfg, B=32)
+    data = synth.generate(cfg, device=dev)
+    samples, delays, bandpass = data["samples"], data["delays"], data["bandpass"]
+    bd = synth.beam_delays(cfg, n_beams, dev)
+    cor = pkg.Correlator(cfg.S, cfg.B, cfg.C, cfg.N, cfg.bits, mode=pkg.COBALT_MODE_TENSOR_FP16 if args.mode == "tensor" else pkg.COBALT_MODE_EXACT_FP32)
+    if args.chunk > 0:
+        cor.set_chunk_subbands(args.chunk)
+    info = cor.info
+    shape, dt = cor.beamform_shape(product, n_beams, n_stokes, t_int)
+    out = torch.empty(shape, dtype=getattr(torch, dt), device=dev)
+    stream = torch.cuda.current_stream()
+    cor.set_timing(True)
+    call = lambda: cor.beamform(samples, delays, bandpass, product, beam_delays=bd, n_stokes=n_stokes, t_int=t_int, out=out)  # noqa: E731
+    for _ in range(args.warmup):
+        call()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(physical_gpu_index(local))
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+    kt = [0.0, 0.0, 0.0, 0.0]
+    launches = 0
+    dist_barrier()
+    torch.cuda.synchronize()
+    sampler.start()
+    ev[0].record(stream)
+    for _ in range(args.steps):
+        call()
+        ms = cor.get_kernel_timing()
+        for k in range(4):
+            kt[k] += ms[k]
+        launches += ms[4]
+    ev[1].record(stream)
+    torch.cuda.synchronize()
+    dist_barrier()
+    clocks = sampler.stop()
+    sec_step = dist_max(ev[0].elapsed_time(ev[1]) / 1e3 / args.steps, dev)
+    t_phase, t_f, t_hist, t_b = (dist_max(v / 1e3 / args.steps, dev) for v in kt)
+    n_chunks = (cfg.B + info.chunk_subbands - 1) // info.chunk_subbands
+    n_cs = float(cfg.B) * cfg.n_t * cfg.C                                    # channel-samples per polarisation stream
+    units = n_beams * n_cs
+    out_bytes = out.numel() * out.element_size()
+    z_bytes = n_cs * 2 * cfg.S * 4                                           # fp16 re + im of every input, read once
+    f_bytes = n_cs * 2 * cfg.S * F_BYTES_PER_SAMPLE[cfg.bits]
+    b_flop = 8.0 * cfg.S * 2 * n_beams * n_cs if product != pkg.COBALT_BF_INCOHERENT_STOKES else 0.0   # complex MAC per (beam, pol, station)
+    roof_f = {"kernel": "fstage_kernel", "bound": "hbm", "achieved": f_bytes / t_f / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+              "frac": f_bytes / t_f / 1e9 / peaks["hbm_gbs"], "traffic": None, "peak_source": peaks["source"],
+              "ms_per_launch": t_f * 1e3 / n_chunks, "launches_per_step": n_chunks, "algorithmic_bytes_per_launch": f_bytes / n_chunks}
+    bname = "incoherent_kernel" if product == pkg.COBALT_BF_INCOHERENT_STOKES else ("bf_tc_kernel" if args.mode == "tensor" else "bf_simt_kernel")
+    roof_b = {"kernel": bname, "bound": "hbm", "achieved": (z_bytes + out_bytes) / t_b / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+              "frac": (z_bytes + out_bytes) / t_b / 1e9 / peaks["hbm_gbs"], "traffic": None, "peak_source": peaks["source"],
+              "ms_per_launch": t_b * 1e3 / n_chunks, "launches_per_step": n_chunks,
+              "algorithmic_bytes_per_launch": (z_bytes + out_bytes) / n_chunks,
+              "tensor_tflops": b_flop / t_b / 1e12, "tensor_frac_of_sustained_peak": b_flop / t_b / 1e12 / peaks["tensor_tflops_sustained"],
+              "note": "algorithmic flops = 8 per (beam, polarisation, station, channel-sample); the kernel issues twice that (the weight rows are zero on the other polarisation)"}
+    dominant, other = (roof_f, roof_b) if t_f >= t_b else (roof_b, roof_f)
+    cor.close()
+    if rank == 0:
+        line = {
+            "metric": "beam-channel-samples/s", "value": whole_job_value(units, world, sec_step), "unit": "beam*channel*samples/s",
+            "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": sec_step * 1e3, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32 (fp16 tensor-core operands, fp32 accumulate; fp64 phase angles)" if args.mode == "tensor" else "f32",
+            "data": "synthetic",
+            "config": {"workload": cfg.name, "call": "cobalt_beamform", "product": args.beamform, "stations": cfg.S, "subbands": cfg.B,
+                       "channels": cfg.C, "beams": n_beams, "n_stokes": n_stokes, "t_int": t_int, "samples_per_integration": cfg.N,
+                       "input_bits": cfg.bits, "mode": args.mode, "chunk_subbands": info.chunk_subbands,
+                       "l2": f"inputs ({cfg.input_bytes / 1e9:.2f} GB per step) exceed the 126 MB L2; no flush needed"},
+            "roofline": dominant, "roofline_other": other,
+            "stage_ms": {"phase_table": t_phase * 1e3, "f_stage": t_f * 1e3, "history": t_hist * 1e3, "beamform": t_b * 1e3},
+            "real_time_factor": (cfg.n_t * cfg.C / F_S) / sec_step, "output_bytes": out_bytes,
+            "clocks": clocks, "gpu_launches": int(launches), "e2e": None, "cpu_baseline": None,
+        }
+        print(json.dumps(line), flush=True)
+    return 0
+
+
 def run_e2e(args, cfg, cor, samples, delays, bandpass, world, dev):
     import torch
 
@@ -441,7 +539,7 @@ def main(argv=None):
         rank = int(os.environ.get("RANK", "0"))
         return run_reference(args, rank, int(os.environ.get("WORLD_SIZE", "1")))
     rank, world, local = dist_setup()
-    rc = run_ours(args, rank, world, local)
+    rc = run_beamform(args, rank, world, local) if args.beamform else run_ours(args, rank, world, local)
     import torch.distributed as dist
 
     if dist.is_available() and dist.is_initialized():

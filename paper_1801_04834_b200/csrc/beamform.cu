@@ -20,7 +20,7 @@
 //       Stokes parameters (A29) are formed in registers; time integration (A30) is a shuffle reduction over t_int lanes.
 // Persistent CTAs; job = (subband, channel, block of <= 64 beams), walked in blocks of 128 spectra with two accumulator
 // sets, so that the MMAs of one block overlap the epilogue of the previous one.  Warp 0 = bulk-copy producer (one copy per
-// 128-spectrum block: the two k-tiles are contiguous), warp 1 = MMA issuer, warps 4-11 = weights + epilogue.
+// 128-spectrum block: the two k-tiles are contiguous), warp 1 = MMA issuer, warps 4-19 = weights + epilogue.
 //
 // bf_simt_kernel (EXACT_FP32 mode): the same sums with fp32 FMAs from the fp32 intermediate (parity instrument, not tuned).
 // incoherent_kernel: sum over stations of the per-station Stokes parameters (A31), reading z once (HBM bound).
@@ -31,7 +31,7 @@ namespace cobalt {
 
 namespace {
 
-constexpr int kBfFirstEpiWarp = 4, kBfEpiWarps = 8;
+constexpr int kBfFirstEpiWarp = 4, kBfEpiWarps = 16, kBfEpiSub = kBfEpiWarps / 4;
 constexpr int kBfThreads = 32 * (kBfFirstEpiWarp + kBfEpiWarps);
 constexpr int kBfEpiThreads = 32 * kBfEpiWarps;
 constexpr int kBfTBlock = 2 * kKTile;          // spectra per accumulator block (M of the instruction)
@@ -49,7 +49,7 @@ struct BfArgs {
     long long n_t, n_out;
     int S, M, Mpad, C, n_kt, n_tb, b0, nb;
     int n_beams, bpb, n_bb, N;      // beams per block, beam blocks, N = 4 bpb accumulator columns
-    int product, n_stokes, t_int;
+    int product, n_stokes, t_int, lg_t_int;
     float inv_s;                    // 1 / s, s = power-of-two scale of the fp16 intermediate
     int stages;
     uint32_t stage_bytes, w_bytes, kt_bytes;
@@ -77,6 +77,120 @@ __device__ __forceinline__ void stokes4(float xr, float xi, float yr, float yi, 
     Q = px - py;
     U = 2.f * (xr * yr + xi * yi);
     V = 2.f * (xi * yr - xr * yi);
+}
+
+// ---- epilogue of one 128-spectrum accumulator block, per warp: lane = spectrum, 16-column chunks = 4 beams x (Xr, Xi, Yr, Yi)
+struct BfEpi {
+    float vs, ps;                 // scale of a voltage (b_j / s) and of a power
+    int lg;                       // t_int = 2^lg
+    long long t, n_t, n_out;      // this lane's spectrum
+    size_t cv_pol, st_k, st_beam; // output strides: polarisation (voltages); Stokes parameter, beam (Stokes)
+    float2 *o_cv;                 // voltages: element (first beam of the block, X, channel, t)
+    float *o_st;                  // Stokes: element (first beam of the block, I, channel, t >> lg)
+    uint32_t taddr;               // TMEM address of column 0 of this warp's lanes
+    int n_chunks, sub, lane, beams_left;
+};
+
+__device__ __forceinline__ void epilogue_voltages(const BfEpi &ep) {
+    const bool live = ep.t < ep.n_t;
+    for (int c16 = ep.sub; c16 < ep.n_chunks; c16 += kBfEpiSub) {
+        uint32_t x[16];
+        tmem_ld16(ep.taddr + 16 * c16, x);
+        tmem_ld_wait();
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            if (live && 4 * c16 + e < ep.beams_left) {
+                float2 *o = ep.o_cv + (size_t)(4 * c16 + e) * 2 * ep.cv_pol;
+                o[0] = make_float2(__uint_as_float(x[4 * e]) * ep.vs, __uint_as_float(x[4 * e + 1]) * ep.vs);
+                o[ep.cv_pol] = make_float2(__uint_as_float(x[4 * e + 2]) * ep.vs, __uint_as_float(x[4 * e + 3]) * ep.vs);
+            }
+        }
+    }
+}
+
+// Sum of v[] over the 2^LGW lanes of a group (reading A30).  While a lane still holds more than one value a step halves
+// the array instead of duplicating the sums (the lanes with the offset bit clear keep the lower half, the others the upper
+// half): V - 1 shuffles for V values instead of V LGW.  On return a lane holds max(1, V >> LGW) sums: the original indices
+// base + j, base = sum over the halving steps i of bit_i(lane) (V >> (i + 1)).
+template <int V, int LGW>
+__device__ __forceinline__ int reduce_lanes(float (&v)[V], int lane) {
+    int base = 0;
+    int n = V;
+#pragma unroll
+    for (int i = 0; i < LGW; ++i) {
+        const int off = 1 << i;
+        if (n > 1) {
+            const int h = n >> 1;
+            const bool up = (lane & off) != 0;
+#pragma unroll
+            for (int j = 0; j < V / 2; ++j) {
+                if (j < h) {
+                    const float send = up ? v[j] : v[h + j];
+                    const float keep = up ? v[h + j] : v[j];
+                    v[j] = keep + __shfl_xor_sync(0xffffffffu, send, off);
+                }
+            }
+            if (up) base += h;
+            n = h;
+        } else {
+            v[0] += __shfl_xor_sync(0xffffffffu, v[0], off);
+        }
+    }
+    return base;
+}
+
+template <int NS, int LGW>
+__device__ __forceinline__ void epilogue_stokes(const BfEpi &ep) {
+    constexpr int V = 4 * NS;                         // values of a chunk per lane: index e NS + k (beam e, parameter k)
+    constexpr int HALVINGS = LGW < (NS == 1 ? 2 : 4) ? LGW : (NS == 1 ? 2 : 4);
+    constexpr int R = V >> HALVINGS;                  // sums a lane holds after the reduction
+    // lanes whose bits [HALVINGS, LGW) are zero write (the others hold duplicates)
+    const bool writer = ((ep.lane >> HALVINGS) & ((1 << (LGW - HALVINGS)) - 1)) == 0 && (ep.t >> ep.lg) < ep.n_out;
+    for (int c16 = ep.sub; c16 < ep.n_chunks; c16 += kBfEpiSub) {
+        uint32_t x[16];
+        tmem_ld16(ep.taddr + 16 * c16, x);
+        tmem_ld_wait();
+        float v[V];
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            const float xr = __uint_as_float(x[4 * e]), xi = __uint_as_float(x[4 * e + 1]);
+            const float yr = __uint_as_float(x[4 * e + 2]), yi = __uint_as_float(x[4 * e + 3]);
+            if (NS == 4) {
+                float I, Q, U, W;
+                stokes4(xr, xi, yr, yi, I, Q, U, W);
+                v[4 * e] = I * ep.ps;
+                v[4 * e + 1] = Q * ep.ps;
+                v[4 * e + 2] = U * ep.ps;
+                v[4 * e + 3] = W * ep.ps;
+            } else {
+                v[e] = fmaf(xr, xr, fmaf(xi, xi, fmaf(yr, yr, yi * yi))) * ep.ps;
+            }
+        }
+        const int base = reduce_lanes<V, LGW>(v, ep.lane);
+        if (writer) {
+#pragma unroll
+            for (int j = 0; j < R; ++j) {
+                const int idx = base + j, e = idx / NS, k = idx % NS;
+                if (4 * c16 + e < ep.beams_left) {
+                    float *o = ep.o_st + (size_t)(4 * c16 + e) * ep.st_beam + (size_t)k * ep.st_k;
+                    if (ep.lg > 5) atomicAdd(o, v[j]);      // t_int = 64, 128: two or four warps per output sample
+                    else *o = v[j];
+                }
+            }
+        }
+    }
+}
+
+template <int NS>
+__device__ __forceinline__ void epilogue_stokes_lg(const BfEpi &ep) {
+    switch (ep.lg < 5 ? ep.lg : 5) {
+        case 0: epilogue_stokes<NS, 0>(ep); break;
+        case 1: epilogue_stokes<NS, 1>(ep); break;
+        case 2: epilogue_stokes<NS, 2>(ep); break;
+        case 3: epilogue_stokes<NS, 3>(ep); break;
+        case 4: epilogue_stokes<NS, 4>(ep); break;
+        default: epilogue_stokes<NS, 5>(ep); break;
+    }
 }
 
 __global__ void __launch_bounds__(kBfThreads, 1) bf_tc_kernel(const BfArgs a) {
@@ -163,7 +277,7 @@ __global__ void __launch_bounds__(kBfThreads, 1) bf_tc_kernel(const BfArgs a) {
     } else if (warp >= kBfFirstEpiWarp) {
         // ------------------------------------------------------------------ weights + epilogue
         const int et = threadIdx.x - 32 * kBfFirstEpiWarp;
-        const int wq = warp & 3, half = (warp - kBfFirstEpiWarp) >> 2;
+        const int wq = warp & 3, sub = (warp - kBfFirstEpiWarp) >> 2;     // TMEM lane quarter; every kBfEpiSub-th 16-column chunk
         const int ns = a.n_stokes;
         uint32_t it = 0;
         for (int jid = blockIdx.x; jid < a.total_jobs; jid += gridDim.x) {
@@ -212,52 +326,31 @@ __global__ void __launch_bounds__(kBfThreads, 1) bf_tc_kernel(const BfArgs a) {
                 bar_sync_named(1, kBfEpiThreads);
                 if (et == 0) mbar_arrive(w_ready);
             }
-            const float bp = a.bandpass[c];
-            const float vs = bp * a.inv_s, ps = vs * vs;      // scale of a voltage / of a power
+            BfEpi ep;
+            ep.vs = a.bandpass[c] * a.inv_s;
+            ep.ps = ep.vs * ep.vs;
+            ep.lg = a.lg_t_int;
+            ep.n_t = a.n_t;
+            ep.n_out = a.n_out;
+            ep.cv_pol = (size_t)a.C * a.n_t;
+            ep.st_k = (size_t)a.C * a.n_out;
+            ep.st_beam = (size_t)ns * ep.st_k;
+            ep.n_chunks = a.N >> 4;
+            ep.sub = sub;
+            ep.lane = lane;
+            const int beam0 = bb * a.bpb;
+            ep.beams_left = a.n_beams - beam0;
             for (int tb = 0; tb < a.n_tb; ++tb, ++it) {
                 const uint32_t buf = it & 1u;
                 mbar_wait(tmem_full + 8 * buf, (it >> 1) & 1u);
                 tc_fence_after();
-                const long long t = (long long)tb * kBfTBlock + 32 * wq + lane;
-                const uint32_t t0 = tmem_base + ((uint32_t)(32 * wq) << 16) + buf * kBfAccStride;
-                for (int c16 = half; c16 < (a.N >> 4); c16 += 2) {
-                    uint32_t x[16];
-                    tmem_ld16(t0 + 16 * c16, x);
-                    tmem_ld_wait();
-#pragma unroll
-                    for (int e = 0; e < 4; ++e) {
-                        const int beam = bb * a.bpb + 4 * c16 + e;
-                        if (beam >= a.n_beams) break;           // warp-uniform
-                        const float xr = __uint_as_float(x[4 * e]), xi = __uint_as_float(x[4 * e + 1]);
-                        const float yr = __uint_as_float(x[4 * e + 2]), yi = __uint_as_float(x[4 * e + 3]);
-                        if (a.product == COBALT_BF_COHERENT_VOLTAGES) {
-                            float2 *o = static_cast<float2 *>(a.out) + ((((size_t)bl * a.n_beams + beam) * 2) * a.C + c) * a.n_t + t;
-                            if (t < a.n_t) {
-                                o[0] = make_float2(xr * vs, xi * vs);
-                                o[(size_t)a.C * a.n_t] = make_float2(yr * vs, yi * vs);
-                            }
-                        } else {
-                            float sv[4];
-                            stokes4(xr, xi, yr, yi, sv[0], sv[1], sv[2], sv[3]);
-                            const int width = a.t_int < 32 ? a.t_int : 32;
-#pragma unroll
-                            for (int k = 0; k < 4; ++k) {
-                                if (k >= ns) break;
-                                float v = sv[k] * ps;
-                                for (int off = 1; off < width; off <<= 1) v += __shfl_xor_sync(0xffffffffu, v, off);
-                                sv[k] = v;
-                            }
-                            const long long u = t / a.t_int;
-                            if ((lane & (width - 1)) == 0 && u < a.n_out) {
-                                float *o = static_cast<float *>(a.out) + ((((size_t)bl * a.n_beams + beam) * ns) * a.C + c) * a.n_out + u;
-                                for (int k = 0; k < ns; ++k) {
-                                    if (a.t_int > 32) atomicAdd(o + (size_t)k * a.C * a.n_out, sv[k]);   // 2 or 4 warps per output sample
-                                    else o[(size_t)k * a.C * a.n_out] = sv[k];
-                                }
-                            }
-                        }
-                    }
-                }
+                ep.t = (long long)tb * kBfTBlock + 32 * wq + lane;
+                ep.taddr = tmem_base + ((uint32_t)(32 * wq) << 16) + buf * kBfAccStride;
+                ep.o_cv = static_cast<float2 *>(a.out) + ((size_t)bl * a.n_beams + beam0) * 2 * ep.cv_pol + (size_t)c * a.n_t + ep.t;
+                ep.o_st = static_cast<float *>(a.out) + ((size_t)bl * a.n_beams + beam0) * ep.st_beam + (size_t)c * a.n_out + (ep.t >> ep.lg);
+                if (a.product == COBALT_BF_COHERENT_VOLTAGES) epilogue_voltages(ep);
+                else if (ns == 1) epilogue_stokes_lg<1>(ep);
+                else epilogue_stokes_lg<4>(ep);
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive(tmem_empty + 8 * buf);
@@ -528,6 +621,8 @@ cudaError_t launch_beamform(const cobalt_plan_s *p, cudaStream_t st, const void 
     a.product = bc.product;
     a.n_stokes = bc.n_stokes;
     a.t_int = bc.t_int;
+    a.lg_t_int = 0;
+    while ((1 << a.lg_t_int) < bc.t_int) ++a.lg_t_int;
     a.inv_s = 1.f / p->zscale;
     a.stages = stages;
     a.stage_bytes = (uint32_t)stage_bytes;

@@ -58,6 +58,9 @@ CONFIGS = {
     3: Config(3, "full-array-16bit", 77, 244, 256, 195312, 16, 100.0, 0.10, 50e-6, 0.1, "sky"),
     4: Config(4, "full-array-8bit", 77, 488, 64, 195312, 8, 16.0, 0.10, 50e-6, 0.0, "sky"),
     5: Config(5, "large-n-stress", 288, 1, 64, 196608, 16, 100.0, 0.0, 0.0, 0.0, "sources"),
+    # not a BASELINE.json config: the beamformer workload of P:L111 ("127 time domain data streams using all 48 core antenna
+    # fields in 16-bit mode at full bandwidth"), at the 256 channels per subband of P:L362; same recipe as config 3
+    6: Config(6, "beamformer-core-16bit", 48, 244, 256, 195312, 16, 100.0, 0.10, 2e-6, 0.1, "sky"),
 }
 
 
@@ -115,6 +118,18 @@ def geometry(cfg: Config, device="cpu"):
     else:
         out["bandpass"] = torch.ones(cfg.C, dtype=torch.float32)
     return {k: v.to(device) for k, v in out.items()}
+
+
+def beam_delays(cfg: Config, n_beams: int, device="cpu") -> torch.Tensor:
+    """Seeded tied-array beam delays tau[b][a] (seconds), [n_beams][S] float64: beam 0 is the phase centre, the others are
+    plane-wave offsets over stations in a 1 km disc, up to ~1 degree off (a few tens of ns)."""
+    gen = torch.Generator(device="cpu").manual_seed(SEED0 + 77 * cfg.index + n_beams)
+    r = 1000.0 * torch.sqrt(torch.rand(cfg.S, generator=gen, dtype=torch.float64))
+    th = 2 * math.pi * torch.rand(cfg.S, generator=gen, dtype=torch.float64)
+    x, y = r * torch.cos(th), r * torch.sin(th)
+    lm = (torch.rand(n_beams, 2, generator=gen, dtype=torch.float64) * 2 - 1) * 0.017
+    lm[0] = 0.0
+    return ((x[None, :] * lm[:, 0:1] + y[None, :] * lm[:, 1:2]) / C_LIGHT).contiguous().to(device)
 
 
 def generate_subband(cfg: Config, sb: int, device="cpu", geo=None) -> torch.Tensor:
