@@ -252,13 +252,13 @@ __global__ void __launch_bounds__(kBfThreads, 1) bf_tc_kernel(const BfArgs a) {
             const uint32_t idesc = make_idesc(kBfTBlock, a.N, 0, /*a_mn=*/1);
             uint32_t it = 0, job = 0;
             for (int jid = blockIdx.x; jid < a.total_jobs; jid += gridDim.x, ++job) {
-                mbar_wait(w_ready, job & 1u);               // this job's W' is in shared memory
+                mbar_wait_spin(w_ready, job & 1u);          // this job's W' is in shared memory
                 tc_fence_after();
                 for (int tb = 0; tb < a.n_tb; ++tb, ++it) {
                     const int s = it % a.stages;
                     const uint32_t buf = it & 1u;
-                    mbar_wait(bar_full + 8 * s, (it / a.stages) & 1u);
-                    mbar_wait(tmem_empty + 8 * buf, ((it >> 1) & 1u) ^ 1u);
+                    mbar_wait_spin(bar_full + 8 * s, (it / a.stages) & 1u);      // one thread: spinning costs nothing, the
+                    mbar_wait_spin(tmem_empty + 8 * buf, ((it >> 1) & 1u) ^ 1u);  // suspended wait's wake-up latency would
                     tc_fence_after();
                     const uint32_t d = tmem_base + buf * kBfAccStride;
                     const uint32_t st_addr = stage_base + (uint32_t)s * a.stage_bytes;
@@ -340,14 +340,16 @@ __global__ void __launch_bounds__(kBfThreads, 1) bf_tc_kernel(const BfArgs a) {
             ep.lane = lane;
             const int beam0 = bb * a.bpb;
             ep.beams_left = a.n_beams - beam0;
+            float2 *cv_job = static_cast<float2 *>(a.out) + ((size_t)bl * a.n_beams + beam0) * 2 * ep.cv_pol + (size_t)c * a.n_t;
+            float *st_job = static_cast<float *>(a.out) + ((size_t)bl * a.n_beams + beam0) * ep.st_beam + (size_t)c * a.n_out;
             for (int tb = 0; tb < a.n_tb; ++tb, ++it) {
                 const uint32_t buf = it & 1u;
-                mbar_wait(tmem_full + 8 * buf, (it >> 1) & 1u);
+                mbar_wait_spin(tmem_full + 8 * buf, (it >> 1) & 1u);
                 tc_fence_after();
                 ep.t = (long long)tb * kBfTBlock + 32 * wq + lane;
                 ep.taddr = tmem_base + ((uint32_t)(32 * wq) << 16) + buf * kBfAccStride;
-                ep.o_cv = static_cast<float2 *>(a.out) + ((size_t)bl * a.n_beams + beam0) * 2 * ep.cv_pol + (size_t)c * a.n_t + ep.t;
-                ep.o_st = static_cast<float *>(a.out) + ((size_t)bl * a.n_beams + beam0) * ep.st_beam + (size_t)c * a.n_out + (ep.t >> ep.lg);
+                ep.o_cv = cv_job + ep.t;
+                ep.o_st = st_job + (ep.t >> ep.lg);
                 if (a.product == COBALT_BF_COHERENT_VOLTAGES) epilogue_voltages(ep);
                 else if (ns == 1) epilogue_stokes_lg<1>(ep);
                 else epilogue_stokes_lg<4>(ep);
