@@ -117,8 +117,9 @@ int cobalt_plan(cobalt_plan_t **out, int stations, int subbands, int channels, i
  * and the last 15 C consumed samples of every stream become the new history (stateful!).
  * The factor w_a[j] = b[j] exp(-2 pi i frac(f[s][j] tau_a)) is constant over the call, so the library correlates F and
  * multiplies each visibility by w_i conj(w_k) (the same product; w from the fp64 phase table, the multiplication in fp32).
- * The call only enqueues kernels on `cuda_stream` (no synchronisation, no allocation): it can be captured in a CUDA
- * graph; the history alternates between two buffers from call to call, so capture calls in pairs.
+ * The call only enqueues kernels on `cuda_stream` (no synchronisation, no allocation) and changes no host-side state, so a
+ * single call can be captured in a CUDA graph and replayed block after block (the history is carried in place).  Exception:
+ * blocks shorter than the history (N_u < 15 C) alternate between two history buffers; capture those in pairs.
  * Only the first N_u = floor(N/C) C samples of each stream are consumed (A11). */
 int cobalt_process(cobalt_plan_t *plan, void *cuda_stream, const void *d_samples,
                    const double *d_delays, const float *d_bandpass, void *d_visibilities);

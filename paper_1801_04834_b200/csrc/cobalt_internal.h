@@ -127,6 +127,9 @@ struct cobalt_plan_s {
 namespace cobalt {
 
 inline size_t sample_bytes(int bits) { return bits == 16 ? 4 : 2; }   // one complex sample
+// the history carry overwrites the buffer it was read from (no host-side state changes from call to call: a single
+// captured call can be replayed); only blocks shorter than the history itself alternate between the two buffers
+inline bool history_in_place(const cobalt_plan_s *p) { return p->N_u >= (long long)(kTaps - 1) * p->C; }
 
 // The per-call inputs beyond the plan (cobalt_io_t) as the launch helpers see them for one chunk.
 struct FCall {

@@ -720,7 +720,9 @@ cudaError_t launch_history_update(const cobalt_plan_s *p, cudaStream_t st, const
     long long blocks = (total + threads - 1) / threads;
     if (blocks > 65535) blocks = 65535;
     const void *ho = p->d_hist[p->hist_cur];
-    void *hn = p->d_hist[p->hist_cur ^ 1];
+    // a block of at least 15 C samples replaces the whole history from the samples alone: written in place (the F-stage of this
+    // chunk, earlier in the stream, was the last reader); shorter blocks (reading R3) mix old and new and go to the other buffer
+    void *hn = p->d_hist[history_in_place(p) ? p->hist_cur : p->hist_cur ^ 1];
     const size_t sb = sample_bytes(p->bits);
     const long long N = call.n_in;
     if (!call.coarse && p->N_u >= HC && (N * sb) % 16 == 0 && ((p->N_u - HC) * sb) % 16 == 0 && (HC * sb) % 16 == 0 &&

@@ -377,7 +377,7 @@ int cobalt_process_ex(cobalt_plan_t *p, void *cuda_stream, const cobalt_io_t *io
         if (rc != COBALT_OK) return rc;
     }
     if (p->timing) p->n_chunks_timed = n_chunks;
-    p->hist_cur ^= 1;   // the history kernels of this call wrote the other buffer (stream ordered)
+    if (!history_in_place(p)) p->hist_cur ^= 1;   // short blocks: the history kernels of this call wrote the other buffer (stream ordered)
     return COBALT_OK;
 }
 
@@ -484,7 +484,7 @@ int cobalt_beamform(cobalt_plan_t *p, void *cuda_stream, const cobalt_bf_io_t *i
         p->launches += (b0 == 0 ? 4 : 3) + extra;
     }
     if (p->timing) p->n_chunks_timed = n_chunks;
-    p->hist_cur ^= 1;
+    if (!history_in_place(p)) p->hist_cur ^= 1;
     return COBALT_OK;
 }
 
@@ -552,7 +552,7 @@ int cobalt_process_host(cobalt_plan_t *p, const void *h_samples, const double *h
                             (size_t)nb * out_b, cudaMemcpyDeviceToHost, s_out));
         CKH(cudaEventRecord(p->ev_out[buf], s_out));
     }
-    p->hist_cur ^= 1;
+    if (!history_in_place(p)) p->hist_cur ^= 1;
     CKH(cudaStreamSynchronize(s_in));
     CKH(cudaStreamSynchronize(s_cmp));
     CKH(cudaStreamSynchronize(s_out));

@@ -441,6 +441,38 @@ def test_streaming_under_a_cuda_graph(cobalt, oracle, dev):
             _assert_parity(got[k][sb], vo, True, f"graph replay, block {k}, subband {sb}")
 
 
+def test_one_captured_call_replays_block_after_block(cobalt, oracle, dev):
+    """A single captured cobalt_process replayed on three consecutive blocks: the FIR history is carried in place, no
+    host-side state changes between calls."""
+    rng = np.random.default_rng(81)
+    S, B, C, n_t = 3, 2, 64, 40
+    N = C * n_t
+    data = [torch.from_numpy(rng.integers(-300, 300, size=(B, S, 2, N, 2)).astype(np.int16)) for _ in range(3)]
+    delays = rng.uniform(-1e-6, 1e-6, S)
+    bp = np.ones(C, dtype=np.float32)
+    with cobalt.Correlator(S, B, C, N, 16) as cor:
+        x = torch.empty_like(data[0], device=dev)
+        v = torch.empty(cor.vis_shape(), dtype=torch.complex64, device=dev)
+        d, b = torch.from_numpy(delays).to(dev), torch.from_numpy(bp).to(dev)
+        g = torch.cuda.CUDAGraph()
+        side = torch.cuda.Stream()
+        torch.cuda.synchronize()
+        with torch.cuda.graph(g, stream=side):
+            cor.process(x, d, b, out=v, stream=torch.cuda.current_stream())
+        cor.reset()
+        got = []
+        for r in range(3):
+            x.copy_(data[r])
+            g.replay()
+            torch.cuda.synchronize()
+            got.append(v.cpu().numpy().copy())
+    for sb in range(B):
+        hist = oracle.new_history(S, C)
+        for k in range(3):
+            vo = oracle.process_subband(data[k].numpy()[sb], C, delays, bp.astype(np.float64), oracle.default_subband_frequency(sb), hist)
+            _assert_parity(got[k][sb], vo, True, f"single-call graph replay, block {k}, subband {sb}")
+
+
 def test_golden_tiny_case_on_gpu(cobalt, dev):
     """The frozen oracle values of tests/golden/ (written by the oracle alone) against both GPU modes."""
     import os
