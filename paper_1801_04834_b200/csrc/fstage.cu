@@ -149,9 +149,7 @@ struct FShape {
     // per-thread tables, one row of 16 float2 per (stream, residue r) at a pitch of 144 bytes (16-byte loads of
     // consecutive rows then hit distinct banks)
     static constexpr int TAB_ROW = 144;
-    static constexpr int OFF_WTAB = OFF_Y + kYBufs * Y_BUF;      // [SPC][R] rows: rotation * bandpass, in register order
-    static constexpr int OFF_ZERO = OFF_WTAB + 16 * TAB_ROW;     // 16 float2 of zeros (spectra beyond n_t)
-    static constexpr int OFF_TW = OFF_ZERO + 128;                // [R] rows: W_C^{r k1}
+    static constexpr int OFF_TW = OFF_Y + kYBufs * Y_BUF;        // [R] rows: W_C^{r k1}
     static constexpr int OFF_STEP = OFF_TW + (R > 1 ? R * TAB_ROW : 0);   // INTERP: [SPC][R] rows of 16 floats, pitch 80 bytes
     static constexpr int STEP_ROW = 80;
     static constexpr int TOTAL = OFF_STEP + (INTERP ? 16 * STEP_ROW : 0);

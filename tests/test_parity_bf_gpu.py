@@ -201,3 +201,37 @@ def test_beamform_rejects_bad_settings(cobalt, dev):
         with pytest.raises(cobalt.CobaltError) as ei:
             cobalt.cobalt_beamform(cor._h, None, x, d, torch.ones(C, dtype=torch.float32, device=dev), bd, 2, cobalt.COBALT_BF_COHERENT_VOLTAGES, 1, 1, out)
         assert ei.value.status == cobalt.COBALT_ERR_BAD_ARG
+
+
+def test_beamformer_workload_shape_sampled(cobalt, oracle, dev):
+    """The shape bench.py --beamform times (48 stations, 256 channels, 195312 samples, 127 beams, Stokes I at t_int = 16; two
+    subbands here, one launch group), checked on sampled (subband, channel) pairs that the oracle computes one by one through its
+    single-sum channeliser (oracle.channel_direct) and its beamformer functions applied to that one channel."""
+    from paper_1801_04834_b200 import synth
+
+    cfg = synth.scaled(synth.CONFIGS[6], B=2)
+    n_beams, t_int = 127, 16
+    data = synth.generate(cfg, device=dev)
+    bd = synth.beam_delays(cfg, n_beams, dev)
+    with cobalt.Correlator(cfg.S, cfg.B, cfg.C, cfg.N, cfg.bits) as cor:
+        got = cor.beamform(data["samples"], data["delays"], data["bandpass"], cobalt.COBALT_BF_COHERENT_STOKES, beam_delays=bd,
+                           n_stokes=1, t_int=t_int)
+        cor.reset()
+        gv = cor.beamform(data["samples"], data["delays"], data["bandpass"], cobalt.COBALT_BF_COHERENT_VOLTAGES, beam_delays=bd)
+        torch.cuda.synchronize()
+        got, gv = got.cpu().numpy(), gv.cpu().numpy()
+    delays, bp, bdh = data["delays"].cpu().numpy(), data["bandpass"].cpu().numpy().astype(np.float64), bd.cpu().numpy()
+    rng = np.random.default_rng(3300)
+    pairs = [(0, 0), (1, cfg.C - 1), (0, cfg.C // 2)] + [(int(rng.integers(cfg.B)), int(rng.integers(cfg.C))) for _ in range(5)]
+    for sb, j in pairs:
+        x = data["samples"][sb].cpu().numpy()
+        f_sb = oracle.default_subband_frequency(sb)
+        zc, _ = oracle.channel_direct(x, cfg.C, j, delays=delays, bandpass=bp, f_sb=f_sb)             # [2S][n_t]
+        z1 = np.ascontiguousarray(zc.reshape(cfg.S, 2, cfg.n_t, 1))                                  # one channel as a C = 1 array
+        f_j = f_sb + (j - cfg.C / 2) * oracle.F_S / cfg.C
+        # oracle_channel_frequency(C = 1, f, f_s, 0) = f - f_s / 2: pass the channel's frequency through that formula
+        y = oracle.beamform_coherent(z1, bdh, f_j + 0.5 * oracle.F_S)[:, :, 0, :]                   # [n_beams][2][n_t]
+        st = oracle.coherent_stokes(z1, bdh, f_j + 0.5 * oracle.F_S, 1, t_int)[:, 0, 0, :]         # [n_beams][n_out]
+        ev = np.sqrt((np.abs(gv[sb, :, :, j, :] - y) ** 2).sum() / (np.abs(y) ** 2).sum())
+        es = np.sqrt(((got[sb, :, 0, j, :] - st) ** 2).sum() / (st ** 2).sum())
+        assert ev <= TOL_TENSOR and es <= TOL_TENSOR, f"subband {sb}, channel {j}: voltages {ev:.3e}, Stokes I {es:.3e}"
