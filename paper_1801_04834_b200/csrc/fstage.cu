@@ -8,9 +8,11 @@
 // instead of once per sample.  Only the time-varying part of cobalt_process_interp (reading A21) is applied here, per sample.
 // A copy kernel carries the FIR history to the next call.
 //
-// fstage_kernel<C, BITS, TENSOR, INTERP> is warp specialised (18 warps, one CTA per SM):
-//   CTA      = 256 / C consecutive streams (subband, station, pol) x a run of 64-spectrum k-tiles,
+// fstage_kernel<C, BITS, TENSOR, INTERP> is warp specialised (18 warps, one persistent CTA per SM):
+//   unit     = 256 / C consecutive streams (subband, station, pol) x a run of 64-spectrum k-tiles,
 //              walked in sub-tiles of 16 spectra; for C = 256 the two polarisations of a station one after the other.
+//              A CTA takes the units b, b + gridDim.x, ... back to back: every role walks the same list with running ring
+//              positions, so the producer already fetches the next unit while the FFT warps finish the current one.
 //   warp 16  = producer: the raw integer rows of the next sub-tiles (time-contiguous, so one bulk
 //              copy -- cp.async.bulk, SASS UBLKCP -- per stream and sub-tile, starting at the station's coarse sample
 //              offset, reading A25) land in a 3-deep shared-memory ring signalled on mbarriers; the first sub-tile of a CTA
@@ -45,6 +47,7 @@ struct FArgs {
     long long N, n_t;               // N = stream stride of `samples`
     size_t z_subband_bytes;
     int S, M, Mpad, n_kt, b0, tiles_per_seg, groups_per_subband;
+    int n_groups, n_seg;            // work units of a launch = (stream group, time segment) pairs, n_groups * n_seg of them
 };
 
 // Packed fp32 pairs (fma.rn.f32x2 family, SASS FFMA2/FADD2/FMUL2): a complex value is one 64-bit
@@ -171,6 +174,28 @@ __device__ __forceinline__ constexpr int out_reg(int i) {
     return R == 4 ? i : dft16_pos(i);
 }
 
+// One work unit of a launch: a group of 256 / C consecutive streams (for C = 256: both polarisations of a station, one after the
+// other) over one time segment.  CTAs are persistent: CTA b takes the units b, b + gridDim.x, ... back to back, so that the
+// producer already fetches the next unit while the FFT warps finish the current one (no pipeline fill / drain, no CTA launch
+// between units); every role walks the same unit list and keeps the same running ring positions.
+struct FUnit {
+    int bl, m0, n_items, kt0, n_sub;
+    long long t0;
+};
+template <int SPC, int IPC>
+__device__ __forceinline__ FUnit decode_unit(const FArgs &a, int u) {
+    FUnit w;
+    const int grp = u % a.n_groups, seg = u / a.n_groups;
+    w.bl = grp / a.groups_per_subband;
+    w.m0 = (grp - w.bl * a.groups_per_subband) * SPC * IPC;            // first stream of the unit
+    w.n_items = min(IPC, (a.M - w.m0 + SPC - 1) / SPC);                // items of the unit that exist
+    w.kt0 = seg * a.tiles_per_seg;
+    const int kt1 = min(w.kt0 + a.tiles_per_seg, a.n_kt);
+    w.n_sub = (kt1 - w.kt0) * (kKTile / kSubTile);
+    w.t0 = (long long)w.kt0 * kKTile;
+    return w;
+}
+
 // INTERP (reading A21): the delay of spectrum t is tau_b + (tau_e - tau_b) t / n_t.
 // The table holds the rotation for tau_b; a second table holds the phase step per spectrum f (tau_e - tau_b) / n_t in
 // cycles (computed in fp64), and the per-spectrum factor exp(-2 pi i frac(t step)) is formed in fp32 ("sin/cos and
@@ -189,15 +214,9 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, con
     const uint32_t bar_stg_empty = bar_stg_full + 8 * kStgBufs;        // [kStgBufs]
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const int grp = blockIdx.x;                          // stream group within the chunk
-    const int bl = grp / a.groups_per_subband;
     constexpr int IPC = Sh::IPC;
-    const int m0 = (grp - bl * a.groups_per_subband) * SPC * IPC;   // first stream of the CTA
-    const int n_items = min(IPC, (a.M - m0 + SPC - 1) / SPC);       // items of this CTA that exist
-    const int kt0 = blockIdx.y * a.tiles_per_seg;
-    const int kt1 = min(kt0 + a.tiles_per_seg, a.n_kt);
-    const int n_sub = (kt1 - kt0) * (kKTile / kSubTile);
-    const long long t0 = (long long)kt0 * kKTile;
+    const int n_units = a.n_groups * a.n_seg;
+    const FUnit first = decode_unit<SPC, IPC>(a, blockIdx.x);            // INTERP: the CTA's only unit (grid = units)
 
     if (tid == 0) {
         for (int s = 0; s < kRawStages; ++s) {
@@ -219,9 +238,9 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, con
         if (INTERP) {
             for (int idx = tid; idx < 256; idx += kFThreads) {
                 const int sl = idx / C, rr = (idx % C) / 16, i = idx % 16;
-                const int m = m0 + sl;
+                const int m = first.m0 + sl;
                 reinterpret_cast<float *>(smem + Sh::OFF_STEP + (idx >> 4) * Sh::STEP_ROW)[i] =
-                    m < a.M ? a.dstep[((size_t)bl * a.S + (m >> 1)) * C + out_channel<R>(rr, i)] : 0.f;
+                    m < a.M ? a.dstep[((size_t)first.bl * a.S + (m >> 1)) * C + out_channel<R>(rr, i)] : 0.f;
             }
         }
         if (R > 1) {
@@ -236,12 +255,17 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, con
 
     if (warp == kProducerWarp) {
         // ------------------------------------------------------------------ producer
+        uint32_t base_raw = 0;                                   // raw sub-tiles of the units before this one
+        for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
+        const FUnit w = decode_unit<SPC, IPC>(a, u);
+        const int bl = w.bl, m0 = w.m0, n_items = w.n_items, n_sub = w.n_sub;
+        const long long t0 = w.t0;
         for (int item = 0; item < n_items; ++item)
         for (int j = 0; j <= n_sub; ++j) {
             const int mi = m0 + item * SPC, n_valid = min(SPC, a.M - mi);
-            const int jg = item * (n_sub + 1) + j;               // position in the ring, over all items
-            const int s = jg % kRawStages;
-            const uint32_t ph = (uint32_t)(jg / kRawStages) & 1u;
+            const uint32_t jg = base_raw + (uint32_t)(item * (n_sub + 1) + j);   // position in the ring, over all units and items
+            const int s = (int)(jg % kRawStages);
+            const uint32_t ph = (jg / kRawStages) & 1u;
             mbar_wait(bar_raw_empty + 8 * s, ph ^ 1u);
             const long long tb = t0 - kSubTile + (long long)j * kSubTile;     // first row of the sub-tile
             const uint32_t full = bar_raw_full + 8 * s;
@@ -285,6 +309,8 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, con
             __syncwarp();
             if (lane == 0) mbar_arrive_expect_tx(full, tx);
         }
+        base_raw += (uint32_t)(n_items * (n_sub + 1));
+        }
     } else if (warp == kStoreWarp) {
         // ------------------------------------------------------------------ tensor-store issuer (step a7)
         // One staged tile = 32 spectra of every (stream, channel) of the CTA.  Row (channel c, k-tile kt, row group
@@ -293,11 +319,15 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, con
         // the 32 spectra of a tile are therefore the 64-byte half (tile & 1) ^ ((m >> 2) & 1) of the row, permuted
         // inside by m & 3 (done by the FFT threads); m >> 2 is the same for the <= 4 streams of a box.
         if (TENSOR && elect_one()) {
+            uint32_t base_tile = 0;                              // staged tiles of the units before this one
+            for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
+            const FUnit w = decode_unit<SPC, IPC>(a, u);
+            const int bl = w.bl, m0 = w.m0, n_items = w.n_items, n_sub = w.n_sub, kt0 = w.kt0;
             for (int item = 0; item < n_items; ++item)
             for (int tile = 0; tile < n_sub / 2; ++tile) {
-                const int tg = item * (n_sub / 2) + tile;        // n_sub / 2 is even: the buffer parity carries over
+                const uint32_t tg = base_tile + (uint32_t)(item * (n_sub / 2) + tile);   // n_sub / 2 is even: the buffer parity carries over
                 const int sbuf = tile & 1;
-                mbar_wait(bar_stg_full + 8 * sbuf, (uint32_t)(tg >> 1) & 1u);
+                mbar_wait(bar_stg_full + 8 * sbuf, (tg >> 1) & 1u);
                 const int kt = kt0 + (tile >> 1);
 #pragma unroll
                 for (int b = 0; b < Sh::BOXES; ++b) {
@@ -312,6 +342,8 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, con
                 asm volatile("cp.async.bulk.commit_group;" ::: "memory");
                 asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // shared memory has been read
                 mbar_arrive(bar_stg_empty + 8 * sbuf);
+            }
+            base_tile += (uint32_t)(n_items * (n_sub / 2));
             }
             asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
         }
@@ -338,18 +370,22 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, con
         const uint32_t raw_thread = sbase + Sh::OFF_RAW + sl * (kSubTile * C * SB) + ph * SB;
         float2 *ybuf = reinterpret_cast<float2 *>(smem + Sh::OFF_Y) + sl * YS + (R == 16 ? 18 * (ph & 15) + (ph >> 4) : ph + (ph >> 4));
 
+        uint32_t base_raw = 0, base_y = 0;
+        for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
+        const FUnit w = decode_unit<SPC, IPC>(a, u);
+        const int n_items = w.n_items, n_sub = w.n_sub;
         for (int item = 0; item < n_items; ++item)
         for (int j = 0; j <= n_sub; ++j) {
-            const int jg = item * (n_sub + 1) + j;
-            const int s = jg % kRawStages;
-            mbar_wait(bar_raw_full + 8 * s, (uint32_t)(jg / kRawStages) & 1u);
+            const uint32_t jg = base_raw + (uint32_t)(item * (n_sub + 1) + j);
+            const int s = (int)(jg % kRawStages);
+            mbar_wait(bar_raw_full + 8 * s, (jg / kRawStages) & 1u);
             const int jj = j - 1;                         // real sub-tile index (j = 0 is the warm-up)
-            const int jjg = item * n_sub + jj;
-            const int yb = jjg % kYBufs;
+            const uint32_t jjg = base_y + (uint32_t)(item * n_sub + jj);   // (unused for the warm-up)
+            const int yb = (int)(jjg % kYBufs);
             const uint32_t raw = raw_thread + s * Sh::RAW_STAGE;
             // The warm-up sub-tile (jj < 0) stores nothing: its 16 samples only re-initialise the pending outputs (every
             // slot gets its first tap from one of them), also when the accumulators still hold the previous item's sums.
-            if (jj >= 0) mbar_wait(bar_y_empty + 8 * yb, ((uint32_t)(jjg / kYBufs) & 1u) ^ 1u);
+            if (jj >= 0) mbar_wait(bar_y_empty + 8 * yb, ((jjg / kYBufs) & 1u) ^ 1u);
             float2 *yrow = ybuf + (size_t)(jj >= 0 ? yb : 0) * (Sh::Y_BUF / 8);
 #pragma unroll
             for (int half = 0; half < 2; ++half) {
@@ -382,6 +418,9 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, con
                 if (jj >= 0) mbar_arrive(bar_y_full + 8 * yb);
             }
         }
+        base_raw += (uint32_t)(n_items * (n_sub + 1));
+        base_y += (uint32_t)(n_items * n_sub);
+        }
     } else {
         // ------------------------------------------------------------------ FFT, rotate, transpose (steps a3-a7)
         // Team tm takes the sub-tiles jj = tm, tm + 2, ...; a thread owns TWO consecutive spectra (so that the fp16
@@ -404,18 +443,22 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, con
         // staging word of (channel c, plane, pair p of the tile): box b = sl / SPB, then [stream][plane][channel][64 B],
         // the 16-byte chunk (p >> 2) stored at (p >> 2) ^ (m & 3), 64-byte swizzled like the tensor store reads it
         const uint32_t stg_thread = (uint32_t)((sl / Sh::SPB) * Sh::BOX_BYTES + (sl % Sh::SPB) * (2 * C * 64));
+        uint32_t base_y = 0;
+        for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
+        const FUnit w = decode_unit<SPC, IPC>(a, u);
+        const int bl = w.bl, m0 = w.m0, n_items = w.n_items, n_sub = w.n_sub, kt0 = w.kt0;
         unsigned char *zsub = a.z + (size_t)bl * a.z_subband_bytes;
 
         for (int item = 0; item < n_items; ++item)
         for (int jj = tm; jj < n_sub; jj += kFftTeams) {
             const int m = m0 + item * SPC + sl;
-            const int jjg = item * n_sub + jj;                   // n_sub is a multiple of 4: team and staging parities carry over
-            const int yb = jjg % kYBufs;
+            const uint32_t jjg = base_y + (uint32_t)(item * n_sub + jj);   // n_sub is a multiple of 4: team and staging parities carry over
+            const int yb = (int)(jjg % kYBufs);
             const int kt = kt0 + (jj >> 2), sub = jj & 3;
             const long long t_spec = (long long)kt * kKTile + sub * kSubTile + 2 * tp;   // first of the two spectra
             float2 *y0 = ybase + (size_t)yb * (Sh::Y_BUF / 8);
             float2 *y1 = y0 + Sh::TS;
-            mbar_wait(bar_y_full + 8 * yb, (uint32_t)(jjg / kYBufs) & 1u);
+            mbar_wait(bar_y_full + 8 * yb, (jjg / kYBufs) & 1u);
             float2 o0[16], o1[16];
             if (R == 16) {
 #pragma unroll
@@ -495,10 +538,11 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, con
             const bool live0 = t_spec < a.n_t, live1 = t_spec + 1 < a.n_t;
             const bool lost = m >= a.M || (a.valid && a.valid[((size_t)(a.b0 + bl) * a.S + (m >> 1)) * a.n_kt + kt] == 0);
             if (TENSOR) {
-                const int tile = jjg >> 1, sbuf = tile & 1;
+                const uint32_t tile = jjg >> 1;
+                const int sbuf = (int)(tile & 1u);
                 const int p = 8 * (jj & 1) + tp;          // pair of spectra within the 32-spectrum tile
                 const uint32_t msk = !live0 || lost ? 0u : live1 ? 0xffffffffu : 0x0000ffffu;   // n_t odd: last pair is half live
-                mbar_wait(bar_stg_empty + 8 * sbuf, ((uint32_t)(tile >> 1) & 1u) ^ 1u);
+                mbar_wait(bar_stg_empty + 8 * sbuf, ((tile >> 1) & 1u) ^ 1u);
                 unsigned char *stg = smem + Sh::OFF_STG + sbuf * Sh::STG + stg_thread;
                 // byte offset of (channel j, plane re, this pair) in the box: 64 j + 16 ((p >> 2) ^ (m & 3)) + 4 (p & 3), then
                 // the store's 64-byte swizzle (bits 4-5 ^= bits 7-8).  Bits 7-8 come from 64 j only, and j = (part fixed by
@@ -547,6 +591,8 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, con
                     }
                 }
             }
+        }
+        base_y += (uint32_t)(n_items * n_sub);
         }
     }
 }
@@ -654,7 +700,12 @@ cudaError_t launch_f(const cobalt_plan_s *p, cudaStream_t st, const FArgs &a, in
     if (n_seg > max_seg) n_seg = max_seg;
     args.tiles_per_seg = (p->n_kt + n_seg - 1) / n_seg;
     n_seg = (p->n_kt + args.tiles_per_seg - 1) / args.tiles_per_seg;
-    dim3 grid((unsigned)groups, (unsigned)n_seg);
+    args.n_groups = (int)groups;
+    args.n_seg = n_seg;
+    // Persistent CTAs, one per SM, each walking its units back to back (decode_unit).  The time-varying-delay instantiation
+    // keeps a per-CTA table of its unit's phase steps: one unit per CTA there.
+    const long long units = groups * n_seg;
+    const unsigned grid = INTERP ? (unsigned)units : (unsigned)(units < p->sm_count ? units : p->sm_count);
     kern<<<grid, kFThreads, smem, st>>>(args, p->zmap);
     return cudaGetLastError();
 }
