@@ -406,7 +406,7 @@ def test_output_pointer_not_16_byte_aligned_is_rejected_in_tensor_mode(cobalt, d
 
 def test_streaming_under_a_cuda_graph(cobalt, oracle, dev):
     """SURVEY.md sec 8(f) row 2 (streaming): cobalt_process only enqueues kernels on the caller's stream, so two
-    consecutive blocks (the FIR history ping-pongs between two buffers, hence pairs of calls) can be captured in a
+    consecutive blocks can be captured in a
     CUDA graph and replayed on new data; the history carries across replays exactly as across plain calls."""
     synth = _synth()
     cfg = synth.scaled(synth.CONFIGS[2], S=3, B=2, C=64, N=64 * 40)
