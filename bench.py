@@ -394,6 +394,34 @@ def run_ours(args, rank, world, local):
     return 0
 
 
+def oracle_beamform_sample(cfg, beam_delays, product, n_stokes, t_int, pkg):
+    """The oracle (as it stands) on a bounded sample of the beamformer workload: the first subband, the first 2 t_int-blocks of
+    at least 32 spectra; float64, direct FIR, naive DFT, a cos/sin per (beam, station, channel, spectrum) term."""
+    import numpy as np
+
+    import oracle
+    from paper_1801_04834_b200 import synth
+
+    oracle.build()
+    n_t_s = max(32, 2 * t_int)
+    geo = synth.geometry(cfg, "cpu")
+    x = synth.generate_subband(cfg, 0, "cpu", geo)[:, :, : n_t_s * cfg.C, :].contiguous().numpy()
+    t0 = time.perf_counter()
+    z = oracle.channelise_subband(x, cfg.C, geo["delays"].numpy(), geo["bandpass"].numpy().astype(np.float64), oracle.default_subband_frequency(0))
+    if product == pkg.COBALT_BF_COHERENT_VOLTAGES:
+        oracle.beamform_coherent(z, beam_delays, oracle.default_subband_frequency(0))
+    elif product == pkg.COBALT_BF_COHERENT_STOKES:
+        oracle.coherent_stokes(z, beam_delays, oracle.default_subband_frequency(0), n_stokes, t_int)
+    else:
+        oracle.incoherent_stokes(z, n_stokes, t_int)
+    sec = time.perf_counter() - t0
+    units = float(beam_delays.shape[0]) * n_t_s * cfg.C
+    return {"value": units / sec, "unit": "beam*channel*samples/s", "cores": oracle.num_threads(), "kind": "oracle", "seconds": sec,
+            "sample": f"oracle channeliser + beamformer on subband 0 of {cfg.B}, first {n_t_s} of {cfg.n_t} spectra ({cfg.S} stations, "
+                      f"{cfg.C} channels, {beam_delays.shape[0]} beams); float64, naive DFT, a cos/sin per term; throughput of the sample, "
+                      "extrapolated linearly to the whole workload"}
+
+
 def run_beamform(args, rank, world, local):
     """`--beamform`: one step = one cobalt_beamform over the whole beamformer workload (F-stage + beamformer kernel)."""
     import torch
@@ -469,6 +497,9 @@ def run_beamform(args, rank, world, local):
               "note": "algorithmic flops = 8 per (beam, polarisation, station, channel-sample); the kernel issues twice that (the weight rows are zero on the other polarisation)"}
     dominant, other = (roof_f, roof_b) if t_f >= t_b else (roof_b, roof_f)
     cor.close()
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        cpu = oracle_beamform_sample(cfg, bd.cpu().numpy(), product, n_stokes, t_int, pkg)
     if rank == 0:
         line = {
             "metric": "beam-channel-samples/s", "value": whole_job_value(units, world, sec_step), "unit": "beam*channel*samples/s",
@@ -482,7 +513,7 @@ def run_beamform(args, rank, world, local):
             "roofline": dominant, "roofline_other": other,
             "stage_ms": {"phase_table": t_phase * 1e3, "f_stage": t_f * 1e3, "history": t_hist * 1e3, "beamform": t_b * 1e3},
             "real_time_factor": (cfg.n_t * cfg.C / F_S) / sec_step, "output_bytes": out_bytes,
-            "clocks": clocks, "gpu_launches": int(launches), "e2e": None, "cpu_baseline": None,
+            "clocks": clocks, "gpu_launches": int(launches), "e2e": None, "cpu_baseline": cpu,
         }
         print(json.dumps(line), flush=True)
     return 0
