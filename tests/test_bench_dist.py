@@ -61,3 +61,21 @@ def test_single_process_helpers_without_a_group():
     assert bench.whole_job_value(10.0, 4, 2.0) == 20.0
     args = bench.parse_args([])
     assert args.gpus == 1 and args.config == 3 and args.warmup >= 3
+
+
+def test_beamformer_bench_host_side():
+    """bench.py --beamform without a GPU: argument parsing, the workload it selects (synth config 6) and the oracle leg of its
+    cpu_baseline on a scaled-down instance."""
+    sys.path.insert(0, ROOT)
+    import bench
+    import paper_1801_04834_b200 as pkg
+    from paper_1801_04834_b200 import synth
+
+    args = bench.parse_args(["--beamform", "stokes-i", "--beams", "5", "--t-int", "4"])
+    cfg = bench.workload(args)
+    assert cfg.name == "beamformer-core-16bit" and (cfg.S, cfg.C) == (48, 256)
+    small = synth.scaled(cfg, S=3, B=1, C=16, N=16 * 64)
+    bd = synth.beam_delays(small, 5, "cpu").numpy()
+    assert bd.shape == (5, 3) and abs(bd[0]).max() == 0.0              # beam 0 is the phase centre
+    r = bench.oracle_beamform_sample(small, bd, pkg.COBALT_BF_COHERENT_STOKES, 1, 4, pkg)
+    assert r["kind"] == "oracle" and r["value"] > 0 and r["cores"] >= 1
