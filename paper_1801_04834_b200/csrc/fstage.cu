@@ -23,6 +23,7 @@
 //              the completed output goes to a 3-deep ring of shared-memory tiles.  The weights carry (-1)^ph (the
 //              ascending-frequency channel order D[(j + C/2) mod C] for free) and the power-of-two scale of the fp16
 //              intermediate (exact).
+//              The FIR -> FFT hand-over uses hardware named barriers (a waiting warp issues nothing).
 //   warps 8-15 = FFT + transpose, two teams of four warps on alternate sub-tiles: thread = (two spectra, 1/16 of their
 //              channels): radix-16 pass in registers, twiddle, warp-local shared-memory exchange, radix-R pass (C = 16 R),
 //              [INTERP: exp(-2 pi i t step)], fp16 (or fp32) conversion, staged transposed in shared memory.  Spectra beyond
@@ -118,6 +119,13 @@ constexpr int kRawStages = 3;      // ring of raw sub-tiles (bulk copies in flig
 constexpr int kYBufs = 3;          // ring of FIR-output sub-tiles
 constexpr int kStgTile = 32;       // spectra per staged output tile (= one tensor store per box)
 constexpr int kStgBufs = 2;
+// Named (hardware) barriers for the FIR -> FFT hand-over of the y ring: a warp waiting in bar.sync issues nothing, a warp polling
+// an mbarrier does (barrier 0 is __syncthreads).  The single-warp waits (producer, store issuer) stay on mbarriers: moving them to
+// named barriers as well measured slower (4.19 / 4.24 ms against 4.15 ms per 61-subband launch).
+// One barrier per (y buffer, consuming FFT team): the two teams are not paced against each other (EXACT mode has no staging
+// that couples them), and a team that runs ahead must not complete the barrier generation meant for the other one.
+constexpr int kBarYFull = 1, kBarYEmpty = kBarYFull + kYBufs * kFftTeams;
+static_assert(kBarYEmpty + kYBufs * kFftTeams <= 16, "named barriers");
 
 template <int C, int BITS, bool TENSOR, bool INTERP = false>
 struct FShape {
@@ -207,11 +215,9 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, con
     extern __shared__ __align__(1024) unsigned char smem[];
     const uint32_t sbase = smem_u32(smem);
     const uint32_t bar_raw_full = sbase + Sh::OFF_BAR;                 // [kRawStages]
-    const uint32_t bar_raw_empty = bar_raw_full + 8 * kRawStages;      // [kRawStages]
-    const uint32_t bar_y_full = bar_raw_empty + 8 * kRawStages;        // [kYBufs]
-    const uint32_t bar_y_empty = bar_y_full + 8 * kYBufs;              // [kYBufs]
-    const uint32_t bar_stg_full = bar_y_empty + 8 * kYBufs;            // [kStgBufs]
-    const uint32_t bar_stg_empty = bar_stg_full + 8 * kStgBufs;        // [kStgBufs]
+    const uint32_t bar_stg_empty = bar_raw_full + 8 * kRawStages;      // [kStgBufs]
+    const uint32_t bar_raw_empty = bar_stg_empty + 8 * kStgBufs;       // [kRawStages]
+    const uint32_t bar_stg_full = bar_raw_empty + 8 * kRawStages;      // [kStgBufs]
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     constexpr int IPC = Sh::IPC;
@@ -219,18 +225,10 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, con
     const FUnit first = decode_unit<SPC, IPC>(a, blockIdx.x);            // INTERP: the CTA's only unit (grid = units)
 
     if (tid == 0) {
-        for (int s = 0; s < kRawStages; ++s) {
-            mbar_init(bar_raw_full + 8 * s, 1);
-            mbar_init(bar_raw_empty + 8 * s, kFirThreads / 32);
-        }
-        for (int b = 0; b < kYBufs; ++b) {
-            mbar_init(bar_y_full + 8 * b, kFirThreads / 32);
-            mbar_init(bar_y_empty + 8 * b, kFftTeam / 32);
-        }
-        for (int b = 0; b < kStgBufs; ++b) {
-            mbar_init(bar_stg_full + 8 * b, kFftThreads / 32);
-            mbar_init(bar_stg_empty + 8 * b, 1);
-        }
+        for (int s = 0; s < kRawStages; ++s) mbar_init(bar_raw_full + 8 * s, 1);
+        for (int b = 0; b < kStgBufs; ++b) mbar_init(bar_stg_empty + 8 * b, 1);
+        for (int s = 0; s < kRawStages; ++s) mbar_init(bar_raw_empty + 8 * s, kFirThreads / 32);
+        for (int b = 0; b < kStgBufs; ++b) mbar_init(bar_stg_full + 8 * b, kFftThreads / 32);
         mbar_fence_init();
     }
     {   // per-CTA tables: the phase step per spectrum of the CTA's streams (INTERP) in the FFT threads' register order, and
@@ -265,8 +263,7 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, con
             const int mi = m0 + item * SPC, n_valid = min(SPC, a.M - mi);
             const uint32_t jg = base_raw + (uint32_t)(item * (n_sub + 1) + j);   // position in the ring, over all units and items
             const int s = (int)(jg % kRawStages);
-            const uint32_t ph = (jg / kRawStages) & 1u;
-            mbar_wait(bar_raw_empty + 8 * s, ph ^ 1u);
+            mbar_wait(bar_raw_empty + 8 * s, ((jg / kRawStages) & 1u) ^ 1u);
             const long long tb = t0 - kSubTile + (long long)j * kSubTile;     // first row of the sub-tile
             const uint32_t full = bar_raw_full + 8 * s;
             uint32_t tx = 0;
@@ -318,34 +315,37 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, con
         // tensor-map coordinates: spectrum, channel, 2 (m / 8) + plane, m % 8, k-tile):
         // the 32 spectra of a tile are therefore the 64-byte half (tile & 1) ^ ((m >> 2) & 1) of the row, permuted
         // inside by m & 3 (done by the FFT threads); m >> 2 is the same for the <= 4 streams of a box.
-        if (TENSOR && elect_one()) {
-            uint32_t base_tile = 0;                              // staged tiles of the units before this one
+        if (TENSOR) {
+            const bool leader = elect_one();
+            uint32_t stg_count = 0;
             for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
             const FUnit w = decode_unit<SPC, IPC>(a, u);
             const int bl = w.bl, m0 = w.m0, n_items = w.n_items, n_sub = w.n_sub, kt0 = w.kt0;
             for (int item = 0; item < n_items; ++item)
             for (int tile = 0; tile < n_sub / 2; ++tile) {
-                const uint32_t tg = base_tile + (uint32_t)(item * (n_sub / 2) + tile);   // n_sub / 2 is even: the buffer parity carries over
                 const int sbuf = tile & 1;
-                mbar_wait(bar_stg_full + 8 * sbuf, (tg >> 1) & 1u);
-                const int kt = kt0 + (tile >> 1);
+                mbar_wait(bar_stg_full + 8 * sbuf, (stg_count >> 1) & 1u);
+                if (leader) {
+                    const int kt = kt0 + (tile >> 1);
 #pragma unroll
-                for (int b = 0; b < Sh::BOXES; ++b) {
-                    const int mb = m0 + item * SPC + b * Sh::SPB;
-                    if (mb >= a.Mpad) break;
-                    const int c0 = 32 * ((tile & 1) ^ ((mb >> 2) & 1));
-                    asm volatile(
-                        "cp.async.bulk.tensor.5d.global.shared::cta.bulk_group [%0, {%2, %3, %4, %5, %6}], [%1];" ::"l"(&zmap),
-                        "r"(sbase + Sh::OFF_STG + sbuf * Sh::STG + b * Sh::BOX_BYTES), "r"(c0), "r"(bl * C), "r"(2 * (mb >> 3)), "r"(mb & 7), "r"(kt)
-                        : "memory");
+                    for (int b = 0; b < Sh::BOXES; ++b) {
+                        const int mb = m0 + item * SPC + b * Sh::SPB;
+                        if (mb >= a.Mpad) break;
+                        const int c0 = 32 * ((tile & 1) ^ ((mb >> 2) & 1));
+                        asm volatile(
+                            "cp.async.bulk.tensor.5d.global.shared::cta.bulk_group [%0, {%2, %3, %4, %5, %6}], [%1];" ::"l"(&zmap),
+                            "r"(sbase + Sh::OFF_STG + sbuf * Sh::STG + b * Sh::BOX_BYTES), "r"(c0), "r"(bl * C), "r"(2 * (mb >> 3)), "r"(mb & 7), "r"(kt)
+                            : "memory");
+                    }
+                    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+                    asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // shared memory has been read
+                    mbar_arrive(bar_stg_empty + 8 * sbuf);
                 }
-                asm volatile("cp.async.bulk.commit_group;" ::: "memory");
-                asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // shared memory has been read
-                mbar_arrive(bar_stg_empty + 8 * sbuf);
+                __syncwarp();
+                ++stg_count;
             }
-            base_tile += (uint32_t)(n_items * (n_sub / 2));
             }
-            asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+            if (leader) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
         }
     } else if (warp < kFirThreads / 32) {
         // ------------------------------------------------------------------ FIR (steps a1, a2)
@@ -385,7 +385,10 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, con
             const uint32_t raw = raw_thread + s * Sh::RAW_STAGE;
             // The warm-up sub-tile (jj < 0) stores nothing: its 16 samples only re-initialise the pending outputs (every
             // slot gets its first tap from one of them), also when the accumulators still hold the previous item's sums.
-            if (jj >= 0) mbar_wait(bar_y_empty + 8 * yb, ((jjg / kYBufs) & 1u) ^ 1u);
+            // FIR -> FFT hand-over of the y ring through NAMED barriers (ids kBarYFull.., kBarYEmpty..; the 256 FIR threads
+            // and the 128 threads of the consuming team): a warp waiting in bar.sync issues nothing, where the eight FIR warps
+            // polling an mbarrier took 8 % of the kernel's issue slots from the FFT warps they were waiting for.
+            if (jj >= 0 && jjg >= (uint32_t)kYBufs) bar_sync_named(kBarYEmpty + kFftTeams * yb + (int)((jjg - kYBufs) & 1u), kFirThreads + kFftTeam);
             float2 *yrow = ybuf + (size_t)(jj >= 0 ? yb : 0) * (Sh::Y_BUF / 8);
 #pragma unroll
             for (int half = 0; half < 2; ++half) {
@@ -413,9 +416,10 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, con
                 }
             }
             __syncwarp();
-            if (lane == 0) {
-                mbar_arrive(bar_raw_empty + 8 * s);
-                if (jj >= 0) mbar_arrive(bar_y_full + 8 * yb);
+            if (lane == 0) mbar_arrive(bar_raw_empty + 8 * s);
+            if (jj >= 0) {
+                __threadfence_block();
+                bar_arrive_named(kBarYFull + kFftTeams * yb + (int)(jjg & 1u), kFirThreads + kFftTeam);
             }
         }
         base_raw += (uint32_t)(n_items * (n_sub + 1));
@@ -458,7 +462,8 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, con
             const long long t_spec = (long long)kt * kKTile + sub * kSubTile + 2 * tp;   // first of the two spectra
             float2 *y0 = ybase + (size_t)yb * (Sh::Y_BUF / 8);
             float2 *y1 = y0 + Sh::TS;
-            mbar_wait(bar_y_full + 8 * yb, (jjg / kYBufs) & 1u);
+            __syncwarp();                                 // bar.sync is warp-aligned: reconverge after the previous sub-tile's stores
+            bar_sync_named(kBarYFull + kFftTeams * yb + tm, kFirThreads + kFftTeam);
             float2 o0[16], o1[16];
             if (R == 16) {
 #pragma unroll
@@ -498,7 +503,7 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, con
                     o1[r2] = y1[18 * r2 + r];
                 }
                 __syncwarp();
-                if (lane == 0) mbar_arrive(bar_y_empty + 8 * yb);
+                bar_arrive_named(kBarYEmpty + kFftTeams * yb + tm, kFirThreads + kFftTeam);
                 dft16(o0);                                // channel r + 16 k2 at o[dft16_pos(k2)]
                 dft16(o1);
             } else if (R == 4) {
@@ -521,7 +526,7 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, con
                     }
                 }
                 __syncwarp();
-                if (lane == 0) mbar_arrive(bar_y_empty + 8 * yb);
+                bar_arrive_named(kBarYEmpty + kFftTeams * yb + tm, kFirThreads + kFftTeam);
 #pragma unroll
                 for (int a4 = 0; a4 < 4; ++a4) {
                     dft4(o0[4 * a4], o0[4 * a4 + 1], o0[4 * a4 + 2], o0[4 * a4 + 3]);
@@ -529,7 +534,7 @@ __global__ void __launch_bounds__(kFThreads, 1) fstage_kernel(const FArgs a, con
                 }
             } else {
                 __syncwarp();
-                if (lane == 0) mbar_arrive(bar_y_empty + 8 * yb);
+                bar_arrive_named(kBarYEmpty + kFftTeams * yb + tm, kFirThreads + kFftTeam);
             }
             // steps a5-a7.  The static rotation * bandpass (a5, a6) is a per-(input, channel) constant and is applied to the
             // visibilities by the X-stage (V_ik <- w_i conj(w_k) V_ik, the same product); here only the time-varying part of

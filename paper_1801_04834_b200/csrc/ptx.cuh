@@ -69,6 +69,12 @@ __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.a
 __device__ __forceinline__ void bar_sync_named(int id, int threads) {
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(threads) : "memory");
 }
+// Producer side of a named barrier (PTX ISA "bar": st.shared ...; bar.arrive in the producer, bar.sync; ld.shared in the consumer):
+// counts the calling warp's threads and does not wait.  A warp blocked in bar.sync is descheduled by the hardware -- unlike an
+// mbarrier wait it issues nothing while it waits.
+__device__ __forceinline__ void bar_arrive_named(int id, int threads) {
+    asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(threads) : "memory");
+}
 
 // One lane of a fully converged warp; ptxas then treats the guarded region as single-threaded and emits the
 // UTCHMMA / UBLKCP / UTMASTG sequence without a per-instruction ELECT loop.

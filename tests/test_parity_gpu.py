@@ -571,3 +571,22 @@ def test_set_sample_rate_rebuilds_the_default_ladder(cobalt, oracle, dev):
     for b in range(cfg.B):
         vo = oracle.process_subband(data["samples"].numpy()[b], cfg.C, delays, bp, 100.0e6 + (12 + b) * f_s, f_s=f_s)
         _assert_parity(vg[b], vo, False, f"default ladder at f_s = {f_s}, subband {b}")
+
+
+@pytest.mark.parametrize("S,B,C,n_t", [(77, 2, 256, 762), (40, 3, 64, 3000)])
+def test_exact_mode_many_units_per_cta(cobalt, oracle, dev, S, B, C, n_t):
+    """Several (stream group, time segment) units per persistent F-stage CTA in EXACT mode, where nothing paces the two FFT
+    teams against each other: the FIR -> FFT hand-over uses one named barrier per (y buffer, team), so a team that runs ahead
+    cannot take the other team's barrier generation (a shared barrier deadlocked here).  Sampled channels against the oracle."""
+    rng = np.random.default_rng(4100 + S)
+    N = n_t * C
+    x = rng.integers(-500, 500, size=(B, S, 2, N, 2)).astype(np.int16)
+    delays = rng.uniform(-1e-6, 1e-6, S)
+    bp = np.ones(C, dtype=np.float32)
+    with cobalt.Correlator(S, B, C, N, 16, mode=cobalt.COBALT_MODE_EXACT_FP32) as cor:
+        vis = cor.process(torch.from_numpy(x).to(dev), torch.from_numpy(delays).to(dev), torch.from_numpy(bp).to(dev))
+        torch.cuda.synchronize()
+        vis = vis.cpu().numpy()
+    for sb, j in [(0, 1), (B - 1, C // 2), (B - 1, C - 1)]:
+        _, vo = oracle.channel_direct(x[sb], C, j, delays=delays, bandpass=bp.astype(np.float64), f_sb=oracle.default_subband_frequency(sb))
+        _assert_parity(vis[sb, j][None], vo[None], False, f"exact mode, subband {sb}, channel {j}")
