@@ -297,6 +297,48 @@ int cobalt_debug_channelised(cobalt_plan_t *plan, void *cuda_stream, const void 
  * d_vis [C][n_bl][2][2] complex64, through the X-stage of the current mode. */
 int cobalt_debug_correlate(cobalt_plan_t *plan, void *cuda_stream, const void *d_z, void *d_vis);
 
+/* --------------------------------------------------------------------------- no-allocation entry point */
+/* cobalt_correlate_noalloc: steps a8-a9 ("computes the correlations of all pairs of antenna fields and averages
+ * in time") of ONE subband without a plan and without a single device or pinned-host allocation, for callers that must
+ * not allocate: a real-time pipeline that took all its buffers from pools before the observation started
+ * cannot afford cudaMalloc / cudaFree in mid-run -- both synchronise the whole device, so every stream stalls and a
+ * late block of antenna data is dropped -- and on a GPU whose memory is budgeted to the last buffer they may
+ * fail; the same goes for code running inside a host application that owns all device memory through its own pool.
+ * Every other entry point needs a cobalt_plan, and cobalt_plan allocates.
+ *
+ * The arithmetic is that of COBALT_MODE_EXACT_FP32 (fp32 FMAs; tolerance vs the float64 oracle 1e-4 of
+ * sqrt(V_ii V_kk)), organised like the split X-stage: the time range is cut into at most COBALT_NOALLOC_MAX_SLICES
+ * slices whose partial visibilities are added in slice order, so the result is deterministic (it differs from
+ * cobalt_debug_correlate only by the order of the fp32 additions).  The partial visibilities live in a fixed
+ * COBALT_NOALLOC_SCRATCH_BYTES array inside the library's device image instead of in allocated memory.  Consequences:
+ *   - every GPU on which the library's module is loaded holds those 16 MiB until the process exits;
+ *   - sizes are limited: channels * n_bl <= COBALT_NOALLOC_MAX_CHANNEL_BASELINES (n_bl = S (S + 1) / 2; e.g. S <= 63
+ *     at 64 channels, S <= 31 at 256).  Anything larger returns COBALT_ERR_BAD_ARG with the numbers in h_err and
+ *     launches nothing;
+ *   - the FIRST call on a device looks up where the array lives on that device (cudaGetSymbolAddress, under a host
+ *     mutex) and remembers it; make that first call during start-up, with the device current, before any stream
+ *     capture is begun on it.  Later calls on that device only launch two kernels on `cuda_stream`;
+ *   - all calls on a device share the array.  It needs no clearing (each call overwrites every slot it later reads),
+ *     and calls on the same stream are safe.  Calls that can overlap on the GPU -- different streams, or several host
+ *     threads each with a stream -- race on it and produce wrong output; the caller must serialise them.
+ *
+ *   cuda_stream  cudaStream_t as void* (NULL = legacy default stream); the call only enqueues, it does not synchronise
+ *   d_z          device, [C][2 S][n_t] complex64, input index 2 * station + pol (the layout of cobalt_debug_correlate);
+ *                read only, 8-byte aligned
+ *   stations     S >= 1;  channels C in {16, 64, 256};  n_spectra n_t in [1, 2^30]
+ *   d_vis        device, [C][n_bl][2][2] complex64, baseline (i <= k) at k (k + 1) / 2 + i (reading A9); fully
+ *                overwritten, 8-byte aligned.  Caller-owned like d_z; both must stay alive until the stream gets there
+ *   h_err        host, NULL or a buffer of h_err_len bytes that receives a 0-terminated description of a failure
+ *                (there is no plan whose cobalt_last_error could hold it); emptied on success
+ * Returns COBALT_OK, COBALT_ERR_BAD_ARG (NULL / misaligned pointer, size out of range or beyond the scratch),
+ * COBALT_ERR_UNSUPPORTED_DEVICE (no CUDA device, or not sm_100 class; no CPU fallback) or COBALT_ERR_CUDA.
+ * Arguments are checked before the device is touched. */
+#define COBALT_NOALLOC_SCRATCH_BYTES 16777216
+#define COBALT_NOALLOC_MAX_SLICES 4
+#define COBALT_NOALLOC_MAX_CHANNEL_BASELINES 131072   /* SCRATCH_BYTES / (MAX_SLICES * 32 bytes per [2][2] complex64) */
+int cobalt_correlate_noalloc(void *cuda_stream, const void *d_z, int stations, int channels, long long n_spectra,
+                             void *d_vis, char *h_err, int h_err_len);
+
 #ifdef __cplusplus
 }
 #endif

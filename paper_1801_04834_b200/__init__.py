@@ -28,6 +28,9 @@ COBALT_LAYOUT_POL_MINOR = 1
 COBALT_BF_COHERENT_VOLTAGES = 0
 COBALT_BF_COHERENT_STOKES = 1
 COBALT_BF_INCOHERENT_STOKES = 2
+COBALT_NOALLOC_SCRATCH_BYTES = 16777216
+COBALT_NOALLOC_MAX_SLICES = 4
+COBALT_NOALLOC_MAX_CHANNEL_BASELINES = 131072
 
 F_S = 195312.5
 
@@ -40,6 +43,7 @@ ABI_SYMBOLS = (
     "cobalt_set_timing", "cobalt_get_timing", "cobalt_get_kernel_timing",
     "cobalt_debug_fir_weights", "cobalt_debug_unpack", "cobalt_debug_channelised", "cobalt_debug_correlate",
     "cobalt_beamform", "cobalt_beamform_output_bytes",
+    "cobalt_correlate_noalloc",
 )
 
 
@@ -124,6 +128,7 @@ def load(path: str | None = None):
     lib.cobalt_beamform.argtypes = [_vp, _vp, ctypes.POINTER(cobalt_bf_io_t)]
     lib.cobalt_beamform_output_bytes.argtypes = [_vp, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int]
     lib.cobalt_beamform_output_bytes.restype = ctypes.c_longlong
+    lib.cobalt_correlate_noalloc.argtypes = [_vp, _vp, ctypes.c_int, ctypes.c_int, ctypes.c_longlong, _vp, ctypes.c_char_p, ctypes.c_int]
     for name in ABI_SYMBOLS:
         fn = getattr(lib, name)
         if name not in ("cobalt_strerror", "cobalt_last_error", "cobalt_beamform_output_bytes"):
@@ -201,6 +206,18 @@ def cobalt_beamform(plan, stream, d_samples, d_delays, d_bandpass, d_beam_delays
     io = cobalt_bf_io_t(_ptr(d_samples), _ptr(d_delays), _ptr(d_delays_end), _ptr(d_bandpass), _ptr(d_valid), _ptr(d_beam_delays),
                         int(n_beams), int(product), int(n_stokes), int(t_int), _ptr(d_out))
     _check(load().cobalt_beamform(plan, _stream_ptr(stream), ctypes.byref(io)), plan)
+
+
+def cobalt_correlate_noalloc(stream, d_z, stations, channels, n_spectra, d_vis):
+    """Steps a8-a9 of one subband for callers that must not allocate device memory (a running real-time pipeline, a host
+    application with its own memory pool): no plan, fp32, partial sums in a fixed 16 MiB array inside the library.
+    d_z [C][2S][n_t] complex64 -> d_vis [C][n_bl][2][2] complex64, both device memory of the caller;
+    channels * n_bl <= COBALT_NOALLOC_MAX_CHANNEL_BASELINES.  Calls that overlap on the GPU race on that array."""
+    err = ctypes.create_string_buffer(512)
+    status = load().cobalt_correlate_noalloc(_stream_ptr(stream), _ptr(d_z), int(stations), int(channels), int(n_spectra),
+                                             _ptr(d_vis), err, len(err))
+    if status != COBALT_OK:
+        raise CobaltError(status, err.value.decode())
 
 
 def cobalt_destroy(plan):

@@ -9,7 +9,7 @@ PKG_DIR = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(PKG_DIR)
 CSRC = os.path.join(PKG_DIR, "csrc")
 LIB = os.path.join(PKG_DIR, "libcobalt_b200.so")
-SOURCES = ["plan.cu", "fstage.cu", "layout.cu", "ingest.cu", "xstage_simt.cu", "xstage_tc.cu", "beamform.cu"]
+SOURCES = ["plan.cu", "fstage.cu", "layout.cu", "ingest.cu", "xstage_simt.cu", "xstage_tc.cu", "beamform.cu", "noalloc.cu"]
 HEADERS = [os.path.join(CSRC, "cobalt_internal.h"), os.path.join(CSRC, "ptx.cuh"), os.path.join(ROOT, "include", "cobalt.h")]
 
 
