@@ -1,7 +1,7 @@
 /*
  * cobalt.h -- C ABI of the B200-native Cobalt correlator hot path.
  *
- * One thing is built: the correlator pipeline of "Cobalt: A GPU-based correlator and
+ * The main thing built is the correlator pipeline of "Cobalt: A GPU-based correlator and
  * beamformer for LOFAR" (arXiv:1801.04834), sec 7.5 ("P:L360"):
  *
  *   "The correlator pipeline first channelizes subbands in a polyphase filter using FIR
@@ -12,8 +12,12 @@
  *
  * plus the fixed->floating conversion of P:L89 (sec 3.2) and the precision rule of P:L368
  * (phase angles in double precision, everything else single precision).  The paper prints
- * no formulas; the exact arithmetic is the reading listed in DESIGN.md ("Readings A1..A20",
- * taken from SURVEY.md sec 8(c)), summarised at cobalt_process() below.
+ * no formulas; the exact arithmetic is the reading listed in DESIGN.md ("Readings A1..A32",
+ * taken from SURVEY.md sec 8(c)), summarised at cobalt_process() below.  On top of it sit the
+ * rows of SURVEY.md sec 8(f): time-varying delays, phase offsets, dumps, lost-data flags, coarse
+ * delays, pol-minor and 4-bit input (cobalt_process_ex and the setters), the beamformer of
+ * P:L362-366 at the plan's channel count (cobalt_beamform), and one plan-less entry point for
+ * callers that must not allocate (cobalt_correlate_noalloc).
  *
  * Conventions
  *   - Every function returns a cobalt_status (0 = OK, negative = error) and never throws,
@@ -25,6 +29,10 @@
  *   - cobalt_process() only ENQUEUES work on `cuda_stream` and returns; buffers must stay
  *     alive and unmodified until the stream reaches the end of the call.
  *   - All sizes are validated; nothing is read or written outside the documented extents.
+ *   - One plan = one stream = one host thread at a time: cobalt_process*, cobalt_beamform and the
+ *     setters update plan state (launch counters, event lists, which history buffer is current)
+ *     without locking, and the plan's scratch is shared by every call on it.  Use one plan per
+ *     concurrent stream; different plans are independent.
  *   - There is no CPU fallback: without a CUDA device of compute capability 10.x every
  *     entry point that needs the device returns COBALT_ERR_UNSUPPORTED_DEVICE / COBALT_ERR_CUDA.
  *
@@ -97,8 +105,10 @@ int cobalt_plan(cobalt_plan_t **out, int stations, int subbands, int channels, i
  * cobalt_process: one integration period of the whole hot path, enqueued on `cuda_stream`
  * (a cudaStream_t passed as void*; NULL = the legacy default stream).
  *
- *   d_samples      device, [B][S][2 pol][N][2 (re,im)] int16 (input_bits 16) or int8 (8),
- *                  time contiguous per polarisation (reading A13); read only.
+ *   d_samples      device, [B][S][2 pol][N][2 (re,im)] int16 (input_bits 16) or int8 (8), or
+ *                  [B][S][2 pol][N] bytes holding one 4-bit complex sample each (input_bits 4, A27),
+ *                  time contiguous per polarisation (reading A13; cobalt_set_input_layout selects
+ *                  LOFAR's pol-minor wire order instead); read only.
  *   d_delays       device, [S] double, seconds; one value per station, both pols (A7).
  *   d_bandpass     device, [C] float, real weight multiplying the voltages (A8).
  *   d_visibilities device, [B][C][n_bl][2][2] complex64 (float re, float im); fully
@@ -176,7 +186,11 @@ int cobalt_process_ex(cobalt_plan_t *plan, void *cuda_stream, const cobalt_io_t 
  * plan's channel count ("Cobalt performs delay compensation, bandpass correction and beamforming at 256 channels per
  * subband"); enqueued on `cuda_stream` like cobalt_process, with the same channelisation (steps a1-a4), delay
  * compensation, bandpass, phase offsets, coarse delays, input layouts and valid-sample flags, and the same history
- * carry (stateful; a plan serves either the correlator or the beamformer stream of an observation).
+ * carry (stateful; a plan serves either the correlator or the beamformer stream of an observation).  Sharing the
+ * correlator's 16-tap channeliser is a reading (A28): in the paper the beamformer "cannot share initial steps
+ * with the correlator" and runs a 256-channel PPF of its own; what this call adds is the beam-forming step.
+ * Not built (A32): the transform to the requested output resolution with its transposes, and beam
+ * delays that vary over the block (beam_delays is one value per (beam, station) and call).
  * With z[a][p][t][j] the delay-compensated, bandpass-corrected channelised sample of station a, polarisation p
  * (cobalt_process, line "z[t][j] = ..."):
  *   coherent beam b (reading A28; "adjusts the beam direction with a phase shift and sums over antenna fields",
@@ -234,7 +248,8 @@ int cobalt_set_subband_frequencies(cobalt_plan_t *plan, const double *h_hz);
 int cobalt_set_sample_rate(cobalt_plan_t *plan, double hz);
 /* Reading A22 ("bandpass and clock corrections"): a constant phase per (station, polarisation) with the
  * sign sense of the delay term, z <- z exp(-i phase0[a][p]).  h_phase0: host [S][2] doubles, radians, or NULL = none.
- * Folded (in fp32) into the rotation table of the F-stage.  Takes effect next call. */
+ * Applied in fp32 together with the delay rotation: to the visibilities in the X-stage epilogue (V_ik *= w_i conj(w_k)) and
+ * to the beam weights of cobalt_beamform.  Takes effect next call. */
 int cobalt_set_phase_offsets(cobalt_plan_t *plan, const double *h_phase0);
 /* Reading A25 ("coarse delay compensation ... by shifting"): station a's block of N samples starts at sample
  * h_offsets[a] of its input stream, which is samples_allocated >= N + max offset samples long (the stream stride of
@@ -252,7 +267,8 @@ int cobalt_set_dumps(cobalt_plan_t *plan, int dumps_per_block);
 #define COBALT_LAYOUT_PLANAR 0
 #define COBALT_LAYOUT_POL_MINOR 1
 int cobalt_set_input_layout(cobalt_plan_t *plan, int layout);
-/* Switch COBALT_MODE_*; reallocates the intermediate scratch, keeps the history. */
+/* Switch COBALT_MODE_*; reallocates the intermediate scratch, keeps the history and a launch-group size set with
+ * cobalt_set_chunk_subbands (otherwise the default group size of the new mode applies). */
 int cobalt_set_mode(cobalt_plan_t *plan, int mode);
 /* Subbands per internal launch group (>= 1, clipped to B).  Reallocates scratch.  Default: as many as fit in 8 GiB of
  * intermediate (at most a quarter of the free device memory), split evenly over the call; cobalt_process_host moves

@@ -408,7 +408,8 @@ def incoherent_stokes(z: np.ndarray, n_stokes: int, t_int: int) -> np.ndarray:
 def channelise_subband(samples: np.ndarray, C: int, delays, bandpass, f_sb: float, hist: np.ndarray | None = None,
                        f_s: float = F_S, T: int = TAPS, delays_end=None, phase0=None, valid=None) -> np.ndarray:
     """Steps 1-7 (+ A22 offsets, A24 flags) of one subband: integer samples [S][2][N][2] -> z complex [S][2][n_t][C]:
-    the input of the beamformer functions above ("the first four kernels in common")."""
+    the input of the beamformer functions above (reading A28: the beamformer of this build is fed by the correlator's
+    channeliser; the paper's has one of its own)."""
     s = np.ascontiguousarray(samples)
     x = _r2c(unpack4(s)) if s.dtype == np.uint8 else _r2c(unpack(s))
     z = fstage(x, C, hist=hist, delays=delays, bandpass=bandpass, f_sb=f_sb, f_s=f_s, T=T, delays_end=delays_end)

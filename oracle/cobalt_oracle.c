@@ -244,6 +244,7 @@ int oracle_fstage_interp_f64(int S, int C, int T, long long N, const double *x /
         double *xh = (double *)malloc(sizeof(double) * 2 * (size_t)(nh + nu));
         double *y = (double *)malloc(sizeof(double) * 2 * (size_t)(nu > 0 ? nu : 1));
         if (!xh || !y) {
+#pragma omp atomic write
             fail = 1;
             free(xh);
             free(y);
@@ -403,7 +404,8 @@ int oracle_correlate_dumps(int S, int C, long long n_t, int D, int tile, const d
  * the beamformer pipeline, at the channel resolution of the
  * plan ("Cobalt performs delay compensation, bandpass correction and beamforming at 256 channels per subband").
  * Input of every function below is z, the delay-compensated, bandpass-corrected channelised data of steps 1-7
- * ("Both beam types have the first four kernels in common").  Readings A28-A31 of DESIGN.md.  The final
+ * (a reading, A28: the paper's beamformer "cannot share initial steps with the correlator", and
+ * channelises on its own).  Readings A28-A31 of DESIGN.md.  The final
  * transformation "to the requested output resolution" (inverse FFT / second FFT) is not part of this row.
  * ===================================================================================================== */
 

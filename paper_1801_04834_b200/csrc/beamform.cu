@@ -1,8 +1,11 @@
 // Beamformer pipeline of SURVEY.md sec 8(f) row 4 (readings A28-A32 of DESIGN.md), at the channel
 // resolution of the plan: "Coherent beamforming first adjusts the beam direction with a phase shift and sums over antenna
 // fields, then optionally computes Stokes parameters, while incoherent beamforming first computes Stokes parameters and
-// then sums over antenna fields."  Input is the channelised intermediate z of the F-stage (steps a1-a4, a7: "Both beam
-// types have the first four kernels in common"); delay compensation, bandpass and the per-input phase offsets (a5, a6, A22)
+// then sums over antenna fields."  Input is the channelised intermediate z of the F-stage (steps a1-a4, a7).  Feeding the
+// beamformer from the correlator's 16-tap channeliser is a READING (A28), not the paper's design: P:L366 says the
+// beamformer "cannot share initial steps with the correlator" (it runs its own 256-channel PPF), and the sentence "Both beam
+// types have the first four kernels in common" is about coherent versus incoherent beams.  Delay compensation,
+// bandpass and the per-input phase offsets (a5, a6, A22)
 // are constants per (input, channel) within a call and are folded into the beam weights.
 //
 // bf_tc_kernel (TENSOR_FP16 mode): the coherent sum
@@ -34,7 +37,6 @@ namespace {
 constexpr int kBfFirstEpiWarp = 4, kBfEpiWarps = 16, kBfEpiSub = kBfEpiWarps / 4;
 constexpr int kBfThreads = 32 * (kBfFirstEpiWarp + kBfEpiWarps);
 constexpr int kBfEpiThreads = 32 * kBfEpiWarps;
-constexpr int kBfTBlock = 2 * kKTile;          // spectra per accumulator block (M of the instruction)
 constexpr int kBfAccStride = 256;              // TMEM columns between the two accumulator sets
 
 struct BfArgs {
@@ -60,7 +62,9 @@ __device__ __forceinline__ float2 cmulf(float2 a, float2 b) { return make_float2
 
 // W[b][a][p] of one (subband, channel): the beam phase in fp64 up to the final rounding, times the station's
 // delay-compensation factor from the fp64 phase table, times the phase offset of the input (A22).
-__device__ __forceinline__ void beam_weight(const BfArgs &a, double f, int sb, int c, int beam, int st, float2 &wx, float2 &wy) {
+// (Args = BfArgs or BfSimtArgs: one routine for the tensor and the fp32 kernel)
+template <class Args>
+__device__ __forceinline__ void beam_weight(const Args &a, double f, int sb, int c, int beam, int st, float2 &wx, float2 &wy) {
     const double cyc = f * a.beam_delays[(size_t)beam * a.S + st];
     const double frac = cyc - floor(cyc);
     float sn, cs;
@@ -218,6 +222,12 @@ __global__ void __launch_bounds__(kBfThreads, 1) bf_tc_kernel(const BfArgs a) {
         mbar_fence_init();
     }
     if (warp == 1) {
+        // All 512 columns (two accumulator sets of up to 256).  Residency assumption: one CTA of this kernel per SM owns the
+        // SM's whole TMEM.  __launch_bounds__(.., 1) does not enforce that -- with a small Mpad the shared memory would let a
+        // second CTA in, and a second plan's bf_tc_kernel / xstage_tc_kernel on another stream can land on the same SM.  Such
+        // a CTA blocks in tcgen05.alloc until this one exits (it never deadlocks: every CTA frees its columns before it
+        // returns and needs no other CTA to make progress), i.e. a correlator plan and a beamformer plan running on two
+        // streams take turns on an SM instead of sharing it.
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tmem_slot), "r"(512) : "memory");
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
     }
@@ -383,16 +393,6 @@ struct BfSimtArgs {
     int S, M, C, b0, n_beams, bpb, product, n_stokes, t_int;
 };
 
-__device__ __forceinline__ void beam_weight_simt(const BfSimtArgs &a, double f, int sb, int c, int beam, int st, float2 &wx, float2 &wy) {
-    const double cyc = f * a.beam_delays[(size_t)beam * a.S + st];
-    const double frac = cyc - floor(cyc);
-    float sn, cs;
-    sincospif(-2.0f * (float)frac, &sn, &cs);
-    const float2 w = cmulf(make_float2(cs, sn), a.phase[((size_t)sb * a.S + st) * a.C + c]);
-    wx = a.poff ? cmulf(w, a.poff[2 * st]) : w;
-    wy = a.poff ? cmulf(w, a.poff[2 * st + 1]) : w;
-}
-
 __global__ void __launch_bounds__(kBfTBlock) bf_simt_kernel(const BfSimtArgs a) {
     extern __shared__ float2 sw[];                         // [bpb][M] weights, then [4][128] floats for the integration
     float *red = reinterpret_cast<float *>(sw + (size_t)a.bpb * a.M);
@@ -403,7 +403,7 @@ __global__ void __launch_bounds__(kBfTBlock) bf_simt_kernel(const BfSimtArgs a) 
     for (int item = threadIdx.x; item < a.bpb * a.S; item += kBfTBlock) {
         const int st = item % a.S, b_loc = item / a.S, beam = bb * a.bpb + b_loc;
         float2 wx = make_float2(0.f, 0.f), wy = wx;
-        if (beam < a.n_beams) beam_weight_simt(a, f, sb, c, beam, st, wx, wy);
+        if (beam < a.n_beams) beam_weight(a, f, sb, c, beam, st, wx, wy);
         sw[(size_t)b_loc * a.M + 2 * st] = wx;
         sw[(size_t)b_loc * a.M + 2 * st + 1] = wy;
     }

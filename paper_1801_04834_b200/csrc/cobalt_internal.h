@@ -18,6 +18,8 @@ constexpr int kTaps = 16;          // P:L360 FIR filter; BASELINE.json: 16-tap
 constexpr int kSubTile = 16;       // spectra per FIR->FFT hand-over
 constexpr int kKTile = 64;         // spectra per X-stage K tile (= one 128-byte fp16 row)
 constexpr int kMaxMmaGroups = 2;   // MMA groups per X-stage job
+constexpr int kBfTBlock = 2 * kKTile;   // beamformer: spectra per accumulator block (M of the instruction) and per CTA of its SIMT kernels
+constexpr int kMaxGridYZ = 65535;  // CUDA's limit on gridDim.y / gridDim.z
 constexpr int kStoreTile = 32;     // spectra per F-stage tensor store (half a k-tile row)
 // streams (rows m) per F-stage tensor-store box: the CTA's 256 / C streams, at most 4 (all with the same m >> 2)
 constexpr int kStoreBoxStreams(int C) { return 256 / C < 4 ? 256 / C : 4; }
@@ -82,6 +84,7 @@ struct cobalt_plan_s {
     long long N = 0, n_t = 0, N_u = 0, n_bl = 0;
     int M = 0, Mpad = 0, n_kt = 0;
     int chunk = 1;
+    int chunk_user = 0;                // what cobalt_set_chunk_subbands asked for (0 = never called: the default rule); kept by cobalt_set_mode
     int host_chunk = 1;                // subbands per group of cobalt_process_host (<= chunk)
     int device = 0, sm_count = 0;
     double f_s = 195312.5;

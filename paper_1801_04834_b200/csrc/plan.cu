@@ -172,23 +172,26 @@ int alloc_scratch(cobalt_plan_s *p, int chunk_request) {
     return COBALT_OK;
 }
 
-// One chunk of subbands [b0, b0 + nb): samples_b0 / vis_b0 point at subband b0 (of dump 0); io holds the per-call pointers.
-int enqueue_chunk(cobalt_plan_s *p, cudaStream_t st, const void *samples_b0, const cobalt_io_t &io, float2 *vis_b0, int b0, int nb,
-                  StageEvents *ev) {
+// Steps a1-a7 + a10 of one chunk of subbands [b0, b0 + nb), shared by the correlator and the beamformer: the fp64 phase table
+// of the whole call (with the first chunk; `table_bandpass` = nullptr builds pure station phases, which is what the beamformer
+// wants -- afterwards p->d_phase belongs to the caller of this function until its chunk loop ends), the ingest pre-pass where
+// the input needs one, the fused F-stage kernel into p->d_z, and the history carry.  Records ev->e[0..3]; adds the launches
+// beyond the usual three (phase table, F-stage, history) to *extra.
+int enqueue_fstage(cobalt_plan_s *p, cudaStream_t st, const void *samples_b0, const double *delays, const float *table_bandpass,
+                   const double *delays_end, const unsigned char *valid, int b0, int nb, StageEvents *ev, int *extra) {
     if (ev) CK(p, cudaEventRecord(ev->e[0], st));
-    if (b0 == 0) CK(p, launch_phase_table(p, st, io.delays, io.bandpass, 0, p->B, io.delays_end));   // every subband's table in one launch
+    if (b0 == 0) CK(p, launch_phase_table(p, st, delays, table_bandpass, 0, p->B, delays_end));   // every subband's table in one launch
     if (ev) CK(p, cudaEventRecord(ev->e[1], st));
     FCall call;
-    call.delays_end = io.delays_end;
-    call.valid = io.valid;
+    call.delays_end = delays_end;
+    call.valid = valid;
     const void *fsamples = samples_b0;
-    int extra = 0;
     if (needs_ingest(p)) {     // pol-minor order / 4-bit samples: re-ordered, widened, coarse offsets applied
         CK(p, launch_ingest(p, st, samples_b0, nb, p->d_ingest));
         fsamples = p->d_ingest;
         call.coarse = nullptr;
         call.n_in = p->N;
-        extra = 1;
+        *extra += 1;
     } else {
         call.coarse = p->d_coarse;
         call.n_in = p->N_in;
@@ -197,6 +200,17 @@ int enqueue_chunk(cobalt_plan_s *p, cudaStream_t st, const void *samples_b0, con
     if (ev) CK(p, cudaEventRecord(ev->e[2], st));
     CK(p, launch_history_update(p, st, fsamples, b0, nb, call));
     if (ev) CK(p, cudaEventRecord(ev->e[3], st));
+    return COBALT_OK;
+}
+
+// One chunk of subbands [b0, b0 + nb): samples_b0 / vis_b0 point at subband b0 (of dump 0); io holds the per-call pointers.
+int enqueue_chunk(cobalt_plan_s *p, cudaStream_t st, const void *samples_b0, const cobalt_io_t &io, float2 *vis_b0, int b0, int nb,
+                  StageEvents *ev) {
+    int extra = 0;
+    {
+        const int rc = enqueue_fstage(p, st, samples_b0, io.delays, io.bandpass, io.delays_end, io.valid, b0, nb, ev, &extra);
+        if (rc != COBALT_OK) return rc;
+    }
     const size_t dump_stride = (size_t)p->B * p->C * p->n_bl * 4;      // float2 between dumps
     XCall xc;
     xc.phase = p->d_phase;
@@ -360,6 +374,11 @@ int cobalt_process_ex(cobalt_plan_t *p, void *cuda_stream, const cobalt_io_t *io
         return fail(p, COBALT_ERR_BAD_ARG, "d_samples must be aligned to one complex sample");
     if (p->mode == COBALT_MODE_TENSOR_FP16 && (reinterpret_cast<uintptr_t>(io->visibilities) & 15u) != 0)
         return fail(p, COBALT_ERR_BAD_ARG, "d_visibilities must be 16-byte aligned in COBALT_MODE_TENSOR_FP16");
+    // the fp32 correlator puts (subband of the group, dump) in gridDim.z: refuse before anything is enqueued (a launch failure
+    // in a later group would leave the in-place FIR history of the earlier groups advanced)
+    if (p->mode == COBALT_MODE_EXACT_FP32 && (long long)p->chunk * p->dumps > kMaxGridYZ)
+        return fail(p, COBALT_ERR_BAD_ARG, "COBALT_MODE_EXACT_FP32: chunk_subbands * dumps = " + std::to_string((long long)p->chunk * p->dumps) +
+                                               " exceeds 65535; lower cobalt_set_chunk_subbands or cobalt_set_dumps");
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     const int n_chunks = (p->B + p->chunk - 1) / p->chunk;
     if (p->timing) {
@@ -427,6 +446,10 @@ int cobalt_beamform(cobalt_plan_t *p, void *cuda_stream, const cobalt_bf_io_t *i
     if ((reinterpret_cast<uintptr_t>(io->samples) & (caller_sample_bytes(p) - 1)) != 0)
         return fail(p, COBALT_ERR_BAD_ARG, "d_samples must be aligned to one complex sample");
     const bool tensor = p->mode == COBALT_MODE_TENSOR_FP16;
+    // the SIMT beamformer kernels (incoherent Stokes in both modes, everything in EXACT mode) put ceil(n_t / 128) in gridDim.y
+    if ((!tensor || io->product == COBALT_BF_INCOHERENT_STOKES) && (p->n_t + kBfTBlock - 1) / kBfTBlock > kMaxGridYZ)
+        return fail(p, COBALT_ERR_BAD_ARG, "n_t = " + std::to_string(p->n_t) + " spectra per block exceed the " + std::to_string((long long)kMaxGridYZ * kBfTBlock) +
+                                               " this beamformer product handles in this mode; use shorter blocks");
     if (tensor && io->product != COBALT_BF_INCOHERENT_STOKES) {
         int bpb, stages;
         size_t wb, sb, sm;
@@ -449,28 +472,12 @@ int cobalt_beamform(cobalt_plan_t *p, void *cuda_stream, const cobalt_bf_io_t *i
         const int nb = (p->B - b0) < p->chunk ? (p->B - b0) : p->chunk;
         const unsigned char *sm = static_cast<const unsigned char *>(io->samples) + (size_t)b0 * subband_input_bytes(p);
         StageEvents *ev = p->timing ? &p->events[ci] : nullptr;
-        if (ev) CK(p, cudaEventRecord(ev->e[0], st));
-        // pure station phases (no bandpass: the beamformer scales its outputs by b[j] in fp32), every subband in one launch
-        if (b0 == 0) CK(p, launch_phase_table(p, st, io->delays, nullptr, 0, p->B, io->delays_end));
-        if (ev) CK(p, cudaEventRecord(ev->e[1], st));
-        FCall call;
-        call.delays_end = io->delays_end;
-        call.valid = io->valid;
-        const void *fsamples = sm;
+        // pure station phases (no bandpass: the beamformer scales its outputs by b[j] in fp32)
         int extra = 0;
-        if (needs_ingest(p)) {
-            CK(p, launch_ingest(p, st, sm, nb, p->d_ingest));
-            fsamples = p->d_ingest;
-            call.n_in = p->N;
-            extra = 1;
-        } else {
-            call.coarse = p->d_coarse;
-            call.n_in = p->N_in;
+        {
+            const int rc = enqueue_fstage(p, st, sm, io->delays, nullptr, io->delays_end, io->valid, b0, nb, ev, &extra);
+            if (rc != COBALT_OK) return rc;
         }
-        CK(p, launch_fstage(p, st, fsamples, b0, nb, call));
-        if (ev) CK(p, cudaEventRecord(ev->e[2], st));
-        CK(p, launch_history_update(p, st, fsamples, b0, nb, call));
-        if (ev) CK(p, cudaEventRecord(ev->e[3], st));
         BfCall bc;
         bc.beam_delays = io->beam_delays;
         bc.bandpass = io->bandpass;
@@ -644,12 +651,13 @@ int cobalt_set_mode(cobalt_plan_t *p, int mode) {
     if (mode == p->mode) return COBALT_OK;
     CK(p, cudaDeviceSynchronize());
     p->mode = mode;
-    return alloc_scratch(p, 0);
+    return alloc_scratch(p, p->chunk_user);   // a group size the caller chose survives the switch; otherwise the default rule of the new mode
 }
 
 int cobalt_set_chunk_subbands(cobalt_plan_t *p, int chunk) {
     if (!p || chunk < 1) return fail(p, COBALT_ERR_BAD_ARG, "chunk must be >= 1");
     CK(p, cudaDeviceSynchronize());
+    p->chunk_user = chunk;
     return alloc_scratch(p, chunk);
 }
 

@@ -126,7 +126,8 @@ def test_incoherent_stokes_match_oracle(cobalt, oracle, dev, C, bits, S, n_t, n_
 @pytest.mark.parametrize("tensor", [False, True])
 def test_every_input_option_and_two_calls(cobalt, oracle, dev, tensor):
     """Phase offsets, lost tiles, one subband per launch group, and a second call that continues from the first call's FIR
-    history: the beamformer shares steps a1-a7 with the correlator ("the first four kernels in common")."""
+    history: in this build the beamformer is fed by the correlator's steps a1-a7 (reading A28; the paper's beamformer has a
+    channeliser of its own)."""
     rng = np.random.default_rng(3100)
     B, S, C, n_t, bits, n_beams = 3, 6, 64, 192, 16, 7
     N = n_t * C
@@ -204,12 +205,12 @@ def test_beamform_rejects_bad_settings(cobalt, dev):
 
 
 def test_beamformer_workload_shape_sampled(cobalt, oracle, dev):
-    """The shape bench.py --beamform times (48 stations, 256 channels, 195312 samples, 127 beams, Stokes I at t_int = 16; two
-    subbands here, one launch group), checked on sampled (subband, channel) pairs that the oracle computes one by one through its
+    """The shape bench.py --beamform times (48 stations, 256 channels, 195312 samples, 127 beams, Stokes I at t_int = 16; three
+    subbands here, one launch group), checked on 32 sampled (subband, channel) pairs that the oracle computes one by one through its
     single-sum channeliser (oracle.channel_direct) and its beamformer functions applied to that one channel."""
     from paper_1801_04834_b200 import synth
 
-    cfg = synth.scaled(synth.CONFIGS[6], B=2)
+    cfg = synth.scaled(synth.CONFIGS[6], B=3)
     n_beams, t_int = 127, 16
     data = synth.generate(cfg, device=dev)
     bd = synth.beam_delays(cfg, n_beams, dev)
@@ -222,7 +223,8 @@ def test_beamformer_workload_shape_sampled(cobalt, oracle, dev):
         got, gv = got.cpu().numpy(), gv.cpu().numpy()
     delays, bp, bdh = data["delays"].cpu().numpy(), data["bandpass"].cpu().numpy().astype(np.float64), bd.cpu().numpy()
     rng = np.random.default_rng(3300)
-    pairs = [(0, 0), (1, cfg.C - 1), (0, cfg.C // 2)] + [(int(rng.integers(cfg.B)), int(rng.integers(cfg.C))) for _ in range(5)]
+    pairs = [(0, 0), (2, cfg.C - 1), (1, cfg.C // 2)] + [(int(rng.integers(cfg.B)), int(rng.integers(cfg.C))) for _ in range(29)]
+    pairs.sort()                                                    # one subband of host memory at a time
     for sb, j in pairs:
         x = data["samples"][sb].cpu().numpy()
         f_sb = oracle.default_subband_frequency(sb)

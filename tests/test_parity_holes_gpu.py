@@ -253,3 +253,41 @@ def test_exact_mode_at_config4_and_config5_shapes(cobalt, oracle, dev, index):
         _, vo = oracle.channel_direct(x, cfg.C, j, delays=delays, bandpass=bp, f_sb=oracle.default_subband_frequency(0))
         e = err_fp32(vis[0, j].cpu().numpy(), vo)
         assert e <= TOL_FP32, f"{cfg.name} channel {j}: error {e:.3e} > {TOL_FP32}"
+
+
+# ------------------------------------------------------------------ plan state and launch limits (round-2 advice)
+def test_set_mode_keeps_a_chunk_size_the_caller_chose(cobalt, dev):
+    with cobalt.Correlator(3, 6, 16, 16 * 64, 16) as cor:
+        default_chunk = cor.info.chunk_subbands
+        cor.set_mode(cobalt.COBALT_MODE_EXACT_FP32)
+        assert cor.info.chunk_subbands == default_chunk                 # never set: the default rule again
+        cor.set_chunk_subbands(2)
+        cor.set_mode(cobalt.COBALT_MODE_TENSOR_FP16)
+        assert cor.info.chunk_subbands == 2
+        cor.set_dumps(1)
+        cor.set_mode(cobalt.COBALT_MODE_EXACT_FP32)
+        assert cor.info.chunk_subbands == 2
+
+
+def test_oversized_grids_are_refused_before_anything_is_enqueued(cobalt, dev):
+    """Settings whose kernels would need gridDim.y / .z > 65535 used to fail at launch, after earlier launch groups had
+    already advanced the in-place FIR history; now they are COBALT_ERR_BAD_ARG up front."""
+    dummy = torch.zeros(1 << 20, dtype=torch.uint8, device=dev)          # never read: the call is refused first
+    with cobalt.Correlator(1, 1024, 16, 16 * 64 * 64, 16, mode=cobalt.COBALT_MODE_EXACT_FP32) as cor:
+        cor.set_chunk_subbands(1024)
+        cor.set_dumps(64)                                                # 1024 * 64 = 65536 (subband, dump) pairs in gridDim.z
+        with pytest.raises(cobalt.CobaltError) as e:
+            cobalt.cobalt_process_ex(cor._h, None, dummy, dummy, dummy, dummy)
+        assert e.value.status == cobalt.COBALT_ERR_BAD_ARG and "65535" in str(e.value)
+        cor.set_chunk_subbands(512)                                      # two groups of 512: fine
+        x = torch.zeros(cor.samples_shape(), dtype=torch.int16, device=dev)
+        x[..., 0] = 3
+        vis = cor.process(x, torch.zeros(1, dtype=torch.float64, device=dev), torch.ones(16, dtype=torch.float32, device=dev))
+        torch.cuda.synchronize()
+        assert vis.shape == (64, 1024, 16, 1, 2, 2) and bool(torch.isfinite(torch.view_as_real(vis)).all())
+        assert float(vis[:, :, 8, 0, 0, 0].real.min()) > 0               # DC input: power in the centre channel of every dump
+    n_t = 65535 * 128 + 1
+    with cobalt.Correlator(1, 1, 16, 16 * n_t, 8, mode=cobalt.COBALT_MODE_EXACT_FP32) as cor:
+        with pytest.raises(cobalt.CobaltError) as e:
+            cobalt.cobalt_beamform(cor._h, None, dummy, dummy, dummy, dummy, 1, cobalt.COBALT_BF_INCOHERENT_STOKES, 1, 1, dummy)
+        assert e.value.status == cobalt.COBALT_ERR_BAD_ARG and "spectra" in str(e.value)
