@@ -42,6 +42,48 @@ __global__ void ingest_kernel(const unsigned char *__restrict__ in, unsigned cha
     }
 }
 
+// The common case of ingest_kernel -- pol-minor int16 / int8 with N a multiple of G -- with 16-byte accesses: a thread takes G =
+// 4 (int16) or 8 (int8) consecutive time samples of one (subband, station), i.e. 32 contiguous bytes of (pol 0, pol 1) pairs, and
+// writes 16 bytes to each polarisation's planar stream.  (The element-wise kernel reads every other 4-byte word per warp and
+// reached 3.6 TB/s of the 6.5 TB/s a copy gets.)  A source that is not 16-byte aligned (odd coarse offset, odd N_in, a caller's
+// base pointer aligned to a sample only) is read sample by sample; the destination (plan-owned) is always aligned.
+template <int BITS>
+__global__ void ingest_polminor_vec_kernel(const unsigned char *__restrict__ in, unsigned char *__restrict__ out, const int *__restrict__ coarse,
+                                           int S, long long N, long long N_in, long long total_groups) {
+    constexpr int SB = BITS == 16 ? 4 : 2;         // bytes per complex sample
+    constexpr int G = 16 / SB;                     // time samples per thread
+    const long long gpr = N / G;                   // groups per (subband, station)
+    for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < total_groups; idx += (long long)gridDim.x * blockDim.x) {
+        const long long g = idx % gpr, bs = idx / gpr;
+        const long long n0 = g * G + (coarse ? coarse[bs % S] : 0);
+        const unsigned char *src = in + ((bs * N_in + n0) * 2) * SB;
+        uint32_t w[8];                             // 32 bytes: int16 (p0 t0)(p1 t0)(p0 t1)...; int8 (p0 t0 | p1 t0)(p0 t1 | p1 t1)...
+        if ((reinterpret_cast<uintptr_t>(src) & 15u) == 0) {
+            const uint4 a = reinterpret_cast<const uint4 *>(src)[0], b = reinterpret_cast<const uint4 *>(src)[1];
+            w[0] = a.x; w[1] = a.y; w[2] = a.z; w[3] = a.w;
+            w[4] = b.x; w[5] = b.y; w[6] = b.z; w[7] = b.w;
+        } else if (SB == 4) {
+#pragma unroll
+            for (int k = 0; k < 8; ++k) w[k] = reinterpret_cast<const uint32_t *>(src)[k];
+        } else {
+#pragma unroll
+            for (int k = 0; k < 8; ++k)
+                w[k] = (uint32_t) reinterpret_cast<const unsigned short *>(src)[2 * k] | ((uint32_t) reinterpret_cast<const unsigned short *>(src)[2 * k + 1] << 16);
+        }
+        uint4 o0, o1;
+        if (SB == 4) {
+            o0 = make_uint4(w[0], w[2], w[4], w[6]);
+            o1 = make_uint4(w[1], w[3], w[5], w[7]);
+        } else {                                   // low halves = pol 0, high halves = pol 1
+            o0 = make_uint4(__byte_perm(w[0], w[1], 0x5410), __byte_perm(w[2], w[3], 0x5410), __byte_perm(w[4], w[5], 0x5410), __byte_perm(w[6], w[7], 0x5410));
+            o1 = make_uint4(__byte_perm(w[0], w[1], 0x7632), __byte_perm(w[2], w[3], 0x7632), __byte_perm(w[4], w[5], 0x7632), __byte_perm(w[6], w[7], 0x7632));
+        }
+        unsigned char *dst = out + ((bs * 2) * N + g * G) * SB;
+        *reinterpret_cast<uint4 *>(dst) = o0;
+        *reinterpret_cast<uint4 *>(dst + N * SB) = o1;
+    }
+}
+
 // counts[b][d][bl(i,k)] = sum over the 64-spectrum tiles v of dump d of valid[b][i][v] * valid[b][k][v] * (spectra in tile v)
 __global__ void valid_counts_kernel(const unsigned char *__restrict__ valid, unsigned int *__restrict__ counts, int b0, int nb, int S,
                                     int n_kt, int D, long long n_t, long long n_bl) {
@@ -95,6 +137,13 @@ cudaError_t launch_ingest(const cobalt_plan_s *p, cudaStream_t st, const void *s
     unsigned char *out = static_cast<unsigned char *>(d_out);
     const unsigned g = grid_for(total, 256);
     const bool pm = p->layout == COBALT_LAYOUT_POL_MINOR;
+    if (pm && p->bits_in != 4 && p->N % (p->bits_in == 16 ? 4 : 8) == 0) {      // 16-byte accesses (see the kernel)
+        const long long groups = (long long)nb * p->S * (p->N / (p->bits_in == 16 ? 4 : 8));
+        const unsigned gv = grid_for(groups, 256);
+        if (p->bits_in == 16) ingest_polminor_vec_kernel<16><<<gv, 256, 0, st>>>(in, out, p->d_coarse, p->S, p->N, p->N_in, groups);
+        else ingest_polminor_vec_kernel<8><<<gv, 256, 0, st>>>(in, out, p->d_coarse, p->S, p->N, p->N_in, groups);
+        return cudaGetLastError();
+    }
 #define COBALT_INGEST(B, PM) ingest_kernel<B, PM><<<g, 256, 0, st>>>(in, out, p->d_coarse, p->S, p->N, p->N_in, total)
     if (p->bits_in == 16) { if (pm) COBALT_INGEST(16, true); else COBALT_INGEST(16, false); }
     else if (p->bits_in == 8) { if (pm) COBALT_INGEST(8, true); else COBALT_INGEST(8, false); }

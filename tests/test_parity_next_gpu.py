@@ -141,10 +141,11 @@ def test_coarse_delays_match_oracle_over_two_calls(cobalt, oracle, dev, C, bits,
 
 
 # ------------------------------------------------------------------ pol-minor order (A26) and 4-bit samples (A27)
+@pytest.mark.parametrize("tail", [9, 8, 4])      # N a multiple of 8 / of 4 only / odd: the 16-byte and the element-wise re-ordering
 @pytest.mark.parametrize("bits", [16, 8])
-def test_pol_minor_input_is_bit_identical_to_planar(cobalt, oracle, dev, bits):
+def test_pol_minor_input_is_bit_identical_to_planar(cobalt, oracle, dev, bits, tail):
     rng = np.random.default_rng(260 + bits)
-    B, S, C, N = 2, 3, 64, 64 * 70 + 9
+    B, S, C, N = 2, 3, 64, 64 * 70 + tail
     x = _data(rng, B, S, N, bits)                                     # planar [B][S][2][N][2]
     xm = np.ascontiguousarray(x.transpose(0, 1, 3, 2, 4))             # pol-minor [B][S][N][2][2]
     assert np.array_equal(oracle.pol_minor_to_planar(xm[0]), x[0])
