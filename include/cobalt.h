@@ -140,6 +140,16 @@ int cobalt_process(cobalt_plan_t *plan, void *cuda_stream, const void *d_samples
  * needed for the copies to overlap; pageable memory works but serialises. */
 int cobalt_process_host(cobalt_plan_t *plan, const void *h_samples, const double *h_delays,
                         const float *h_bandpass, void *h_visibilities);
+/* cobalt_process_host with the optional members of cobalt_io_t (declared below, at cobalt_process_ex): every pointer
+ * of `h_io` is a HOST pointer with the layout of its device counterpart -- samples, delays, bandpass, visibilities
+ * ([D][B][C][n_bl][2][2] with D = cobalt_set_dumps) required; delays_end [S], valid [B][S][n_tiles] and valid_counts
+ * [B][D][n_bl] optional (NULL = absent).  In the paper the lost-data flags arrive from the host side together with the
+ * samples and the blocks are streamed through pinned buffers: this is that path.  The small
+ * arrays are copied whole ahead of the first group, the samples and visibilities group by group, double buffered, on
+ * three internal streams; valid_counts comes back after the last group.  Synchronous like cobalt_process_host, same
+ * history carry; results are bit-identical to cobalt_process_ex on device copies of the same buffers. */
+struct cobalt_io_s;
+int cobalt_process_host_ex(cobalt_plan_t *plan, const struct cobalt_io_s *h_io);
 
 /* cobalt_process with a delay that varies over the block ("we compute the
  * channel-dependent phase angles [from the residual delay at the start and the end of the block] in double
@@ -170,7 +180,7 @@ int cobalt_process_interp(cobalt_plan_t *plan, void *cuda_stream, const void *d_
  *                  baseline are valid -- the weight that goes with the visibility (n_t per dump when valid == NULL);
  *   visibilities   [D][B][C][n_bl][2][2] complex64 with D = cobalt_set_dumps (default 1: the layout of cobalt_process).
  */
-typedef struct {
+typedef struct cobalt_io_s {
     const void *samples;
     const double *delays;
     const double *delays_end;

@@ -43,7 +43,7 @@ ABI_SYMBOLS = (
     "cobalt_set_timing", "cobalt_get_timing", "cobalt_get_kernel_timing",
     "cobalt_debug_fir_weights", "cobalt_debug_unpack", "cobalt_debug_channelised", "cobalt_debug_correlate",
     "cobalt_beamform", "cobalt_beamform_output_bytes",
-    "cobalt_correlate_noalloc",
+    "cobalt_correlate_noalloc", "cobalt_process_host_ex",
 )
 
 
@@ -102,6 +102,7 @@ def load(path: str | None = None):
     lib.cobalt_process_interp.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp, _vp]
     lib.cobalt_process_ex.argtypes = [_vp, _vp, ctypes.POINTER(cobalt_io_t)]
     lib.cobalt_process_host.argtypes = [_vp, _vp, _vp, _vp, _vp]
+    lib.cobalt_process_host_ex.argtypes = [_vp, ctypes.POINTER(cobalt_io_t)]
     lib.cobalt_set_phase_offsets.argtypes = [_vp, _vp]
     lib.cobalt_set_coarse_delays.argtypes = [_vp, _vp, ctypes.c_longlong]
     lib.cobalt_set_dumps.argtypes = [_vp, ctypes.c_int]
@@ -199,6 +200,12 @@ def cobalt_process_ex(plan, stream, d_samples, d_delays, d_bandpass, d_visibilit
 
 def cobalt_process_host(plan, h_samples, h_delays, h_bandpass, h_visibilities):
     _check(load().cobalt_process_host(plan, _ptr(h_samples), _ptr(h_delays), _ptr(h_bandpass), _ptr(h_visibilities)), plan)
+
+
+def cobalt_process_host_ex(plan, h_samples, h_delays, h_bandpass, h_visibilities, h_delays_end=None, h_valid=None, h_valid_counts=None):
+    io = cobalt_io_t(_ptr(h_samples), _ptr(h_delays), _ptr(h_delays_end), _ptr(h_bandpass), _ptr(h_valid), _ptr(h_visibilities),
+                     _ptr(h_valid_counts))
+    _check(load().cobalt_process_host_ex(plan, ctypes.byref(io)), plan)
 
 
 def cobalt_beamform(plan, stream, d_samples, d_delays, d_bandpass, d_beam_delays, n_beams, product, n_stokes, t_int, d_out,
@@ -411,14 +418,24 @@ class Correlator:
                         delays_end, valid)
         return out
 
-    def process_host(self, samples, delays, bandpass, out):
-        """Host buffers (numpy arrays or pinned CPU tensors), same layouts; synchronous."""
+    def process_host(self, samples, delays, bandpass, out, delays_end=None, valid=None, valid_counts=None):
+        """Host buffers (numpy arrays or pinned CPU tensors), same layouts; synchronous.  The optional arrays select
+        cobalt_process_host_ex (also used when the plan writes several dumps per block)."""
         i = self.info
-        for a, nbytes in ((samples, i.input_bytes), (delays, 8 * i.stations), (bandpass, 4 * i.channels),
-                          (out, i.output_bytes)):
+        sizes = [(samples, i.input_bytes), (delays, 8 * i.stations), (bandpass, 4 * i.channels), (out, i.output_bytes)]
+        if delays_end is not None:
+            sizes.append((delays_end, 8 * i.stations))
+        if valid is not None:
+            sizes.append((valid, i.subbands * i.stations * i.n_tiles))
+        if valid_counts is not None:
+            sizes.append((valid_counts, 4 * i.subbands * i.dumps * i.n_baselines))
+        for a, nbytes in sizes:
             n = a.numel() * a.element_size() if hasattr(a, "numel") else a.nbytes
             assert n == nbytes, (n, nbytes)
-        cobalt_process_host(self._h, samples, delays, bandpass, out)
+        if delays_end is None and valid is None and valid_counts is None:
+            cobalt_process_host(self._h, samples, delays, bandpass, out)
+        else:
+            cobalt_process_host_ex(self._h, samples, delays, bandpass, out, delays_end, valid, valid_counts)
         return out
 
     # -- debug taps

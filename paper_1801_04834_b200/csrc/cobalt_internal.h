@@ -117,6 +117,9 @@ struct cobalt_plan_s {
     void *d_in[2] = {nullptr, nullptr};
     void *d_out[2] = {nullptr, nullptr};
     double *d_delays_h = nullptr;
+    double *d_delays_end_h = nullptr;
+    unsigned char *d_valid_h = nullptr;    // [B][S][n_kt] flags of a cobalt_process_host_ex call
+    unsigned int *d_counts_h = nullptr;    // [B][D][n_bl] weights of a cobalt_process_host_ex call
     float *d_bandpass_h = nullptr;
     cudaEvent_t ev_in[2] = {nullptr, nullptr}, ev_cmp[2] = {nullptr, nullptr}, ev_out[2] = {nullptr, nullptr};
     // timing

@@ -74,6 +74,10 @@ void free_scratch(cobalt_plan_s *p) {
         cudaFree(p->d_out[i]);
         p->d_in[i] = p->d_out[i] = nullptr;
     }
+    cudaFree(p->d_valid_h);
+    cudaFree(p->d_counts_h);
+    p->d_valid_h = nullptr;
+    p->d_counts_h = nullptr;
 }
 
 // Tensor map of the fp16 intermediate of one chunk for the F-stage's tensor stores (fstage.cu, store issuer).
@@ -204,14 +208,14 @@ int enqueue_fstage(cobalt_plan_s *p, cudaStream_t st, const void *samples_b0, co
 }
 
 // One chunk of subbands [b0, b0 + nb): samples_b0 / vis_b0 point at subband b0 (of dump 0); io holds the per-call pointers.
-int enqueue_chunk(cobalt_plan_s *p, cudaStream_t st, const void *samples_b0, const cobalt_io_t &io, float2 *vis_b0, int b0, int nb,
-                  StageEvents *ev) {
+// dump_stride: float2 between consecutive dumps at vis_b0 (the caller's [D][B][...] array, or a group-sized staging buffer).
+int enqueue_chunk(cobalt_plan_s *p, cudaStream_t st, const void *samples_b0, const cobalt_io_t &io, float2 *vis_b0, size_t dump_stride, int b0,
+                  int nb, StageEvents *ev) {
     int extra = 0;
     {
         const int rc = enqueue_fstage(p, st, samples_b0, io.delays, io.bandpass, io.delays_end, io.valid, b0, nb, ev, &extra);
         if (rc != COBALT_OK) return rc;
     }
-    const size_t dump_stride = (size_t)p->B * p->C * p->n_bl * 4;      // float2 between dumps
     XCall xc;
     xc.phase = p->d_phase;
     xc.poff = p->d_poff;
@@ -352,6 +356,7 @@ int cobalt_destroy(cobalt_plan_t *p) {
     cudaFree(p->d_coarse);
     cudaFree(p->d_poff);
     cudaFree(p->d_delays_h);
+    cudaFree(p->d_delays_end_h);
     cudaFree(p->d_bandpass_h);
     for (auto &e : p->events)
         for (auto &ev : e.e) cudaEventDestroy(ev);
@@ -392,7 +397,7 @@ int cobalt_process_ex(cobalt_plan_t *p, void *cuda_stream, const cobalt_io_t *io
         const int nb = (p->B - b0) < p->chunk ? (p->B - b0) : p->chunk;
         const unsigned char *sm = static_cast<const unsigned char *>(io->samples) + (size_t)b0 * subband_input_bytes(p);
         float2 *vis = reinterpret_cast<float2 *>(static_cast<unsigned char *>(io->visibilities) + (size_t)b0 * subband_output_bytes(p));
-        int rc = enqueue_chunk(p, st, sm, *io, vis, b0, nb, p->timing ? &p->events[ci] : nullptr);
+        int rc = enqueue_chunk(p, st, sm, *io, vis, (size_t)p->B * p->C * p->n_bl * 4, b0, nb, p->timing ? &p->events[ci] : nullptr);
         if (rc != COBALT_OK) return rc;
     }
     if (p->timing) p->n_chunks_timed = n_chunks;
@@ -495,13 +500,15 @@ int cobalt_beamform(cobalt_plan_t *p, void *cuda_stream, const cobalt_bf_io_t *i
     return COBALT_OK;
 }
 
-int cobalt_process_host(cobalt_plan_t *p, const void *h_samples, const double *h_delays, const float *h_bandpass,
-                        void *h_visibilities) {
+int cobalt_process_host_ex(cobalt_plan_t *p, const cobalt_io_t *h) {
     if (!p) return fail(nullptr, COBALT_ERR_BAD_ARG, "plan is NULL");
-    if (!h_samples || !h_delays || !h_bandpass || !h_visibilities) return fail(p, COBALT_ERR_BAD_ARG, "NULL buffer");
+    if (!h || !h->samples || !h->delays || !h->bandpass || !h->visibilities) return fail(p, COBALT_ERR_BAD_ARG, "NULL buffer");
     if (!p->scratch_ok) return fail(p, COBALT_ERR_NO_MEMORY, "the plan has no scratch (an earlier cobalt_set_mode / cobalt_set_chunk_subbands failed)");
-    if (p->dumps != 1) return fail(p, COBALT_ERR_BAD_ARG, "cobalt_process_host writes one dump per block (cobalt_set_dumps(plan, 1))");
+    if (p->mode == COBALT_MODE_EXACT_FP32 && (long long)p->host_chunk * p->dumps > kMaxGridYZ)
+        return fail(p, COBALT_ERR_BAD_ARG, "COBALT_MODE_EXACT_FP32: subbands per group * dumps exceeds 65535; lower cobalt_set_chunk_subbands or cobalt_set_dumps");
     const size_t in_b = subband_input_bytes(p), out_b = subband_output_bytes(p);
+    const int D = p->dumps;
+    const size_t valid_b = (size_t)p->B * p->S * p->n_kt, counts_b = (size_t)p->B * D * p->n_bl * sizeof(unsigned int);
     if (!p->hs[0]) {
         for (int i = 0; i < 3; ++i) CK(p, cudaStreamCreateWithFlags(&p->hs[i], cudaStreamNonBlocking));
         for (int i = 0; i < 2; ++i) {
@@ -510,14 +517,17 @@ int cobalt_process_host(cobalt_plan_t *p, const void *h_samples, const double *h
             CK(p, cudaEventCreateWithFlags(&p->ev_out[i], cudaEventDisableTiming));
         }
         CK(p, cudaMalloc(&p->d_delays_h, (size_t)p->S * sizeof(double)));
+        CK(p, cudaMalloc(&p->d_delays_end_h, (size_t)p->S * sizeof(double)));
         CK(p, cudaMalloc(&p->d_bandpass_h, (size_t)p->C * sizeof(float)));
     }
-    if (!p->d_in[0]) {
+    if (!p->d_in[0]) {        // (re)allocated after every change of mode / group size / dumps / layout (free_scratch)
         for (int i = 0; i < 2; ++i) {
             CK(p, cudaMalloc(&p->d_in[i], (size_t)p->host_chunk * in_b));
-            CK(p, cudaMalloc(&p->d_out[i], (size_t)p->host_chunk * out_b));
+            CK(p, cudaMalloc(&p->d_out[i], (size_t)p->host_chunk * out_b * D));     // [D][group][C][n_bl][2][2]
         }
     }
+    if (h->valid && !p->d_valid_h) CK(p, cudaMalloc(&p->d_valid_h, valid_b));
+    if (h->valid_counts && !p->d_counts_h) CK(p, cudaMalloc(&p->d_counts_h, counts_b));
     cudaStream_t s_in = p->hs[0], s_cmp = p->hs[1], s_out = p->hs[2];
     // On any failure below the copies already enqueued still touch the caller's host buffers: drain the three
     // streams before returning the error.
@@ -533,8 +543,18 @@ int cobalt_process_host(cobalt_plan_t *p, const void *h_samples, const double *h
         if (e__ != cudaSuccess)                                                                               \
             return drain(fail(p, COBALT_ERR_CUDA, std::string(#call) + ": " + cudaGetErrorString(e__)));      \
     } while (0)
-    CKH(cudaMemcpyAsync(p->d_delays_h, h_delays, (size_t)p->S * sizeof(double), cudaMemcpyHostToDevice, s_cmp));
-    CKH(cudaMemcpyAsync(p->d_bandpass_h, h_bandpass, (size_t)p->C * sizeof(float), cudaMemcpyHostToDevice, s_cmp));
+    // the small per-call arrays travel whole, ahead of the first group, on the compute stream
+    CKH(cudaMemcpyAsync(p->d_delays_h, h->delays, (size_t)p->S * sizeof(double), cudaMemcpyHostToDevice, s_cmp));
+    CKH(cudaMemcpyAsync(p->d_bandpass_h, h->bandpass, (size_t)p->C * sizeof(float), cudaMemcpyHostToDevice, s_cmp));
+    if (h->delays_end) CKH(cudaMemcpyAsync(p->d_delays_end_h, h->delays_end, (size_t)p->S * sizeof(double), cudaMemcpyHostToDevice, s_cmp));
+    if (h->valid) CKH(cudaMemcpyAsync(p->d_valid_h, h->valid, valid_b, cudaMemcpyHostToDevice, s_cmp));
+    cobalt_io_t io{};
+    io.delays = p->d_delays_h;
+    io.bandpass = p->d_bandpass_h;
+    io.delays_end = h->delays_end ? p->d_delays_end_h : nullptr;
+    io.valid = h->valid ? p->d_valid_h : nullptr;
+    io.valid_counts = h->valid_counts ? p->d_counts_h : nullptr;
+    const size_t group_stride = (size_t)p->host_chunk * p->C * p->n_bl * 4;     // float2 between dumps in d_out[buf]
     const int n_chunks = (p->B + p->host_chunk - 1) / p->host_chunk;
     p->launches = 0;
     p->n_chunks_timed = 0;
@@ -543,28 +563,38 @@ int cobalt_process_host(cobalt_plan_t *p, const void *h_samples, const double *h
         const int b0 = ci * p->host_chunk;
         const int nb = (p->B - b0) < p->host_chunk ? (p->B - b0) : p->host_chunk;
         if (ci >= 2) CKH(cudaStreamWaitEvent(s_in, p->ev_cmp[buf], 0));     // d_in[buf] consumed
-        CKH(cudaMemcpyAsync(p->d_in[buf], static_cast<const unsigned char *>(h_samples) + (size_t)b0 * in_b,
+        CKH(cudaMemcpyAsync(p->d_in[buf], static_cast<const unsigned char *>(h->samples) + (size_t)b0 * in_b,
                             (size_t)nb * in_b, cudaMemcpyHostToDevice, s_in));
         CKH(cudaEventRecord(p->ev_in[buf], s_in));
         CKH(cudaStreamWaitEvent(s_cmp, p->ev_in[buf], 0));
         if (ci >= 2) CKH(cudaStreamWaitEvent(s_cmp, p->ev_out[buf], 0));    // d_out[buf] drained
-        cobalt_io_t io{};
-        io.delays = p->d_delays_h;
-        io.bandpass = p->d_bandpass_h;
-        int rc = enqueue_chunk(p, s_cmp, p->d_in[buf], io, static_cast<float2 *>(p->d_out[buf]), b0, nb, nullptr);
+        int rc = enqueue_chunk(p, s_cmp, p->d_in[buf], io, static_cast<float2 *>(p->d_out[buf]), group_stride, b0, nb, nullptr);
         if (rc != COBALT_OK) return drain(rc);
         CKH(cudaEventRecord(p->ev_cmp[buf], s_cmp));
         CKH(cudaStreamWaitEvent(s_out, p->ev_cmp[buf], 0));
-        CKH(cudaMemcpyAsync(static_cast<unsigned char *>(h_visibilities) + (size_t)b0 * out_b, p->d_out[buf],
-                            (size_t)nb * out_b, cudaMemcpyDeviceToHost, s_out));
+        for (int d = 0; d < D; ++d)      // dump d of the group -> subbands [b0, b0 + nb) of dump d of the caller's [D][B][...] array
+            CKH(cudaMemcpyAsync(static_cast<unsigned char *>(h->visibilities) + ((size_t)d * p->B + b0) * out_b,
+                                static_cast<const unsigned char *>(p->d_out[buf]) + (size_t)d * group_stride * sizeof(float2),
+                                (size_t)nb * out_b, cudaMemcpyDeviceToHost, s_out));
         CKH(cudaEventRecord(p->ev_out[buf], s_out));
     }
+    if (h->valid_counts) CKH(cudaMemcpyAsync(h->valid_counts, p->d_counts_h, counts_b, cudaMemcpyDeviceToHost, s_cmp));
     if (!history_in_place(p)) p->hist_cur ^= 1;
     CKH(cudaStreamSynchronize(s_in));
     CKH(cudaStreamSynchronize(s_cmp));
     CKH(cudaStreamSynchronize(s_out));
 #undef CKH
     return COBALT_OK;
+}
+
+int cobalt_process_host(cobalt_plan_t *p, const void *h_samples, const double *h_delays, const float *h_bandpass,
+                        void *h_visibilities) {
+    cobalt_io_t h{};
+    h.samples = h_samples;
+    h.delays = h_delays;
+    h.bandpass = h_bandpass;
+    h.visibilities = h_visibilities;
+    return cobalt_process_host_ex(p, &h);
 }
 
 int cobalt_set_subband_frequencies(cobalt_plan_t *p, const double *h_hz) {

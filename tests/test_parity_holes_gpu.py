@@ -291,3 +291,43 @@ def test_oversized_grids_are_refused_before_anything_is_enqueued(cobalt, dev):
         with pytest.raises(cobalt.CobaltError) as e:
             cobalt.cobalt_beamform(cor._h, None, dummy, dummy, dummy, dummy, 1, cobalt.COBALT_BF_INCOHERENT_STOKES, 1, 1, dummy)
         assert e.value.status == cobalt.COBALT_ERR_BAD_ARG and "spectra" in str(e.value)
+
+
+# ------------------------------------------------------------------ the host-buffer call with every optional array
+@pytest.mark.parametrize("tensor", [False, True])
+def test_process_host_ex_is_bit_identical_to_the_device_path(cobalt, dev, tensor):
+    """cobalt_process_host_ex (pinned host buffers: dumps, lost-data flags, weights, time-varying delay; groups of 2 + 2 + 1
+    subbands) on one plan against cobalt_process_ex with device copies of the same buffers on a second plan, over two
+    consecutive blocks (history carry): the same kernels on the same data, so bit for bit.  Then the plain
+    cobalt_process_host on plans that write two dumps per block (it used to refuse them)."""
+    from paper_1801_04834_b200 import synth
+
+    cfg = synth.scaled(synth.CONFIGS[3], S=6, B=5, C=64, N=64 * 64 * 4)
+    D = 2
+    rng = np.random.default_rng(4500)
+    with cobalt.Correlator(cfg.S, cfg.B, cfg.C, cfg.N, cfg.bits, mode=_mode(cobalt, tensor)) as on_dev, \
+            cobalt.Correlator(cfg.S, cfg.B, cfg.C, cfg.N, cfg.bits, mode=_mode(cobalt, tensor)) as on_host:
+        for cor in (on_dev, on_host):
+            cor.set_chunk_subbands(2)
+            cor.set_dumps(D)
+        i = on_host.info
+        for call in range(2):
+            data = synth.generate(synth.scaled(cfg, sigma=cfg.sigma * (1 + call)), device="cpu")
+            tau_e = data["delays"] + torch.from_numpy(rng.uniform(-1, 1, cfg.S) * 2e-8)
+            valid = torch.from_numpy((rng.uniform(size=(cfg.B, cfg.S, i.n_tiles)) > 0.3).astype(np.uint8))
+            want_counts = torch.zeros((cfg.B, D, i.n_baselines), dtype=torch.int32, device=dev)
+            want = on_dev.process(data["samples"].to(dev), data["delays"].to(dev), data["bandpass"].to(dev), delays_end=tau_e.to(dev),
+                                  valid=valid.to(dev), valid_counts=want_counts).cpu().numpy()
+            out = torch.full(on_host.vis_shape(), float("nan"), dtype=torch.complex64).pin_memory()
+            counts = torch.full((cfg.B, D, i.n_baselines), -1, dtype=torch.int32).pin_memory()
+            on_host.process_host(data["samples"].pin_memory(), data["delays"], data["bandpass"], out, delays_end=tau_e, valid=valid.pin_memory(),
+                                 valid_counts=counts)
+            assert out.shape[0] == D and want.shape == tuple(out.shape)
+            assert np.array_equal(want.view(np.float32), out.numpy().view(np.float32)), f"block {call}"
+            assert np.array_equal(want_counts.cpu().numpy(), counts.numpy()), f"block {call}"
+        for cor in (on_dev, on_host):
+            cor.reset()
+        plain_d = on_dev.process(data["samples"].to(dev), data["delays"].to(dev), data["bandpass"].to(dev)).cpu().numpy()
+        plain_h = torch.empty(on_host.vis_shape(), dtype=torch.complex64).pin_memory()
+        on_host.process_host(data["samples"].pin_memory(), data["delays"], data["bandpass"], plain_h)
+        assert np.array_equal(plain_d.view(np.float32), plain_h.numpy().view(np.float32))
